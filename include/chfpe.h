@@ -1,0 +1,132 @@
+/*
+ * chfpe.h -- C-ABI boundary of the B200-native multimode CHFPE hot path (libchfpe.so).
+ *
+ * Method: R. Hoshino and Y. Tanimura, "A Multimode Classical Hierarchical Fokker-Planck Equations
+ * Approach to Molecular Vibrations: Simulating Two-Dimensional Spectra" (arXiv 2509.25840).
+ * Citations below are line numbers of the paper text plus the equation they fall in;
+ * "R<n>" are the readings of garbled / silent passages listed in DESIGN.md.
+ *
+ * The library time-propagates the whole hierarchy W^(n)(q1,p1,...,qM,pM), M = 1..3, on a uniform
+ * phase-space grid in fp64, applies Poisson-bracket kicks, reduces phase-space expectations and runs
+ * the 1D / 2D response protocols.  Every step runs in hand-written sm_100a CUDA kernels; there is no
+ * CPU fallback (calls fail with CHFPE_ERR_CUDA when no device / kernel image is available).
+ *
+ * Conventions
+ *   - All functions return int: CHFPE_OK (0) or a negative CHFPE_ERR_* code.  They never throw,
+ *     abort or print.  chfpe_last_error() returns a static or handle-owned message.
+ *   - "host" / "device" is stated for every pointer.  Device memory and the CUDA stream are OWNED BY
+ *     THE CALLER: the library carves its state arrays, stage buffers, tables and reduction scratch out
+ *     of the single workspace passed to chfpe_create and never allocates device memory itself.
+ *   - Calls are asynchronous on the stream given at create time, except those that return host data
+ *     (expect, response_*, equilibrate with residual_out, export to host), which synchronise that
+ *     stream only.  A handle is not thread-safe; distinct handles are independent.
+ *   - Canonical (import/export) layout of one replica: X[k][i_q1][i_p1]...[i_qM][i_pM], last axis
+ *     fastest, hierarchy element k outermost ("hierarchy-major"), fp64.  X = W (gauge W) or
+ *     X = f = W / sqrt(W_eq) (gauge SQRT_EQ, default).  The internal device layout differs (q-major /
+ *     p-minor bricks) and is not exposed.
+ *   - Element order (R5, R6): all n in N^M with n_1+...+n_M <= depth; ascending |n|, ties by
+ *     descending lexicographic (n_1,...,n_M).
+ */
+#ifndef CHFPE_H
+#define CHFPE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  CHFPE_OK = 0,
+  CHFPE_ERR_INVALID = -1,    /* bad descriptor / argument (M not in 1..3, < 5 grid points, degree > 4, ...) */
+  CHFPE_ERR_WORKSPACE = -2,  /* workspace too small or not 256-byte aligned */
+  CHFPE_ERR_CUDA = -3,       /* CUDA runtime error; message from cudaGetErrorString */
+  CHFPE_ERR_DIVERGED = -4,   /* non-finite expectation value encountered */
+  CHFPE_ERR_STATE = -5       /* call sequence error (e.g. response before equilibrate/import) */
+};
+
+enum { CHFPE_CENTRAL4 = 0, CHFPE_CENTRAL2 = 1, CHFPE_COMPACT6 = 2 };   /* derivative scheme */
+enum { CHFPE_GAUGE_SQRT_EQ = 0, CHFPE_GAUGE_W = 1 };                   /* propagated variable (R7) */
+
+/* coef * q1^e1 q2^e2 q3^e3 ; total degree <= 4.  Eq. (3)-(4). */
+typedef struct { double coef; int32_t expo[3]; } chfpe_monomial;
+
+/* Model + discretisation.  Copied at create time.  Entries beyond n_modes are ignored. */
+typedef struct {
+  int32_t n_modes;                    /* M = 1..3 */
+  double  mass[3];                    /* m_s, Eq. (2) :45 */
+  int32_t n_terms; const chfpe_monomial* U;   /* host; U(q) incl. harmonic, anharmonic and mode-mode terms */
+  double  V_LL[3], V_SL[3];           /* V_s = V_LL q + V_SL q^2/2 */
+  double  zeta[3], gamma[3], beta;    /* Drude baths Eq. (7) :67, inverse temperature */
+  int32_t nq[3], np[3];               /* grid points per axis (>= 5) */
+  double  qmin[3], qmax[3], pmin[3], pmax[3];   /* nodal uniform grid, end points included (R8) */
+  int32_t depth;                      /* N: elements n with sum(n) <= N */
+  int32_t scheme;                     /* CHFPE_CENTRAL4 (default) | CHFPE_CENTRAL2 | CHFPE_COMPACT6 */
+  int32_t gauge;                      /* CHFPE_GAUGE_SQRT_EQ (default) | CHFPE_GAUGE_W (literal Eq. 8) */
+  int32_t batch;                      /* B >= 1 independent replicas (state slots) sharing the operator */
+} chfpe_desc;
+
+/* X(q,p) = c0 + sum lin_q[s] q_s + 1/2 sum quad[s][s'] q_s q_s' + sum lin_p[s] p_s ; Eq. (13)-(14) :108-113.
+   lin_p and c0 are used by chfpe_expect only (kick needs dX/dq_s). */
+typedef struct { double c0, lin_q[3], quad[3][3], lin_p[3]; } chfpe_observable;
+
+typedef struct chfpe_handle chfpe_handle;     /* opaque, host side, owned by the library */
+
+/* Device bytes the caller must provide for this descriptor (256-byte aligned).  out: host. */
+int chfpe_workspace_bytes(const chfpe_desc* desc, size_t* bytes);
+
+/* Build tables (setup step a0), carve the workspace, zero all replicas.  dev_workspace: device, caller-owned,
+   must outlive the handle.  cuda_stream: a cudaStream_t (0 = legacy default stream).  Section IV.A, :217-219. */
+int chfpe_create(const chfpe_desc* desc, void* dev_workspace, size_t bytes, void* cuda_stream, chfpe_handle** out);
+
+/* Frees the host struct only (the workspace stays with the caller). */
+int chfpe_destroy(chfpe_handle* h);
+
+int chfpe_num_elements(const chfpe_handle* h, int32_t* K);                  /* K = C(N+M, M) */
+int chfpe_element_index(const chfpe_handle* h, int32_t k, int32_t n_out[3]); /* canonical order */
+
+/* All replicas: X_0 <- analytic equilibrium (e^{-beta H}/Z or phi/Z_f), X_{k>0} <- 0, then n_steps RK4 steps
+   (section IV.B, :221-223; R18).  residual_out (host, may be NULL) <- ||F(X)||_2 / ||X||_2 of replica 0. */
+int chfpe_equilibrate(chfpe_handle* h, int64_t n_steps, double dt, double* residual_out);
+
+/* n_steps fourth-order Runge-Kutta steps of Eq. (8) :77-80 on every replica (R13: evaluated in the
+   Horner form of the same degree-4 polynomial in dt*L, the generator being linear and autonomous). */
+int chfpe_step(chfpe_handle* h, int64_t n_steps, double dt);
+
+/* Every element of every replica: X_k <- sum_s (dX/dq_s) (d/dp_s) X_k, Eq. (18) :131, literal (no sign; R3, R11). */
+int chfpe_kick(chfpe_handle* h, const chfpe_observable* X);
+
+/* out[b] (host, length batch) <- integral of O(q,p) W^(0) over phase space for replica b, Eq. (15) :119 (R10, R12). */
+int chfpe_expect(chfpe_handle* h, const chfpe_observable* O, double* out);
+
+/* Same reduction on element k of replica `replica` (tests of the hierarchy normalisation). out: host, 1 double. */
+int chfpe_expect_element(chfpe_handle* h, int32_t replica, int32_t k, const chfpe_observable* O, double* out);
+
+/* R1: replica 0 <- Kick(A) replica 0; for i in 0..n_samples-1: R[i] = <C>, then `stride` steps.
+   Literal Eq. (15) :119, section IV.C.1 :229-233.  R: host, n_samples doubles.  Other replicas untouched. */
+int chfpe_response_1d(chfpe_handle* h, const chfpe_observable* A, const chfpe_observable* C,
+                      int64_t n_samples, int64_t stride, double dt, double* R);
+
+/* R2[k][j]: T <- Kick(A) replica 0, advanced along t1; at t1_steps[k] a copy of T gets Kick(B) and is propagated
+   over the t2 grid, <C> recorded after t2_steps[j] steps.  Literal Eq. (16) :121-122, section IV.C.2 :235-237.
+   Step lists: host, ascending, >= 0.  R: host, row-major [n1][n2].  With batch >= 2, batch-1 replicas (different
+   t1) are propagated together per launch; with batch == 1 an extra workspace slot is used sequentially. */
+int chfpe_response_2d(chfpe_handle* h, const chfpe_observable* A, const chfpe_observable* B, const chfpe_observable* C,
+                      const int64_t* t1_steps, int32_t n1, const int64_t* t2_steps, int32_t n2,
+                      double dt, double* R);
+
+/* Canonical-layout copy of one replica out of / into the library (K*cells doubles). dst/src: device if *_is_device. */
+int chfpe_export_state(chfpe_handle* h, int32_t replica, double* dst, int dst_is_device);
+int chfpe_import_state(chfpe_handle* h, int32_t replica, const double* src, int src_is_device);
+
+/* F(X) of replica `replica` (right-hand side of Eq. (8)), canonical layout, for operator-level parity tests. */
+int chfpe_export_rhs(chfpe_handle* h, int32_t replica, double* dst, int dst_is_device);
+
+/* Number of kernels the library has launched on this handle since create (bench.py's gpu_launches). */
+int chfpe_launch_count(const chfpe_handle* h, int64_t* n);
+
+const char* chfpe_last_error(const chfpe_handle* h);   /* h may be NULL: last create-time error */
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,266 @@
+"""ctypes binding of include/chfpe.h (same names, argument marshalling only)."""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+EXPORTED_SYMBOLS = [
+    "chfpe_workspace_bytes", "chfpe_create", "chfpe_destroy", "chfpe_num_elements", "chfpe_element_index",
+    "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
+    "chfpe_response_1d", "chfpe_response_2d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
+    "chfpe_launch_count", "chfpe_last_error",
+]
+
+
+class ChfpeError(RuntimeError):
+    pass
+
+
+class Monomial(C.Structure):
+    _fields_ = [("coef", C.c_double), ("expo", C.c_int32 * 3)]
+
+
+class Desc(C.Structure):
+    _fields_ = [("n_modes", C.c_int32), ("mass", C.c_double * 3),
+                ("n_terms", C.c_int32), ("U", C.POINTER(Monomial)),
+                ("V_LL", C.c_double * 3), ("V_SL", C.c_double * 3),
+                ("zeta", C.c_double * 3), ("gamma", C.c_double * 3), ("beta", C.c_double),
+                ("nq", C.c_int32 * 3), ("np", C.c_int32 * 3),
+                ("qmin", C.c_double * 3), ("qmax", C.c_double * 3),
+                ("pmin", C.c_double * 3), ("pmax", C.c_double * 3),
+                ("depth", C.c_int32), ("scheme", C.c_int32), ("gauge", C.c_int32), ("batch", C.c_int32)]
+
+
+class Observable(C.Structure):
+    _fields_ = [("c0", C.c_double), ("lin_q", C.c_double * 3), ("quad", (C.c_double * 3) * 3),
+                ("lin_p", C.c_double * 3)]
+
+
+SCHEMES = {"central4": 0, "central2": 1, "compact6": 2}
+GAUGES = {"sqrt_eq": 0, "w": 1}
+_lib = None
+
+
+def lib():
+    """Load libchfpe.so (building it in-tree with nvcc if absent).  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    try:
+        so = _build.build()
+    except Exception as exc:   # no nvcc and no prebuilt library: fail loudly, never fall back
+        if not os.path.exists(_build.SO):
+            raise ChfpeError("libchfpe.so is missing and could not be built with nvcc: %s" % exc)
+        so = _build.SO
+    L = C.CDLL(so)
+    vp, dp, i64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)
+    op = C.POINTER(Observable)
+    L.chfpe_workspace_bytes.argtypes = [C.POINTER(Desc), C.POINTER(C.c_size_t)]
+    L.chfpe_create.argtypes = [C.POINTER(Desc), vp, C.c_size_t, vp, C.POINTER(vp)]
+    L.chfpe_destroy.argtypes = [vp]
+    L.chfpe_num_elements.argtypes = [vp, C.POINTER(C.c_int32)]
+    L.chfpe_element_index.argtypes = [vp, C.c_int32, C.POINTER(C.c_int32)]
+    L.chfpe_equilibrate.argtypes = [vp, C.c_int64, C.c_double, dp]
+    L.chfpe_step.argtypes = [vp, C.c_int64, C.c_double]
+    L.chfpe_kick.argtypes = [vp, op]
+    L.chfpe_expect.argtypes = [vp, op, dp]
+    L.chfpe_expect_element.argtypes = [vp, C.c_int32, C.c_int32, op, dp]
+    L.chfpe_response_1d.argtypes = [vp, op, op, C.c_int64, C.c_int64, C.c_double, dp]
+    L.chfpe_response_2d.argtypes = [vp, op, op, op, i64p, C.c_int32, i64p, C.c_int32, C.c_double, dp]
+    L.chfpe_export_state.argtypes = [vp, C.c_int32, vp, C.c_int]
+    L.chfpe_import_state.argtypes = [vp, C.c_int32, vp, C.c_int]
+    L.chfpe_export_rhs.argtypes = [vp, C.c_int32, vp, C.c_int]
+    L.chfpe_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.chfpe_last_error.argtypes = [vp]
+    L.chfpe_last_error.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _vec3(vals, fill=0.0):
+    v = list(vals) + [fill] * (3 - len(vals))
+    return (C.c_double * 3)(*v)
+
+
+def make_observable(c0=0.0, lin_q=(), quad=None, lin_p=()):
+    o = Observable()
+    o.c0 = c0
+    for s, v in enumerate(lin_q):
+        o.lin_q[s] = v
+    for s, v in enumerate(lin_p):
+        o.lin_p[s] = v
+    if quad is not None:
+        for a, row in enumerate(quad):
+            for b, v in enumerate(row):
+                o.quad[a][b] = v
+    return o
+
+
+def make_desc(cfg, batch=1):
+    """Fill a chfpe_desc from a plain parameter dict (chfpe_inputs.config).  Returns (desc, keepalive)."""
+    M = cfg["n_modes"]
+    d = Desc()
+    d.n_modes = M
+    d.mass = _vec3(cfg.get("mass", [1.0] * M), 1.0)
+    terms = cfg["U"]
+    arr = (Monomial * max(1, len(terms)))()
+    for i, (coef, expo) in enumerate(terms):
+        arr[i].coef = coef
+        arr[i].expo = (C.c_int32 * 3)(*(list(expo) + [0] * (3 - len(expo))))
+    d.n_terms = len(terms)
+    d.U = C.cast(arr, C.POINTER(Monomial))
+    d.V_LL = _vec3(cfg["V_LL"])
+    d.V_SL = _vec3(cfg["V_SL"])
+    d.zeta = _vec3(cfg["zeta"])
+    d.gamma = _vec3(cfg["gamma"], 1.0)
+    d.beta = cfg.get("beta", 1.0)
+    d.nq = (C.c_int32 * 3)(*(list(cfg["nq"]) + [0] * (3 - M)))
+    d.np = (C.c_int32 * 3)(*(list(cfg["np"]) + [0] * (3 - M)))
+    d.qmin = _vec3(cfg["qmin"])
+    d.qmax = _vec3(cfg["qmax"])
+    d.pmin = _vec3(cfg["pmin"])
+    d.pmax = _vec3(cfg["pmax"])
+    d.depth = cfg["depth"]
+    d.scheme = SCHEMES[cfg.get("scheme", "central4")]
+    d.gauge = GAUGES[cfg.get("gauge", "sqrt_eq")]
+    d.batch = batch
+    return d, arr
+
+
+def workspace_bytes(cfg, batch=1):
+    d, _keep = make_desc(cfg, batch)
+    n = C.c_size_t()
+    rc = lib().chfpe_workspace_bytes(C.byref(d), C.byref(n))
+    if rc != 0:
+        raise ChfpeError("chfpe_workspace_bytes: %d %s" % (rc, lib().chfpe_last_error(None).decode()))
+    return n.value
+
+
+class CHFPE:
+    """One library handle.  The workspace is a torch uint8 CUDA tensor owned by this object."""
+
+    def __init__(self, cfg, batch=1, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise ChfpeError("CUDA device required: the CHFPE path has no CPU fallback")
+        L = lib()
+        self._torch = torch
+        self.device = torch.device(device)
+        d, keep = make_desc(cfg, batch)
+        nbytes = workspace_bytes(cfg, batch)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            base = self.workspace.data_ptr()
+            aligned = (base + 255) & ~255
+            self._h = C.c_void_p()
+            rc = L.chfpe_create(C.byref(d), C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream),
+                                C.byref(self._h))
+        if rc != 0:
+            raise ChfpeError("chfpe_create: %d %s" % (rc, L.chfpe_last_error(None).decode()))
+        self.cfg = cfg
+        self.batch = batch
+        self.M = cfg["n_modes"]
+        k = C.c_int32()
+        L.chfpe_num_elements(self._h, C.byref(k))
+        self.K = k.value
+        self.shape = tuple(x for s in range(self.M) for x in (cfg["nq"][s], cfg["np"][s]))
+        self.cells = int(np.prod(self.shape))
+
+    def _ck(self, rc, what):
+        if rc != 0:
+            raise ChfpeError("%s: %d %s" % (what, rc, lib().chfpe_last_error(self._h).decode()))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().chfpe_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def element_index(self, k):
+        n = (C.c_int32 * 3)()
+        self._ck(lib().chfpe_element_index(self._h, k, n), "chfpe_element_index")
+        return tuple(n[: self.M])
+
+    def elements(self):
+        return [self.element_index(k) for k in range(self.K)]
+
+    def equilibrate(self, n_steps=0, dt=0.0, residual=True):
+        r = C.c_double()
+        self._ck(lib().chfpe_equilibrate(self._h, n_steps, dt, C.byref(r) if residual else None), "chfpe_equilibrate")
+        return r.value if residual else None
+
+    def step(self, n_steps, dt):
+        self._ck(lib().chfpe_step(self._h, n_steps, dt), "chfpe_step")
+
+    def kick(self, obs):
+        self._ck(lib().chfpe_kick(self._h, C.byref(obs)), "chfpe_kick")
+
+    def expect(self, obs):
+        out = np.empty(self.batch)
+        self._ck(lib().chfpe_expect(self._h, C.byref(obs), out.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_expect")
+        return out
+
+    def expect_element(self, obs, k, replica=0):
+        out = C.c_double()
+        self._ck(lib().chfpe_expect_element(self._h, replica, k, C.byref(obs), C.byref(out)), "chfpe_expect_element")
+        return out.value
+
+    def response_1d(self, A, Cobs, n_samples, stride, dt):
+        R = np.empty(n_samples)
+        self._ck(lib().chfpe_response_1d(self._h, C.byref(A), C.byref(Cobs), n_samples, stride, dt,
+                                         R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_response_1d")
+        return R
+
+    def response_2d(self, A, B, Cobs, t1_steps, t2_steps, dt):
+        t1 = np.ascontiguousarray(t1_steps, dtype=np.int64)
+        t2 = np.ascontiguousarray(t2_steps, dtype=np.int64)
+        R = np.empty((len(t1), len(t2)))
+        self._ck(lib().chfpe_response_2d(self._h, C.byref(A), C.byref(B), C.byref(Cobs),
+                                         t1.ctypes.data_as(C.POINTER(C.c_int64)), len(t1),
+                                         t2.ctypes.data_as(C.POINTER(C.c_int64)), len(t2), dt,
+                                         R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_response_2d")
+        return R
+
+    def export_state(self, replica=0):
+        X = np.empty((self.K,) + self.shape)
+        self._ck(lib().chfpe_export_state(self._h, replica, C.c_void_p(X.ctypes.data), 0), "chfpe_export_state")
+        return X
+
+    def export_state_device(self, replica=0):
+        t = self._torch.empty((self.K,) + self.shape, dtype=self._torch.float64, device=self.device)
+        self._ck(lib().chfpe_export_state(self._h, replica, C.c_void_p(t.data_ptr()), 1), "chfpe_export_state")
+        return t
+
+    def import_state(self, X, replica=0):
+        if hasattr(X, "data_ptr"):
+            assert X.is_cuda and X.is_contiguous() and X.numel() == self.K * self.cells
+            self._ck(lib().chfpe_import_state(self._h, replica, C.c_void_p(X.data_ptr()), 1), "chfpe_import_state")
+            self.stream.synchronize()
+            return
+        X = np.ascontiguousarray(X, dtype=np.float64)
+        assert X.size == self.K * self.cells
+        self._ck(lib().chfpe_import_state(self._h, replica, C.c_void_p(X.ctypes.data), 0), "chfpe_import_state")
+
+    def export_rhs(self, replica=0):
+        F = np.empty((self.K,) + self.shape)
+        self._ck(lib().chfpe_export_rhs(self._h, replica, C.c_void_p(F.ctypes.data), 0), "chfpe_export_rhs")
+        return F
+
+    def export_rhs_device(self, replica=0):
+        t = self._torch.empty((self.K,) + self.shape, dtype=self._torch.float64, device=self.device)
+        self._ck(lib().chfpe_export_rhs(self._h, replica, C.c_void_p(t.data_ptr()), 1), "chfpe_export_rhs")
+        return t
+
+    def launch_count(self):
+        n = C.c_int64()
+        self._ck(lib().chfpe_launch_count(self._h, C.byref(n)), "chfpe_launch_count")
+        return n.value

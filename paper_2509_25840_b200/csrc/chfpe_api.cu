@@ -1,0 +1,471 @@
+// Host side of the C-ABI (include/chfpe.h): validation, setup tables (step a0), workspace carving and the
+// drivers that sequence kernel launches (equilibrate a6, step a1-a3, kick a4, expect a5, R1 a7, R2 a8).
+// No arithmetic of the method runs on the host beyond the one-off tables of `create`.
+#include <cmath>
+#include <cstring>
+#include "chfpe_internal.cuh"
+
+static thread_local std::string g_create_err;
+
+#define FAIL(h, code, msg)                  \
+  do {                                      \
+    (h)->err = (msg);                       \
+    return (code);                          \
+  } while (0)
+
+#define CU(h, call)                                              \
+  do {                                                           \
+    cudaError_t e_ = (call);                                     \
+    if (e_ != cudaSuccess) {                                     \
+      (h)->err = std::string(#call) + ": " + cudaGetErrorString(e_); \
+      return CHFPE_ERR_CUDA;                                     \
+    }                                                            \
+  } while (0)
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static int enumerate_elements(int M, int depth, std::vector<int>* out) {
+  int K = 0;
+  for (int lev = 0; lev <= depth; lev++) {
+    for (int a = lev; a >= 0; a--) {
+      if (M == 1) { if (a != lev) break; if (out) { out->push_back(a); out->push_back(0); out->push_back(0); } K++; continue; }
+      for (int b = lev - a; b >= 0; b--) {
+        if (M == 2) { if (b != lev - a) break; if (out) { out->push_back(a); out->push_back(b); out->push_back(0); } K++; continue; }
+        if (out) { out->push_back(a); out->push_back(b); out->push_back(lev - a - b); }
+        K++;
+      }
+    }
+  }
+  return K;
+}
+
+static int validate(const chfpe_desc* d, std::string* why) {
+  if (!d) { *why = "null descriptor"; return CHFPE_ERR_INVALID; }
+  if (d->n_modes < 1 || d->n_modes > 3) { *why = "n_modes must be 1..3"; return CHFPE_ERR_INVALID; }
+  if (d->depth < 0 || d->depth > 64) { *why = "depth out of range"; return CHFPE_ERR_INVALID; }
+  if (!(d->beta > 0)) { *why = "beta must be > 0"; return CHFPE_ERR_INVALID; }
+  if (d->scheme != CHFPE_CENTRAL4 && d->scheme != CHFPE_CENTRAL2 && d->scheme != CHFPE_COMPACT6) { *why = "unknown scheme"; return CHFPE_ERR_INVALID; }
+  if (d->scheme == CHFPE_COMPACT6) { *why = "COMPACT6 (conditional step a9) is not built in this round"; return CHFPE_ERR_INVALID; }
+  if (d->gauge != CHFPE_GAUGE_SQRT_EQ && d->gauge != CHFPE_GAUGE_W) { *why = "unknown gauge"; return CHFPE_ERR_INVALID; }
+  if (d->batch < 1 || d->batch > 4096) { *why = "batch must be 1..4096"; return CHFPE_ERR_INVALID; }
+  if (d->n_terms < 0 || (d->n_terms > 0 && !d->U)) { *why = "bad potential term list"; return CHFPE_ERR_INVALID; }
+  for (int t = 0; t < d->n_terms; t++) {
+    int deg = 0;
+    for (int s = 0; s < 3; s++) {
+      if (d->U[t].expo[s] < 0) { *why = "negative exponent"; return CHFPE_ERR_INVALID; }
+      if (s < d->n_modes) deg += d->U[t].expo[s];
+    }
+    if (deg > 4) { *why = "potential degree > 4"; return CHFPE_ERR_INVALID; }
+  }
+  for (int s = 0; s < d->n_modes; s++) {
+    if (d->nq[s] < 5 || d->np[s] < 5) { *why = "need >= 5 grid points per axis"; return CHFPE_ERR_INVALID; }
+    if (!(d->mass[s] > 0) || !(d->gamma[s] > 0) || d->zeta[s] < 0) { *why = "mass, gamma must be > 0 and zeta >= 0"; return CHFPE_ERR_INVALID; }
+    if (!(d->qmax[s] > d->qmin[s]) || !(d->pmax[s] > d->pmin[s])) { *why = "empty coordinate range"; return CHFPE_ERR_INVALID; }
+  }
+  return CHFPE_OK;
+}
+
+struct Plan {
+  int M, K, batch, n_arrays, red_blocks;
+  long long cells, nqc;
+  size_t off_tables, tables_bytes, off_partial, off_results, off_arrays, total;
+  static const long long RESULTS = 1 << 16;
+};
+
+static Plan make_plan(const chfpe_desc* d) {
+  Plan p;
+  p.M = d->n_modes; p.batch = d->batch;
+  p.K = enumerate_elements(p.M, d->depth, nullptr);
+  p.cells = 1; p.nqc = 1;
+  long long sum_n = 0;
+  for (int s = 0; s < p.M; s++) { p.cells *= (long long)d->nq[s] * d->np[s]; p.nqc *= d->nq[s]; sum_n += d->np[s]; }
+  p.n_arrays = 3 * p.batch + (p.batch == 1 ? 1 : 0);
+  p.red_blocks = 592;
+  size_t o = 0;
+  p.off_tables = o;
+  size_t tb = 0;
+  tb += align256(sizeof(double) * p.nqc) * (p.M + 1);          // dU[s], eU
+  tb += align256(sizeof(double) * sum_n);                      // ep
+  tb += align256(sizeof(int) * 3 * p.K) * 3;                   // up, dn, nvec
+  tb += align256(sizeof(double) * p.K);                        // Gamma
+  p.tables_bytes = tb; o += tb;
+  p.off_partial = o; o += align256(sizeof(double) * p.red_blocks * (size_t)p.batch);
+  p.off_results = o; o += align256(sizeof(double) * Plan::RESULTS);
+  p.off_arrays = o; o += align256(sizeof(double) * (size_t)p.n_arrays * p.K * p.cells);
+  p.total = o;
+  return p;
+}
+
+extern "C" int chfpe_workspace_bytes(const chfpe_desc* desc, size_t* bytes) {
+  std::string why;
+  int rc = validate(desc, &why);
+  if (rc != CHFPE_OK || !bytes) { g_create_err = why.empty() ? "null output" : why; return CHFPE_ERR_INVALID; }
+  *bytes = make_plan(desc).total;
+  return CHFPE_OK;
+}
+
+static double ipow(double x, int e) { double r = 1.0; for (int i = 0; i < e; i++) r *= x; return r; }
+
+extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void* cuda_stream, chfpe_handle** out) {
+  std::string why;
+  int rc = validate(desc, &why);
+  if (rc != CHFPE_OK) { g_create_err = why; return rc; }
+  if (!out) { g_create_err = "null output"; return CHFPE_ERR_INVALID; }
+  Plan pl = make_plan(desc);
+  if (!ws || bytes < pl.total || ((uintptr_t)ws & 255)) { g_create_err = "workspace too small or misaligned"; return CHFPE_ERR_WORKSPACE; }
+  int ndev = 0;
+  cudaError_t ce = cudaGetDeviceCount(&ndev);
+  if (ce != cudaSuccess || ndev == 0) { g_create_err = std::string("no CUDA device: ") + cudaGetErrorString(ce); return CHFPE_ERR_CUDA; }
+
+  chfpe_handle* h = new chfpe_handle();
+  h->desc = *desc;
+  h->U.assign(desc->U, desc->U + desc->n_terms);
+  h->desc.U = h->U.data();
+  h->stream = (cudaStream_t)cuda_stream;
+  h->K = pl.K; h->batch = pl.batch; h->n_arrays = pl.n_arrays; h->cells = pl.cells;
+  h->state_doubles = (size_t)pl.K * pl.cells;
+  h->red_blocks = pl.red_blocks;
+  h->initialised = false; h->launches = 0;
+  const int M = pl.M;
+  enumerate_elements(M, desc->depth, &h->elem);
+
+  DevOp& op = h->op;
+  memset(&op, 0, sizeof(op));
+  op.M = M; op.nax = 2 * M; op.K = pl.K; op.scheme = desc->scheme; op.gauge = desc->gauge; op.beta = desc->beta;
+  for (int s = 0; s < M; s++) {
+    op.n[s] = desc->nq[s]; op.n[M + s] = desc->np[s];
+    op.x0[s] = desc->qmin[s]; op.x0[M + s] = desc->pmin[s];
+    op.h[s] = (desc->qmax[s] - desc->qmin[s]) / (desc->nq[s] - 1);
+    op.h[M + s] = (desc->pmax[s] - desc->pmin[s]) / (desc->np[s] - 1);
+    op.inv_mass[s] = 1.0 / desc->mass[s];
+    op.cdn[s] = desc->zeta[s] * desc->gamma[s] * desc->mass[s] / desc->beta;
+    if (desc->gauge == CHFPE_GAUGE_W) { op.kup[s] = 0.0; op.kdn[s] = desc->beta / desc->mass[s]; }
+    else { op.kup[s] = -desc->beta / (2 * desc->mass[s]); op.kdn[s] = desc->beta / (2 * desc->mass[s]); }
+    op.VLL[s] = desc->V_LL[s]; op.VSL[s] = desc->V_SL[s];
+  }
+  op.cells = pl.cells; op.nqc = pl.nqc; op.pb = pl.cells / pl.nqc;
+  op.dV = 1.0;
+  long long st = 1;
+  for (int a = 2 * M - 1; a >= 0; a--) {
+    op.st[a] = st; st *= op.n[a]; op.dV *= op.h[a];
+    if (desc->scheme == CHFPE_CENTRAL4) { op.c1[a] = 8.0 / (12.0 * op.h[a]); op.c2[a] = -1.0 / (12.0 * op.h[a]); }
+    else { op.c1[a] = 1.0 / (2.0 * op.h[a]); op.c2[a] = 0.0; }
+  }
+
+  // ---- host tables (setup step a0) ----
+  std::vector<double> dU[3], eU(pl.nqc);
+  for (int s = 0; s < M; s++) dU[s].resize(pl.nqc);
+  const double wfac = (desc->gauge == CHFPE_GAUGE_W) ? 1.0 : 0.5;     // weight exponent: e^{-beta H} or e^{-beta H/2}
+  for (long long l = 0; l < pl.nqc; l++) {
+    int iq[3] = {0, 0, 0}; long long r = l;
+    for (int s = M - 1; s >= 0; s--) { iq[s] = (int)(r % op.n[s]); r /= op.n[s]; }
+    double q[3] = {0, 0, 0};
+    for (int s = 0; s < M; s++) q[s] = op.x0[s] + iq[s] * op.h[s];
+    double u = 0.0, du[3] = {0, 0, 0};
+    for (const chfpe_monomial& t : h->U) {
+      double v = t.coef;
+      for (int s = 0; s < M; s++) v *= ipow(q[s], t.expo[s]);
+      u += v;
+      for (int s = 0; s < M; s++) {
+        if (t.expo[s] == 0) continue;
+        double w = t.coef * t.expo[s] * ipow(q[s], t.expo[s] - 1);
+        for (int r2 = 0; r2 < M; r2++) if (r2 != s) w *= ipow(q[r2], t.expo[r2]);
+        du[s] += w;
+      }
+    }
+    eU[l] = exp(-wfac * desc->beta * u);
+    for (int s = 0; s < M; s++) dU[s][l] = du[s];
+  }
+  std::vector<double> ep;
+  size_t ep_off[3] = {0, 0, 0};
+  for (int s = 0; s < M; s++) {
+    ep_off[s] = ep.size();
+    for (int i = 0; i < op.n[M + s]; i++) {
+      double p = op.x0[M + s] + i * op.h[M + s];
+      ep.push_back(exp(-wfac * desc->beta * p * p / (2.0 * desc->mass[s])));
+    }
+  }
+  std::vector<int> up(3 * pl.K, -1), dn(3 * pl.K, -1), nv(3 * pl.K, 0);
+  std::vector<double> Gam(pl.K, 0.0);
+  auto find = [&](const int n[3]) {
+    for (int k = 0; k < pl.K; k++)
+      if (h->elem[3 * k] == n[0] && h->elem[3 * k + 1] == n[1] && h->elem[3 * k + 2] == n[2]) return k;
+    return -1;
+  };
+  for (int k = 0; k < pl.K; k++)
+    for (int s = 0; s < M; s++) {
+      int n[3] = {h->elem[3 * k], h->elem[3 * k + 1], h->elem[3 * k + 2]};
+      nv[3 * k + s] = n[s];
+      Gam[k] += n[s] * desc->gamma[s];
+      n[s] += 1; up[3 * k + s] = find(n);
+      n[s] -= 2; if (n[s] >= 0) dn[3 * k + s] = find(n);
+    }
+
+  // ---- carve and upload ----
+  char* base = (char*)ws;
+  char* tp = base + pl.off_tables;
+  auto put = [&](const void* src, size_t nbytes) -> void* {
+    void* dst = tp;
+    cudaMemcpyAsync(dst, src, nbytes, cudaMemcpyHostToDevice, h->stream);
+    tp += align256(nbytes);
+    return dst;
+  };
+  for (int s = 0; s < M; s++) op.dU[s] = (const double*)put(dU[s].data(), sizeof(double) * pl.nqc);
+  op.eU = (const double*)put(eU.data(), sizeof(double) * pl.nqc);
+  const double* epd = (const double*)put(ep.data(), sizeof(double) * ep.size());
+  for (int s = 0; s < M; s++) op.ep[s] = epd + ep_off[s];
+  op.up = (const int*)put(up.data(), sizeof(int) * up.size());
+  op.dn = (const int*)put(dn.data(), sizeof(int) * dn.size());
+  op.nvec = (const int*)put(nv.data(), sizeof(int) * nv.size());
+  op.Gamma = (const double*)put(Gam.data(), sizeof(double) * Gam.size());
+  h->partial = (double*)(base + pl.off_partial);
+  h->results = (double*)(base + pl.off_results);
+  h->arrays = (double*)(base + pl.off_arrays);
+  ce = cudaMemsetAsync(h->arrays, 0, sizeof(double) * (size_t)pl.n_arrays * h->state_doubles, h->stream);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(h->stream);       // host tables go out of scope below
+  if (ce != cudaSuccess) {
+    g_create_err = std::string("create: ") + cudaGetErrorString(ce);
+    delete h;
+    return CHFPE_ERR_CUDA;
+  }
+  *out = h;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_destroy(chfpe_handle* h) { delete h; return CHFPE_OK; }
+
+extern "C" const char* chfpe_last_error(const chfpe_handle* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+extern "C" int chfpe_num_elements(const chfpe_handle* h, int32_t* K) {
+  if (!h || !K) return CHFPE_ERR_INVALID;
+  *K = h->K; return CHFPE_OK;
+}
+
+extern "C" int chfpe_element_index(const chfpe_handle* h, int32_t k, int32_t n_out[3]) {
+  if (!h || !n_out || k < 0 || k >= h->K) return CHFPE_ERR_INVALID;
+  for (int s = 0; s < 3; s++) n_out[s] = h->elem[3 * k + s];
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_launch_count(const chfpe_handle* h, int64_t* n) {
+  if (!h || !n) return CHFPE_ERR_INVALID;
+  *n = h->launches; return CHFPE_OK;
+}
+
+static DevObs to_dev(const chfpe_observable* o) {
+  DevObs d;
+  memset(&d, 0, sizeof(d));
+  if (o) memcpy(&d, o, sizeof(d));
+  return d;
+}
+
+static int check_launch(chfpe_handle* h) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { h->err = std::string("kernel launch: ") + cudaGetErrorString(e); return CHFPE_ERR_CUDA; }
+  return CHFPE_OK;
+}
+
+// n RK4 steps (Horner form, R13) on slots [b0, b0+nb)
+static int step_slots(chfpe_handle* h, int b0, int nb, int64_t n_steps, double dt) {
+  if (nb <= 0 || n_steps <= 0) return CHFPE_OK;
+  const size_t ss = 3 * h->state_doubles;
+  double *y = h->y(b0), *va = h->va(b0), *vb = h->vb(b0);
+  for (int64_t i = 0; i < n_steps; i++) {
+    h->launches += launch_stage(h->op, y, y, va, 1.0, dt / 4.0, nb, ss, h->stream);
+    h->launches += launch_stage(h->op, va, y, vb, 1.0, dt / 3.0, nb, ss, h->stream);
+    h->launches += launch_stage(h->op, vb, y, va, 1.0, dt / 2.0, nb, ss, h->stream);
+    h->launches += launch_stage(h->op, va, y, y, 1.0, dt, nb, ss, h->stream);
+  }
+  return check_launch(h);
+}
+
+static int kick_slots(chfpe_handle* h, int b0, int nb, const chfpe_observable* X) {
+  const size_t ss = 3 * h->state_doubles;
+  DevObs o = to_dev(X);
+  h->launches += launch_kick(h->op, o, h->y(b0), h->va(b0), nb, ss, h->stream);
+  for (int b = b0; b < b0 + nb; b++)
+    CU(h, cudaMemcpyAsync(h->y(b), h->va(b), sizeof(double) * h->state_doubles, cudaMemcpyDeviceToDevice, h->stream));
+  return check_launch(h);
+}
+
+// <O> on element k of slots [b0, b0+nb) -> results[res_off + i*res_stride]
+static int expect_slots(chfpe_handle* h, int b0, int nb, int k, const chfpe_observable* O, long long res_off,
+                        long long res_stride) {
+  DevObs o = to_dev(O);
+  h->launches += launch_reduce(h->op, o, RED_EXPECT, h->y(b0), k, h->cells, nb, 3 * h->state_doubles, h->op.dV,
+                               h->partial, h->red_blocks, h->results + res_off, res_stride, h->stream);
+  return check_launch(h);
+}
+
+static int fetch_results(chfpe_handle* h, long long n, double* host) {
+  CU(h, cudaMemcpyAsync(host, h->results, sizeof(double) * n, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  for (long long i = 0; i < n; i++)
+    if (!std::isfinite(host[i])) FAIL(h, CHFPE_ERR_DIVERGED, "non-finite expectation value");
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_equilibrate(chfpe_handle* h, int64_t n_steps, double dt, double* residual_out) {
+  if (!h || n_steps < 0) return CHFPE_ERR_INVALID;
+  DevObs none = to_dev(nullptr);
+  h->launches += launch_init_eq(h->op, h->y(0), h->stream);
+  const int mode = (h->op.gauge == CHFPE_GAUGE_SQRT_EQ) ? RED_SUMSQ : RED_SUM;   // Z_f = dV sum phi^2, Z_W = dV sum e^{-beta H}
+  h->launches += launch_reduce(h->op, none, mode, h->y(0), 0, h->cells, 1, 0, h->op.dV, h->partial, h->red_blocks,
+                               h->results, 1, h->stream);
+  h->launches += launch_scale(h->y(0), h->cells, h->results, 1.0, h->stream);
+  for (int b = 1; b < h->batch; b++)
+    CU(h, cudaMemcpyAsync(h->y(b), h->y(0), sizeof(double) * h->state_doubles, cudaMemcpyDeviceToDevice, h->stream));
+  int rc = check_launch(h);
+  if (rc) return rc;
+  h->initialised = true;
+  rc = step_slots(h, 0, h->batch, n_steps, dt);
+  if (rc) return rc;
+  if (residual_out) {
+    h->launches += launch_stage(h->op, h->y(0), h->y(0), h->va(0), 0.0, 1.0, 1, 0, h->stream);
+    h->launches += launch_reduce(h->op, none, RED_SUMSQ, h->va(0), 0, (long long)h->state_doubles, 1, 0, 1.0,
+                                 h->partial, h->red_blocks, h->results, 1, h->stream);
+    h->launches += launch_reduce(h->op, none, RED_SUMSQ, h->y(0), 0, (long long)h->state_doubles, 1, 0, 1.0,
+                                 h->partial, h->red_blocks, h->results + 1, 1, h->stream);
+    rc = check_launch(h);
+    if (rc) return rc;
+    double r[2];
+    rc = fetch_results(h, 2, r);
+    if (rc) return rc;
+    *residual_out = sqrt(r[0] / r[1]);
+  }
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_step(chfpe_handle* h, int64_t n_steps, double dt) {
+  if (!h || n_steps < 0) return CHFPE_ERR_INVALID;
+  return step_slots(h, 0, h->batch, n_steps, dt);
+}
+
+extern "C" int chfpe_kick(chfpe_handle* h, const chfpe_observable* X) {
+  if (!h || !X) return CHFPE_ERR_INVALID;
+  return kick_slots(h, 0, h->batch, X);
+}
+
+extern "C" int chfpe_expect(chfpe_handle* h, const chfpe_observable* O, double* out) {
+  if (!h || !O || !out) return CHFPE_ERR_INVALID;
+  int rc = expect_slots(h, 0, h->batch, 0, O, 0, 1);
+  if (rc) return rc;
+  return fetch_results(h, h->batch, out);
+}
+
+extern "C" int chfpe_expect_element(chfpe_handle* h, int32_t replica, int32_t k, const chfpe_observable* O, double* out) {
+  if (!h || !O || !out || replica < 0 || replica >= h->batch || k < 0 || k >= h->K) return CHFPE_ERR_INVALID;
+  int rc = expect_slots(h, replica, 1, k, O, 0, 1);
+  if (rc) return rc;
+  return fetch_results(h, 1, out);
+}
+
+extern "C" int chfpe_response_1d(chfpe_handle* h, const chfpe_observable* A, const chfpe_observable* C,
+                                 int64_t n_samples, int64_t stride, double dt, double* R) {
+  if (!h || !A || !C || !R || n_samples < 0 || stride < 0) return CHFPE_ERR_INVALID;
+  if (!h->initialised) FAIL(h, CHFPE_ERR_STATE, "response_1d before equilibrate/import");
+  int rc = kick_slots(h, 0, 1, A);
+  if (rc) return rc;
+  int64_t done = 0;
+  while (done < n_samples) {                         // results buffer holds Plan::RESULTS samples per round trip
+    int64_t chunk = n_samples - done;
+    if (chunk > Plan::RESULTS) chunk = Plan::RESULTS;
+    for (int64_t i = 0; i < chunk; i++) {
+      rc = expect_slots(h, 0, 1, 0, C, i, 1);
+      if (rc) return rc;
+      if (done + i + 1 < n_samples) { rc = step_slots(h, 0, 1, stride, dt); if (rc) return rc; }
+    }
+    rc = fetch_results(h, chunk, R + done);
+    if (rc) return rc;
+    done += chunk;
+  }
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_response_2d(chfpe_handle* h, const chfpe_observable* A, const chfpe_observable* B,
+                                 const chfpe_observable* C, const int64_t* t1, int32_t n1, const int64_t* t2,
+                                 int32_t n2, double dt, double* R) {
+  if (!h || !A || !B || !C || !t1 || !t2 || !R || n1 < 1 || n2 < 1) return CHFPE_ERR_INVALID;
+  if (!h->initialised) FAIL(h, CHFPE_ERR_STATE, "response_2d before equilibrate/import");
+  for (int i = 0; i < n1; i++) if (t1[i] < 0 || (i && t1[i] < t1[i - 1])) FAIL(h, CHFPE_ERR_INVALID, "t1_steps must be ascending and >= 0");
+  for (int i = 0; i < n2; i++) if (t2[i] < 0 || (i && t2[i] < t2[i - 1])) FAIL(h, CHFPE_ERR_INVALID, "t2_steps must be ascending and >= 0");
+  const size_t sbytes = sizeof(double) * h->state_doubles;
+  int rc = kick_slots(h, 0, 1, A);                   // T <- A^x X, slot 0 carries the t1 trajectory
+  if (rc) return rc;
+  int64_t now1 = 0;
+  const int per_round = (h->batch >= 2) ? h->batch - 1 : 1;
+  const long long rows_per_fetch = Plan::RESULTS / n2;
+  if (rows_per_fetch < 1) FAIL(h, CHFPE_ERR_INVALID, "n2 too large for the results buffer");
+  int k = 0, row0 = 0;                               // rows [row0, k) are in the device results buffer
+  while (k < n1) {
+    int nb = n1 - k; if (nb > per_round) nb = per_round;
+    if (k + nb - row0 > rows_per_fetch) {            // flush before the buffer overflows
+      rc = fetch_results(h, (long long)(k - row0) * n2, R + (size_t)row0 * n2); if (rc) return rc;
+      row0 = k;
+    }
+    int first;                                       // first slot of the replica group
+    if (h->batch >= 2) {
+      first = 1;
+      for (int b = 0; b < nb; b++) {
+        rc = step_slots(h, 0, 1, t1[k + b] - now1, dt); if (rc) return rc;
+        now1 = t1[k + b];
+        CU(h, cudaMemcpyAsync(h->y(1 + b), h->y(0), sbytes, cudaMemcpyDeviceToDevice, h->stream));
+      }
+    } else {
+      first = 0;
+      rc = step_slots(h, 0, 1, t1[k] - now1, dt); if (rc) return rc;
+      now1 = t1[k];
+      CU(h, cudaMemcpyAsync(h->spare(), h->y(0), sbytes, cudaMemcpyDeviceToDevice, h->stream));
+    }
+    rc = kick_slots(h, first, nb, B); if (rc) return rc;
+    int64_t now2 = 0;
+    for (int j = 0; j < n2; j++) {
+      rc = step_slots(h, first, nb, t2[j] - now2, dt); if (rc) return rc;
+      now2 = t2[j];
+      rc = expect_slots(h, first, nb, 0, C, (long long)(k - row0) * n2 + j, n2); if (rc) return rc;
+    }
+    if (h->batch < 2) CU(h, cudaMemcpyAsync(h->y(0), h->spare(), sbytes, cudaMemcpyDeviceToDevice, h->stream));
+    k += nb;
+  }
+  return fetch_results(h, (long long)(k - row0) * n2, R + (size_t)row0 * n2);
+}
+
+extern "C" int chfpe_export_state(chfpe_handle* h, int32_t replica, double* dst, int dst_is_device) {
+  if (!h || !dst || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
+  if (dst_is_device) {
+    h->launches += launch_permute(h->op, h->y(replica), dst, 0, h->stream);
+    return check_launch(h);
+  }
+  h->launches += launch_permute(h->op, h->y(replica), h->va(replica), 0, h->stream);
+  int rc = check_launch(h); if (rc) return rc;
+  CU(h, cudaMemcpyAsync(dst, h->va(replica), sizeof(double) * h->state_doubles, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_import_state(chfpe_handle* h, int32_t replica, const double* src, int src_is_device) {
+  if (!h || !src || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
+  if (src_is_device) {
+    h->launches += launch_permute(h->op, src, h->y(replica), 1, h->stream);
+  } else {
+    CU(h, cudaMemcpyAsync(h->va(replica), src, sizeof(double) * h->state_doubles, cudaMemcpyHostToDevice, h->stream));
+    h->launches += launch_permute(h->op, h->va(replica), h->y(replica), 1, h->stream);
+    CU(h, cudaStreamSynchronize(h->stream));          // the caller may free src on return
+  }
+  h->initialised = true;
+  return check_launch(h);
+}
+
+extern "C" int chfpe_export_rhs(chfpe_handle* h, int32_t replica, double* dst, int dst_is_device) {
+  if (!h || !dst || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
+  h->launches += launch_stage(h->op, h->y(replica), h->y(replica), h->va(replica), 0.0, 1.0, 1, 0, h->stream);
+  if (dst_is_device) {
+    h->launches += launch_permute(h->op, h->va(replica), dst, 0, h->stream);
+    return check_launch(h);
+  }
+  h->launches += launch_permute(h->op, h->va(replica), h->vb(replica), 0, h->stream);
+  int rc = check_launch(h); if (rc) return rc;
+  CU(h, cudaMemcpyAsync(dst, h->vb(replica), sizeof(double) * h->state_doubles, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  return CHFPE_OK;
+}

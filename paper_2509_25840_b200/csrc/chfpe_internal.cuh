@@ -1,0 +1,78 @@
+// Internal declarations shared by the host API (chfpe_api.cu) and the kernels (chfpe_kernels.cu).
+// Not part of the C-ABI; nothing here is used by the oracle.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include "../../include/chfpe.h"
+
+#define CHFPE_MAXAX 6
+
+// Device-side view of the operator: passed BY VALUE to every kernel (< 1 KB of kernel parameter space).
+// Internal axis order ("q-major / p-minor bricks"): a = 0..M-1 are q_1..q_M, a = M..2M-1 are p_1..p_M,
+// last axis fastest, so all momenta of one q-point form one contiguous "p-brick" of pb cells.
+struct DevOp {
+  int M, nax, K, scheme, gauge;
+  int n[CHFPE_MAXAX];                 // points per internal axis
+  long long st[CHFPE_MAXAX];          // internal strides (doubles)
+  long long cells, nqc, pb;           // cells per element, q-points, p-brick size
+  double x0[CHFPE_MAXAX], h[CHFPE_MAXAX];
+  double c1[CHFPE_MAXAX], c2[CHFPE_MAXAX];   // pre-multiplied stencil coefficients (+-1, +-2 neighbours)
+  double inv_mass[3], kup[3], kdn[3], cdn[3], VLL[3], VSL[3], beta;
+  double dV;
+  const double* dU[3];                // dU/dq_s on the q-subgrid, q_1 slowest   (device)
+  const double* eU;                   // exp(-beta U/2) (sqrt gauge) or exp(-beta U) (W gauge) on the q-subgrid
+  const double* ep[3];                // exp(-beta p^2/(4m)) resp. exp(-beta p^2/(2m)) per p-axis
+  const int* up;                      // [K][3] element index of n + e_s or -1
+  const int* dn;                      // [K][3] element index of n - e_s or -1
+  const int* nvec;                    // [K][3]
+  const double* Gamma;                // [K] sum_s n_s gamma_s
+};
+
+struct DevObs {                       // observable polynomial, Eq. (13)-(14)
+  double c0, lin_q[3], quad[3][3], lin_p[3];
+};
+
+enum ReduceMode { RED_EXPECT = 0, RED_SUMSQ = 1, RED_SUM = 2 };
+
+struct chfpe_handle {
+  chfpe_desc desc;
+  std::vector<chfpe_monomial> U;
+  DevOp op;
+  cudaStream_t stream;
+  int K, batch, n_arrays;
+  long long cells;
+  size_t state_doubles;               // K * cells
+  double* arrays;                     // n_arrays * state_doubles, carved from the workspace
+  // slot b uses arrays[3b] (state y), arrays[3b+1], arrays[3b+2] (stage buffers); optional spare array last
+  double* partial;                    // reduction scratch
+  double* results;                    // batch doubles (device)
+  int red_blocks;
+  std::vector<int> elem;              // host copy [K][3]
+  bool initialised;
+  int64_t launches;
+  std::string err;
+  double* y(int b) const { return arrays + (size_t)(3 * b) * state_doubles; }
+  double* va(int b) const { return arrays + (size_t)(3 * b + 1) * state_doubles; }
+  double* vb(int b) const { return arrays + (size_t)(3 * b + 2) * state_doubles; }
+  double* spare() const { return arrays + (size_t)(3 * batch) * state_doubles; }
+};
+
+// ---- launchers implemented in chfpe_kernels.cu (all asynchronous on `s`; return the launch count) ----
+// out = a*y + c*F(in) for slots [b0, b0+nb); slot stride = 3*state_doubles for all three pointers.
+int launch_stage(const DevOp& op, const double* in, const double* y, double* out, double a, double c,
+                 int nb, size_t slot_stride, cudaStream_t s);
+// out = Kick_obs(in) on every element, slots [b0, b0+nb)
+int launch_kick(const DevOp& op, const DevObs& o, const double* in, double* out, int nb, size_t slot_stride,
+                cudaStream_t s);
+// results[b*res_stride] = scale * sum over ncells cells starting at element k of slot b of the integrand;
+// deterministic two-pass reduction (fixed block partition, fixed-order final pass)
+int launch_reduce(const DevOp& op, const DevObs& o, int mode, const double* x, int k, long long ncells,
+                  int nb, size_t slot_stride, double scale, double* partial, int red_blocks, double* results,
+                  long long res_stride, cudaStream_t s);
+// element 0 <- unnormalised equilibrium profile, other elements <- 0 (one slot)
+int launch_init_eq(const DevOp& op, double* x, cudaStream_t s);
+int launch_scale(double* x, long long n, const double* denom_dev, double mult, cudaStream_t s);
+// layout conversion between canonical (q1,p1,...,qM,pM) and internal (q..., p...) for all K elements
+int launch_permute(const DevOp& op, const double* src, double* dst, int to_internal, cudaStream_t s);

@@ -1,0 +1,272 @@
+// sm_100a kernels of the CHFPE hot path: RK stage (Liouvillian stencil + hierarchy couplings + stage combine),
+// kick, expectation reduction, equilibrium initialisation, layout conversion.
+// Equations: PAPER.md Eq. (8)-(12) :77-100, (15)-(18) :119-131; readings R1, R3, R7, R9-R13 of DESIGN.md.
+#include "chfpe_internal.cuh"
+
+namespace {
+
+template <int NAX>
+__device__ __forceinline__ void decode(const DevOp& op, long long cell, int (&idx)[NAX]) {
+#pragma unroll
+  for (int a = NAX - 1; a >= 0; a--) {
+    long long q = cell / op.n[a];
+    idx[a] = (int)(cell - q * op.n[a]);
+    cell = q;
+  }
+}
+
+// explicit antisymmetric stencil with zero ghosts (R9): c1 (f[+1]-f[-1]) + c2 (f[+2]-f[-2])
+__device__ __forceinline__ double dstencil(const double* __restrict__ f, long long cell, long long st, int i, int n,
+                                           double c1, double c2, bool wide) {
+  double fp1 = (i + 1 < n) ? __ldg(f + cell + st) : 0.0;
+  double fm1 = (i >= 1) ? __ldg(f + cell - st) : 0.0;
+  double d = c1 * (fp1 - fm1);
+  if (wide) {
+    double fp2 = (i + 2 < n) ? __ldg(f + cell + 2 * st) : 0.0;
+    double fm2 = (i >= 2) ? __ldg(f + cell - 2 * st) : 0.0;
+    d = fma(c2, fp2 - fm2, d);
+  }
+  return d;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Generic RK stage: out = a*y + c*F(in), one thread per (cell, element, slot).  Correct for every M, grid
+// and explicit scheme; the brick kernels below replace it where they apply.
+// ------------------------------------------------------------------------------------------------
+template <int M>
+__global__ void __launch_bounds__(256) k_stage_generic(DevOp op, const double* __restrict__ in,
+                                                       const double* y, double* out,
+                                                       double a, double c, size_t slot_stride) {
+  long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (cell >= op.cells) return;
+  const int k = blockIdx.y;
+  const size_t boff = (size_t)blockIdx.z * slot_stride;
+  const double* X = in + boff;
+  const double* Xk = X + (size_t)k * op.cells;
+  int idx[2 * M];
+  decode<2 * M>(op, cell, idx);
+  const long long ql = cell / op.pb;
+  const bool wide = (op.scheme == CHFPE_CENTRAL4);
+  double acc = -__ldg(op.Gamma + k) * __ldg(Xk + cell);
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const int aq = s, ap = M + s;
+    const double q = op.x0[aq] + idx[aq] * op.h[aq];
+    const double p = op.x0[ap] + idx[ap] * op.h[ap];
+    const double dq = dstencil(Xk, cell, op.st[aq], idx[aq], op.n[aq], op.c1[aq], op.c2[aq], wide);
+    const double dp = dstencil(Xk, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
+    acc = fma(-(p * op.inv_mass[s]), dq, acc);                      // -(p_s/m_s) dW/dq_s
+    acc = fma(__ldg(op.dU[s] + ql), dp, acc);                       // +(dU/dq_s) dW/dp_s
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+    if (ku >= 0) {                                                  // Phi_s W^(n+e_s)
+      const double* Xu = X + (size_t)ku * op.cells;
+      double d = dstencil(Xu, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
+      acc = fma(Vp, fma(op.kup[s] * p, __ldg(Xu + cell), d), acc);
+    }
+    if (kd >= 0) {                                                  // n_s Theta_s W^(n-e_s)
+      const double* Xd = X + (size_t)kd * op.cells;
+      double d = dstencil(Xd, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
+      acc = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp, fma(op.kdn[s] * p, __ldg(Xd + cell), d), acc);
+    }
+  }
+  const size_t o = boff + (size_t)k * op.cells + cell;
+  out[o] = fma(c, acc, a * y[o]);
+}
+
+// Kick, Eq. (18): out_k = sum_s dX/dq_s (D_{p_s} + kup_s p_s) in_k
+template <int M>
+__global__ void __launch_bounds__(256) k_kick_generic(DevOp op, DevObs ob, const double* __restrict__ in,
+                                                      double* __restrict__ out, size_t slot_stride) {
+  long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (cell >= op.cells) return;
+  const int k = blockIdx.y;
+  const size_t boff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells;
+  const double* Xk = in + boff;
+  int idx[2 * M];
+  decode<2 * M>(op, cell, idx);
+  const bool wide = (op.scheme == CHFPE_CENTRAL4);
+  double q[M];
+#pragma unroll
+  for (int s = 0; s < M; s++) q[s] = op.x0[s] + idx[s] * op.h[s];
+  const double xc = __ldg(Xk + cell);
+  double acc = 0.0;
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const int ap = M + s;
+    const double p = op.x0[ap] + idx[ap] * op.h[ap];
+    double g = ob.lin_q[s];
+#pragma unroll
+    for (int r = 0; r < M; r++) g = fma(0.5 * (ob.quad[s][r] + ob.quad[r][s]), q[r], g);
+    double d = dstencil(Xk, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
+    acc = fma(g, fma(op.kup[s] * p, xc, d), acc);
+  }
+  out[boff + cell] = acc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Deterministic reductions: per-block partials (warp shuffle -> shared) then a fixed-order final pass.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double block_sum_256(double v) {
+  __shared__ double sm[8];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (threadIdx.x < 32) {
+    r = (threadIdx.x < 8) ? sm[threadIdx.x] : 0.0;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
+  }
+  __syncthreads();
+  return r;   // valid in thread 0
+}
+
+template <int M>
+__global__ void __launch_bounds__(256) k_reduce_partial(DevOp op, DevObs ob, int mode, const double* __restrict__ x,
+                                                        long long elem_off, long long ncells, size_t slot_stride,
+                                                        double* __restrict__ partial) {
+  const double* X = x + (size_t)blockIdx.y * slot_stride + elem_off;
+  // contiguous chunk per block so that the summation order is fixed by (ncells, gridDim.x) alone
+  const long long per = (ncells + gridDim.x - 1) / gridDim.x;
+  const long long lo = (long long)blockIdx.x * per;
+  long long hi = lo + per; if (hi > ncells) hi = ncells;
+  double acc = 0.0;
+  for (long long c = lo + threadIdx.x; c < hi; c += 256) {
+    const double v = X[c];
+    if (mode == RED_SUMSQ) { acc = fma(v, v, acc); continue; }
+    if (mode == RED_SUM) { acc += v; continue; }
+    int idx[2 * M];
+    decode<2 * M>(op, c % op.cells, idx);
+    double O = ob.c0, w = 1.0;
+    double q[M];
+#pragma unroll
+    for (int s = 0; s < M; s++) q[s] = op.x0[s] + idx[s] * op.h[s];
+#pragma unroll
+    for (int s = 0; s < M; s++) {
+      const double p = op.x0[M + s] + idx[M + s] * op.h[M + s];
+      O = fma(ob.lin_q[s], q[s], O);
+      O = fma(ob.lin_p[s], p, O);
+#pragma unroll
+      for (int r = 0; r < M; r++) O = fma(0.5 * ob.quad[s][r] * q[s], q[r], O);
+      if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.ep[s] + idx[M + s]);
+    }
+    if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.eU + (c % op.cells) / op.pb);
+    acc = fma(O * w, v, acc);
+  }
+  const double r = block_sum_256(acc);
+  if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = r;
+}
+
+__global__ void __launch_bounds__(256) k_reduce_final(const double* __restrict__ partial, int nblocks, double scale,
+                                                      double* __restrict__ results, long long res_stride) {
+  const double* P = partial + (size_t)blockIdx.x * nblocks;
+  double acc = 0.0;
+  for (int i = threadIdx.x; i < nblocks; i += 256) acc += P[i];
+  const double r = block_sum_256(acc);
+  if (threadIdx.x == 0) results[(long long)blockIdx.x * res_stride] = r * scale;
+}
+
+// element 0 <- exp factor tables product (phi or e^{-beta H}), others <- 0
+template <int M>
+__global__ void __launch_bounds__(256) k_init_eq(DevOp op, double* __restrict__ x) {
+  long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (cell >= op.cells) return;
+  const int k = blockIdx.y;
+  double v = 0.0;
+  if (k == 0) {
+    int idx[2 * M];
+    decode<2 * M>(op, cell, idx);
+    v = __ldg(op.eU + cell / op.pb);
+#pragma unroll
+    for (int s = 0; s < M; s++) v *= __ldg(op.ep[s] + idx[M + s]);
+  }
+  x[(size_t)k * op.cells + cell] = v;
+}
+
+__global__ void __launch_bounds__(256) k_scale(double* __restrict__ x, long long n, const double* __restrict__ denom,
+                                               double mult) {
+  const double f = mult / denom[0];
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < n; i += (long long)gridDim.x * 256) x[i] *= f;
+}
+
+template <int M>
+__global__ void __launch_bounds__(256) k_permute(DevOp op, const double* __restrict__ src, double* __restrict__ dst,
+                                                 int to_internal) {
+  long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (cell >= op.cells) return;
+  int idx[2 * M];
+  decode<2 * M>(op, cell, idx);
+  long long canon = 0;                       // canonical order q1,p1,...,qM,pM, last fastest
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    canon = canon * op.n[s] + idx[s];
+    canon = canon * op.n[M + s] + idx[M + s];
+  }
+  const size_t e = (size_t)blockIdx.y * op.cells;
+  if (to_internal) dst[e + cell] = src[e + canon];
+  else dst[e + canon] = src[e + cell];
+}
+
+}  // namespace
+
+#define DISPATCH_M(M, CALL)            \
+  do {                                 \
+    if ((M) == 1) { CALL(1); }         \
+    else if ((M) == 2) { CALL(2); }    \
+    else { CALL(3); }                  \
+  } while (0)
+
+int launch_stage(const DevOp& op, const double* in, const double* y, double* out, double a, double c, int nb,
+                 size_t slot_stride, cudaStream_t s) {
+  dim3 grid((unsigned)((op.cells + 255) / 256), op.K, nb);
+#define CALL(MM) k_stage_generic<MM><<<grid, 256, 0, s>>>(op, in, y, out, a, c, slot_stride)
+  DISPATCH_M(op.M, CALL);
+#undef CALL
+  return 1;
+}
+
+int launch_kick(const DevOp& op, const DevObs& o, const double* in, double* out, int nb, size_t slot_stride,
+                cudaStream_t s) {
+  dim3 grid((unsigned)((op.cells + 255) / 256), op.K, nb);
+#define CALL(MM) k_kick_generic<MM><<<grid, 256, 0, s>>>(op, o, in, out, slot_stride)
+  DISPATCH_M(op.M, CALL);
+#undef CALL
+  return 1;
+}
+
+int launch_reduce(const DevOp& op, const DevObs& o, int mode, const double* x, int k, long long ncells, int nb,
+                  size_t slot_stride, double scale, double* partial, int red_blocks, double* results,
+                  long long res_stride, cudaStream_t s) {
+  dim3 grid(red_blocks, nb);
+  const long long off = (long long)k * op.cells;
+#define CALL(MM) k_reduce_partial<MM><<<grid, 256, 0, s>>>(op, o, mode, x, off, ncells, slot_stride, partial)
+  DISPATCH_M(op.M, CALL);
+#undef CALL
+  k_reduce_final<<<nb, 256, 0, s>>>(partial, red_blocks, scale, results, res_stride);
+  return 2;
+}
+
+int launch_init_eq(const DevOp& op, double* x, cudaStream_t s) {
+  dim3 grid((unsigned)((op.cells + 255) / 256), op.K);
+#define CALL(MM) k_init_eq<MM><<<grid, 256, 0, s>>>(op, x)
+  DISPATCH_M(op.M, CALL);
+#undef CALL
+  return 1;
+}
+
+int launch_scale(double* x, long long n, const double* denom_dev, double mult, cudaStream_t s) {
+  long long blocks = (n + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  k_scale<<<(unsigned)blocks, 256, 0, s>>>(x, n, denom_dev, mult);
+  return 1;
+}
+
+int launch_permute(const DevOp& op, const double* src, double* dst, int to_internal, cudaStream_t s) {
+  dim3 grid((unsigned)((op.cells + 255) / 256), op.K);
+#define CALL(MM) k_permute<MM><<<grid, 256, 0, s>>>(op, src, dst, to_internal)
+  DISPATCH_M(op.M, CALL);
+#undef CALL
+  return 1;
+}

@@ -1,0 +1,68 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol that
+include/chfpe.h declares; descriptor validation and workspace sizing run on the CPU."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import chfpe_inputs as ci
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def header_functions():
+    text = open(os.path.join(ROOT, "include", "chfpe.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(chfpe_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol():
+    import paper_2509_25840_b200 as P
+    L = P.lib()
+    names = header_functions()
+    assert len(names) >= 15
+    for n in names:
+        assert hasattr(L, n), "libchfpe.so does not export %s" % n
+    assert sorted(P.EXPORTED_SYMBOLS) == names
+
+
+def test_oracle_and_product_share_no_code():
+    """The oracle never imports the product and vice versa; the product never touches oracle/."""
+    for sub, banned in (("oracle", "paper_2509_25840_b200"), ("paper_2509_25840_b200", "oracle")):
+        for dirpath, _, files in os.walk(os.path.join(ROOT, sub)):
+            for f in files:
+                if f.endswith((".py", ".c", ".h", ".cu", ".cuh")):
+                    src = open(os.path.join(dirpath, f)).read()
+                    assert ("import " + banned) not in src and ("from " + banned) not in src
+                    if sub == "paper_2509_25840_b200":
+                        assert "chfpe_ref" not in src
+
+
+def test_workspace_bytes_and_validation():
+    import paper_2509_25840_b200 as P
+    for name, arrays in (("cfg1", 4), ("cfg4", 4)):
+        cfg = ci.config(name)
+        K = {"cfg1": 9, "cfg4": 20}[name]
+        cells = 1
+        for s in range(cfg["n_modes"]):
+            cells *= cfg["nq"][s] * cfg["np"][s]
+        nbytes = P.workspace_bytes(cfg, batch=1)
+        assert arrays * K * cells * 8 <= nbytes <= arrays * K * cells * 8 + (8 << 20)
+    n5 = P.workspace_bytes(ci.config("cfg5"), batch=5)
+    assert n5 < 180e9                       # config 5 with 5 slots (trajectory + 4 replicas) fits one B200
+    for bad in (dict(nq=[4]), dict(depth=-1), dict(beta=0.0), dict(gamma=[0.0]), dict(U=[(1.0, (5,))]),
+                dict(scheme="compact6")):
+        with pytest.raises(P.ChfpeError):
+            P.workspace_bytes(ci.config("cfg1", **bad))
+    with pytest.raises(P.ChfpeError):
+        P.workspace_bytes(ci.config("cfg1"), batch=0)
+
+
+def test_create_rejects_bad_workspace_without_touching_the_gpu():
+    import paper_2509_25840_b200 as P
+    from paper_2509_25840_b200 import binding
+    d, keep = binding.make_desc(ci.config("cfg1"))
+    h = C.c_void_p()
+    rc = P.lib().chfpe_create(C.byref(d), None, 0, None, C.byref(h))
+    assert rc == -2 and not h.value          # CHFPE_ERR_WORKSPACE

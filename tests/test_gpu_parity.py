@@ -1,0 +1,235 @@
+"""Parity of the CUDA path (through the C-ABI binding) with the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): per-step relative L2 <= 1e-12; response functions relative max
+error <= 1e-8.  Operator-level checks use 1e-13.  All tests need a GPU (`-m gpu`).
+"""
+import numpy as np
+import pytest
+
+import chfpe_inputs as ci
+import oracle
+from conftest import make_obs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def gpu_mod():
+    import paper_2509_25840_b200 as P
+    return P
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def both(cfg, batch=1):
+    P = gpu_mod()
+    return P.CHFPE(cfg, batch=batch), oracle.RefCHFPE(cfg)
+
+
+def obs_pair(kind, M):
+    d = ci.observable(kind, M)
+    return make_obs(gpu_mod(), d), make_obs(oracle, d)
+
+
+SMALL = [
+    ("m1_sqrt", ci.config("cfg2", nq=[37], np=[41], depth=5)),
+    ("m1_w_c2", ci.config("cfg2", nq=[33], np=[29], depth=3, gauge="w", scheme="central2")),
+    ("m2_sqrt", ci.config("cfg3s", nq=[13, 11], np=[12, 14], depth=3)),
+    ("m2_w", ci.config("cfg3s", nq=[9, 10], np=[11, 8], depth=2, gauge="w", mass=[1.0, 1.3])),
+    ("m3_sqrt", ci.config("cfg4s8", nq=[7, 8, 6], np=[8, 6, 9], depth=3)),
+    ("m3_w_c2", ci.config("cfg4s8", nq=[6, 5, 7], np=[5, 7, 6], depth=2, gauge="w", scheme="central2",
+                          mass=[1.0, 0.8, 1.2])),
+    ("m3_cube8", ci.config("cfg4s8")),
+]
+
+
+@pytest.mark.parametrize("name,cfg", SMALL, ids=[c[0] for c in SMALL])
+def test_operator_step_kick_expect(name, cfg):
+    g, o = both(cfg)
+    M = cfg["n_modes"]
+    assert g.elements() == o.elements() and g.K == o.K
+    levels = [sum(n) for n in o.elements()]
+    X = ci.seeded_state(cfg, levels, seed=1)
+    g.import_state(X); o.import_state(X)
+    assert np.array_equal(g.export_state(), X)                         # canonical round trip is exact
+    # right-hand side of Eq. (8)
+    Fg, Fo = g.export_rhs(), o.rhs(X)
+    assert rel_l2(Fg, Fo) < 1e-13
+    for k in range(o.K):
+        assert np.linalg.norm(Fg[k] - Fo[k]) <= 1e-13 * np.linalg.norm(Fo)
+    # expectation of a general observable (element 0 and a higher element)
+    gen = dict(c0=0.3, lin_q=[0.7, -0.4, 0.2][:M], quad=[[0.5, 0.2, -0.1][:M], [0.1, -0.3, 0.25][:M], [0.05, 0.15, 0.4][:M]][:M],
+               lin_p=[0.3, -0.2, 0.1][:M])
+    og, oo = make_obs(gpu_mod(), gen), make_obs(oracle, gen)
+    eg, eo = g.expect(og)[0], o.expect(oo)
+    assert abs(eg - eo) <= 1e-12 * max(1.0, abs(eo))
+    assert abs(g.expect_element(og, o.K - 1) - o.expect(oo, element=o.K - 1)) <= 1e-12 * max(1.0, abs(eo))
+    # one step and ten steps
+    g.step(1, cfg["dt"]); o.step(1, cfg["dt"])
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+    g.step(9, cfg["dt"]); o.step(9, cfg["dt"])
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+    # kick (Eq. 18) with a general observable
+    g.import_state(X); o.import_state(X)
+    g.kick(og); o.kick(oo)
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-13
+    g.close()
+
+
+@pytest.mark.parametrize("name,cfg", SMALL[:5], ids=[c[0] for c in SMALL[:5]])
+def test_equilibrate(name, cfg):
+    g, o = both(cfg)
+    rg = g.equilibrate(3, cfg["dt"])
+    ro = o.equilibrate(3, cfg["dt"])
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+    assert abs(rg - ro) <= 1e-9 * ro
+    one_g, one_o = obs_pair("one", cfg["n_modes"])
+    assert abs(g.expect(one_g)[0] - o.expect(one_o)) < 1e-12
+    g.close()
+
+
+def test_response_1d_config1_full():
+    """BASELINE config 1 at full size: 2000 steps, <q> every step; also against the closed form."""
+    cfg = ci.config("cfg1")
+    g, o = both(cfg)
+    mu_g, mu_o = obs_pair("mu", 1)
+    g.equilibrate(); o.equilibrate()
+    Rg = g.response_1d(mu_g, mu_g, 2001, 1, cfg["dt"])
+    Ro = o.response_1d(mu_o, mu_o, 2001, 1, cfg["dt"])
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    r = np.roots([1.0, 1.0, 1.5, 1.0])
+    dp = 3 * r * r + 2 * r + 1.5
+    t = np.arange(2001) * cfg["dt"]
+    bo = np.real(sum((ri + 1.0) / di * np.exp(ri * t) for ri, di in zip(r, dp)))
+    assert np.max(np.abs(-Rg - bo)) < 6e-5            # h^4 error of the sqrt(W_eq) gauge on 64 x 64 (pin P1)
+    g.close()
+
+
+def test_response_1d_config2_full():
+    """BASELINE config 2 at full size: 10^4 steps of dt = 5e-4, mu = q + 0.1 q^2, sampled every 10 steps."""
+    cfg = ci.config("cfg2")
+    g, o = both(cfg)
+    mu_g, mu_o = obs_pair("mu_nl", 1)
+    g.equilibrate(); o.equilibrate()
+    Rg = g.response_1d(mu_g, mu_g, 1001, 10, cfg["dt"])
+    Ro = o.response_1d(mu_o, mu_o, 1001, 10, cfg["dt"])
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    g.close()
+
+
+@pytest.mark.parametrize("name,cfg,nsteps", [("cfg3s", ci.config("cfg3s"), 200),
+                                             ("cfg4s8", ci.config("cfg4s8"), 100)])
+def test_response_1d_shrunken_multimode(name, cfg, nsteps):
+    g, o = both(cfg)
+    M = cfg["n_modes"]
+    for kind in ("mu", "alpha"):
+        a_g, a_o = obs_pair(kind, M)
+        g.equilibrate(); o.equilibrate()
+        Rg = g.response_1d(a_g, a_g, nsteps // 10 + 1, 10, cfg["dt"])
+        Ro = o.response_1d(a_o, a_o, nsteps // 10 + 1, 10, cfg["dt"])
+        assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    g.close()
+
+
+@pytest.mark.parametrize("batch", [1, 2, 4])
+def test_response_2d_batched(batch):
+    """R2 (Eq. 16) with t1 replicas propagated together; batched == unbatched == oracle."""
+    cfg = ci.config("cfg4s8", nq=[6, 6, 6], np=[6, 6, 6])
+    g, o = both(cfg, batch=batch)
+    mu_g, mu_o = obs_pair("mu", 3)
+    al_g, al_o = obs_pair("alpha", 3)
+    t1 = [0, 2, 3, 7, 8]; t2 = [0, 1, 4, 6]
+    g.equilibrate(); o.equilibrate()
+    Rg = g.response_2d(mu_g, al_g, al_g, t1, t2, cfg["dt"] * 10)
+    Ro = o.response_2d(mu_o, al_o, al_o, t1, t2, cfg["dt"] * 10)
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    if batch > 1:
+        g1 = gpu_mod().CHFPE(cfg, batch=1)
+        g1.equilibrate()
+        R1 = g1.response_2d(mu_g, al_g, al_g, t1, t2, cfg["dt"] * 10)
+        assert np.max(np.abs(Rg - R1)) <= 1e-14 * np.max(np.abs(R1))
+        g1.close()
+    g.close()
+
+
+def test_batched_step_equals_single():
+    cfg = ci.config("cfg3s", nq=[10, 9], np=[9, 10], depth=2)
+    P = gpu_mod()
+    g = P.CHFPE(cfg, batch=3)
+    o = oracle.RefCHFPE(cfg)
+    levels = [sum(n) for n in o.elements()]
+    Xs = [ci.seeded_state(cfg, levels, seed=s) for s in range(3)]
+    for b in range(3):
+        g.import_state(Xs[b], replica=b)
+    g.step(4, cfg["dt"])
+    mu_g, mu_o = obs_pair("mu", 2)
+    e = g.expect(mu_g)
+    for b in range(3):
+        o.import_state(Xs[b]); o.step(4, cfg["dt"])
+        assert rel_l2(g.export_state(b), o.export_state()) < 1e-12
+        assert abs(e[b] - o.expect(mu_o)) <= 1e-12 * max(1.0, abs(o.expect(mu_o)))
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_sampled_rhs_and_step_properties(name):
+    """BASELINE configs 3 and 4 at full size, in the launch configuration bench.py times: sampled entries of the
+    right-hand side against the oracle's point formula, plus size-independent properties of a step."""
+    cfg = ci.config(name)
+    P = gpu_mod()
+    g = P.CHFPE(cfg, batch=1)
+    o = oracle.RefCHFPE(cfg)
+    levels = [sum(n) for n in o.elements()]
+    X = ci.seeded_state(cfg, levels, seed=0)
+    g.import_state(X)
+    F = g.export_rhs()
+    rng = np.random.default_rng(5)
+    Ff = F.reshape(o.K, -1)
+    scale = float(np.sqrt(np.mean(Ff[:, ::997] ** 2)))
+    shape = o.shape
+    samples = [(int(rng.integers(o.K)), int(rng.integers(o.cells))) for _ in range(3000)]
+    # add corners / edges of the grid (zero-ghost boundary handling)
+    for k in (0, o.K - 1):
+        for cell in (0, o.cells - 1, shape[-1] - 1, o.cells - shape[-1], o.cells // 2):
+            samples.append((k, cell))
+    worst = 0.0
+    for k, cell in samples:
+        worst = max(worst, abs(Ff[k, cell] - o.rhs_at(X, k, cell)))
+    assert worst <= 1e-12 * scale
+    # properties of one full-size step: the scaled norm must not grow (sqrt gauge, pin P6) and <1> drifts by O(dt h^4)
+    one_g, _ = obs_pair("one", cfg["n_modes"])
+    n0 = g.expect(one_g)[0]
+    g.step(2, cfg["dt"])
+    Y = g.export_state()
+    w = []
+    for n in o.elements():
+        f = 1.0
+        for s, ns in enumerate(n):
+            for j in range(1, ns + 1):
+                f *= j * cfg["zeta"][s] * cfg["gamma"][s] * cfg["mass"][s] / cfg["beta"]
+        w.append(f)
+    norm = lambda Z: sum(float(np.sum(Z[k] ** 2)) / w[k] for k in range(o.K))
+    assert norm(Y) <= norm(X) * (1 + 1e-12)
+    assert np.all(np.isfinite(Y))
+    assert abs(g.expect(one_g)[0] - n0) < 1e-2 * abs(n0)
+    g.close()
+
+
+def test_error_paths():
+    P = gpu_mod()
+    bad = ci.config("cfg1", nq=[3])
+    with pytest.raises(P.ChfpeError):
+        P.CHFPE(bad)
+    with pytest.raises(P.ChfpeError):
+        P.CHFPE(ci.config("cfg1", depth=-1))
+    g = P.CHFPE(ci.config("cfg1"))
+    mu_g, _ = obs_pair("mu", 1)
+    with pytest.raises(P.ChfpeError):
+        g.response_1d(mu_g, mu_g, 3, 1, 1e-3)          # before equilibrate / import
+    g.equilibrate()
+    with pytest.raises(P.ChfpeError):
+        g.response_2d(mu_g, mu_g, mu_g, [3, 1], [0], 1e-3)   # unsorted t1
+    g.close()
