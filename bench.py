@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""Benchmark of the CHFPE hot path (arXiv 2509.25840) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4]
+
+A "step" is one pass of the whole hot path over one batch: one fourth-order Runge-Kutta step of the whole
+hierarchy (steps a1-a3 of DESIGN.md: Liouvillian stencil + hierarchy couplings + stage combine, 4 fused stage
+kernels) followed by the phase-space expectation <C> of element 0 (step a5), i.e. one sample of the linear
+response protocol of section IV.C.1.  Metric (BASELINE.json): phase-space cell-updates/s in
+fp64 = cells * steps / time; one cell-update advances all K hierarchy elements of one grid cell by one step.
+
+Workload at N = 1: BASELINE.json configs[3] ("cfg4": 3 modes, 16^6 grid, depth 3 -> 20 elements), the
+configuration the north-star target is quoted on.  Inputs are synthetic (chfpe_inputs.py): the state is the
+analytic equilibrium kicked by mu = q1+q2+q3.  One state array (2.7 GB) exceeds the 126 MB L2, so every timed
+iteration streams from HBM ("inputs larger than L2").
+
+N > 1 (torchrun): a single propagation does not shard ("replicas only"); every rank propagates its
+own replica, no data-path collective, scaling = weak; time = max over ranks.
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) as it stands on the host cores, rank 0 only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import chfpe_inputs as ci  # noqa: E402
+
+METRIC = "phase-space cell-updates/s (fp64)"
+UNIT = "cell-updates/s"
+BYTES_PER_VALUE_STEP_SURVEY = 128.0        # classical RK4, 4 arrays, 9R + 7W per value per step
+HBM_NOMINAL_GBS = 8000.0                   # "about 8 TB/s", BASELINE.json north_star
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.proc is not None:
+            self.proc.terminate()          # exact PID of the child we started
+        self.join(timeout=2.0)
+        sm, mx, reasons = [], 0.0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        med = sm[len(sm) // 2] if sm else None
+        return {"sm_mhz": med, "sm_max_mhz": mx or None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def obs(mod, kind, M):
+    d = ci.observable(kind, M)
+    return mod.make_observable(d["c0"], d["lin_q"], d["quad"], d["lin_p"])
+
+
+def cpu_oracle_time(cfg, steps, warmup=0):
+    """Time the oracle as it stands: equilibrium, kick(mu), then `steps` x (RK4 step + <mu>).  Returns
+    (seconds, threads, K, cells)."""
+    import oracle
+    o = oracle.RefCHFPE(cfg)
+    mu = obs(oracle, "mu", cfg["n_modes"])
+    o.equilibrate()
+    o.kick(mu)
+    for _ in range(warmup):
+        o.step(1, cfg["dt"]); o.expect(mu)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(1, cfg["dt"]); o.expect(mu)
+    dt = time.perf_counter() - t0
+    K, cells = o.K, o.cells
+    o.close()
+    return dt, oracle.set_threads(0), K, cells
+
+
+def pick_cpu_sample(workload):
+    """Bounded sample of the workload for the oracle: the full grid if the host has the RAM (4 state-sized
+    arrays + scratch), else the 12^6 shrink of the same model (stated in `sample`)."""
+    cfg = ci.config(workload)
+    cells = 1
+    for s in range(cfg["n_modes"]):
+        cells *= cfg["nq"][s] * cfg["np"][s]
+    K = {1: cfg["depth"] + 1, 2: (cfg["depth"] + 1) * (cfg["depth"] + 2) // 2,
+         3: (cfg["depth"] + 1) * (cfg["depth"] + 2) * (cfg["depth"] + 3) // 6}[cfg["n_modes"]]
+    need = 5 * K * cells * 8
+    try:
+        import psutil
+        avail = psutil.virtual_memory().available
+    except Exception:
+        avail = 0
+    if workload == "cfg4" and avail < need + (8 << 30):
+        return ci.config("cfg4s12"), "cfg4 model on a 12^6 grid (host RAM too small for 16^6)"
+    return cfg, "%s at full size" % workload
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg, sample = pick_cpu_sample(args.workload)
+    steps = max(1, args.steps)
+    # keep the whole run within a few minutes: the oracle does ~1e7 value-updates/s on 8 cores
+    t_probe, threads, K, cells = cpu_oracle_time(cfg, 1, 0)
+    budget = 150.0
+    max_steps = max(1, int(budget / max(t_probe, 1e-3)) - 1)
+    warm = min(args.warmup, max(0, max_steps // 4))
+    steps = min(steps, max(1, max_steps - warm))
+    dt, threads, K, cells = cpu_oracle_time(cfg, steps, warm)
+    val = cells * steps / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warm, "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "sample": sample, "K": K, "cells": cells,
+                       "note": "CPU oracle (oracle/chfpe_ref.c, OpenMP) on the host cores; a deliberately plain program"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
+                             "sample": "%s, %d RK4 steps + <mu> each" % (sample, steps)},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import paper_2509_25840_b200 as P
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: a CUDA device is required (the CHFPE path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = ci.config(args.workload)
+    M = cfg["n_modes"]
+    g = P.CHFPE(cfg, batch=1, device="cuda:%d" % local)
+    mu = obs(P, "mu", M)
+    dt = cfg["dt"]
+    K, cells = g.K, g.cells
+    values = K * cells
+    steps, warm = args.steps, max(args.warmup, 3)
+
+    # ---- device-resident arm: equilibrium, kick(mu), W warm-up steps, then exactly K x (step + <mu>) ----
+    g.equilibrate(residual=False)
+    g.kick(mu)
+    g.response_1d(None, mu, warm + 1, 1, dt)
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.3)
+    n0 = g.launch_count()
+    g.profile_enable(True)
+    g.profile_read()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    R = g.response_1d(None, mu, steps + 1, 1, dt)        # K steps, K+1 expectation samples, one D2H of K+1 doubles
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    stage_ms, stage_n = g.profile_read()
+    g.profile_enable(False)
+    launches = g.launch_count() - n0
+    clocks = sampler.stop() if sampler else None
+    if not np.all(np.isfinite(R)):
+        raise SystemExit("bench.py: non-finite response")
+
+    # ---- end-to-end arm: host state in pinned memory -> import (H2D) -> kick, K x (step + <mu>) -> R on host ----
+    X0 = g.export_state_device().cpu().pin_memory()       # canonical layout, K*cells doubles, pinned
+    R_host_bytes = 8 * (steps + 1)
+    barrier()
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record()
+    g.import_state(X0.numpy())
+    g.response_1d(None, mu, steps + 1, 1, dt)
+    e3.record()
+    barrier()
+    ms_e2e = e2.elapsed_time(e3)
+
+    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, ms_e2e = float(t[0]), float(t[1])
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        value = world * cells * steps / (ms * 1e-3)
+        e2e = world * cells * steps / (ms_e2e * 1e-3)
+        # dominant kernel: the fused RK-stage kernel.  Algorithmic (compulsory) bytes per launch, DESIGN.md section 5:
+        # stage 1 reads y and writes v (16 B/value), stages 2-4 read v, read y, write the next v (24 B/value);
+        # averaged over the four launches of a step: 22 B/value/launch = 88 B/value/step.
+        alg_bytes_launch = values * 22.0
+        kern_ms = stage_ms / max(stage_n, 1)
+        achieved = alg_bytes_launch / (kern_ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
+            "ms_per_step": ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "modes": M, "grid": "x".join(str(x) for x in g.shape), "K": K,
+                       "cells": cells, "depth": cfg["depth"], "dt": dt, "scheme": cfg["scheme"], "gauge": cfg["gauge"],
+                       "integrator": "RK4 (Horner form)", "l2": "inputs larger than L2 (state array 2.7 GB vs 126 MB)",
+                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU"},
+            "value_updates_per_s": value * K,
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": values * 8.0 / steps,
+                    "d2h_bytes_per_step": R_host_bytes / steps,
+                    "note": "one chfpe_import_state of the pinned host state (H2D, whole state once per job) + "
+                            "chfpe_response_1d returning R on the host, all inside the timed region"},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "kernel": "RK stage (k_stage_*)",
+                         "kernel_ms": kern_ms, "kernel_launches_timed": int(stage_n),
+                         "kernel_share_of_step": stage_ms / ms,
+                         "algorithmic_bytes_per_launch": alg_bytes_launch,
+                         "frac_survey_128B_of_8TBs": values * BYTES_PER_VALUE_STEP_SURVEY * steps
+                         / (ms * 1e-3) / 1e9 / HBM_NOMINAL_GBS},
+        }
+        if world == 1 and not args.no_cpu:
+            cfg_c, sample = pick_cpu_sample(args.workload)
+            tc, threads, Kc, cells_c = cpu_oracle_time(cfg_c, 1, 0)
+            line["cpu_baseline"] = {"value": cells_c / tc, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                    "sample": "%s, 1 RK4 step + <mu> (%.1f s)" % (sample, tc)}
+        print(json.dumps(line))
+    g.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

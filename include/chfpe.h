@@ -101,8 +101,9 @@ int chfpe_expect(chfpe_handle* h, const chfpe_observable* O, double* out);
 /* Same reduction on element k of replica `replica` (tests of the hierarchy normalisation). out: host, 1 double. */
 int chfpe_expect_element(chfpe_handle* h, int32_t replica, int32_t k, const chfpe_observable* O, double* out);
 
-/* R1: replica 0 <- Kick(A) replica 0; for i in 0..n_samples-1: R[i] = <C>, then `stride` steps.
-   Literal Eq. (15) :119, section IV.C.1 :229-233.  R: host, n_samples doubles.  Other replicas untouched. */
+/* R1: replica 0 <- Kick(A) replica 0; for i in 0..n_samples-1: R[i] = <C>, then `stride` steps (none after the
+   last sample).  Literal Eq. (15) :119, section IV.C.1 :229-233.  R: host, n_samples doubles.  Other replicas
+   untouched.  A == NULL skips the kick and continues the trajectory replica 0 already holds. */
 int chfpe_response_1d(chfpe_handle* h, const chfpe_observable* A, const chfpe_observable* C,
                       int64_t n_samples, int64_t stride, double dt, double* R);
 
@@ -123,6 +124,13 @@ int chfpe_export_rhs(chfpe_handle* h, int32_t replica, double* dst, int dst_is_d
 
 /* Number of kernels the library has launched on this handle since create (bench.py's gpu_launches). */
 int chfpe_launch_count(const chfpe_handle* h, int64_t* n);
+
+/* Device timing of the dominant kernel (the fused RK-stage kernel, steps a1-a3).  While enabled, every stage
+   launch is bracketed by two CUDA events on the handle's stream.  chfpe_profile_read synchronises the stream,
+   returns the summed duration (milliseconds) and the number of stage launches since the last read (host
+   pointers), and resets both.  Off by default; the events cost about a microsecond per launch. */
+int chfpe_profile_enable(chfpe_handle* h, int on);
+int chfpe_profile_read(chfpe_handle* h, double* total_ms, int64_t* n_launches);
 
 const char* chfpe_last_error(const chfpe_handle* h);   /* h may be NULL: last create-time error */
 

@@ -10,7 +10,7 @@ EXPORTED_SYMBOLS = [
     "chfpe_workspace_bytes", "chfpe_create", "chfpe_destroy", "chfpe_num_elements", "chfpe_element_index",
     "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
     "chfpe_response_1d", "chfpe_response_2d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
-    "chfpe_launch_count", "chfpe_last_error",
+    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_last_error",
 ]
 
 
@@ -73,6 +73,8 @@ def lib():
     L.chfpe_import_state.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_export_rhs.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.chfpe_profile_enable.argtypes = [vp, C.c_int]
+    L.chfpe_profile_read.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.chfpe_last_error.argtypes = [vp]
     L.chfpe_last_error.restype = C.c_char_p
     _lib = L
@@ -215,8 +217,10 @@ class CHFPE:
         return out.value
 
     def response_1d(self, A, Cobs, n_samples, stride, dt):
+        """A may be None: no kick, continue the trajectory replica 0 holds."""
         R = np.empty(n_samples)
-        self._ck(lib().chfpe_response_1d(self._h, C.byref(A), C.byref(Cobs), n_samples, stride, dt,
+        self._ck(lib().chfpe_response_1d(self._h, C.byref(A) if A is not None else None, C.byref(Cobs),
+                                         n_samples, stride, dt,
                                          R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_response_1d")
         return R
 
@@ -259,6 +263,15 @@ class CHFPE:
         t = self._torch.empty((self.K,) + self.shape, dtype=self._torch.float64, device=self.device)
         self._ck(lib().chfpe_export_rhs(self._h, replica, C.c_void_p(t.data_ptr()), 1), "chfpe_export_rhs")
         return t
+
+    def profile_enable(self, on=True):
+        self._ck(lib().chfpe_profile_enable(self._h, 1 if on else 0), "chfpe_profile_enable")
+
+    def profile_read(self):
+        """(summed stage-kernel milliseconds, stage launches) since the last read; synchronises the stream."""
+        ms, n = C.c_double(), C.c_int64()
+        self._ck(lib().chfpe_profile_read(self._h, C.byref(ms), C.byref(n)), "chfpe_profile_read")
+        return ms.value, n.value
 
     def launch_count(self):
         n = C.c_int64()

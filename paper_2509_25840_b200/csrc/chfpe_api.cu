@@ -125,7 +125,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   h->K = pl.K; h->batch = pl.batch; h->n_arrays = pl.n_arrays; h->cells = pl.cells;
   h->state_doubles = (size_t)pl.K * pl.cells;
   h->red_blocks = pl.red_blocks;
-  h->initialised = false; h->launches = 0;
+  h->initialised = false; h->launches = 0; h->prof = false; h->prof_used = 0;
   const int M = pl.M;
   enumerate_elements(M, desc->depth, &h->elem);
 
@@ -232,7 +232,11 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   return CHFPE_OK;
 }
 
-extern "C" int chfpe_destroy(chfpe_handle* h) { delete h; return CHFPE_OK; }
+extern "C" int chfpe_destroy(chfpe_handle* h) {
+  if (h) for (cudaEvent_t e : h->prof_ev) cudaEventDestroy(e);
+  delete h;
+  return CHFPE_OK;
+}
 
 extern "C" const char* chfpe_last_error(const chfpe_handle* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
 
@@ -265,18 +269,54 @@ static int check_launch(chfpe_handle* h) {
   return CHFPE_OK;
 }
 
+// one RK stage launch, bracketed by events when profiling is on
+static void stage(chfpe_handle* h, const double* in, const double* y, double* out, double a, double c, int nb,
+                  size_t ss) {
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (h->prof) {
+    if (h->prof_used + 2 > h->prof_ev.size()) {
+      cudaEvent_t a0, a1;
+      if (cudaEventCreate(&a0) == cudaSuccess && cudaEventCreate(&a1) == cudaSuccess) { h->prof_ev.push_back(a0); h->prof_ev.push_back(a1); }
+    }
+    if (h->prof_used + 2 <= h->prof_ev.size()) { e0 = h->prof_ev[h->prof_used]; e1 = h->prof_ev[h->prof_used + 1]; h->prof_used += 2; }
+  }
+  if (e0) cudaEventRecord(e0, h->stream);
+  h->launches += launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);
+  if (e1) cudaEventRecord(e1, h->stream);
+}
+
 // n RK4 steps (Horner form, R13) on slots [b0, b0+nb)
 static int step_slots(chfpe_handle* h, int b0, int nb, int64_t n_steps, double dt) {
   if (nb <= 0 || n_steps <= 0) return CHFPE_OK;
   const size_t ss = 3 * h->state_doubles;
   double *y = h->y(b0), *va = h->va(b0), *vb = h->vb(b0);
   for (int64_t i = 0; i < n_steps; i++) {
-    h->launches += launch_stage(h->op, y, y, va, 1.0, dt / 4.0, nb, ss, h->stream);
-    h->launches += launch_stage(h->op, va, y, vb, 1.0, dt / 3.0, nb, ss, h->stream);
-    h->launches += launch_stage(h->op, vb, y, va, 1.0, dt / 2.0, nb, ss, h->stream);
-    h->launches += launch_stage(h->op, va, y, y, 1.0, dt, nb, ss, h->stream);
+    stage(h, y, y, va, 1.0, dt / 4.0, nb, ss);
+    stage(h, va, y, vb, 1.0, dt / 3.0, nb, ss);
+    stage(h, vb, y, va, 1.0, dt / 2.0, nb, ss);
+    stage(h, va, y, y, 1.0, dt, nb, ss);
   }
   return check_launch(h);
+}
+
+extern "C" int chfpe_profile_enable(chfpe_handle* h, int on) {
+  if (!h) return CHFPE_ERR_INVALID;
+  h->prof = on != 0;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_profile_read(chfpe_handle* h, double* total_ms, int64_t* n_launches) {
+  if (!h || !total_ms || !n_launches) return CHFPE_ERR_INVALID;
+  CU(h, cudaStreamSynchronize(h->stream));
+  double tot = 0.0;
+  for (size_t i = 0; i + 1 < h->prof_used; i += 2) {
+    float ms = 0.f;
+    CU(h, cudaEventElapsedTime(&ms, h->prof_ev[i], h->prof_ev[i + 1]));
+    tot += ms;
+  }
+  *total_ms = tot; *n_launches = (int64_t)(h->prof_used / 2);
+  h->prof_used = 0;
+  return CHFPE_OK;
 }
 
 static int kick_slots(chfpe_handle* h, int b0, int nb, const chfpe_observable* X) {
@@ -362,9 +402,9 @@ extern "C" int chfpe_expect_element(chfpe_handle* h, int32_t replica, int32_t k,
 
 extern "C" int chfpe_response_1d(chfpe_handle* h, const chfpe_observable* A, const chfpe_observable* C,
                                  int64_t n_samples, int64_t stride, double dt, double* R) {
-  if (!h || !A || !C || !R || n_samples < 0 || stride < 0) return CHFPE_ERR_INVALID;
+  if (!h || !C || !R || n_samples < 0 || stride < 0) return CHFPE_ERR_INVALID;
   if (!h->initialised) FAIL(h, CHFPE_ERR_STATE, "response_1d before equilibrate/import");
-  int rc = kick_slots(h, 0, 1, A);
+  int rc = A ? kick_slots(h, 0, 1, A) : CHFPE_OK;
   if (rc) return rc;
   int64_t done = 0;
   while (done < n_samples) {                         // results buffer holds Plan::RESULTS samples per round trip

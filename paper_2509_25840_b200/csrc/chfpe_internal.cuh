@@ -52,6 +52,9 @@ struct chfpe_handle {
   std::vector<int> elem;              // host copy [K][3]
   bool initialised;
   int64_t launches;
+  bool prof;                          // bracket every stage launch with CUDA events (chfpe_profile_*)
+  std::vector<cudaEvent_t> prof_ev;   // pairs (start, stop); prof_used of them are pending
+  size_t prof_used;
   std::string err;
   double* y(int b) const { return arrays + (size_t)(3 * b) * state_doubles; }
   double* va(int b) const { return arrays + (size_t)(3 * b + 1) * state_doubles; }
