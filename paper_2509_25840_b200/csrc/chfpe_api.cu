@@ -2,6 +2,7 @@
 // drivers that sequence kernel launches (equilibrate a6, step a1-a3, kick a4, expect a5, R1 a7, R2 a8).
 // No arithmetic of the method runs on the host beyond the one-off tables of `create`.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include "chfpe_internal.cuh"
 
@@ -88,12 +89,89 @@ static Plan make_plan(const chfpe_desc* d) {
   tb += align256(sizeof(double) * sum_n);                      // ep
   tb += align256(sizeof(int) * 3 * p.K) * 3;                   // up, dn, nvec
   tb += align256(sizeof(double) * p.K);                        // Gamma
+  tb += align256(sizeof(int) * p.K);                           // brick-kernel element order
+  tb += align256(sizeof(double) * (p.cells / p.nqc));          // brick of zeros (ghost bricks)
   p.tables_bytes = tb; o += tb;
   p.off_partial = o; o += align256(sizeof(double) * p.red_blocks * (size_t)p.batch);
   p.off_results = o; o += align256(sizeof(double) * Plan::RESULTS);
   p.off_arrays = o; o += align256(sizeof(double) * (size_t)p.n_arrays * p.K * p.cells);
   p.total = o;
   return p;
+}
+
+static int env_int(const char* name, int dflt) {
+  const char* v = getenv(name);
+  return (v && *v) ? atoi(v) : dflt;
+}
+
+// Choose the brick-kernel decomposition (chfpe_brick.cu) and the element groups that sweep q_1 in lock-step.
+// order_out: elements with the groups contiguous.  Tunables (experiments only): CHFPE_BRICK=0 disables the brick
+// kernels, CHFPE_BRICK_M forces the p_1 interleave m, CHFPE_GROUP the group size.
+static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std::vector<int>& up, const std::vector<int>& dn,
+                                 std::vector<int>* order_out) {
+  BrickPlan bp;
+  memset(&bp, 0, sizeof(bp));
+  const int M = pl.M, K = pl.K;
+  order_out->resize(K);
+  for (int k = 0; k < K; k++) (*order_out)[k] = k;
+  bp.g = 1; bp.n_groups = K;
+  if (M < 2 || d->scheme == CHFPE_COMPACT6 || !env_int("CHFPE_BRICK", 1)) return bp;
+  bp.P1 = d->np[0]; bp.P2 = d->np[1]; bp.P3 = (M == 3) ? d->np[2] : 1;
+  bp.PB2 = bp.P2 * bp.P3;
+  const int forced_m = env_int("CHFPE_BRICK_M", 0);
+  int best_m = 0, best_nc = 0, best_score = -1;
+  for (int m = 1; m * bp.PB2 <= 512 && m <= bp.P1; m++) {
+    if (forced_m && m != forced_m) continue;
+    const int need = (bp.P1 + m - 1) / m;
+    if (need > 24) continue;
+    const int nc = need <= 8 ? 8 : (need <= 16 ? 16 : 24);
+    const int nt = m * bp.PB2;
+    int score = (nt % 32 == 0 ? 1000 : 0) + (24 - nc) * 10 + nt / 64;
+    if (M == 3 && m == 1 && bp.P1 <= 16 && !forced_m) score += 100000;     // whole p_1 line in registers
+    if (score > best_score) { best_score = score; best_m = m; best_nc = nc; }
+  }
+  if (!best_m) return bp;
+  bp.m = best_m; bp.nc = best_nc; bp.nt = best_m * bp.PB2;
+  bp.p1reg = (M == 3 && best_m == 1 && bp.P1 <= 16) ? 1 : 0;
+  bp.o1 = bp.p1reg ? 0 : 2;
+  if (M == 3) { bp.S2 = bp.P3 + 4; bp.S1 = (bp.P2 + 4) * bp.S2; } else { bp.S2 = 1; bp.S1 = bp.P2 + 4; }
+  bp.smem_doubles = (bp.P1 + 2 * bp.o1) * bp.S1;
+  if ((size_t)bp.smem_doubles * sizeof(double) > 200 * 1024) return bp;
+  // group size: five q_1 planes of g elements should stay L2-resident (126 MB on B200; budget 90 MB)
+  const double plane_bytes = 8.0 * (double)pl.cells / d->nq[0];
+  int g = (int)(90.0e6 / (5.0 * plane_bytes));
+  if (g < 1) g = 1;
+  if (g > K) g = K;
+  g = env_int("CHFPE_GROUP", g);
+  if (g < 1) g = 1;
+  if (g > K) g = K;
+  // greedy grouping: grow each group by the unassigned element with most hierarchy links into it
+  std::vector<int> assigned(K, 0), order;
+  for (int k0 = 0; k0 < K; k0++) {
+    if (assigned[k0]) continue;
+    std::vector<int> grp(1, k0);
+    assigned[k0] = 1;
+    while ((int)grp.size() < g) {
+      int best = -1, best_links = -1;
+      for (int c = 0; c < K; c++) {
+        if (assigned[c]) continue;
+        int links = 0;
+        for (int e : grp)
+          for (int s = 0; s < M; s++) links += (up[3 * e + s] == c) + (dn[3 * e + s] == c);
+        if (links > best_links) { best_links = links; best = c; }
+      }
+      if (best < 0) break;
+      assigned[best] = 1; grp.push_back(best);
+    }
+    for (int e : grp) order.push_back(e);
+  }
+  *order_out = order;
+  bp.g = g; bp.n_groups = (K + g - 1) / g;
+  bp.blocks_per_full_group = (long long)g * pl.nqc;
+  bp.rest = pl.nqc / d->nq[0];
+  bp.enabled = 1;
+  bp.fixed = env_int("CHFPE_BRICK_FIXED", 1) ? brick_has_fixed(M, bp.P1, bp.P2, bp.P3) : 0;
+  return bp;
 }
 
 extern "C" int chfpe_workspace_bytes(const chfpe_desc* desc, size_t* bytes) {
@@ -218,6 +296,15 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   op.dn = (const int*)put(dn.data(), sizeof(int) * dn.size());
   op.nvec = (const int*)put(nv.data(), sizeof(int) * nv.size());
   op.Gamma = (const double*)put(Gam.data(), sizeof(double) * Gam.size());
+  std::vector<int> order;
+  h->bp = make_brick_plan(desc, pl, up, dn, &order);
+  h->bp.order = (const int*)put(order.data(), sizeof(int) * order.size());
+  {
+    std::vector<double> zeros((size_t)(pl.cells / pl.nqc), 0.0);
+    h->bp.zero_brick = (const double*)put(zeros.data(), sizeof(double) * zeros.size());
+    cudaStreamSynchronize(h->stream);                                  // `zeros` goes out of scope
+  }
+  if (h->bp.enabled && brick_configure(h->bp, M) != 0) { cudaGetLastError(); h->bp.enabled = 0; }
   h->partial = (double*)(base + pl.off_partial);
   h->results = (double*)(base + pl.off_results);
   h->arrays = (double*)(base + pl.off_arrays);
@@ -269,6 +356,12 @@ static int check_launch(chfpe_handle* h) {
   return CHFPE_OK;
 }
 
+static int run_stage(chfpe_handle* h, const double* in, const double* y, double* out, double a, double c, int nb,
+                     size_t ss) {
+  if (h->bp.enabled) return launch_stage_brick(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
+  return launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);
+}
+
 // one RK stage launch, bracketed by events when profiling is on
 static void stage(chfpe_handle* h, const double* in, const double* y, double* out, double a, double c, int nb,
                   size_t ss) {
@@ -281,7 +374,7 @@ static void stage(chfpe_handle* h, const double* in, const double* y, double* ou
     if (h->prof_used + 2 <= h->prof_ev.size()) { e0 = h->prof_ev[h->prof_used]; e1 = h->prof_ev[h->prof_used + 1]; h->prof_used += 2; }
   }
   if (e0) cudaEventRecord(e0, h->stream);
-  h->launches += launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);
+  h->launches += run_stage(h, in, y, out, a, c, nb, ss);
   if (e1) cudaEventRecord(e1, h->stream);
 }
 
@@ -361,7 +454,7 @@ extern "C" int chfpe_equilibrate(chfpe_handle* h, int64_t n_steps, double dt, do
   rc = step_slots(h, 0, h->batch, n_steps, dt);
   if (rc) return rc;
   if (residual_out) {
-    h->launches += launch_stage(h->op, h->y(0), h->y(0), h->va(0), 0.0, 1.0, 1, 0, h->stream);
+    h->launches += run_stage(h, h->y(0), h->y(0), h->va(0), 0.0, 1.0, 1, 0);
     h->launches += launch_reduce(h->op, none, RED_SUMSQ, h->va(0), 0, (long long)h->state_doubles, 1, 0, 1.0,
                                  h->partial, h->red_blocks, h->results, 1, h->stream);
     h->launches += launch_reduce(h->op, none, RED_SUMSQ, h->y(0), 0, (long long)h->state_doubles, 1, 0, 1.0,
@@ -498,7 +591,7 @@ extern "C" int chfpe_import_state(chfpe_handle* h, int32_t replica, const double
 
 extern "C" int chfpe_export_rhs(chfpe_handle* h, int32_t replica, double* dst, int dst_is_device) {
   if (!h || !dst || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
-  h->launches += launch_stage(h->op, h->y(replica), h->y(replica), h->va(replica), 0.0, 1.0, 1, 0, h->stream);
+  h->launches += run_stage(h, h->y(replica), h->y(replica), h->va(replica), 0.0, 1.0, 1, 0);
   if (dst_is_device) {
     h->launches += launch_permute(h->op, h->va(replica), dst, 0, h->stream);
     return check_launch(h);

@@ -30,6 +30,25 @@ struct DevOp {
   const double* Gamma;                // [K] sum_s n_s gamma_s
 };
 
+// Launch plan of the brick kernels (chfpe_brick.cu): one CTA per (element, q-point) p-brick.
+// The brick is viewed as [P1][PB2] (PB2 = product of the trailing p-extents).  Thread t owns the cells
+// (i1_0 + j*m, r), j = 0..NC-1, with r = t % PB2 and i1_0 = t / PB2, so its trailing momenta are constants.
+struct BrickPlan {
+  int enabled;
+  int nt, m, nc, p1reg;               // threads per CTA, p1-interleave, cells per thread (template), p1 line in registers
+  int P1, P2, P3, PB2;                // p-extents (P3 = 1 for M = 2)
+  int o1;                             // p1 padding of the shared brick (0 when p1reg)
+  int S1, S2;                         // shared-memory strides of i1 and i2 (padded)
+  int smem_doubles;
+  int g;                              // elements per lock-step group (L2 window)
+  int n_groups;
+  long long blocks_per_full_group;    // g * nqc
+  long long rest;                     // q-points per q1 plane
+  const int* order;                   // [K] element order, groups contiguous (device)
+  int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3>) exists
+  const double* zero_brick;           // pb zeros (device): stands in for bricks outside the grid
+};
+
 struct DevObs {                       // observable polynomial, Eq. (13)-(14)
   double c0, lin_q[3], quad[3][3], lin_p[3];
 };
@@ -40,6 +59,7 @@ struct chfpe_handle {
   chfpe_desc desc;
   std::vector<chfpe_monomial> U;
   DevOp op;
+  BrickPlan bp;
   cudaStream_t stream;
   int K, batch, n_arrays;
   long long cells;
@@ -66,6 +86,12 @@ struct chfpe_handle {
 // out = a*y + c*F(in) for slots [b0, b0+nb); slot stride = 3*state_doubles for all three pointers.
 int launch_stage(const DevOp& op, const double* in, const double* y, double* out, double a, double c,
                  int nb, size_t slot_stride, cudaStream_t s);
+// same operation by the brick kernel (chfpe_brick.cu); requires bp.enabled
+int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out,
+                       double a, double c, int nb, size_t slot_stride, cudaStream_t s);
+// one-off opt-in to > 48 KB dynamic shared memory for the brick kernels; returns a cudaError_t as int
+int brick_configure(const BrickPlan& bp, int M);
+int brick_has_fixed(int M, int P1, int P2, int P3);
 // out = Kick_obs(in) on every element, slots [b0, b0+nb)
 int launch_kick(const DevOp& op, const DevObs& o, const double* in, double* out, int nb, size_t slot_stride,
                 cudaStream_t s);
