@@ -89,7 +89,7 @@ static Plan make_plan(const chfpe_desc* d) {
   tb += align256(sizeof(double) * sum_n);                      // ep
   tb += align256(sizeof(int) * 3 * p.K) * 3;                   // up, dn, nvec
   tb += align256(sizeof(double) * p.K);                        // Gamma
-  tb += align256(sizeof(int) * p.K);                           // brick-kernel element order
+  tb += align256(sizeof(int) * p.K) * 2;                       // brick-kernel element order and its inverse
   tb += align256(sizeof(double) * (p.cells / p.nqc));          // brick of zeros (ghost bricks)
   p.tables_bytes = tb; o += tb;
   p.off_partial = o; o += align256(sizeof(double) * p.red_blocks * (size_t)p.batch);
@@ -299,6 +299,10 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   std::vector<int> order;
   h->bp = make_brick_plan(desc, pl, up, dn, &order);
   h->bp.order = (const int*)put(order.data(), sizeof(int) * order.size());
+  std::vector<int> pos(order.size());
+  for (size_t i = 0; i < order.size(); i++) pos[order[i]] = (int)i;
+  h->bp.pos = (const int*)put(pos.data(), sizeof(int) * pos.size());
+  h->bp.l2mode = env_int("CHFPE_L2MODE", 1);
   {
     std::vector<double> zeros((size_t)(pl.cells / pl.nqc), 0.0);
     h->bp.zero_brick = (const double*)put(zeros.data(), sizeof(double) * zeros.size());

@@ -14,6 +14,32 @@
 
 namespace {
 
+// L2 eviction policies (createpolicy + ld/st .L2::cache_hint): the stage input of the elements of the current
+// group must survive in L2 for five q_1 planes, everything that is touched once (y, out, bricks of elements outside
+// the group) is marked evict_first so that it cannot push the window out.
+__device__ __forceinline__ unsigned long long l2_policy(int kind) {   // 0 normal, 1 evict_first, 2 evict_last
+  unsigned long long p;
+  if (kind == 1) asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  else if (kind == 2) asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  else asm("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ double ldg_hint(const double* p, unsigned long long pol) {   // read-only data
+  double v;
+  asm("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ double ld_hint(const double* p, unsigned long long pol) {    // may alias the output
+  double v;
+  asm volatile("ld.global.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(p), "l"(pol) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_hint(double* p, double v, unsigned long long pol) {
+  asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(p), "d"(v), "l"(pol) : "memory");
+}
+
+__device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 template <int M, int NC, bool P1REG>
 __global__ void __launch_bounds__(512, 1)
 k_stage_brick(DevOp op, BrickPlan bp, const double* __restrict__ in, const double* y, double* out, double a,
@@ -216,16 +242,75 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     g3[rw * G3_ROW + (c4 < 2 ? c4 : P3 + c4)] = 0.0;
   }
 
+  const unsigned long long pol_own = l2_policy((bp.l2mode & 2) ? 2 : 0);
+  const unsigned long long pol_str = l2_policy((bp.l2mode & 1) ? 1 : 0);
   const bool wide = (op.scheme == CHFPE_CENTRAL4);
   const double p1_0 = op.x0[3], h1 = op.h[3];
   const double p2 = op.x0[4] + i2 * op.h[4], p3 = op.x0[5] + i3 * op.h[5];
   const double Gam = __ldg(op.Gamma + k);
 
-  double xk[NC], acc[NC];
+  // Everything this brick needs from HBM (its own stage input, the bricks of its hierarchy neighbours, y) is
+  // requested into L2 now -- one 128-byte line per thread and array -- and consumed after the q-derivative part,
+  // whose loads are L2 hits on the q_1-plane window and take long enough to cover the DRAM latency.
+  {
+    constexpr int LINES = P1 * NT / 16;                             // 128-byte lines per brick
+    const size_t e0 = (size_t)k * op.cells + brick;
+    for (int l = tid; l < LINES; l += NT) {
+      prefetch_l2(X + e0 + 16 * l);
+      if (!y_is_in) prefetch_l2(y + boff + e0 + 16 * l);
 #pragma unroll
-  for (int j = 0; j < NC; j++) xk[j] = __ldg(Xk + j * NT);
+      for (int s = 0; s < 3; s++) {
+        const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+        if (ku >= 0) prefetch_l2(X + (size_t)ku * op.cells + brick + 16 * l);
+        if (kd >= 0) prefetch_l2(X + (size_t)kd * op.cells + brick + 16 * l);
+      }
+    }
+  }
+  double acc[NC];
 #pragma unroll
-  for (int j = 0; j < NC; j++) acc[j] = -Gam * xk[j];
+  for (int j = 0; j < NC; j++) acc[j] = 0.0;
+
+  // -(p_s/m_s) dW/dq_s
+#pragma unroll
+  for (int s = 0; s < 3; s++) {
+    const long long st = op.st[s];
+    const int i = iq[s], n = op.n[s];
+    const double* zb = zero_brick + tid;
+    const double* qp1 = (i + 1 < n) ? Xk + st : zb;
+    const double* qm1 = (i >= 1) ? Xk - st : zb;
+    const double* qp2 = (i + 2 < n) ? Xk + 2 * st : zb;
+    const double* qm2 = (i >= 2) ? Xk - 2 * st : zb;
+    const double wq = -(wide ? -op.c2[s] : op.c1[s]) * op.inv_mass[s];
+    const double cq23 = wq * (s == 1 ? p2 : p3);
+    constexpr int HB = (NC % 2 == 0) ? NC / 2 : NC;                 // loads are issued in batches of 4*HB
+#pragma unroll
+    for (int j0 = 0; j0 < NC; j0 += HB) {
+      double fp1[HB], fm1[HB], fp2[HB], fm2[HB];
+#pragma unroll
+      for (int j = 0; j < HB; j++) {
+        fp1[j] = ldg_hint(qp1 + (j0 + j) * NT, pol_own);
+        fm1[j] = ldg_hint(qm1 + (j0 + j) * NT, pol_own);
+        if (wide) {
+          fp2[j] = ldg_hint(qp2 + (j0 + j) * NT, pol_own);
+          fm2[j] = ldg_hint(qm2 + (j0 + j) * NT, pol_own);
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < HB; j++) {
+        const double d1 = fp1[j] - fm1[j];
+        double e = d1;
+        if (wide) e = fma(8.0, d1, -(fp2[j] - fm2[j]));
+        const double cq = (s == 0) ? wq * fma((double)(j0 + j), h1, p1_0) : cq23;
+        acc[j0 + j] = fma(cq, e, acc[j0 + j]);
+      }
+    }
+  }
+
+  double xk[NC];
+#pragma unroll
+  for (int j = 0; j < NC; j++) xk[j] = ldg_hint(Xk + j * NT, pol_own);
+#pragma unroll
+  for (int j = 0; j < NC; j++) acc[j] = fma(-Gam, xk[j], acc[j]);
 
   double w2 = 0.0, w3 = 0.0;                                        // 1/(12h) or 1/(2h) of p_2, p_3
 #pragma unroll
@@ -239,14 +324,16 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     const double pu = cu * op.kup[s], pd = cd * op.kdn[s];
     const double* Xu = (ku >= 0) ? X + (size_t)ku * op.cells + brick + tid : zero_brick + tid;
     const double* Xd = (kd >= 0) ? X + (size_t)kd * op.cells + brick + tid : zero_brick + tid;
+    const unsigned long long pol_u = (ku >= 0 && __ldg(bp.pos + ku) / bp.g == G) ? pol_own : pol_str;
+    const unsigned long long pol_d = (kd >= 0 && __ldg(bp.pos + kd) / bp.g == G) ? pol_own : pol_str;
     const double wp = wide ? -op.c2[3 + s] : op.c1[3 + s];
     if (s == 1) w2 = wp;
     if (s == 2) w3 = wp;
     const double wp8 = wide ? 8.0 * wp : wp, wp1 = wide ? wp : 0.0;
 #pragma unroll
     for (int j = 0; j < NC; j++) {
-      const double xu = (ku >= 0) ? __ldg(Xu + j * NT) : 0.0;
-      const double xd = (kd >= 0) ? __ldg(Xd + j * NT) : 0.0;
+      const double xu = (ku >= 0) ? ldg_hint(Xu + j * NT, pol_u) : 0.0;
+      const double xd = (kd >= 0) ? ldg_hint(Xd + j * NT, pol_d) : 0.0;
       double gg = dUs * xk[j];
       gg = fma(cu, xu, gg);
       gg = fma(cd, xd, gg);
@@ -284,39 +371,17 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     }
   }
 
-  // -(p_s/m_s) dW/dq_s
-#pragma unroll
-  for (int s = 0; s < 3; s++) {
-    const long long st = op.st[s];
-    const int i = iq[s], n = op.n[s];
-    const double* zb = zero_brick + tid;
-    const double* qp1 = (i + 1 < n) ? Xk + st : zb;
-    const double* qm1 = (i >= 1) ? Xk - st : zb;
-    const double* qp2 = (i + 2 < n) ? Xk + 2 * st : zb;
-    const double* qm2 = (i >= 2) ? Xk - 2 * st : zb;
-    const double wq = -(wide ? -op.c2[s] : op.c1[s]) * op.inv_mass[s];
-    const double cq23 = wq * (s == 1 ? p2 : p3);
-#pragma unroll
-    for (int j = 0; j < NC; j++) {
-      const double d1 = __ldg(qp1 + j * NT) - __ldg(qm1 + j * NT);
-      double e = d1;
-      if (wide) e = fma(8.0, d1, -(__ldg(qp2 + j * NT) - __ldg(qm2 + j * NT)));
-      const double cq = (s == 0) ? wq * fma((double)j, h1, p1_0) : cq23;
-      acc[j] = fma(cq, e, acc[j]);
-    }
-  }
-
   // stage combine.  y may alias out (last stage, in place): a thread reads only the cells it writes, and all
   // its reads are issued before its first write.
   const size_t o0 = boff + (size_t)k * op.cells + brick + tid;
   if (!y_is_in) {
 #pragma unroll
-    for (int j = 0; j < NC; j++) xk[j] = y[o0 + (size_t)j * NT];
+    for (int j = 0; j < NC; j++) xk[j] = ld_hint(y + o0 + (size_t)j * NT, pol_str);
   }
 #pragma unroll
   for (int j = 0; j < NC; j++) acc[j] = fma(cc, acc[j], a * xk[j]);
 #pragma unroll
-  for (int j = 0; j < NC; j++) out[o0 + (size_t)j * NT] = acc[j];
+  for (int j = 0; j < NC; j++) st_hint(out + o0 + (size_t)j * NT, acc[j], pol_str);
 }
 
 template <int P1, int P2, int P3>

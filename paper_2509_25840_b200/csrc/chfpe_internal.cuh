@@ -45,6 +45,8 @@ struct BrickPlan {
   long long blocks_per_full_group;    // g * nqc
   long long rest;                     // q-points per q1 plane
   const int* order;                   // [K] element order, groups contiguous (device)
+  const int* pos;                     // [K] position of element k in `order`
+  int l2mode;                         // bit 0: once-touched data evict_first, bit 1: window data evict_last
   int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3>) exists
   const double* zero_brick;           // pb zeros (device): stands in for bricks outside the grid
 };
