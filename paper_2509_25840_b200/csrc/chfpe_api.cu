@@ -171,6 +171,8 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   bp.rest = pl.nqc / d->nq[0];
   bp.enabled = 1;
   bp.fixed = env_int("CHFPE_BRICK_FIXED", 1) ? brick_has_fixed(M, bp.P1, bp.P2, bp.P3) : 0;
+  bp.pipe_stages = env_int("CHFPE_PIPE_STAGES", 2);
+  bp.pipe = env_int("CHFPE_PIPE", 1) ? pipe_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.pipe_stages) : 0;
   return bp;
 }
 
@@ -309,6 +311,18 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
     cudaStreamSynchronize(h->stream);                                  // `zeros` goes out of scope
   }
   if (h->bp.enabled && brick_configure(h->bp, M) != 0) { cudaGetLastError(); h->bp.enabled = 0; }
+  if (h->bp.enabled && h->bp.pipe) {
+    int dev = 0, sms = 148, smem_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+    const size_t need = pipe_smem_bytes(h->bp) + 1024;                  // + per-CTA reservation
+    int per_sm = need ? (int)((size_t)smem_sm / need) : 0;
+    if (per_sm > 2) per_sm = 2;
+    per_sm = env_int("CHFPE_PIPE_PER_SM", per_sm);
+    if (per_sm < 1 || pipe_configure(h->bp) != 0) { cudaGetLastError(); h->bp.pipe = 0; }
+    h->bp.pipe_ctas = sms * per_sm;
+  }
   h->partial = (double*)(base + pl.off_partial);
   h->results = (double*)(base + pl.off_results);
   h->arrays = (double*)(base + pl.off_arrays);
@@ -362,6 +376,7 @@ static int check_launch(chfpe_handle* h) {
 
 static int run_stage(chfpe_handle* h, const double* in, const double* y, double* out, double a, double c, int nb,
                      size_t ss) {
+  if (h->bp.enabled && h->bp.pipe) return launch_stage_pipe(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
   if (h->bp.enabled) return launch_stage_brick(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
   return launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);
 }

@@ -49,6 +49,8 @@ struct BrickPlan {
   int l2mode;                         // bit 0: once-touched data evict_first, bit 1: window data evict_last
   int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3>) exists
   const double* zero_brick;           // pb zeros (device): stands in for bricks outside the grid
+  int pipe;                           // use the plane-pipelined kernel (chfpe_pipe.cu)
+  int pipe_stages, pipe_ctas;         // shared-memory stages per CTA, persistent CTAs in the grid
 };
 
 struct DevObs {                       // observable polynomial, Eq. (13)-(14)
@@ -94,6 +96,12 @@ int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, c
 // one-off opt-in to > 48 KB dynamic shared memory for the brick kernels; returns a cudaError_t as int
 int brick_configure(const BrickPlan& bp, int M);
 int brick_has_fixed(int M, int P1, int P2, int P3);
+// plane-pipelined variant (chfpe_pipe.cu): bulk async copies into a shared-memory ring, persistent CTAs
+int pipe_has_fixed(int M, int P1, int P2, int P3, int stages);
+size_t pipe_smem_bytes(const BrickPlan& bp);
+int pipe_configure(const BrickPlan& bp);
+int launch_stage_pipe(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out, double a,
+                      double c, int nb, size_t slot_stride, cudaStream_t s);
 // out = Kick_obs(in) on every element, slots [b0, b0+nb)
 int launch_kick(const DevOp& op, const DevObs& o, const double* in, double* out, int nb, size_t slot_stride,
                 cudaStream_t s);
