@@ -137,9 +137,9 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   if (M == 3) { bp.S2 = bp.P3 + 4; bp.S1 = (bp.P2 + 4) * bp.S2; } else { bp.S2 = 1; bp.S1 = bp.P2 + 4; }
   bp.smem_doubles = (bp.P1 + 2 * bp.o1) * bp.S1;
   if ((size_t)bp.smem_doubles * sizeof(double) > 200 * 1024) return bp;
-  // group size: five q_1 planes of g elements should stay L2-resident (126 MB on B200; budget 90 MB)
+  // group size: five q_1 planes of g elements should stay L2-resident (126 MB on B200, shared with the once-touched streams; budget 60 MB)
   const double plane_bytes = 8.0 * (double)pl.cells / d->nq[0];
-  int g = (int)(90.0e6 / (5.0 * plane_bytes));
+  int g = (int)(60.0e6 / (5.0 * plane_bytes));
   if (g < 1) g = 1;
   if (g > K) g = K;
   g = env_int("CHFPE_GROUP", g);
@@ -170,9 +170,17 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   bp.blocks_per_full_group = (long long)g * pl.nqc;
   bp.rest = pl.nqc / d->nq[0];
   bp.enabled = 1;
-  bp.fixed = env_int("CHFPE_BRICK_FIXED", 1) ? brick_has_fixed(M, bp.P1, bp.P2, bp.P3) : 0;
+  // specialised kernel: threads per CTA = split * P2*P3/2 (128-bit accesses); aim at 256 threads, 16 cells each
+  int split_default = 1;
+  while (split_default < bp.P1 && bp.P1 % (2 * split_default) == 0 && bp.P1 / (2 * split_default) >= 4 &&
+         split_default * bp.PB2 / 2 < 256)
+    split_default *= 2;
+  if (bp.P1 == 12) split_default = 2;
+  bp.split = env_int("CHFPE_BRICK_SPLIT", split_default);
+  bp.minb = env_int("CHFPE_BRICK_MINB", (bp.PB2 * bp.split / 2 <= 256) ? 2 : 1);
+  bp.fixed = env_int("CHFPE_BRICK_FIXED", 1) ? brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb) : 0;
   bp.pipe_stages = env_int("CHFPE_PIPE_STAGES", 2);
-  bp.pipe = env_int("CHFPE_PIPE", 1) ? pipe_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.pipe_stages) : 0;
+  bp.pipe = env_int("CHFPE_PIPE", 0) ? pipe_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.pipe_stages) : 0;
   return bp;
 }
 

@@ -189,24 +189,46 @@ k_stage_brick(DevOp op, BrickPlan bp, const double* __restrict__ in, const doubl
 }
 
 // ------------------------------------------------------------------------------------------------
-// Specialised M = 3 brick kernel with compile-time momentum extents (P1, P2, P3): NT = P2*P3 threads, thread
-// (i2, i3) owns the whole p_1 line (cells tid + j*NT, j = i1).  The p_1 stencil of G_1 runs in registers in
-// scatter form (each G_1 value is added to its four neighbours' accumulators as soon as it is formed); G_2 and
-// G_3 go to two shared arrays padded along their own axis only, so one __syncthreads per brick suffices.
+// Specialised M = 3 brick kernel with compile-time momentum extents (P1, P2, P3), 128-bit accesses.
+// A thread owns a PAIR of cells adjacent along p_3 (one double2) on NC = P1/SPLIT consecutive p_1 planes; the SPLIT
+// thread groups of a CTA share one brick.  On B200 a 16-byte-per-lane load moves twice the bytes of an 8-byte one
+// per outstanding request, and the L2->SM rate of this kernel is set by the requests in flight (measured: 11 vs
+// 20 TB/s at 16 warps per SM).  The p_1 stencil of G_1 runs in registers in scatter form (each G_1 value is added
+// to its four neighbours' accumulators as soon as it is formed; segment edges are exchanged through shared memory);
+// G_2 and G_3 go to two shared arrays padded along their own axis only, so one __syncthreads per brick suffices.
 // Absent q-neighbours (zero ghosts, R9) are redirected to a brick of zeros, which keeps every load unpredicated.
 // ------------------------------------------------------------------------------------------------
-template <int P1, int P2, int P3>
-__global__ void __launch_bounds__(P2 * P3, (P2 * P3 <= 256) ? 2 : 1)
+__device__ __forceinline__ double2 ldg2_hint(const double2* p, unsigned long long pol) {
+  double2 v;
+  asm("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+  return v;
+}
+__device__ __forceinline__ double2 ld2_hint(const double2* p, unsigned long long pol) {
+  double2 v;
+  asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st2_hint(double2* p, double2 v, unsigned long long pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ double2 fma2(double c, double2 a, double2 b) { return make_double2(fma(c, a.x, b.x), fma(c, a.y, b.y)); }
+
+template <int P1, int P2, int P3, int SPLIT, int MINB>
+__global__ void __launch_bounds__(SPLIT * P2 * P3 / 2, MINB)
 k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const double* y, double* out, double a,
                double cc, size_t slot_stride, int y_is_in, const double* __restrict__ zero_brick) {
-  constexpr int NT = P2 * P3, NC = P1;
+  static_assert(P3 % 2 == 0 && P1 % SPLIT == 0 && (SPLIT == 1 || P1 / SPLIT >= 2), "unsupported brick shape");
+  constexpr int PLANE = P2 * P3, PL2 = PLANE / 2, NTT = SPLIT * PL2, NC = P1 / SPLIT;
   constexpr int G2_ROW = P3, G2_PLANE = (P2 + 4) * P3;              // G_2[i1][i2+2][i3]
   constexpr int G3_ROW = P3 + 4, G3_PLANE = P2 * (P3 + 4);          // G_3[i1][i2][i3+2]
-  extern __shared__ double sm[];
+  extern __shared__ __align__(16) double sm[];
   double* g2 = sm;
   double* g3 = sm + P1 * G2_PLANE;
-  const int tid = threadIdx.x;
-  const int i2 = tid / P3, i3 = tid - i2 * P3;
+  double* xg = g3 + P1 * G3_PLANE;                                  // [SPLIT][4][PLANE]: first/last two G_1 planes of a segment
+  const int seg = (SPLIT == 1) ? 0 : threadIdx.x / PL2;
+  const int tid = threadIdx.x - seg * PL2;                          // pair index inside the plane
+  const int jbase = seg * NC;                                       // first p_1 plane of this thread
+  const int i2 = tid / (P3 / 2), i3 = 2 * (tid - i2 * (P3 / 2));
 
   long long L = blockIdx.x;
   const int G = (int)(L / bp.blocks_per_full_group);
@@ -227,17 +249,17 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   }
   const size_t boff = (size_t)blockIdx.y * slot_stride;
   const double* X = in + boff;
-  const size_t brick = (size_t)ql * (P1 * NT);
-  const double* Xk = X + (size_t)k * op.cells + brick + tid;
+  const size_t brick = (size_t)ql * (P1 * PLANE);
+  const size_t toff = (size_t)jbase * PLANE + 2 * tid;              // this thread's first cell inside the brick
+  const double2* Xk = reinterpret_cast<const double2*>(X + (size_t)k * op.cells + brick + toff);
+  const double2* zb = reinterpret_cast<const double2*>(zero_brick + toff);
 
   // zero the ghost rows / columns of the two shared bricks
-#pragma unroll
-  for (int i = tid; i < P1 * 4 * P3; i += NT) {                     // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
+  for (int i = threadIdx.x; i < P1 * 4 * P3; i += NTT) {            // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
     const int pl = i / (4 * P3), rr = i - pl * (4 * P3), row = rr / P3, col = rr - row * P3;
     g2[pl * G2_PLANE + (row < 2 ? row : P2 + row) * G2_ROW + col] = 0.0;
   }
-#pragma unroll
-  for (int i = tid; i < P1 * P2 * 4; i += NT) {                     // G_3: columns i3 = -2,-1,P3,P3+1 of every row
+  for (int i = threadIdx.x; i < P1 * P2 * 4; i += NTT) {            // G_3: columns i3 = -2,-1,P3,P3+1 of every row
     const int rw = i >> 2, c4 = i & 3;
     g3[rw * G3_ROW + (c4 < 2 ? c4 : P3 + c4)] = 0.0;
   }
@@ -245,17 +267,18 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const unsigned long long pol_own = l2_policy((bp.l2mode & 2) ? 2 : 0);
   const unsigned long long pol_str = l2_policy((bp.l2mode & 1) ? 1 : 0);
   const bool wide = (op.scheme == CHFPE_CENTRAL4);
-  const double p1_0 = op.x0[3], h1 = op.h[3];
-  const double p2 = op.x0[4] + i2 * op.h[4], p3 = op.x0[5] + i3 * op.h[5];
+  const double h1 = op.h[3], p1_0 = op.x0[3] + jbase * h1;
+  const double p2 = op.x0[4] + i2 * op.h[4];
+  const double p3a = op.x0[5] + i3 * op.h[5], p3b = op.x0[5] + (i3 + 1) * op.h[5];
   const double Gam = __ldg(op.Gamma + k);
 
   // Everything this brick needs from HBM (its own stage input, the bricks of its hierarchy neighbours, y) is
   // requested into L2 now -- one 128-byte line per thread and array -- and consumed after the q-derivative part,
   // whose loads are L2 hits on the q_1-plane window and take long enough to cover the DRAM latency.
   {
-    constexpr int LINES = P1 * NT / 16;                             // 128-byte lines per brick
+    constexpr int LINES = P1 * PLANE / 16;                          // 128-byte lines per brick
     const size_t e0 = (size_t)k * op.cells + brick;
-    for (int l = tid; l < LINES; l += NT) {
+    for (int l = threadIdx.x; l < LINES; l += NTT) {
       prefetch_l2(X + e0 + 16 * l);
       if (!y_is_in) prefetch_l2(y + boff + e0 + 16 * l);
 #pragma unroll
@@ -266,53 +289,54 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
       }
     }
   }
-  double acc[NC];
+  double2 acc[NC];
 #pragma unroll
-  for (int j = 0; j < NC; j++) acc[j] = 0.0;
+  for (int j = 0; j < NC; j++) acc[j] = make_double2(0.0, 0.0);
 
   // -(p_s/m_s) dW/dq_s
 #pragma unroll
   for (int s = 0; s < 3; s++) {
-    const long long st = op.st[s];
+    const long long st = op.st[s] / 2;                              // brick strides are even
     const int i = iq[s], n = op.n[s];
-    const double* zb = zero_brick + tid;
-    const double* qp1 = (i + 1 < n) ? Xk + st : zb;
-    const double* qm1 = (i >= 1) ? Xk - st : zb;
-    const double* qp2 = (i + 2 < n) ? Xk + 2 * st : zb;
-    const double* qm2 = (i >= 2) ? Xk - 2 * st : zb;
+    const bool hp1 = i + 1 < n, hm1 = i >= 1, hp2 = wide && i + 2 < n, hm2 = wide && i >= 2;   // CTA-uniform
     const double wq = -(wide ? -op.c2[s] : op.c1[s]) * op.inv_mass[s];
-    const double cq23 = wq * (s == 1 ? p2 : p3);
-    constexpr int HB = (NC % 2 == 0) ? NC / 2 : NC;                 // loads are issued in batches of 4*HB
+    const double cqa = wq * (s == 1 ? p2 : p3a), cqb = wq * (s == 1 ? p2 : p3b);
+    constexpr bool TIGHT = (NTT * MINB > 512);                      // <= 64 registers per thread
+    constexpr int HB = TIGHT ? 2 : ((NC > 4 && NC % 2 == 0) ? NC / 2 : NC);   // loads are issued in batches of 4*HB
+    const double2 zero2 = make_double2(0.0, 0.0);
 #pragma unroll
     for (int j0 = 0; j0 < NC; j0 += HB) {
-      double fp1[HB], fm1[HB], fp2[HB], fm2[HB];
+      double2 fp1[HB], fm1[HB], fp2[HB], fm2[HB];
 #pragma unroll
-      for (int j = 0; j < HB; j++) {
-        fp1[j] = ldg_hint(qp1 + (j0 + j) * NT, pol_own);
-        fm1[j] = ldg_hint(qm1 + (j0 + j) * NT, pol_own);
-        if (wide) {
-          fp2[j] = ldg_hint(qp2 + (j0 + j) * NT, pol_own);
-          fm2[j] = ldg_hint(qm2 + (j0 + j) * NT, pol_own);
-        }
+      for (int j = 0; j < HB; j++) {                                // ghost bricks (R9) are zero: no load at all
+        fp1[j] = hp1 ? ldg2_hint(Xk + st + (j0 + j) * PL2, pol_own) : zero2;
+        fm1[j] = hm1 ? ldg2_hint(Xk - st + (j0 + j) * PL2, pol_own) : zero2;
+        fp2[j] = hp2 ? ldg2_hint(Xk + 2 * st + (j0 + j) * PL2, pol_own) : zero2;
+        fm2[j] = hm2 ? ldg2_hint(Xk - 2 * st + (j0 + j) * PL2, pol_own) : zero2;
       }
 #pragma unroll
       for (int j = 0; j < HB; j++) {
-        const double d1 = fp1[j] - fm1[j];
-        double e = d1;
-        if (wide) e = fma(8.0, d1, -(fp2[j] - fm2[j]));
-        const double cq = (s == 0) ? wq * fma((double)(j0 + j), h1, p1_0) : cq23;
-        acc[j0 + j] = fma(cq, e, acc[j0 + j]);
+        double ex = fp1[j].x - fm1[j].x, ey = fp1[j].y - fm1[j].y;
+        if (wide) {
+          ex = fma(8.0, ex, -(fp2[j].x - fm2[j].x));
+          ey = fma(8.0, ey, -(fp2[j].y - fm2[j].y));
+        }
+        const double c1 = wq * fma((double)(j0 + j), h1, p1_0);
+        acc[j0 + j].x = fma(s == 0 ? c1 : cqa, ex, acc[j0 + j].x);
+        acc[j0 + j].y = fma(s == 0 ? c1 : cqb, ey, acc[j0 + j].y);
       }
     }
   }
 
-  double xk[NC];
+  double2 xk[NC];
 #pragma unroll
-  for (int j = 0; j < NC; j++) xk[j] = ldg_hint(Xk + j * NT, pol_own);
+  for (int j = 0; j < NC; j++) xk[j] = ldg2_hint(Xk + j * PL2, pol_own);
 #pragma unroll
-  for (int j = 0; j < NC; j++) acc[j] = fma(-Gam, xk[j], acc[j]);
+  for (int j = 0; j < NC; j++) acc[j] = fma2(-Gam, xk[j], acc[j]);
 
   double w2 = 0.0, w3 = 0.0;                                        // 1/(12h) or 1/(2h) of p_2, p_3
+  constexpr bool KEEP_G3 = (NTT * MINB <= 512);                    // else re-read the own G_3 pair from shared memory
+  double2 g3own[KEEP_G3 ? NC : 1];
 #pragma unroll
   for (int s = 0; s < 3; s++) {
     const double qs = op.x0[s] + iq[s] * op.h[s];
@@ -322,8 +346,8 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     const double cu = (ku >= 0) ? Vp : 0.0;
     const double cd = (kd >= 0) ? __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp : 0.0;
     const double pu = cu * op.kup[s], pd = cd * op.kdn[s];
-    const double* Xu = (ku >= 0) ? X + (size_t)ku * op.cells + brick + tid : zero_brick + tid;
-    const double* Xd = (kd >= 0) ? X + (size_t)kd * op.cells + brick + tid : zero_brick + tid;
+    const double2* Xu = (ku >= 0) ? reinterpret_cast<const double2*>(X + (size_t)ku * op.cells + brick + toff) : zb;
+    const double2* Xd = (kd >= 0) ? reinterpret_cast<const double2*>(X + (size_t)kd * op.cells + brick + toff) : zb;
     const unsigned long long pol_u = (ku >= 0 && __ldg(bp.pos + ku) / bp.g == G) ? pol_own : pol_str;
     const unsigned long long pol_d = (kd >= 0 && __ldg(bp.pos + kd) / bp.g == G) ? pol_own : pol_str;
     const double wp = wide ? -op.c2[3 + s] : op.c1[3 + s];
@@ -332,60 +356,101 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     const double wp8 = wide ? 8.0 * wp : wp, wp1 = wide ? wp : 0.0;
 #pragma unroll
     for (int j = 0; j < NC; j++) {
-      const double xu = (ku >= 0) ? ldg_hint(Xu + j * NT, pol_u) : 0.0;
-      const double xd = (kd >= 0) ? ldg_hint(Xd + j * NT, pol_d) : 0.0;
-      double gg = dUs * xk[j];
-      gg = fma(cu, xu, gg);
-      gg = fma(cd, xd, gg);
-      const double ps = (s == 0) ? fma((double)j, h1, p1_0) : (s == 1 ? p2 : p3);
-      acc[j] = fma(ps, fma(pd, xd, pu * xu), acc[j]);
+      double2 gg = make_double2(dUs * xk[j].x, dUs * xk[j].y);
+      const double psa = (s == 0) ? fma((double)j, h1, p1_0) : (s == 1 ? p2 : p3a);
+      const double psb = (s == 2) ? p3b : psa;
+      if (ku >= 0) {                                                // Phi_s W^(n+e_s), CTA-uniform branch
+        const double2 xu = ldg2_hint(Xu + j * PL2, pol_u);
+        gg = fma2(cu, xu, gg);
+        acc[j].x = fma(psa * pu, xu.x, acc[j].x);
+        acc[j].y = fma(psb * pu, xu.y, acc[j].y);
+      }
+      if (kd >= 0) {                                                // n_s Theta_s W^(n-e_s)
+        const double2 xd = ldg2_hint(Xd + j * PL2, pol_d);
+        gg = fma2(cd, xd, gg);
+        acc[j].x = fma(psa * pd, xd.x, acc[j].x);
+        acc[j].y = fma(psb * pd, xd.y, acc[j].y);
+      }
       if (s == 0) {                                                 // D_{p_1} G_1 in scatter form
-        if (j >= 1) acc[j - 1] = fma(wp8, gg, acc[j - 1]);
-        if (j + 1 < NC) acc[j + 1] = fma(-wp8, gg, acc[j + 1]);
-        if (j >= 2) acc[j - 2] = fma(-wp1, gg, acc[j - 2]);
-        if (j + 2 < NC) acc[j + 2] = fma(wp1, gg, acc[j + 2]);
+        if (j >= 1) acc[j - 1] = fma2(wp8, gg, acc[j - 1]);
+        if (j + 1 < NC) acc[j + 1] = fma2(-wp8, gg, acc[j + 1]);
+        if (j >= 2) acc[j - 2] = fma2(-wp1, gg, acc[j - 2]);
+        if (j + 2 < NC) acc[j + 2] = fma2(wp1, gg, acc[j + 2]);
+        if (SPLIT > 1) {                                            // segment edges: hand G_1 to the neighbour segment
+          if (j < 2) *reinterpret_cast<double2*>(xg + (seg * 4 + j) * PLANE + 2 * tid) = gg;
+          if (j >= NC - 2) *reinterpret_cast<double2*>(xg + (seg * 4 + 2 + j - (NC - 2)) * PLANE + 2 * tid) = gg;
+        }
       } else if (s == 1) {
-        g2[j * G2_PLANE + (i2 + 2) * G2_ROW + i3] = gg;
+        *reinterpret_cast<double2*>(g2 + (jbase + j) * G2_PLANE + (i2 + 2) * G2_ROW + i3) = gg;
       } else {
-        g3[j * G3_PLANE + i2 * G3_ROW + i3 + 2] = gg;
+        *reinterpret_cast<double2*>(g3 + (jbase + j) * G3_PLANE + i2 * G3_ROW + i3 + 2) = gg;
+        if (KEEP_G3) g3own[j] = gg;
       }
     }
   }
   __syncthreads();
+  if (SPLIT > 1) {
+    const double wp = wide ? -op.c2[3] : op.c1[3];
+    const double wp8 = wide ? 8.0 * wp : wp, wp1 = wide ? wp : 0.0;
+    if (seg > 0) {                                                  // G_1 at planes jbase-2, jbase-1
+      const double2 gm2 = *reinterpret_cast<const double2*>(xg + ((seg - 1) * 4 + 2) * PLANE + 2 * tid);
+      const double2 gm1 = *reinterpret_cast<const double2*>(xg + ((seg - 1) * 4 + 3) * PLANE + 2 * tid);
+      acc[0] = fma2(-wp8, gm1, acc[0]);
+      acc[0] = fma2(wp1, gm2, acc[0]);
+      acc[1] = fma2(wp1, gm1, acc[1]);
+    }
+    if (seg + 1 < SPLIT) {                                          // G_1 at planes jbase+NC, jbase+NC+1
+      const double2 gp0 = *reinterpret_cast<const double2*>(xg + ((seg + 1) * 4 + 0) * PLANE + 2 * tid);
+      const double2 gp1 = *reinterpret_cast<const double2*>(xg + ((seg + 1) * 4 + 1) * PLANE + 2 * tid);
+      acc[NC - 1] = fma2(wp8, gp0, acc[NC - 1]);
+      acc[NC - 1] = fma2(-wp1, gp1, acc[NC - 1]);
+      acc[NC - 2] = fma2(-wp1, gp0, acc[NC - 2]);
+    }
+  }
   {
-    const double* c2 = g2 + (i2 + 2) * G2_ROW + i3;
-    const double* c3 = g3 + i2 * G3_ROW + i3 + 2;
+    const double* c2 = g2 + jbase * G2_PLANE + (i2 + 2) * G2_ROW + i3;
+    const double* c3 = g3 + jbase * G3_PLANE + i2 * G3_ROW + i3 + 2;
 #pragma unroll
     for (int j = 0; j < NC; j++) {
       const double* a2 = c2 + j * G2_PLANE;
       const double* a3 = c3 + j * G3_PLANE;
-      const double d2 = a2[G2_ROW] - a2[-G2_ROW];
-      const double d3 = a3[1] - a3[-1];
-      double e2 = d2, e3 = d3;
+      const double2 u1 = *reinterpret_cast<const double2*>(a2 + G2_ROW), d1 = *reinterpret_cast<const double2*>(a2 - G2_ROW);
+      double e2x = u1.x - d1.x, e2y = u1.y - d1.y;
+      const double2 lft = *reinterpret_cast<const double2*>(a3 - 2), rgt = *reinterpret_cast<const double2*>(a3 + 2);
+      // pair (i3, i3+1): neighbours i3-2..i3+3 = lft.x lft.y [own.x own.y] rgt.x rgt.y
+      const double2 own = KEEP_G3 ? g3own[KEEP_G3 ? j : 0] : *reinterpret_cast<const double2*>(a3);
+      double e3x = own.y - lft.y, e3y = rgt.x - own.x;
       if (wide) {
-        e2 = fma(8.0, d2, -(a2[2 * G2_ROW] - a2[-2 * G2_ROW]));
-        e3 = fma(8.0, d3, -(a3[2] - a3[-2]));
+        const double2 u2 = *reinterpret_cast<const double2*>(a2 + 2 * G2_ROW), d2 = *reinterpret_cast<const double2*>(a2 - 2 * G2_ROW);
+        e2x = fma(8.0, e2x, -(u2.x - d2.x));
+        e2y = fma(8.0, e2y, -(u2.y - d2.y));
+        e3x = fma(8.0, e3x, -(rgt.x - lft.x));
+        e3y = fma(8.0, e3y, -(rgt.y - lft.y));
       }
-      acc[j] = fma(w2, e2, acc[j]);
-      acc[j] = fma(w3, e3, acc[j]);
+      acc[j].x = fma(w2, e2x, acc[j].x);
+      acc[j].y = fma(w2, e2y, acc[j].y);
+      acc[j].x = fma(w3, e3x, acc[j].x);
+      acc[j].y = fma(w3, e3y, acc[j].y);
     }
   }
 
   // stage combine.  y may alias out (last stage, in place): a thread reads only the cells it writes, and all
   // its reads are issued before its first write.
-  const size_t o0 = boff + (size_t)k * op.cells + brick + tid;
+  const size_t o0 = boff + (size_t)k * op.cells + brick + toff;
   if (!y_is_in) {
 #pragma unroll
-    for (int j = 0; j < NC; j++) xk[j] = ld_hint(y + o0 + (size_t)j * NT, pol_str);
+    for (int j = 0; j < NC; j++) xk[j] = ld2_hint(reinterpret_cast<const double2*>(y + o0) + j * PL2, pol_str);
   }
 #pragma unroll
-  for (int j = 0; j < NC; j++) acc[j] = fma(cc, acc[j], a * xk[j]);
+  for (int j = 0; j < NC; j++) acc[j] = make_double2(fma(cc, acc[j].x, a * xk[j].x), fma(cc, acc[j].y, a * xk[j].y));
 #pragma unroll
-  for (int j = 0; j < NC; j++) st_hint(out + o0 + (size_t)j * NT, acc[j], pol_str);
+  for (int j = 0; j < NC; j++) st2_hint(reinterpret_cast<double2*>(out + o0) + j * PL2, acc[j], pol_str);
 }
 
-template <int P1, int P2, int P3>
-constexpr int brick3_smem_bytes() { return (int)sizeof(double) * (P1 * (P2 + 4) * P3 + P1 * P2 * (P3 + 4)); }
+template <int P1, int P2, int P3, int SPLIT>
+constexpr int brick3_smem_bytes() {
+  return (int)sizeof(double) * (P1 * (P2 + 4) * P3 + P1 * P2 * (P3 + 4) + (SPLIT > 1 ? SPLIT * 4 * P2 * P3 : 0));
+}
 
 template <int M, int NC, bool P1REG>
 cudaError_t configure_one(int smem_bytes) {
@@ -407,11 +472,11 @@ cudaError_t configure_one(int smem_bytes) {
     }                                                                              \
   } while (0)
 
-#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16) X(20, 20, 20) X(8, 8, 8) X(12, 12, 12)
+#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 2, 2) X(16, 16, 16, 2, 1) X(16, 16, 16, 4, 2) X(16, 16, 16, 4, 1) X(20, 20, 20, 2, 1) X(20, 20, 20, 4, 1) X(8, 8, 8, 1, 2) X(8, 8, 8, 2, 2) X(12, 12, 12, 2, 2) X(12, 12, 12, 3, 2)
 
-int brick_has_fixed(int M, int P1, int P2, int P3) {
+int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {
   if (M != 3) return 0;
-#define X(A, B, C) if (P1 == A && P2 == B && P3 == C) return 1;
+#define X(A, B, C, S, MB) if (P1 == A && P2 == B && P3 == C && split == S && minb == MB) return 1;
   BRICK3_SPECIALISATIONS(X)
 #undef X
   return 0;
@@ -420,10 +485,10 @@ int brick_has_fixed(int M, int P1, int P2, int P3) {
 int brick_configure(const BrickPlan& bp, int M) {
   cudaError_t e = cudaSuccess;
   if (bp.fixed) {
-#define X(A, B, C)                                                                                        \
-    if (bp.P1 == A && bp.P2 == B && bp.P3 == C)                                                           \
-      e = cudaFuncSetAttribute(k_stage_brick3<A, B, C>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
-                               brick3_smem_bytes<A, B, C>());
+#define X(A, B, C, S, MB)                                                                                 \
+    if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                         \
+      e = cudaFuncSetAttribute(k_stage_brick3<A, B, C, S, MB>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                               brick3_smem_bytes<A, B, C, S>());
     BRICK3_SPECIALISATIONS(X)
 #undef X
     return (int)e;
@@ -441,10 +506,10 @@ int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, c
   const size_t smem = (size_t)bp.smem_doubles * sizeof(double);
   const int y_is_in = (y == in) ? 1 : 0;
   if (bp.fixed) {
-#define X(A, B, C)                                                                                         \
-    if (bp.P1 == A && bp.P2 == B && bp.P3 == C)                                                            \
-      k_stage_brick3<A, B, C><<<grid, B * C, brick3_smem_bytes<A, B, C>(), s>>>(op, bp, in, y, out, a, c,   \
-                                                                                slot_stride, y_is_in, bp.zero_brick);
+#define X(A, B, C, S, MB)                                                                                  \
+    if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                          \
+      k_stage_brick3<A, B, C, S, MB><<<grid, S * B * C / 2, brick3_smem_bytes<A, B, C, S>(), s>>>(             \
+          op, bp, in, y, out, a, c, slot_stride, y_is_in, bp.zero_brick);
     BRICK3_SPECIALISATIONS(X)
 #undef X
     return 1;

@@ -47,6 +47,8 @@ struct BrickPlan {
   const int* order;                   // [K] element order, groups contiguous (device)
   const int* pos;                     // [K] position of element k in `order`
   int l2mode;                         // bit 0: once-touched data evict_first, bit 1: window data evict_last
+  int minb;                           // CTAs per SM the specialised kernel is compiled for (register budget)
+  int split;                          // p_1 segments (thread groups) per brick in the specialised kernel
   int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3>) exists
   const double* zero_brick;           // pb zeros (device): stands in for bricks outside the grid
   int pipe;                           // use the plane-pipelined kernel (chfpe_pipe.cu)
@@ -95,7 +97,7 @@ int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, c
                        double a, double c, int nb, size_t slot_stride, cudaStream_t s);
 // one-off opt-in to > 48 KB dynamic shared memory for the brick kernels; returns a cudaError_t as int
 int brick_configure(const BrickPlan& bp, int M);
-int brick_has_fixed(int M, int P1, int P2, int P3);
+int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb);
 // plane-pipelined variant (chfpe_pipe.cu): bulk async copies into a shared-memory ring, persistent CTAs
 int pipe_has_fixed(int M, int P1, int P2, int P3, int stages);
 size_t pipe_smem_bytes(const BrickPlan& bp);
