@@ -38,6 +38,18 @@ BYTES_PER_VALUE_STEP_SURVEY = 128.0        # classical RK4, 4 ar
 HBM_NOMINAL_GBS = 8000.0                   # "about 8 TB/s", BASELINE.json north_star
 
 
+def profiled_traffic():
+    """DRAM bytes per launch of the stage kernel from the committed ncu --set full summary (profiles/), or None."""
+    import glob
+    import re
+    best = None
+    for f in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_stage_kernel_ncu_full.txt"))):
+        m = re.search(r"^dram_bytes_per_launch=([0-9.eE+]+)", open(f).read(), flags=re.M)
+        if m:
+            best = float(m.group(1))
+    return best
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -259,7 +271,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src, "kernel": "RK stage (k_stage_*)",
+                         "traffic": profiled_traffic() if args.workload == "cfg4" else None, "peak_source": peak_src, "kernel": "RK stage (k_stage_*)",
                          "kernel_ms": kern_ms, "kernel_launches_timed": int(stage_n),
                          "kernel_share_of_step": stage_ms / ms,
                          "algorithmic_bytes_per_launch": alg_bytes_launch,
