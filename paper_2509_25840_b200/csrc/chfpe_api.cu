@@ -104,9 +104,10 @@ static int env_int(const char* name, int dflt) {
   return (v && *v) ? atoi(v) : dflt;
 }
 
-// Choose the brick-kernel decomposition (chfpe_brick.cu) and the element groups that sweep q_1 in lock-step.
+// Choose the brick-kernel variant (chfpe_brick.cu) and the element groups that sweep q_1 in lock-step.
 // order_out: elements with the groups contiguous.  Tunables (experiments only): CHFPE_BRICK=0 disables the brick
-// kernels, CHFPE_BRICK_M forces the p_1 interleave m, CHFPE_GROUP the group size.
+// kernels, CHFPE_GROUP the group size, CHFPE_BRICK_SPLIT / CHFPE_BRICK_MINB the thread decomposition,
+// CHFPE_PIPE=1 the plane-pipelined variant.
 static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std::vector<int>& up, const std::vector<int>& dn,
                                  std::vector<int>* order_out) {
   BrickPlan bp;
@@ -115,29 +116,21 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   order_out->resize(K);
   for (int k = 0; k < K; k++) (*order_out)[k] = k;
   bp.g = 1; bp.n_groups = K;
-  if (M < 2 || d->scheme == CHFPE_COMPACT6 || !env_int("CHFPE_BRICK", 1)) return bp;
-  bp.P1 = d->np[0]; bp.P2 = d->np[1]; bp.P3 = (M == 3) ? d->np[2] : 1;
+  if (M != 3 || d->scheme == CHFPE_COMPACT6 || !env_int("CHFPE_BRICK", 1)) return bp;
+  bp.P1 = d->np[0]; bp.P2 = d->np[1]; bp.P3 = d->np[2];
   bp.PB2 = bp.P2 * bp.P3;
-  const int forced_m = env_int("CHFPE_BRICK_M", 0);
-  int best_m = 0, best_nc = 0, best_score = -1;
-  for (int m = 1; m * bp.PB2 <= 512 && m <= bp.P1; m++) {
-    if (forced_m && m != forced_m) continue;
-    const int need = (bp.P1 + m - 1) / m;
-    if (need > 24) continue;
-    const int nc = need <= 8 ? 8 : (need <= 16 ? 16 : 24);
-    const int nt = m * bp.PB2;
-    int score = (nt % 32 == 0 ? 1000 : 0) + (24 - nc) * 10 + nt / 64;
-    if (M == 3 && m == 1 && bp.P1 <= 16 && !forced_m) score += 100000;     // whole p_1 line in registers
-    if (score > best_score) { best_score = score; best_m = m; best_nc = nc; }
-  }
-  if (!best_m) return bp;
-  bp.m = best_m; bp.nc = best_nc; bp.nt = best_m * bp.PB2;
-  bp.p1reg = (M == 3 && best_m == 1 && bp.P1 <= 16) ? 1 : 0;
-  bp.o1 = bp.p1reg ? 0 : 2;
-  if (M == 3) { bp.S2 = bp.P3 + 4; bp.S1 = (bp.P2 + 4) * bp.S2; } else { bp.S2 = 1; bp.S1 = bp.P2 + 4; }
-  bp.smem_doubles = (bp.P1 + 2 * bp.o1) * bp.S1;
-  if ((size_t)bp.smem_doubles * sizeof(double) > 200 * 1024) return bp;
-  // group size: five q_1 planes of g elements should stay L2-resident (126 MB on B200, shared with the once-touched streams; budget 60 MB)
+  // threads per CTA = split * P2*P3/2 (128-bit accesses); aim at 256 threads with 16 cells each
+  int split_default = 1;
+  while (split_default < bp.P1 && bp.P1 % (2 * split_default) == 0 && bp.P1 / (2 * split_default) >= 4 &&
+         split_default * bp.PB2 / 2 < 256)
+    split_default *= 2;
+  if (bp.P1 == 12) split_default = 2;
+  bp.split = env_int("CHFPE_BRICK_SPLIT", split_default);
+  bp.minb = env_int("CHFPE_BRICK_MINB", (bp.PB2 * bp.split / 2 <= 256) ? 2 : 1);
+  bp.fixed = brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb);
+  if (!bp.fixed) return bp;
+  // group size: five q_1 planes of g elements should stay L2-resident (126 MB on B200, shared with the once-touched
+  // streams; budget 60 MB)
   const double plane_bytes = 8.0 * (double)pl.cells / d->nq[0];
   int g = (int)(60.0e6 / (5.0 * plane_bytes));
   if (g < 1) g = 1;
@@ -170,15 +163,6 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   bp.blocks_per_full_group = (long long)g * pl.nqc;
   bp.rest = pl.nqc / d->nq[0];
   bp.enabled = 1;
-  // specialised kernel: threads per CTA = split * P2*P3/2 (128-bit accesses); aim at 256 threads, 16 cells each
-  int split_default = 1;
-  while (split_default < bp.P1 && bp.P1 % (2 * split_default) == 0 && bp.P1 / (2 * split_default) >= 4 &&
-         split_default * bp.PB2 / 2 < 256)
-    split_default *= 2;
-  if (bp.P1 == 12) split_default = 2;
-  bp.split = env_int("CHFPE_BRICK_SPLIT", split_default);
-  bp.minb = env_int("CHFPE_BRICK_MINB", (bp.PB2 * bp.split / 2 <= 256) ? 2 : 1);
-  bp.fixed = env_int("CHFPE_BRICK_FIXED", 1) ? brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb) : 0;
   bp.pipe_stages = env_int("CHFPE_PIPE_STAGES", 2);
   bp.pipe = env_int("CHFPE_PIPE", 0) ? pipe_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.pipe_stages) : 0;
   return bp;

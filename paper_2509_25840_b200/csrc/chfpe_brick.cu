@@ -1,15 +1,14 @@
-// Brick kernel of the RK stage (steps a1-a3 of DESIGN.md) for M = 2, 3 on sm_100a.
+// Brick kernel of the RK stage (steps a1-a3 of DESIGN.md) for three modes on sm_100a.
 //
 // Internal layout [k][q_1..q_M][p_1..p_M] makes all momenta of one (element, q-point) a contiguous "p-brick".
 // Everything in Eq. (8) :77-80 except the q-derivatives of Eq. (9)-(10) :86-91 is local to the bricks of one
 // q-point: the p_s-derivatives of W^(n) (Eq. 10), of W^(n+e_s) (Phi, Eq. 11 :96) and of W^(n-e_s) (Theta, Eq. 12
 // :100) have q-only coefficients, so they are taken ONCE on the combination
 //     G_s = (dU/dq_s) X_k + V'_s X_up(k,s) + n_s c_s V'_s X_dn(k,s)                      (per cell, 3 flops)
-// which is staged in shared memory (zero-padded: the ghost values of reading R9) or, for the slowest momentum
-// when a thread owns the whole p_1 line, kept in registers.  The gauge terms kappa p_s X_{up,dn} are pointwise.
-// The q-derivatives are pointwise in the brick: coalesced loads of the same cell of the 4 M neighbouring bricks
-// of the same element, which the L2 serves (CTAs are ordered q_1-plane by q_1-plane, element group by group).
-// One CTA = one brick; thread t owns cells t, t + NT, ... (fixed trailing momenta, p_1 index i1_0 + j m).
+// The gauge terms kappa p_s X_{up,dn} are pointwise.  The q-derivatives are pointwise in the brick: coalesced loads
+// of the same cell of the 12 neighbouring bricks of the same element, which the L2 serves (CTAs are ordered q_1-plane
+// by q_1-plane, element group by group).  One CTA = one brick.  Grids without a compile-time specialisation run the
+// generic kernel of chfpe_kernels.cu (a run-time-shaped brick kernel was measured slower than it and removed).
 #include "chfpe_internal.cuh"
 
 namespace {
@@ -25,154 +24,6 @@ __device__ __forceinline__ unsigned long long l2_policy(int kind) {   // 0 norma
   return p;
 }
 __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-
-template <int M, int NC, bool P1REG>
-__global__ void __launch_bounds__(512, 1)
-k_stage_brick(DevOp op, BrickPlan bp, const double* __restrict__ in, const double* y, double* out, double a,
-              double cc, size_t slot_stride, int y_is_in) {
-  extern __shared__ double sm[];
-  const int tid = threadIdx.x;
-  const int nt = bp.nt;
-
-  // ---- block -> (element k, q-point ql): groups of bp.g elements, q_1 plane by q_1 plane inside a group ----
-  long long L = blockIdx.x;
-  const int G = (int)(L / bp.blocks_per_full_group);
-  L -= (long long)G * bp.blocks_per_full_group;
-  int gs = op.K - G * bp.g;
-  if (gs > bp.g) gs = bp.g;
-  const long long per_plane = (long long)gs * bp.rest;
-  const int iq1 = (int)(L / per_plane);
-  const long long r2 = L - (long long)iq1 * per_plane;
-  const int kk = (int)(r2 / bp.rest);
-  const long long ql = (long long)iq1 * bp.rest + (r2 - (long long)kk * bp.rest);
-  const int k = __ldg(bp.order + G * bp.g + kk);
-  int iq[M];
-  {
-    long long t = ql;
-#pragma unroll
-    for (int s = M - 1; s >= 0; s--) { long long u = t / op.n[s]; iq[s] = (int)(t - u * op.n[s]); t = u; }
-  }
-  const size_t boff = (size_t)blockIdx.y * slot_stride;
-  const double* X = in + boff;
-  const size_t brick = (size_t)ql * op.pb;
-  const double* Xk = X + (size_t)k * op.cells + brick;
-
-  // ---- thread -> cells ----
-  const int r = tid % bp.PB2, i1_0 = tid / bp.PB2;
-  int i2, i3 = 0;
-  if (M == 3) { i2 = r / bp.P3; i3 = r - i2 * bp.P3; } else { i2 = r; }
-  const int sstep = bp.m * bp.S1;                                   // shared-memory distance between owned cells
-  const int sbase = (M == 3) ? (i1_0 + bp.o1) * bp.S1 + (i2 + 2) * bp.S2 + (i3 + 2)
-                             : (i1_0 + bp.o1) * bp.S1 + (i2 + 2);
-  double pc[M];                                                     // momenta of the owned cells (p_1 of cell 0)
-  pc[0] = op.x0[M] + i1_0 * op.h[M];
-  pc[1] = op.x0[M + 1] + i2 * op.h[M + 1];
-  if (M == 3) pc[2] = op.x0[M + 2] + i3 * op.h[M + 2];
-  const double p1step = bp.m * op.h[M];
-  const bool wide = (op.scheme == CHFPE_CENTRAL4);
-
-  // zero the padded brick once (ghost values, R9); interior cells are overwritten before every use
-  for (int i = tid; i < bp.smem_doubles; i += nt) sm[i] = 0.0;
-
-  bool valid[NC];
-  double xk[NC], acc[NC];
-  const double Gam = __ldg(op.Gamma + k);
-#pragma unroll
-  for (int j = 0; j < NC; j++) {
-    valid[j] = (i1_0 + j * bp.m) < bp.P1;
-    xk[j] = valid[j] ? __ldg(Xk + tid + j * nt) : 0.0;
-    acc[j] = -Gam * xk[j];                                          // -(sum_s n_s gamma_s) W^(n)
-  }
-
-#pragma unroll
-  for (int s = 0; s < M; s++) {
-    const int ap = M + s;
-    const double qs = op.x0[s] + iq[s] * op.h[s];
-    const double Vp = fma(op.VSL[s], qs, op.VLL[s]);                // V'_s(q_s)
-    const double dUs = __ldg(op.dU[s] + ql);
-    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
-    const double cu = (ku >= 0) ? Vp : 0.0;
-    const double cd = (kd >= 0) ? __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp : 0.0;
-    const double pu = cu * op.kup[s], pd = cd * op.kdn[s];
-    const double* Xu = X + (size_t)(ku >= 0 ? ku : k) * op.cells + brick;
-    const double* Xd = X + (size_t)(kd >= 0 ? kd : k) * op.cells + brick;
-    const double wp = wide ? -op.c2[ap] : op.c1[ap];                // 1/(12h) or 1/(2h)
-    const bool regpath = P1REG && s == 0;
-    double g[NC];
-#pragma unroll
-    for (int j = 0; j < NC; j++) {
-      const double xu = (ku >= 0 && valid[j]) ? __ldg(Xu + tid + j * nt) : 0.0;
-      const double xd = (kd >= 0 && valid[j]) ? __ldg(Xd + tid + j * nt) : 0.0;
-      double gg = dUs * xk[j];
-      gg = fma(cu, xu, gg);
-      gg = fma(cd, xd, gg);
-      const double ps = (s == 0) ? fma((double)j, p1step, pc[0]) : pc[s];
-      acc[j] = fma(ps, fma(pd, xd, pu * xu), acc[j]);               // kappa p_s (V' X_up + n c V' X_dn)
-      g[j] = gg;
-    }
-    if (regpath) {                                                  // whole p_1 line in registers, m == 1
-#pragma unroll
-      for (int j = 0; j < NC; j++) {
-        const double d1 = ((j + 1 < NC) ? g[(j + 1 < NC) ? j + 1 : j] : 0.0) - ((j >= 1) ? g[(j >= 1) ? j - 1 : j] : 0.0);
-        double e = d1;
-        if (wide) {
-          const double d2 = ((j + 2 < NC) ? g[(j + 2 < NC) ? j + 2 : j] : 0.0) - ((j >= 2) ? g[(j >= 2) ? j - 2 : j] : 0.0);
-          e = fma(8.0, d1, -d2);
-        }
-        acc[j] = fma(wp, e, acc[j]);
-      }
-    } else {
-      const int str = (s == 0) ? bp.S1 : ((M == 3 && s == 1) ? bp.S2 : 1);
-      __syncthreads();                                              // previous readers done (and pads zeroed)
-#pragma unroll
-      for (int j = 0; j < NC; j++)
-        if (valid[j]) sm[sbase + j * sstep] = g[j];
-      __syncthreads();
-#pragma unroll
-      for (int j = 0; j < NC; j++) {
-        if (!valid[j]) continue;
-        const double* c0 = sm + sbase + j * sstep;
-        const double d1 = c0[str] - c0[-str];
-        double e = d1;
-        if (wide) e = fma(8.0, d1, -(c0[2 * str] - c0[-2 * str]));
-        acc[j] = fma(wp, e, acc[j]);
-      }
-    }
-  }
-
-  // ---- -(p_s/m_s) dW/dq_s: same cell of the neighbouring bricks of the same element ----
-#pragma unroll
-  for (int s = 0; s < M; s++) {
-    const long long st = op.st[s];
-    const int i = iq[s], n = op.n[s];
-    const bool hp1 = i + 1 < n, hm1 = i >= 1, hp2 = wide && (i + 2 < n), hm2 = wide && (i >= 2);
-    const double wq = -(wide ? -op.c2[s] : op.c1[s]) * op.inv_mass[s];
-#pragma unroll
-    for (int j = 0; j < NC; j++) {
-      if (!valid[j]) continue;
-      const double* c0 = Xk + tid + j * nt;
-      const double fp1 = hp1 ? __ldg(c0 + st) : 0.0, fm1 = hm1 ? __ldg(c0 - st) : 0.0;
-      const double d1 = fp1 - fm1;
-      double e = d1;
-      if (wide) {
-        const double fp2 = hp2 ? __ldg(c0 + 2 * st) : 0.0, fm2 = hm2 ? __ldg(c0 - 2 * st) : 0.0;
-        e = fma(8.0, d1, -(fp2 - fm2));
-      }
-      const double ps = (s == 0) ? fma((double)j, p1step, pc[0]) : pc[s];
-      acc[j] = fma(wq * ps, e, acc[j]);
-    }
-  }
-
-  // ---- stage combine: out = a y + c F(in) ----
-  const size_t o0 = boff + (size_t)k * op.cells + brick + tid;
-#pragma unroll
-  for (int j = 0; j < NC; j++) {
-    if (!valid[j]) continue;
-    const size_t o = o0 + (size_t)j * nt;
-    const double yv = y_is_in ? xk[j] : y[o];
-    out[o] = fma(cc, acc[j], a * yv);
-  }
-}
 
 // ------------------------------------------------------------------------------------------------
 // Specialised M = 3 brick kernel with compile-time momentum extents (P1, P2, P3), 128-bit accesses.
@@ -438,25 +289,7 @@ constexpr int brick3_smem_bytes() {
   return (int)sizeof(double) * (P1 * (P2 + 4) * P3 + P1 * P2 * (P3 + 4) + (SPLIT > 1 ? SPLIT * 4 * P2 * P3 : 0));
 }
 
-template <int M, int NC, bool P1REG>
-cudaError_t configure_one(int smem_bytes) {
-  return cudaFuncSetAttribute(k_stage_brick<M, NC, P1REG>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-}
-
 }  // namespace
-
-#define BRICK_DISPATCH(M, NC, P1REG, CALL)                                         \
-  do {                                                                             \
-    if ((M) == 3) {                                                                \
-      if ((NC) == 8) { if (P1REG) { CALL(3, 8, true); } else { CALL(3, 8, false); } }        \
-      else if ((NC) == 16) { if (P1REG) { CALL(3, 16, true); } else { CALL(3, 16, false); } } \
-      else { CALL(3, 24, false); }                                                 \
-    } else {                                                                       \
-      if ((NC) == 8) { CALL(2, 8, false); }                                        \
-      else if ((NC) == 16) { CALL(2, 16, false); }                                 \
-      else { CALL(2, 24, false); }                                                 \
-    }                                                                              \
-  } while (0)
 
 #define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 2, 2) X(16, 16, 16, 2, 1) X(16, 16, 16, 4, 2) X(16, 16, 16, 4, 1) X(20, 20, 20, 2, 1) X(20, 20, 20, 4, 1) X(8, 8, 8, 1, 2) X(8, 8, 8, 2, 2) X(12, 12, 12, 2, 2) X(12, 12, 12, 3, 2)
 
@@ -469,40 +302,26 @@ int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {
 }
 
 int brick_configure(const BrickPlan& bp, int M) {
-  cudaError_t e = cudaSuccess;
-  if (bp.fixed) {
+  cudaError_t e = cudaErrorInvalidValue;
+  if (M != 3) return (int)e;
 #define X(A, B, C, S, MB)                                                                                 \
-    if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                         \
-      e = cudaFuncSetAttribute(k_stage_brick3<A, B, C, S, MB>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
-                               brick3_smem_bytes<A, B, C, S>());
-    BRICK3_SPECIALISATIONS(X)
+  if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                           \
+    e = cudaFuncSetAttribute(k_stage_brick3<A, B, C, S, MB>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                             brick3_smem_bytes<A, B, C, S>());
+  BRICK3_SPECIALISATIONS(X)
 #undef X
-    return (int)e;
-  }
-  const int bytes = bp.smem_doubles * (int)sizeof(double);
-#define CALL(MM, NN, PP) e = configure_one<MM, NN, PP>(bytes)
-  BRICK_DISPATCH(M, bp.nc, bp.p1reg, CALL);
-#undef CALL
   return (int)e;
 }
 
 int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out, double a,
                        double c, int nb, size_t slot_stride, cudaStream_t s) {
   dim3 grid((unsigned)((long long)op.K * op.nqc), nb);
-  const size_t smem = (size_t)bp.smem_doubles * sizeof(double);
   const int y_is_in = (y == in) ? 1 : 0;
-  if (bp.fixed) {
 #define X(A, B, C, S, MB)                                                                                  \
-    if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                          \
-      k_stage_brick3<A, B, C, S, MB><<<grid, S * B * C / 2, brick3_smem_bytes<A, B, C, S>(), s>>>(             \
-          op, bp, in, y, out, a, c, slot_stride, y_is_in, bp.zero_brick);
-    BRICK3_SPECIALISATIONS(X)
+  if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                            \
+    k_stage_brick3<A, B, C, S, MB><<<grid, S * B * C / 2, brick3_smem_bytes<A, B, C, S>(), s>>>(           \
+        op, bp, in, y, out, a, c, slot_stride, y_is_in, bp.zero_brick);
+  BRICK3_SPECIALISATIONS(X)
 #undef X
-    return 1;
-  }
-#define CALL(MM, NN, PP) \
-  k_stage_brick<MM, NN, PP><<<grid, bp.nt, smem, s>>>(op, bp, in, y, out, a, c, slot_stride, y_is_in)
-  BRICK_DISPATCH(op.M, bp.nc, bp.p1reg, CALL);
-#undef CALL
   return 1;
 }

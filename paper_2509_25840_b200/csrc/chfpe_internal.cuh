@@ -30,16 +30,10 @@ struct DevOp {
   const double* Gamma;                // [K] sum_s n_s gamma_s
 };
 
-// Launch plan of the brick kernels (chfpe_brick.cu): one CTA per (element, q-point) p-brick.
-// The brick is viewed as [P1][PB2] (PB2 = product of the trailing p-extents).  Thread t owns the cells
-// (i1_0 + j*m, r), j = 0..NC-1, with r = t % PB2 and i1_0 = t / PB2, so its trailing momenta are constants.
+// Launch plan of the brick kernels (chfpe_brick.cu, chfpe_pipe.cu): one CTA per (element, q-point) p-brick.
 struct BrickPlan {
   int enabled;
-  int nt, m, nc, p1reg;               // threads per CTA, p1-interleave, cells per thread (template), p1 line in registers
-  int P1, P2, P3, PB2;                // p-extents (P3 = 1 for M = 2)
-  int o1;                             // p1 padding of the shared brick (0 when p1reg)
-  int S1, S2;                         // shared-memory strides of i1 and i2 (padded)
-  int smem_doubles;
+  int P1, P2, P3, PB2;                // p-extents, PB2 = P2*P3
   int g;                              // elements per lock-step group (L2 window)
   int n_groups;
   long long blocks_per_full_group;    // g * nqc
@@ -49,8 +43,8 @@ struct BrickPlan {
   int l2mode;                         // bit 0: once-touched data evict_first, bit 1: window data evict_last
   int minb;                           // CTAs per SM the specialised kernel is compiled for (register budget)
   int split;                          // p_1 segments (thread groups) per brick in the specialised kernel
-  int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3>) exists
-  const double* zero_brick;           // pb zeros (device): stands in for bricks outside the grid
+  int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3,...>) exists
+  const double* zero_brick;           // pb zeros (device)
   int pipe;                           // use the plane-pipelined kernel (chfpe_pipe.cu)
   int pipe_stages, pipe_ctas;         // shared-memory stages per CTA, persistent CTAs in the grid
 };

@@ -43,6 +43,9 @@ SMALL = [
     ("m3_w_c2", ci.config("cfg4s8", nq=[6, 5, 7], np=[5, 7, 6], depth=2, gauge="w", scheme="central2",
                           mass=[1.0, 0.8, 1.2])),
     ("m3_cube8", ci.config("cfg4s8")),
+    ("m3_cube12", ci.config("cfg4s12", nq=[5, 6, 7])),
+    ("m3_cube16_w", ci.config("cfg4", nq=[5, 5, 6], gauge="w")),
+    ("m3_cube20_c2", ci.config("cfg5", nq=[5, 5, 5], depth=2, scheme="central2")),
 ]
 
 
@@ -174,7 +177,21 @@ def test_batched_step_equals_single():
     g.close()
 
 
-@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_pipelined_kernel_variant(monkeypatch):
+    """The plane-pipelined stage kernel (cp.async.bulk + mbarrier ring, CHFPE_PIPE=1) computes the same step."""
+    monkeypatch.setenv("CHFPE_PIPE", "1")
+    for cfg in (ci.config("cfg4s8"), ci.config("cfg4", nq=[5, 6, 5], depth=2)):
+        g, o = both(cfg)
+        levels = [sum(n) for n in o.elements()]
+        X = ci.seeded_state(cfg, levels, seed=4)
+        g.import_state(X); o.import_state(X)
+        assert rel_l2(g.export_rhs(), o.rhs(X)) < 1e-13
+        g.step(3, cfg["dt"]); o.step(3, cfg["dt"])
+        assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+        g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4", "cfg5"])
 def test_full_size_sampled_rhs_and_step_properties(name):
     """BASELINE configs 3 and 4 at full size, in the launch configuration bench.py times: sampled entries of the
     right-hand side against the oracle's point formula, plus size-independent properties of a step."""
