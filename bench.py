@@ -290,6 +290,48 @@ def run_ours(args):
     return 0
 
 
+def run_2d(args):
+    """Secondary metric of BASELINE.json: wall time of the 2D THz-Raman response R2(t2, t1) (configs[4]: 20^6 grid,
+    64 t1 x 256 t2 delays, t1 replicas batched into HBM).  Times chfpe_response_2d end to end (replica copies, kicks,
+    batched propagation, expectations, D2H of R) on a bounded sample of the delay grid and extrapolates linearly in
+    replica-steps to the full grid; says so."""
+    import numpy as np
+    import torch
+    import paper_2509_25840_b200 as P
+    wl = args.workload if args.workload != "cfg4" else "cfg5"
+    cfg = ci.config(wl)
+    M = cfg["n_modes"]
+    g = P.CHFPE(cfg, batch=args.batch)
+    mu, al = obs(P, "mu", M), obs(P, "alpha", M)
+    g.equilibrate(residual=False)
+    n1, n2 = args.n1, args.n2
+    t1, t2 = list(range(n1)), list(range(n2))
+    g.response_2d(mu, al, al, t1[:2], t2[:2], cfg["dt"])            # warm-up
+    g.equilibrate(residual=False)
+    n0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    R = g.response_2d(mu, al, al, t1, t2, cfg["dt"])
+    e1.record()
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    rsteps = (n1 - 1) + n1 * (n2 - 1)                               # trajectory steps + replica steps
+    full = 63 + 64 * 255
+    line = {"metric": "2D THz-Raman wall time", "value": sec * full / rsteps, "unit": "s", "higher_is_better": False,
+            "n_gpus": 1, "dtype": "f64", "data": "synthetic", "extrapolated": True,
+            "config": {"workload": wl + " response_2d", "grid": "x".join(str(x) for x in g.shape), "K": g.K,
+                       "batch_slots": args.batch, "workspace_GB": P.workspace_bytes(cfg, args.batch) / 1e9,
+                       "timed_sample": "%d t1 x %d t2 delays, stride 1, A=mu B=alpha C=alpha" % (n1, n2),
+                       "full_protocol": "64 t1 x 256 t2 (16383 replica-steps), linear extrapolation in replica-steps"},
+            "sample_seconds": sec, "replica_steps_timed": rsteps, "ms_per_replica_step": 1e3 * sec / rsteps,
+            "cell_updates_per_s": g.cells * rsteps / sec, "gpu_launches": int(g.launch_count() - n0),
+            "finite": bool(np.all(np.isfinite(R)))}
+    print(json.dumps(line))
+    g.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -298,9 +340,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--protocol", default="step", choices=["step", "2d"],
+                    help="'2d': time chfpe_response_2d on config 5 (secondary metric: 2D THz-Raman wall time)")
+    ap.add_argument("--batch", type=int, default=5, help="replica slots for --protocol 2d (trajectory + t1 replicas)")
+    ap.add_argument("--n1", type=int, default=8)
+    ap.add_argument("--n2", type=int, default=16)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.protocol == "2d":
+        return run_2d(args)
     return run_ours(args)
 
 

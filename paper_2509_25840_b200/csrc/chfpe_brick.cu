@@ -37,7 +37,7 @@ __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("pre
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double2 ldg2_hint(const double2* p, unsigned long long pol) {
   double2 v;
-  asm("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+  asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
   return v;
 }
 __device__ __forceinline__ double2 ld2_hint(const double2* p, unsigned long long pol) {

@@ -72,6 +72,8 @@ struct chfpe_handle {
   std::vector<int> elem;              // host copy [K][3]
   bool initialised;
   int64_t launches;
+  int coop_mode;                      // CHFPE_COOP: 0 off, 1 tiny states only, 2 every L2-resident state
+  bool coop;                          // persistent cooperative kernel allowed for L2-resident states
   bool prof;                          // bracket every stage launch with CUDA events (chfpe_profile_*)
   std::vector<cudaEvent_t> prof_ev;   // pairs (start, stop); prof_used of them are pending
   size_t prof_used;
@@ -86,6 +88,11 @@ struct chfpe_handle {
 // out = a*y + c*F(in) for slots [b0, b0+nb); slot stride = 3*state_doubles for all three pointers.
 int launch_stage(const DevOp& op, const double* in, const double* y, double* out, double a, double c,
                  int nb, size_t slot_stride, cudaStream_t s);
+// persistent cooperative kernel for L2-resident states (one replica): n_samples x (stride steps [+ <O> sample]);
+// returns 0 if a cooperative launch is not possible
+int launch_steps_coop(const DevOp& op, const DevObs& o, double* y, double* va, double* vb, double dt,
+                      long long n_samples, long long stride, int do_expect, double* partial, double* results,
+                      cudaStream_t s);
 // same operation by the brick kernel (chfpe_brick.cu); requires bp.enabled
 int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out,
                        double a, double c, int nb, size_t slot_stride, cudaStream_t s);

@@ -1,6 +1,7 @@
 // sm_100a kernels of the CHFPE hot path: RK stage (Liouvillian stencil + hierarchy couplings + stage combine),
 // kick, expectation reduction, equilibrium initialisation, layout conversion.
 // Equations: PAPER.md Eq. (8)-(12) :77-100, (15)-(18) :119-131; readings R1, R3, R7, R9-R13 of DESIGN.md.
+#include <cooperative_groups.h>
 #include "chfpe_internal.cuh"
 
 namespace {
@@ -29,9 +30,63 @@ __device__ __forceinline__ double dstencil(const double* __restrict__ f, long lo
   return d;
 }
 
+// Loads of the stage input: read-only path inside one-stage launches, L2-coherent (.cg) inside the persistent
+// multi-stage kernel, where other SMs have just written the array.
+template <bool COHERENT>
+__device__ __forceinline__ double ldx(const double* p) { return COHERENT ? __ldcg(p) : __ldg(p); }
+
+template <bool COHERENT>
+__device__ __forceinline__ double dstencil_x(const double* __restrict__ f, long long cell, long long st, int i, int n,
+                                             double c1, double c2, bool wide) {
+  double fp1 = (i + 1 < n) ? ldx<COHERENT>(f + cell + st) : 0.0;
+  double fm1 = (i >= 1) ? ldx<COHERENT>(f + cell - st) : 0.0;
+  double d = c1 * (fp1 - fm1);
+  if (wide) {
+    double fp2 = (i + 2 < n) ? ldx<COHERENT>(f + cell + 2 * st) : 0.0;
+    double fm2 = (i >= 2) ? ldx<COHERENT>(f + cell - 2 * st) : 0.0;
+    d = fma(c2, fp2 - fm2, d);
+  }
+  return d;
+}
+
+// F_k(X)(cell), right-hand side of Eq. (8) :77-80 for one (element, cell): Liouvillian Eq. (9)-(10), Phi Eq. (11),
+// n_s Theta Eq. (12) + R1, damping.  X points at element 0 of the replica.
+template <int M, bool COHERENT>
+__device__ __forceinline__ double rhs_value(const DevOp& op, const double* __restrict__ X, int k, long long cell) {
+  const double* Xk = X + (size_t)k * op.cells;
+  int idx[2 * M];
+  decode<2 * M>(op, cell, idx);
+  const long long ql = cell / op.pb;
+  const bool wide = (op.scheme == CHFPE_CENTRAL4);
+  double acc = -__ldg(op.Gamma + k) * ldx<COHERENT>(Xk + cell);
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const int aq = s, ap = M + s;
+    const double q = op.x0[aq] + idx[aq] * op.h[aq];
+    const double p = op.x0[ap] + idx[ap] * op.h[ap];
+    const double dq = dstencil_x<COHERENT>(Xk, cell, op.st[aq], idx[aq], op.n[aq], op.c1[aq], op.c2[aq], wide);
+    const double dp = dstencil_x<COHERENT>(Xk, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
+    acc = fma(-(p * op.inv_mass[s]), dq, acc);                      // -(p_s/m_s) dW/dq_s
+    acc = fma(__ldg(op.dU[s] + ql), dp, acc);                       // +(dU/dq_s) dW/dp_s
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+    if (ku >= 0) {                                                  // Phi_s W^(n+e_s)
+      const double* Xu = X + (size_t)ku * op.cells;
+      double d = dstencil_x<COHERENT>(Xu, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
+      acc = fma(Vp, fma(op.kup[s] * p, ldx<COHERENT>(Xu + cell), d), acc);
+    }
+    if (kd >= 0) {                                                  // n_s Theta_s W^(n-e_s)
+      const double* Xd = X + (size_t)kd * op.cells;
+      double d = dstencil_x<COHERENT>(Xd, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
+      acc = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp, fma(op.kdn[s] * p, ldx<COHERENT>(Xd + cell), d), acc);
+    }
+  }
+  return acc;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Generic RK stage: out = a*y + c*F(in), one thread per (cell, element, slot).  Correct for every M, grid
-// and explicit scheme; the brick kernels below replace it where they apply.
+// and explicit scheme; the brick kernels replace it where they apply.
 // ------------------------------------------------------------------------------------------------
 template <int M>
 __global__ void __launch_bounds__(256) k_stage_generic(DevOp op, const double* __restrict__ in,
@@ -41,35 +96,7 @@ __global__ void __launch_bounds__(256) k_stage_generic(DevOp op, const double* _
   if (cell >= op.cells) return;
   const int k = blockIdx.y;
   const size_t boff = (size_t)blockIdx.z * slot_stride;
-  const double* X = in + boff;
-  const double* Xk = X + (size_t)k * op.cells;
-  int idx[2 * M];
-  decode<2 * M>(op, cell, idx);
-  const long long ql = cell / op.pb;
-  const bool wide = (op.scheme == CHFPE_CENTRAL4);
-  double acc = -__ldg(op.Gamma + k) * __ldg(Xk + cell);
-#pragma unroll
-  for (int s = 0; s < M; s++) {
-    const int aq = s, ap = M + s;
-    const double q = op.x0[aq] + idx[aq] * op.h[aq];
-    const double p = op.x0[ap] + idx[ap] * op.h[ap];
-    const double dq = dstencil(Xk, cell, op.st[aq], idx[aq], op.n[aq], op.c1[aq], op.c2[aq], wide);
-    const double dp = dstencil(Xk, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
-    acc = fma(-(p * op.inv_mass[s]), dq, acc);                      // -(p_s/m_s) dW/dq_s
-    acc = fma(__ldg(op.dU[s] + ql), dp, acc);                       // +(dU/dq_s) dW/dp_s
-    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
-    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
-    if (ku >= 0) {                                                  // Phi_s W^(n+e_s)
-      const double* Xu = X + (size_t)ku * op.cells;
-      double d = dstencil(Xu, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
-      acc = fma(Vp, fma(op.kup[s] * p, __ldg(Xu + cell), d), acc);
-    }
-    if (kd >= 0) {                                                  // n_s Theta_s W^(n-e_s)
-      const double* Xd = X + (size_t)kd * op.cells;
-      double d = dstencil(Xd, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
-      acc = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp, fma(op.kdn[s] * p, __ldg(Xd + cell), d), acc);
-    }
-  }
+  const double acc = rhs_value<M, false>(op, in + boff, k, cell);
   const size_t o = boff + (size_t)k * op.cells + cell;
   out[o] = fma(c, acc, a * y[o]);
 }
@@ -123,6 +150,28 @@ __device__ __forceinline__ double block_sum_256(double v) {
   return r;   // valid in thread 0
 }
 
+// O(q,p) * w(q,p) at one cell: observable polynomial Eq. (13)-(14) times the gauge weight (1 or phi = e^{-beta H/2})
+template <int M>
+__device__ __forceinline__ double expect_weight(const DevOp& op, const DevObs& ob, long long cell) {
+  int idx[2 * M];
+  decode<2 * M>(op, cell, idx);
+  double O = ob.c0, w = 1.0;
+  double q[M];
+#pragma unroll
+  for (int s = 0; s < M; s++) q[s] = op.x0[s] + idx[s] * op.h[s];
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const double p = op.x0[M + s] + idx[M + s] * op.h[M + s];
+    O = fma(ob.lin_q[s], q[s], O);
+    O = fma(ob.lin_p[s], p, O);
+#pragma unroll
+    for (int r = 0; r < M; r++) O = fma(0.5 * ob.quad[s][r] * q[s], q[r], O);
+    if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.ep[s] + idx[M + s]);
+  }
+  if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.eU + cell / op.pb);
+  return O * w;
+}
+
 template <int M>
 __global__ void __launch_bounds__(256) k_reduce_partial(DevOp op, DevObs ob, int mode, const double* __restrict__ x,
                                                         long long elem_off, long long ncells, size_t slot_stride,
@@ -137,23 +186,7 @@ __global__ void __launch_bounds__(256) k_reduce_partial(DevOp op, DevObs ob, int
     const double v = X[c];
     if (mode == RED_SUMSQ) { acc = fma(v, v, acc); continue; }
     if (mode == RED_SUM) { acc += v; continue; }
-    int idx[2 * M];
-    decode<2 * M>(op, c % op.cells, idx);
-    double O = ob.c0, w = 1.0;
-    double q[M];
-#pragma unroll
-    for (int s = 0; s < M; s++) q[s] = op.x0[s] + idx[s] * op.h[s];
-#pragma unroll
-    for (int s = 0; s < M; s++) {
-      const double p = op.x0[M + s] + idx[M + s] * op.h[M + s];
-      O = fma(ob.lin_q[s], q[s], O);
-      O = fma(ob.lin_p[s], p, O);
-#pragma unroll
-      for (int r = 0; r < M; r++) O = fma(0.5 * ob.quad[s][r] * q[s], q[r], O);
-      if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.ep[s] + idx[M + s]);
-    }
-    if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.eU + (c % op.cells) / op.pb);
-    acc = fma(O * w, v, acc);
+    acc = fma(expect_weight<M>(op, ob, c % op.cells), v, acc);
   }
   const double r = block_sum_256(acc);
   if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = r;
@@ -207,6 +240,55 @@ __global__ void __launch_bounds__(256) k_permute(DevOp op, const double* __restr
   const size_t e = (size_t)blockIdx.y * op.cells;
   if (to_internal) dst[e + cell] = src[e + canon];
   else dst[e + canon] = src[e + cell];
+}
+
+// ------------------------------------------------------------------------------------------------
+// Persistent multi-step kernel for states that live in L2 (configs 1-2 and small grids): all four RK stages of
+// `stride` steps and, optionally, one expectation sample per `stride` steps in ONE cooperative launch; stages are
+// separated by grid-wide barriers instead of kernel boundaries (6 launches of ~9 us per step otherwise).
+// ------------------------------------------------------------------------------------------------
+template <int M>
+__device__ __forceinline__ void coop_stage(const DevOp& op, const double* in, const double* y, double* out, double c,
+                                           long long total) {
+  for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < total; v += (long long)gridDim.x * blockDim.x) {
+    const int k = (int)(v / op.cells);
+    const long long cell = v - (long long)k * op.cells;
+    const double acc = rhs_value<M, true>(op, in, k, cell);
+    out[v] = fma(c, acc, __ldcg(y + v));
+  }
+}
+
+template <int M>
+__global__ void __launch_bounds__(256) k_steps_coop(DevOp op, DevObs ob, double* y, double* va, double* vb, double dt,
+                                                    long long n_samples, long long stride, int do_expect,
+                                                    double* partial, double* results) {
+  namespace cg = cooperative_groups;
+  cg::grid_group grid = cg::this_grid();
+  const long long total = (long long)op.K * op.cells;
+  for (long long smp = 0; smp < n_samples; smp++) {
+    for (long long st = 0; st < stride; st++) {                    // Horner form of RK4 (R13)
+      coop_stage<M>(op, y, y, va, dt / 4.0, total);  grid.sync();
+      coop_stage<M>(op, va, y, vb, dt / 3.0, total); grid.sync();
+      coop_stage<M>(op, vb, y, va, dt / 2.0, total); grid.sync();
+      coop_stage<M>(op, va, y, y, dt, total);        grid.sync();
+    }
+    if (do_expect) {                                               // <O> on element 0, fixed summation order
+      const long long per = (op.cells + gridDim.x - 1) / gridDim.x;
+      const long long lo = (long long)blockIdx.x * per;
+      long long hi = lo + per; if (hi > op.cells) hi = op.cells;
+      double acc = 0.0;
+      for (long long c = lo + threadIdx.x; c < hi; c += 256) acc = fma(expect_weight<M>(op, ob, c), __ldcg(y + c), acc);
+      const double r = block_sum_256(acc);
+      if (threadIdx.x == 0) partial[blockIdx.x] = r;
+      grid.sync();
+      if (blockIdx.x == 0) {
+        double a2 = 0.0;
+        for (int i = threadIdx.x; i < (int)gridDim.x; i += 256) a2 += __ldcg(partial + i);
+        const double r2 = block_sum_256(a2);
+        if (threadIdx.x == 0) results[smp] = r2 * op.dV;
+      }
+    }
+  }
 }
 
 }  // namespace
@@ -268,5 +350,33 @@ int launch_permute(const DevOp& op, const double* src, double* dst, int to_inter
 #define CALL(MM) k_permute<MM><<<grid, 256, 0, s>>>(op, src, dst, to_internal)
   DISPATCH_M(op.M, CALL);
 #undef CALL
+  return 1;
+}
+
+// n_samples x (stride RK4 steps [+ one expectation sample]) on ONE replica in one cooperative launch.  Returns the
+// number of launches (1) or 0 when the device cannot co-schedule the grid (the caller then uses per-stage launches).
+int launch_steps_coop(const DevOp& op, const DevObs& o, double* y, double* va, double* vb, double dt,
+                      long long n_samples, long long stride, int do_expect, double* partial, double* results,
+                      cudaStream_t s) {
+  int dev = 0, coop = 0, sms = 0, per_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (!coop) return 0;
+  const void* fn = nullptr;
+  if (op.M == 1) fn = (const void*)k_steps_coop<1>;
+  else if (op.M == 2) fn = (const void*)k_steps_coop<2>;
+  else fn = (const void*)k_steps_coop<3>;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, 256, 0) != cudaSuccess || per_sm < 1) return 0;
+  if (per_sm > 8) per_sm = 8;
+  const long long total = (long long)op.K * op.cells;
+  long long blocks = (total + 255) / 256;
+  if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
+  DevOp opv = op; DevObs ov = o;
+  void* args[] = {&opv, &ov, &y, &va, &vb, &dt, &n_samples, &stride, &do_expect, &partial, &results};
+  if (cudaLaunchCooperativeKernel(fn, dim3((unsigned)blocks), dim3(256), args, 0, s) != cudaSuccess) {
+    cudaGetLastError();
+    return 0;
+  }
   return 1;
 }

@@ -177,6 +177,25 @@ def test_batched_step_equals_single():
     g.close()
 
 
+@pytest.mark.parametrize("coop", ["0", "2"])
+def test_cooperative_and_per_stage_paths_agree(monkeypatch, coop):
+    """Persistent cooperative multi-step kernel (CHFPE_COOP=2: every L2-resident state) vs per-stage launches
+    (CHFPE_COOP=0): both against the oracle, M = 1, 2, 3."""
+    monkeypatch.setenv("CHFPE_COOP", coop)
+    for cfg in (ci.config("cfg2", nq=[37], np=[41], depth=5), ci.config("cfg3s", nq=[9, 10], np=[11, 8], depth=2),
+                ci.config("cfg4s8", nq=[6, 5, 7], np=[8, 8, 8], depth=2)):
+        g, o = both(cfg)
+        M = cfg["n_modes"]
+        mu_g, mu_o = obs_pair("mu_nl", M)
+        g.equilibrate(); o.equilibrate()
+        Rg = g.response_1d(mu_g, mu_g, 7, 3, cfg["dt"])
+        Ro = o.response_1d(mu_o, mu_o, 7, 3, cfg["dt"])
+        assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+        assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+        assert (g.launch_count() < 40) if coop == "2" else (g.launch_count() > 60)
+        g.close()
+
+
 def test_pipelined_kernel_variant(monkeypatch):
     """The plane-pipelined stage kernel (cp.async.bulk + mbarrier ring, CHFPE_PIPE=1) computes the same step."""
     monkeypatch.setenv("CHFPE_PIPE", "1")
