@@ -119,25 +119,40 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   if (M != 3 || d->scheme == CHFPE_COMPACT6 || !env_int("CHFPE_BRICK", 1)) return bp;
   bp.P1 = d->np[0]; bp.P2 = d->np[1]; bp.P3 = d->np[2];
   bp.PB2 = bp.P2 * bp.P3;
-  // threads per CTA = split * P2*P3/2 (128-bit accesses); aim at 256 threads with 16 cells each
+  // threads per CTA = split * P2*P3/2 (128-bit accesses); aim at ~512 threads (one CTA per SM at 128 registers)
+  // with >= 4 planes per thread: at 16^3 the 256-thread / 2-CTA variant times the same but its register allocation
+  // sits on the spill edge (a few more live scalars cost 15 %)
   int split_default = 1;
   while (split_default < bp.P1 && bp.P1 % (2 * split_default) == 0 && bp.P1 / (2 * split_default) >= 4 &&
-         split_default * bp.PB2 / 2 < 256)
+         split_default * bp.PB2 / 2 < 384)
     split_default *= 2;
   if (bp.P1 == 12) split_default = 2;
   bp.split = env_int("CHFPE_BRICK_SPLIT", split_default);
   bp.minb = env_int("CHFPE_BRICK_MINB", (bp.PB2 * bp.split / 2 <= 256) ? 2 : 1);
   bp.fixed = brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb);
   if (!bp.fixed) return bp;
-  // group size: five q_1 planes of g elements should stay L2-resident (126 MB on B200, shared with the once-touched
-  // streams; budget 60 MB)
+  // L2 reuse window = five q_1 planes x (q_2 chunk + 2+2 halo rows) x g elements of the stage input; budget 64 MiB
+  // of the 126 MB L2 (the rest serves the once-touched streams).  Pairs of linked elements (g = 2) save one
+  // neighbour-brick read per pair if at least 6 q_2 rows per chunk still fit, else one element at a time.
   const double plane_bytes = 8.0 * (double)pl.cells / d->nq[0];
-  int g = (int)(60.0e6 / (5.0 * plane_bytes));
-  if (g < 1) g = 1;
-  if (g > K) g = K;
+  const double row_bytes = plane_bytes / d->nq[1];                 // one q_2 row of one q_1 plane
+  const double budget = 64.0 * 1024 * 1024;
+  auto rows_that_fit = [&](int gg) { return (int)(budget / (5.0 * row_bytes * gg)) - 4; };
+  int g = (K >= 2 && rows_that_fit(2) >= 6) ? 2 : 1;
   g = env_int("CHFPE_GROUP", g);
   if (g < 1) g = 1;
   if (g > K) g = K;
+  int cs = rows_that_fit(g);
+  if (cs >= d->nq[1]) cs = d->nq[1];
+  else {
+    if (cs < 4) cs = 4;
+    const int nch = (d->nq[1] + cs - 1) / cs;                      // equalise the chunks
+    cs = (d->nq[1] + nch - 1) / nch;
+  }
+  cs = env_int("CHFPE_Q2CHUNK", cs);
+  if (cs < 1) cs = 1;
+  if (cs > d->nq[1]) cs = d->nq[1];
+  bp.q2chunk = cs;
   // greedy grouping: grow each group by the unassigned element with most hierarchy links into it
   std::vector<int> assigned(K, 0), order;
   for (int k0 = 0; k0 < K; k0++) {

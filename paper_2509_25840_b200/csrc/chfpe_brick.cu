@@ -67,23 +67,10 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const int jbase = seg * NC;                                       // first p_1 plane of this thread
   const int i2 = tid / (P3 / 2), i3 = 2 * (tid - i2 * (P3 / 2));
 
-  long long L = blockIdx.x;
-  const int G = (int)(L / bp.blocks_per_full_group);
-  L -= (long long)G * bp.blocks_per_full_group;
-  int gs = op.K - G * bp.g;
-  if (gs > bp.g) gs = bp.g;
-  const long long per_plane = (long long)gs * bp.rest;
-  const int iq1 = (int)(L / per_plane);
-  const long long r2 = L - (long long)iq1 * per_plane;
-  const int kk = (int)(r2 / bp.rest);
-  const long long ql = (long long)iq1 * bp.rest + (r2 - (long long)kk * bp.rest);
-  const int k = __ldg(bp.order + G * bp.g + kk);
-  int iq[3];
-  {
-    long long t = ql;
-#pragma unroll
-    for (int s = 2; s >= 0; s--) { long long u = t / op.n[s]; iq[s] = (int)(t - u * op.n[s]); t = u; }
-  }
+  const BrickId bid = decode_brick_id(op, bp, blockIdx.x);
+  const int k = bid.k, G = bid.G;
+  const long long ql = bid.ql;
+  const int iq[3] = {bid.iq[0], bid.iq[1], bid.iq[2]};
   const size_t boff = (size_t)blockIdx.y * slot_stride;
   const double* X = in + boff;
   const size_t brick = (size_t)ql * (P1 * PLANE);

@@ -73,19 +73,9 @@ __device__ __forceinline__ BrickInfo decode_brick(const DevOp& op, const BrickPl
   const long long per_slot = (long long)op.K * op.nqc;
   const long long slot = Lt / per_slot;
   long long L = Lt - slot * per_slot;
-  b.G = (int)(L / bp.blocks_per_full_group);
-  L -= (long long)b.G * bp.blocks_per_full_group;
-  int gs = op.K - b.G * bp.g;
-  if (gs > bp.g) gs = bp.g;
-  const long long per_plane = (long long)gs * bp.rest;
-  const int iq1 = (int)(L / per_plane);
-  const long long r2 = L - (long long)iq1 * per_plane;
-  const int kk = (int)(r2 / bp.rest);
-  b.ql = (long long)iq1 * bp.rest + (r2 - (long long)kk * bp.rest);
-  b.k = __ldg(bp.order + b.G * bp.g + kk);
-  long long t = b.ql;
-#pragma unroll
-  for (int s = 2; s >= 0; s--) { long long u = t / op.n[s]; b.iq[s] = (int)(t - u * op.n[s]); t = u; }
+  const BrickId id = decode_brick_id(op, bp, L);
+  b.G = id.G; b.k = id.k; b.ql = id.ql;
+  b.iq[0] = id.iq[0]; b.iq[1] = id.iq[1]; b.iq[2] = id.iq[2];
   b.elem_off = (size_t)b.k * op.cells + (size_t)b.ql * op.pb;
   b.slot_off = (size_t)slot * slot_stride;
   return b;
