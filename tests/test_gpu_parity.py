@@ -269,3 +269,58 @@ def test_error_paths():
     with pytest.raises(P.ChfpeError):
         g.response_2d(mu_g, mu_g, mu_g, [3, 1], [0], 1e-3)   # unsorted t1
     g.close()
+
+
+def test_degenerate_and_edge_cases():
+    """Depth 0 (one element, no hierarchy links), minimum 5-point axes, zeta = 0, zero steps, zero stride,
+    repeated delays, more replica slots than t1 rows, n_samples = 0."""
+    mu1_g, mu1_o = obs_pair("mu", 1)
+    # depth 0 on a 5 x 5 grid: pure Liouvillian, K = 1
+    cfg = ci.config("cfg1", nq=[5], np=[5], depth=0)
+    g, o = both(cfg)
+    assert g.K == 1
+    X = ci.seeded_state(cfg, [0], seed=2)
+    g.import_state(X); o.import_state(X)
+    assert rel_l2(g.export_rhs(), o.rhs(X)) < 1e-13
+    g.step(0, cfg["dt"])                                       # no-op
+    assert np.array_equal(g.export_state(), X)
+    g.step(5, cfg["dt"]); o.step(5, cfg["dt"])
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+    assert g.response_1d(mu1_g, mu1_g, 0, 1, cfg["dt"]).size == 0
+    g.close()
+    # zeta = 0: the hierarchy decouples downwards (rigid rotation, pin P5), stride 0 repeats the same sample
+    cfg = ci.config("cfg1", nq=[21], np=[23], depth=2, zeta=[0.0])
+    g, o = both(cfg)
+    g.equilibrate(); o.equilibrate()
+    p_g, p_o = (m.make_observable(0.0, [0.0], [[0.0]], [1.0]) for m in (gpu_mod(), oracle))   # C = p: <p>(0+) = -1
+    Rg = g.response_1d(mu1_g, p_g, 4, 0, cfg["dt"])
+    Ro = o.response_1d(mu1_o, p_o, 4, 0, cfg["dt"])
+    assert abs(Ro[0] + 1.0) < 5e-3                              # h^4 error of the 21 x 23 grid
+    assert np.allclose(Rg, Rg[0], rtol=1e-13, atol=0) and np.max(np.abs(Rg - Ro)) <= 1e-12
+    g.close()
+    # 2D: repeated t1 / t2 entries, batch larger than the number of rows
+    cfg = ci.config("cfg3s", nq=[6, 7], np=[7, 6], depth=2)
+    g, o = both(cfg, batch=4)
+    mu_g, mu_o = obs_pair("mu", 2)
+    al_g, al_o = obs_pair("alpha", 2)
+    g.equilibrate(); o.equilibrate()
+    t1, t2 = [0, 0, 2], [0, 3, 3, 5]
+    Rg = g.response_2d(mu_g, al_g, mu_g, t1, t2, 10 * cfg["dt"])
+    Ro = o.response_2d(mu_o, al_o, mu_o, t1, t2, 10 * cfg["dt"])
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    assert np.array_equal(Rg[0], Rg[1]) and np.array_equal(Rg[:, 1], Rg[:, 2])
+    g.close()
+
+
+def test_two_dimensional_closed_form_on_gpu():
+    """Pin P4 on the CUDA path itself: harmonic + LL, A = C = q, B = q^2 in the W gauge:
+    R2_lib(t2, t1) = 2 R_phys(t1) R_phys(t2) (tests/golden/r2_closed_form.txt)."""
+    cfg = ci.config("cfg1", nq=[48], np=[48], depth=4, gauge="w")
+    P = gpu_mod()
+    g = P.CHFPE(cfg, batch=2)
+    q = P.make_observable(0.0, [1.0], [[0.0]], [0.0])
+    q2 = P.make_observable(0.0, [0.0], [[2.0]], [0.0])
+    g.equilibrate()
+    R = g.response_2d(q, q2, q, [800], [1200], 1e-3)
+    assert abs(R[0, 0] - 1.153396427) < 2e-6
+    g.close()
