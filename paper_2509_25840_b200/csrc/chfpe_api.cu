@@ -1,6 +1,7 @@
 // Host side of the C-ABI (include/chfpe.h): validation, setup tables (step a0), workspace carving and the
 // drivers that sequence kernel launches (equilibrate a6, step a1-a3, kick a4, expect a5, R1 a7, R2 a8).
 // No arithmetic of the method runs on the host beyond the one-off tables of `create`.
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -91,6 +92,7 @@ static Plan make_plan(const chfpe_desc* d) {
   tb += align256(sizeof(double) * p.K);                        // Gamma
   tb += align256(sizeof(int) * p.K) * 2;                       // brick-kernel element order and its inverse
   tb += align256(sizeof(double) * (p.cells / p.nqc));          // brick of zeros (ghost bricks)
+  tb += align256(sizeof(int) * 4 * (size_t)p.K * p.nqc);       // brick-order table of the three-mode kernels
   p.tables_bytes = tb; o += tb;
   p.off_partial = o; o += align256(sizeof(double) * p.red_blocks * (size_t)p.batch);
   p.off_results = o; o += align256(sizeof(double) * Plan::RESULTS);
@@ -117,6 +119,7 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   for (int k = 0; k < K; k++) (*order_out)[k] = k;
   bp.g = 1; bp.n_groups = K;
   if (M != 3 || d->scheme == CHFPE_COMPACT6 || !env_int("CHFPE_BRICK", 1)) return bp;
+  if (d->nq[0] > 1023 || d->nq[1] > 1023 || d->nq[2] > 1023 || (long long)pl.K * pl.nqc > 0x7fffffffLL) return bp;
   bp.P1 = d->np[0]; bp.P2 = d->np[1]; bp.P3 = d->np[2];
   bp.PB2 = bp.P2 * bp.P3;
   // threads per CTA = split * P2*P3/2 (128-bit accesses); aim at ~512 threads (one CTA per SM at 128 registers)
@@ -314,6 +317,38 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   for (size_t i = 0; i < order.size(); i++) pos[order[i]] = (int)i;
   h->bp.pos = (const int*)put(pos.data(), sizeof(int) * pos.size());
   h->bp.l2mode = env_int("CHFPE_L2MODE", 1);
+  if (h->bp.enabled) {                                                 // tabulate the brick order (decode_brick_id)
+    const BrickPlan& b = h->bp;
+    const int n1 = desc->nq[0], n2 = desc->nq[1], n3 = desc->nq[2], cs = b.q2chunk;
+    const int nch = (n2 + cs - 1) / cs;
+    std::vector<int> tab;
+    tab.reserve((size_t)4 * pl.K * pl.nqc);
+    for (int G = 0; G < b.n_groups; G++) {
+      const int gs = std::min(b.g, pl.K - G * b.g);
+      for (int ch = 0; ch < nch; ch++) {
+        const int w = std::min(cs, n2 - ch * cs);
+        for (int i1 = 0; i1 < n1; i1++)
+          for (int kk = 0; kk < gs; kk++) {
+            const int k = order[G * b.g + kk];
+            int own = 0;
+            for (int s = 0; s < 3; s++) {
+              if (up[3 * k + s] >= 0 && pos[up[3 * k + s]] / b.g == G) own |= 1 << (2 * s);
+              if (dn[3 * k + s] >= 0 && pos[dn[3 * k + s]] / b.g == G) own |= 1 << (2 * s + 1);
+            }
+            for (int r2 = 0; r2 < w; r2++)
+              for (int i3 = 0; i3 < n3; i3++) {
+                const int i2 = ch * cs + r2;
+                tab.push_back(k);
+                tab.push_back((i1 * n2 + i2) * n3 + i3);
+                tab.push_back(i1 | (i2 << 10) | (i3 << 20));
+                tab.push_back(G | (own << 16));
+              }
+          }
+      }
+    }
+    h->bp.table = (const int4*)put(tab.data(), sizeof(int) * tab.size());
+    cudaStreamSynchronize(h->stream);                                  // `tab` goes out of scope
+  }
   {
     std::vector<double> zeros((size_t)(pl.cells / pl.nqc), 0.0);
     h->bp.zero_brick = (const double*)put(zeros.data(), sizeof(double) * zeros.size());

@@ -9,6 +9,7 @@
 // of the same cell of the 12 neighbouring bricks of the same element, which the L2 serves (CTAs are ordered q_1-plane
 // by q_1-plane, element group by group).  One CTA = one brick.  Grids without a compile-time specialisation run the
 // generic kernel of chfpe_kernels.cu (a run-time-shaped brick kernel was measured slower than it and removed).
+#include <type_traits>
 #include "chfpe_internal.cuh"
 
 namespace {
@@ -28,27 +29,40 @@ __device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("pre
 // ------------------------------------------------------------------------------------------------
 // Specialised M = 3 brick kernel with compile-time momentum extents (P1, P2, P3), 128-bit accesses.
 // A thread owns a PAIR of cells adjacent along p_3 (one double2) on NC = P1/SPLIT consecutive p_1 planes; the SPLIT
-// thread groups of a CTA share one brick.  On B200 a 16-byte-per-lane load moves twice the bytes of an 8-byte one
-// per outstanding request, and the L2->SM rate of this kernel is set by the requests in flight (measured: 11 vs
-// 20 TB/s at 16 warps per SM).  The p_1 stencil of G_1 runs in registers in scatter form (each G_1 value is added
-// to its four neighbours' accumulators as soon as it is formed; segment edges are exchanged through shared memory);
-// G_2 and G_3 go to two shared arrays padded along their own axis only, so one __syncthreads per brick suffices.
-// Absent q-neighbours (zero ghosts, R9) are redirected to a brick of zeros, which keeps every load unpredicated.
+// thread groups of a CTA share one brick.  The p_1 stencil of G_1 runs in registers in scatter form (each G_1 value
+// is added to its four neighbours' accumulators as soon as it is formed; segment edges are exchanged through shared
+// memory); G_2 and G_3 go to two shared arrays padded along their own axis only, so one __syncthreads per brick
+// suffices.  The kernel is latency-bound at 16 warps per SM, so its time follows its instruction count: every load
+// is "one 64-bit base per brick and direction + compile-time byte offset", the brick decode is 32-bit, and ghost
+// bricks (R9) are handled by CTA-uniform branches (an all-interior fast path per q axis), not by selects.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double2 ldg2_hint(const double2* p, unsigned long long pol) {
+template <int OFF>   // OFF in double2 units, folded into the instruction as an immediate byte offset
+__device__ __forceinline__ double2 ldg2o(const double2* base, unsigned long long pol) {
   double2 v;
-  asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+  asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2+%4], %3;"
+      : "=d"(v.x), "=d"(v.y) : "l"(base), "l"(pol), "n"(OFF * 16));
   return v;
 }
-__device__ __forceinline__ double2 ld2_hint(const double2* p, unsigned long long pol) {
+template <int OFF>
+__device__ __forceinline__ double2 ld2o(const double2* base, unsigned long long pol) {   // may alias the output
   double2 v;
-  asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
+  asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2+%4], %3;"
+               : "=d"(v.x), "=d"(v.y) : "l"(base), "l"(pol), "n"(OFF * 16) : "memory");
   return v;
 }
-__device__ __forceinline__ void st2_hint(double2* p, double2 v, unsigned long long pol) {
-  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+template <int OFF>
+__device__ __forceinline__ void st2o(double2* base, double2 v, unsigned long long pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0+%4], {%1, %2}, %3;" ::"l"(base), "d"(v.x), "d"(v.y), "l"(pol), "n"(OFF * 16) : "memory");
 }
 __device__ __forceinline__ double2 fma2(double c, double2 a, double2 b) { return make_double2(fma(c, a.x, b.x), fma(c, a.y, b.y)); }
+
+// compile-time loop helpers (the load offsets must be template arguments)
+template <int J, int N> struct Unroll {
+  template <typename F> __device__ __forceinline__ static void run(F&& f) { f(std::integral_constant<int, J>()); Unroll<J + 1, N>::run(f); }
+};
+template <int N> struct Unroll<N, N> {
+  template <typename F> __device__ __forceinline__ static void run(F&&) {}
+};
 
 template <int P1, int P2, int P3, int SPLIT, int MINB>
 __global__ void __launch_bounds__(SPLIT * P2 * P3 / 2, MINB)
@@ -67,16 +81,17 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const int jbase = seg * NC;                                       // first p_1 plane of this thread
   const int i2 = tid / (P3 / 2), i3 = 2 * (tid - i2 * (P3 / 2));
 
+  // ---- brick of this CTA (32-bit arithmetic: at most K * n_q < 2^31 bricks) ----
   const BrickId bid = decode_brick_id(op, bp, blockIdx.x);
-  const int k = bid.k, G = bid.G;
-  const long long ql = bid.ql;
-  const int iq[3] = {bid.iq[0], bid.iq[1], bid.iq[2]};
+  const int k = bid.k;
+  const unsigned ql = (unsigned)bid.ql;
   const size_t boff = (size_t)blockIdx.y * slot_stride;
-  const double* X = in + boff;
-  const size_t brick = (size_t)ql * (P1 * PLANE);
-  const size_t toff = (size_t)jbase * PLANE + 2 * tid;              // this thread's first cell inside the brick
-  const double2* Xk = reinterpret_cast<const double2*>(X + (size_t)k * op.cells + brick + toff);
-  const double2* zb = reinterpret_cast<const double2*>(zero_brick + toff);
+  const double2* X2 = reinterpret_cast<const double2*>(in + boff);  // replica base
+  const unsigned cells2 = (unsigned)(op.cells >> 1);                // element stride in double2
+  const unsigned tpart = (unsigned)(jbase * PL2 + tid);             // this thread's first pair inside a brick
+  const unsigned brick2 = ql * (unsigned)(P1 * PL2);                // brick offset inside an element
+  const double2* Xk = X2 + ((size_t)k * cells2 + brick2 + tpart);   // own pairs: Xk[j * PL2]
+  (void)zero_brick;
 
   // zero the ghost rows / columns of the two shared bricks
   for (int i = threadIdx.x; i < P1 * 4 * P3; i += NTT) {            // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
@@ -95,21 +110,23 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const double p2 = op.x0[4] + i2 * op.h[4];
   const double p3a = op.x0[5] + i3 * op.h[5], p3b = op.x0[5] + (i3 + 1) * op.h[5];
   const double Gam = __ldg(op.Gamma + k);
+  int kup[3], kdn[3];
+#pragma unroll
+  for (int s = 0; s < 3; s++) { kup[s] = __ldg(op.up + 3 * k + s); kdn[s] = __ldg(op.dn + 3 * k + s); }
 
   // Everything this brick needs from HBM (its own stage input, the bricks of its hierarchy neighbours, y) is
-  // requested into L2 now -- one 128-byte line per thread and array -- and consumed after the q-derivative part,
-  // whose loads are L2 hits on the q_1-plane window and take long enough to cover the DRAM latency.
+  // requested into L2 now -- one 128-byte line per thread and array -- and consumed after the q-derivative part.
   {
     constexpr int LINES = P1 * PLANE / 16;                          // 128-byte lines per brick
-    const size_t e0 = (size_t)k * op.cells + brick;
+    const double* Xd = in + boff;
+    const size_t e0 = (size_t)k * op.cells + (size_t)ql * (P1 * PLANE);
     for (int l = threadIdx.x; l < LINES; l += NTT) {
-      prefetch_l2(X + e0 + 16 * l);
+      prefetch_l2(Xd + e0 + 16 * l);
       if (!y_is_in) prefetch_l2(y + boff + e0 + 16 * l);
 #pragma unroll
       for (int s = 0; s < 3; s++) {
-        const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
-        if (ku >= 0) prefetch_l2(X + (size_t)ku * op.cells + brick + 16 * l);
-        if (kd >= 0) prefetch_l2(X + (size_t)kd * op.cells + brick + 16 * l);
+        if (kup[s] >= 0) prefetch_l2(Xd + (size_t)kup[s] * op.cells + (size_t)ql * (P1 * PLANE) + 16 * l);
+        if (kdn[s] >= 0) prefetch_l2(Xd + (size_t)kdn[s] * op.cells + (size_t)ql * (P1 * PLANE) + 16 * l);
       }
     }
   }
@@ -117,44 +134,56 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
 #pragma unroll
   for (int j = 0; j < NC; j++) acc[j] = make_double2(0.0, 0.0);
 
-  // -(p_s/m_s) dW/dq_s
+  // ---- -(p_s/m_s) dW/dq_s: same pair of the 4 neighbouring bricks of this element along every q axis ----
 #pragma unroll
   for (int s = 0; s < 3; s++) {
-    const long long st = op.st[s] / 2;                              // brick strides are even
-    const int i = iq[s], n = op.n[s];
-    const bool hp1 = i + 1 < n, hm1 = i >= 1, hp2 = wide && i + 2 < n, hm2 = wide && i >= 2;   // CTA-uniform
-    const double wq = -(wide ? -op.c2[s] : op.c1[s]) * op.inv_mass[s];
+    const long long st2 = op.st[s] >> 1;                            // brick stride of q_s in double2 (even)
+    const int i = bid.iq[s], n = op.n[s];
+    const double wq = -(wide ? -op.c2[s] : op.c1[s]) * op.inv_mass[s];   // -(1/m_s) / (12 h) or / (2 h)
     const double cqa = wq * (s == 1 ? p2 : p3a), cqb = wq * (s == 1 ? p2 : p3b);
-    constexpr bool TIGHT = (NTT * MINB > 512);                      // <= 64 registers per thread
-    constexpr int HB = TIGHT ? 2 : ((NC > 4 && NC % 2 == 0) ? NC / 2 : NC);   // loads are issued in batches of 4*HB
-    const double2 zero2 = make_double2(0.0, 0.0);
+    const double2* bp1 = Xk + st2;
+    const double2* bm1 = Xk - st2;
+    if (wide && i >= 2 && i + 2 < n) {                              // interior in q_s: all four neighbours exist
+      const double2* bp2 = Xk + 2 * st2;
+      const double2* bm2 = Xk - 2 * st2;
+      double2 vp1[NC], vm1[NC], vp2[NC], vm2[NC];
+      Unroll<0, NC>::run([&](auto J) {
+        constexpr int j = decltype(J)::value;
+        vp1[j] = ldg2o<j * PL2>(bp1, pol_own);
+        vm1[j] = ldg2o<j * PL2>(bm1, pol_own);
+        vp2[j] = ldg2o<j * PL2>(bp2, pol_own);
+        vm2[j] = ldg2o<j * PL2>(bm2, pol_own);
+      });
 #pragma unroll
-    for (int j0 = 0; j0 < NC; j0 += HB) {
-      double2 fp1[HB], fm1[HB], fp2[HB], fm2[HB];
-#pragma unroll
-      for (int j = 0; j < HB; j++) {                                // ghost bricks (R9) are zero: no load at all
-        fp1[j] = hp1 ? ldg2_hint(Xk + st + (j0 + j) * PL2, pol_own) : zero2;
-        fm1[j] = hm1 ? ldg2_hint(Xk - st + (j0 + j) * PL2, pol_own) : zero2;
-        fp2[j] = hp2 ? ldg2_hint(Xk + 2 * st + (j0 + j) * PL2, pol_own) : zero2;
-        fm2[j] = hm2 ? ldg2_hint(Xk - 2 * st + (j0 + j) * PL2, pol_own) : zero2;
+      for (int j = 0; j < NC; j++) {
+        const double ex = fma(8.0, vp1[j].x - vm1[j].x, -(vp2[j].x - vm2[j].x));
+        const double ey = fma(8.0, vp1[j].y - vm1[j].y, -(vp2[j].y - vm2[j].y));
+        const double c1 = wq * fma((double)j, h1, p1_0);
+        acc[j].x = fma(s == 0 ? c1 : cqa, ex, acc[j].x);
+        acc[j].y = fma(s == 0 ? c1 : cqb, ey, acc[j].y);
       }
+    } else {                                                        // edge of the q_s axis: one direction at a time
 #pragma unroll
-      for (int j = 0; j < HB; j++) {
-        double ex = fp1[j].x - fm1[j].x, ey = fp1[j].y - fm1[j].y;
-        if (wide) {
-          ex = fma(8.0, ex, -(fp2[j].x - fm2[j].x));
-          ey = fma(8.0, ey, -(fp2[j].y - fm2[j].y));
+      for (int d = 0; d < 4; d++) {
+        const int off = (d == 0) ? 1 : (d == 1 ? -1 : (d == 2 ? 2 : -2));
+        if (i + off < 0 || i + off >= n || (!wide && d >= 2)) continue;          // ghost brick: contributes zero
+        const double wd = wide ? ((d == 0) ? 8.0 : (d == 1 ? -8.0 : (d == 2 ? -1.0 : 1.0))) : ((d == 0) ? 1.0 : -1.0);
+        const double2* b = Xk + off * st2;
+        double2 v[NC];
+        Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; v[j] = ldg2o<j * PL2>(b, pol_own); });
+#pragma unroll
+        for (int j = 0; j < NC; j++) {
+          const double c1 = wq * fma((double)j, h1, p1_0);
+          acc[j].x = fma((s == 0 ? c1 : cqa) * wd, v[j].x, acc[j].x);
+          acc[j].y = fma((s == 0 ? c1 : cqb) * wd, v[j].y, acc[j].y);
         }
-        const double c1 = wq * fma((double)(j0 + j), h1, p1_0);
-        acc[j0 + j].x = fma(s == 0 ? c1 : cqa, ex, acc[j0 + j].x);
-        acc[j0 + j].y = fma(s == 0 ? c1 : cqb, ey, acc[j0 + j].y);
       }
     }
   }
 
+  // ---- own brick, hierarchy neighbours: G_s and the pointwise gauge terms ----
   double2 xk[NC];
-#pragma unroll
-  for (int j = 0; j < NC; j++) xk[j] = ldg2_hint(Xk + j * PL2, pol_own);
+  Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; xk[j] = ldg2o<j * PL2>(Xk, pol_own); });
 #pragma unroll
   for (int j = 0; j < NC; j++) acc[j] = fma2(-Gam, xk[j], acc[j]);
 
@@ -163,52 +192,64 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   double2 g3own[KEEP_G3 ? NC : 1];
 #pragma unroll
   for (int s = 0; s < 3; s++) {
-    const double qs = op.x0[s] + iq[s] * op.h[s];
+    const double qs = op.x0[s] + bid.iq[s] * op.h[s];
     const double Vp = fma(op.VSL[s], qs, op.VLL[s]);
     const double dUs = __ldg(op.dU[s] + ql);
-    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
-    const double cu = (ku >= 0) ? Vp : 0.0;
-    const double cd = (kd >= 0) ? __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp : 0.0;
+    const int ku = kup[s], kd = kdn[s];
+    const double cu = Vp;
+    const double cd = __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp;
     const double pu = cu * op.kup[s], pd = cd * op.kdn[s];
-    const double2* Xu = (ku >= 0) ? reinterpret_cast<const double2*>(X + (size_t)ku * op.cells + brick + toff) : zb;
-    const double2* Xd = (kd >= 0) ? reinterpret_cast<const double2*>(X + (size_t)kd * op.cells + brick + toff) : zb;
-    const unsigned long long pol_u = (ku >= 0 && __ldg(bp.pos + ku) / bp.g == G) ? pol_own : pol_str;
-    const unsigned long long pol_d = (kd >= 0 && __ldg(bp.pos + kd) / bp.g == G) ? pol_own : pol_str;
     const double wp = wide ? -op.c2[3 + s] : op.c1[3 + s];
     if (s == 1) w2 = wp;
     if (s == 2) w3 = wp;
     const double wp8 = wide ? 8.0 * wp : wp, wp1 = wide ? wp : 0.0;
+    double2 gg[NC];
+#pragma unroll
+    for (int j = 0; j < NC; j++) gg[j] = make_double2(dUs * xk[j].x, dUs * xk[j].y);
+    if (ku >= 0) {                                                  // Phi_s W^(n+e_s), CTA-uniform branch
+      const double2* Xu = X2 + ((size_t)ku * cells2 + brick2 + tpart);
+      const unsigned long long pol_u = ((bid.own >> (2 * s)) & 1) ? pol_own : pol_str;
+      double2 v[NC];
+      Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; v[j] = ldg2o<j * PL2>(Xu, pol_u); });
+#pragma unroll
+      for (int j = 0; j < NC; j++) {
+        const double psa = (s == 0) ? fma((double)j, h1, p1_0) : (s == 1 ? p2 : p3a);
+        const double psb = (s == 2) ? p3b : psa;
+        gg[j] = fma2(cu, v[j], gg[j]);
+        acc[j].x = fma(psa * pu, v[j].x, acc[j].x);
+        acc[j].y = fma(psb * pu, v[j].y, acc[j].y);
+      }
+    }
+    if (kd >= 0) {                                                  // n_s Theta_s W^(n-e_s)
+      const double2* Xd = X2 + ((size_t)kd * cells2 + brick2 + tpart);
+      const unsigned long long pol_d = ((bid.own >> (2 * s + 1)) & 1) ? pol_own : pol_str;
+      double2 v[NC];
+      Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; v[j] = ldg2o<j * PL2>(Xd, pol_d); });
+#pragma unroll
+      for (int j = 0; j < NC; j++) {
+        const double psa = (s == 0) ? fma((double)j, h1, p1_0) : (s == 1 ? p2 : p3a);
+        const double psb = (s == 2) ? p3b : psa;
+        gg[j] = fma2(cd, v[j], gg[j]);
+        acc[j].x = fma(psa * pd, v[j].x, acc[j].x);
+        acc[j].y = fma(psb * pd, v[j].y, acc[j].y);
+      }
+    }
 #pragma unroll
     for (int j = 0; j < NC; j++) {
-      double2 gg = make_double2(dUs * xk[j].x, dUs * xk[j].y);
-      const double psa = (s == 0) ? fma((double)j, h1, p1_0) : (s == 1 ? p2 : p3a);
-      const double psb = (s == 2) ? p3b : psa;
-      if (ku >= 0) {                                                // Phi_s W^(n+e_s), CTA-uniform branch
-        const double2 xu = ldg2_hint(Xu + j * PL2, pol_u);
-        gg = fma2(cu, xu, gg);
-        acc[j].x = fma(psa * pu, xu.x, acc[j].x);
-        acc[j].y = fma(psb * pu, xu.y, acc[j].y);
-      }
-      if (kd >= 0) {                                                // n_s Theta_s W^(n-e_s)
-        const double2 xd = ldg2_hint(Xd + j * PL2, pol_d);
-        gg = fma2(cd, xd, gg);
-        acc[j].x = fma(psa * pd, xd.x, acc[j].x);
-        acc[j].y = fma(psb * pd, xd.y, acc[j].y);
-      }
       if (s == 0) {                                                 // D_{p_1} G_1 in scatter form
-        if (j >= 1) acc[j - 1] = fma2(wp8, gg, acc[j - 1]);
-        if (j + 1 < NC) acc[j + 1] = fma2(-wp8, gg, acc[j + 1]);
-        if (j >= 2) acc[j - 2] = fma2(-wp1, gg, acc[j - 2]);
-        if (j + 2 < NC) acc[j + 2] = fma2(wp1, gg, acc[j + 2]);
+        if (j >= 1) acc[j - 1] = fma2(wp8, gg[j], acc[j - 1]);
+        if (j + 1 < NC) acc[j + 1] = fma2(-wp8, gg[j], acc[j + 1]);
+        if (j >= 2) acc[j - 2] = fma2(-wp1, gg[j], acc[j - 2]);
+        if (j + 2 < NC) acc[j + 2] = fma2(wp1, gg[j], acc[j + 2]);
         if (SPLIT > 1) {                                            // segment edges: hand G_1 to the neighbour segment
-          if (j < 2) *reinterpret_cast<double2*>(xg + (seg * 4 + j) * PLANE + 2 * tid) = gg;
-          if (j >= NC - 2) *reinterpret_cast<double2*>(xg + (seg * 4 + 2 + j - (NC - 2)) * PLANE + 2 * tid) = gg;
+          if (j < 2) *reinterpret_cast<double2*>(xg + (seg * 4 + j) * PLANE + 2 * tid) = gg[j];
+          if (j >= NC - 2) *reinterpret_cast<double2*>(xg + (seg * 4 + 2 + j - (NC - 2)) * PLANE + 2 * tid) = gg[j];
         }
       } else if (s == 1) {
-        *reinterpret_cast<double2*>(g2 + (jbase + j) * G2_PLANE + (i2 + 2) * G2_ROW + i3) = gg;
+        *reinterpret_cast<double2*>(g2 + (jbase + j) * G2_PLANE + (i2 + 2) * G2_ROW + i3) = gg[j];
       } else {
-        *reinterpret_cast<double2*>(g3 + (jbase + j) * G3_PLANE + i2 * G3_ROW + i3 + 2) = gg;
-        if (KEEP_G3) g3own[j] = gg;
+        *reinterpret_cast<double2*>(g3 + (jbase + j) * G3_PLANE + i2 * G3_ROW + i3 + 2) = gg[j];
+        if (KEEP_G3) g3own[j] = gg[j];
       }
     }
   }
@@ -260,15 +301,14 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
 
   // stage combine.  y may alias out (last stage, in place): a thread reads only the cells it writes, and all
   // its reads are issued before its first write.
-  const size_t o0 = boff + (size_t)k * op.cells + brick + toff;
   if (!y_is_in) {
-#pragma unroll
-    for (int j = 0; j < NC; j++) xk[j] = ld2_hint(reinterpret_cast<const double2*>(y + o0) + j * PL2, pol_str);
+    const double2* Y = reinterpret_cast<const double2*>(y + boff) + ((size_t)k * cells2 + brick2 + tpart);
+    Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; xk[j] = ld2o<j * PL2>(Y, pol_str); });
   }
 #pragma unroll
   for (int j = 0; j < NC; j++) acc[j] = make_double2(fma(cc, acc[j].x, a * xk[j].x), fma(cc, acc[j].y, a * xk[j].y));
-#pragma unroll
-  for (int j = 0; j < NC; j++) st2_hint(reinterpret_cast<double2*>(out + o0) + j * PL2, acc[j], pol_str);
+  double2* O = reinterpret_cast<double2*>(out + boff) + ((size_t)k * cells2 + brick2 + tpart);
+  Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; st2o<j * PL2>(O, acc[j], pol_str); });
 }
 
 template <int P1, int P2, int P3, int SPLIT>

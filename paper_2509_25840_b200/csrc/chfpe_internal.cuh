@@ -41,6 +41,7 @@ struct BrickPlan {
   int q2chunk;                        // q_2 rows per sweep chunk (= n_q2 unless five q_1 planes exceed the L2 budget)
   const int* order;                   // [K] element order, groups contiguous (device)
   const int* pos;                     // [K] position of element k in `order`
+  const int4* table;                  // [K * n_q] brick order (device), see decode_brick_id
   int l2mode;                         // bit 0: once-touched data evict_first, bit 1: window data evict_last
   int minb;                           // CTAs per SM the specialised kernel is compiled for (register budget)
   int split;                          // p_1 segments (thread groups) per brick in the specialised kernel
@@ -53,28 +54,18 @@ struct BrickPlan {
 #ifdef __CUDACC__
 // Brick order of the three-mode kernels: element group -> q_2 chunk -> q_1 plane -> element in group -> (q_2, q_3).
 // The five q_1 planes (of one chunk of q_2 rows) of the group's stage input are the L2 reuse window.
-struct BrickId { int k, G, iq[3]; long long ql; };
-__device__ __forceinline__ BrickId decode_brick_id(const DevOp& op, const BrickPlan& bp, long long L) {
+struct BrickId { int k, G, iq[3], own; long long ql; };
+// The order is tabulated once per handle by the host (make_brick_plan): one int4 per brick,
+// {k, linear q index, iq_1 | iq_2 << 10 | iq_3 << 20, group | own-mask << 16}; own-mask bit 2s (+1) says that the
+// up (down) neighbour along s belongs to the same group, i.e. its bricks are part of the L2 window.
+__device__ __forceinline__ BrickId decode_brick_id(const DevOp&, const BrickPlan& bp, long long L) {
+  const int4 t = __ldg(bp.table + L);
   BrickId b;
-  b.G = (int)(L / bp.blocks_per_full_group);
-  L -= (long long)b.G * bp.blocks_per_full_group;
-  int gs = op.K - b.G * bp.g;
-  if (gs > bp.g) gs = bp.g;
-  const int n1 = op.n[0], n2 = op.n[1], n3 = op.n[2], cs = bp.q2chunk;
-  const int nch = (n2 + cs - 1) / cs;
-  int ch = (int)(L / ((long long)n1 * gs * cs * n3));
-  if (ch > nch - 1) ch = nch - 1;
-  L -= (long long)ch * n1 * gs * cs * n3;
-  const int w = (n2 - ch * cs < cs) ? n2 - ch * cs : cs;
-  const long long per_plane = (long long)gs * w * n3;
-  b.iq[0] = (int)(L / per_plane);
-  const long long r = L - (long long)b.iq[0] * per_plane;
-  const int kk = (int)(r / (w * n3));
-  const int rr = (int)(r - (long long)kk * (w * n3));
-  b.iq[1] = ch * cs + rr / n3;
-  b.iq[2] = rr - (rr / n3) * n3;
-  b.ql = ((long long)b.iq[0] * n2 + b.iq[1]) * n3 + b.iq[2];
-  b.k = __ldg(bp.order + b.G * bp.g + kk);
+  b.k = t.x;
+  b.ql = t.y;
+  b.iq[0] = t.z & 1023; b.iq[1] = (t.z >> 10) & 1023; b.iq[2] = (t.z >> 20) & 1023;
+  b.G = t.w & 0xffff;
+  b.own = t.w >> 16;
   return b;
 }
 #endif

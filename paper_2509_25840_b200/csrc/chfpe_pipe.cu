@@ -61,7 +61,7 @@ enum { ROW_XK = 0, ROW_NB = 1 /* +2s (up), +2s+1 (down) */, ROW_Q = 7 /* +4s: -2
 
 // what every thread of the CTA needs to know about a brick (CTA-uniform)
 struct BrickInfo {
-  int k, G;
+  int k, G, own;
   long long ql;
   int iq[3];
   size_t elem_off;       // k*cells + ql*pb (doubles, inside one replica)
@@ -74,7 +74,7 @@ __device__ __forceinline__ BrickInfo decode_brick(const DevOp& op, const BrickPl
   const long long slot = Lt / per_slot;
   long long L = Lt - slot * per_slot;
   const BrickId id = decode_brick_id(op, bp, L);
-  b.G = id.G; b.k = id.k; b.ql = id.ql;
+  b.G = id.G; b.k = id.k; b.ql = id.ql; b.own = id.own;
   b.iq[0] = id.iq[0]; b.iq[1] = id.iq[1]; b.iq[2] = id.iq[2];
   b.elem_off = (size_t)b.k * op.cells + (size_t)b.ql * op.pb;
   b.slot_off = (size_t)slot * slot_stride;
@@ -133,7 +133,7 @@ k_stage_pipe(DevOp op, BrickPlan bp, const double* __restrict__ in, const double
         const int kn = ((lane - ROW_NB) & 1) ? __ldg(op.dn + 3 * b.k + s) : __ldg(op.up + 3 * b.k + s);
         if (kn >= 0) {
           src = X + (size_t)kn * op.cells + (size_t)b.ql * op.pb;
-          own = (__ldg(bp.pos + kn) / bp.g == b.G);
+          own = ((b.own >> (lane - ROW_NB)) & 1) != 0;
         }
       } else if (lane < ROW_Y) {
         const int s = (lane - ROW_Q) >> 2, r = (lane - ROW_Q) & 3;
