@@ -24,7 +24,9 @@ __device__ __forceinline__ unsigned long long l2_policy(int kind) {   // 0 norma
   else asm("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
   return p;
 }
-__device__ __forceinline__ void prefetch_l2(const double* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, unsigned bytes) {   // bytes: multiple of 16
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 
 // ------------------------------------------------------------------------------------------------
 // Specialised M = 3 brick kernel with compile-time momentum extents (P1, P2, P3), 128-bit accesses.
@@ -64,8 +66,15 @@ template <int N> struct Unroll<N, N> {
   template <typename F> __device__ __forceinline__ static void run(F&&) {}
 };
 
+// registers per thread that let MINB CTAs of NT threads share the 64 K registers of an SM
+constexpr int brick3_maxreg(int nt, int minb) {
+  const int warps = ((nt + 127) / 128) * 4;                        // warps are allocated in groups of four
+  const int r = (65536 / (minb * warps * 32)) & ~7;
+  return r > 255 ? 255 : r;
+}
+
 template <int P1, int P2, int P3, int SPLIT, int MINB>
-__global__ void __launch_bounds__(SPLIT * P2 * P3 / 2, MINB)
+__global__ void __launch_bounds__(SPLIT * P2 * P3 / 2) __maxnreg__(brick3_maxreg(SPLIT * P2 * P3 / 2, MINB))
 k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const double* y, double* out, double a,
                double cc, size_t slot_stride, int y_is_in, const double* __restrict__ zero_brick) {
   static_assert(P3 % 2 == 0 && P1 % SPLIT == 0 && (SPLIT == 1 || P1 / SPLIT >= 2), "unsupported brick shape");
@@ -80,18 +89,6 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const int tid = threadIdx.x - seg * PL2;                          // pair index inside the plane
   const int jbase = seg * NC;                                       // first p_1 plane of this thread
   const int i2 = tid / (P3 / 2), i3 = 2 * (tid - i2 * (P3 / 2));
-
-  // ---- brick of this CTA (32-bit arithmetic: at most K * n_q < 2^31 bricks) ----
-  const BrickId bid = decode_brick_id(op, bp, blockIdx.x);
-  const int k = bid.k;
-  const unsigned ql = (unsigned)bid.ql;
-  const size_t boff = (size_t)blockIdx.y * slot_stride;
-  const double2* X2 = reinterpret_cast<const double2*>(in + boff);  // replica base
-  const unsigned cells2 = (unsigned)(op.cells >> 1);                // element stride in double2
-  const unsigned tpart = (unsigned)(jbase * PL2 + tid);             // this thread's first pair inside a brick
-  const unsigned brick2 = ql * (unsigned)(P1 * PL2);                // brick offset inside an element
-  const double2* Xk = X2 + ((size_t)k * cells2 + brick2 + tpart);   // own pairs: Xk[j * PL2]
-  (void)zero_brick;
 
   // zero the ghost rows / columns of the two shared bricks
   for (int i = threadIdx.x; i < P1 * 4 * P3; i += NTT) {            // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
@@ -109,25 +106,38 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const double h1 = op.h[3], p1_0 = op.x0[3] + jbase * h1;
   const double p2 = op.x0[4] + i2 * op.h[4];
   const double p3a = op.x0[5] + i3 * op.h[5], p3b = op.x0[5] + (i3 + 1) * op.h[5];
+  // ---- bricks of this CTA: bp.bpc consecutive entries of the brick order (setup above is paid once) ----
+  const long long n_bricks = (long long)op.K * op.nqc;
+  for (long long L = (long long)blockIdx.x * bp.bpc, Lend = L + bp.bpc; L < Lend && L < n_bricks; L++) {
+  const BrickId bid = decode_brick_id(op, bp, L);
+  const int k = bid.k;
+  const unsigned ql = (unsigned)bid.ql;
+  const size_t boff = (size_t)blockIdx.y * slot_stride;
+  const double2* X2 = reinterpret_cast<const double2*>(in + boff);  // replica base
+  const unsigned cells2 = (unsigned)(op.cells >> 1);                // element stride in double2
+  const unsigned tpart = (unsigned)(jbase * PL2 + tid);             // this thread's first pair inside a brick
+  const unsigned brick2 = ql * (unsigned)(P1 * PL2);                // brick offset inside an element
+  const double2* Xk = X2 + ((size_t)k * cells2 + brick2 + tpart);   // own pairs: Xk[j * PL2]
+  (void)zero_brick;
+
   const double Gam = __ldg(op.Gamma + k);
   int kup[3], kdn[3];
 #pragma unroll
   for (int s = 0; s < 3; s++) { kup[s] = __ldg(op.up + 3 * k + s); kdn[s] = __ldg(op.dn + 3 * k + s); }
 
   // Everything this brick needs from HBM (its own stage input, the bricks of its hierarchy neighbours, y) is
-  // requested into L2 now -- one 128-byte line per thread and array -- and consumed after the q-derivative part.
-  {
-    constexpr int LINES = P1 * PLANE / 16;                          // 128-byte lines per brick
+  // requested into L2 now -- one bulk prefetch per array, issued by one thread -- and consumed after the
+  // q-derivative part, whose loads are L2 hits on the q_1-plane window and cover the DRAM latency.
+  if (threadIdx.x == 0) {
+    constexpr unsigned BB = P1 * PLANE * sizeof(double);
     const double* Xd = in + boff;
-    const size_t e0 = (size_t)k * op.cells + (size_t)ql * (P1 * PLANE);
-    for (int l = threadIdx.x; l < LINES; l += NTT) {
-      prefetch_l2(Xd + e0 + 16 * l);
-      if (!y_is_in) prefetch_l2(y + boff + e0 + 16 * l);
+    const size_t b0 = (size_t)ql * (P1 * PLANE);
+    bulk_prefetch_l2(Xd + (size_t)k * op.cells + b0, BB);
+    if (!y_is_in) bulk_prefetch_l2(y + boff + (size_t)k * op.cells + b0, BB);
 #pragma unroll
-      for (int s = 0; s < 3; s++) {
-        if (kup[s] >= 0) prefetch_l2(Xd + (size_t)kup[s] * op.cells + (size_t)ql * (P1 * PLANE) + 16 * l);
-        if (kdn[s] >= 0) prefetch_l2(Xd + (size_t)kdn[s] * op.cells + (size_t)ql * (P1 * PLANE) + 16 * l);
-      }
+    for (int s = 0; s < 3; s++) {
+      if (kup[s] >= 0) bulk_prefetch_l2(Xd + (size_t)kup[s] * op.cells + b0, BB);
+      if (kdn[s] >= 0) bulk_prefetch_l2(Xd + (size_t)kdn[s] * op.cells + b0, BB);
     }
   }
   double2 acc[NC];
@@ -146,22 +156,26 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     if (wide && i >= 2 && i + 2 < n) {                              // interior in q_s: all four neighbours exist
       const double2* bp2 = Xk + 2 * st2;
       const double2* bm2 = Xk - 2 * st2;
-      double2 vp1[NC], vm1[NC], vp2[NC], vm2[NC];
-      Unroll<0, NC>::run([&](auto J) {
-        constexpr int j = decltype(J)::value;
-        vp1[j] = ldg2o<j * PL2>(bp1, pol_own);
-        vm1[j] = ldg2o<j * PL2>(bm1, pol_own);
-        vp2[j] = ldg2o<j * PL2>(bp2, pol_own);
-        vm2[j] = ldg2o<j * PL2>(bm2, pol_own);
-      });
+      constexpr int CH = (NC <= 5) ? NC : (NC % 5 == 0 ? 5 : (NC % 4 == 0 ? 4 : (NC % 3 == 0 ? 3 : 1)));   // planes per load batch
+      Unroll<0, NC / CH>::run([&](auto C0) {
+        constexpr int j0 = decltype(C0)::value * CH;
+        double2 vp1[CH], vm1[CH], vp2[CH], vm2[CH];
+        Unroll<0, CH>::run([&](auto J) {
+          constexpr int j = decltype(J)::value;
+          vp1[j] = ldg2o<(j0 + j) * PL2>(bp1, pol_own);
+          vm1[j] = ldg2o<(j0 + j) * PL2>(bm1, pol_own);
+          vp2[j] = ldg2o<(j0 + j) * PL2>(bp2, pol_own);
+          vm2[j] = ldg2o<(j0 + j) * PL2>(bm2, pol_own);
+        });
 #pragma unroll
-      for (int j = 0; j < NC; j++) {
-        const double ex = fma(8.0, vp1[j].x - vm1[j].x, -(vp2[j].x - vm2[j].x));
-        const double ey = fma(8.0, vp1[j].y - vm1[j].y, -(vp2[j].y - vm2[j].y));
-        const double c1 = wq * fma((double)j, h1, p1_0);
-        acc[j].x = fma(s == 0 ? c1 : cqa, ex, acc[j].x);
-        acc[j].y = fma(s == 0 ? c1 : cqb, ey, acc[j].y);
-      }
+        for (int j = 0; j < CH; j++) {
+          const double ex = fma(8.0, vp1[j].x - vm1[j].x, -(vp2[j].x - vm2[j].x));
+          const double ey = fma(8.0, vp1[j].y - vm1[j].y, -(vp2[j].y - vm2[j].y));
+          const double c1 = wq * fma((double)(j0 + j), h1, p1_0);
+          acc[j0 + j].x = fma(s == 0 ? c1 : cqa, ex, acc[j0 + j].x);
+          acc[j0 + j].y = fma(s == 0 ? c1 : cqb, ey, acc[j0 + j].y);
+        }
+      });
     } else {                                                        // edge of the q_s axis: one direction at a time
 #pragma unroll
       for (int d = 0; d < 4; d++) {
@@ -188,7 +202,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   for (int j = 0; j < NC; j++) acc[j] = fma2(-Gam, xk[j], acc[j]);
 
   double w2 = 0.0, w3 = 0.0;                                        // 1/(12h) or 1/(2h) of p_2, p_3
-  constexpr bool KEEP_G3 = (NTT * MINB <= 512);                    // else re-read the own G_3 pair from shared memory
+  constexpr bool KEEP_G3 = (NC <= 8);                              // else re-read the own G_3 pair from shared memory
   double2 g3own[KEEP_G3 ? NC : 1];
 #pragma unroll
   for (int s = 0; s < 3; s++) {
@@ -203,55 +217,60 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     if (s == 1) w2 = wp;
     if (s == 2) w3 = wp;
     const double wp8 = wide ? 8.0 * wp : wp, wp1 = wide ? wp : 0.0;
-    double2 gg[NC];
+    const double2* Xu = X2 + ((size_t)(ku >= 0 ? ku : k) * cells2 + brick2 + tpart);
+    const double2* Xd = X2 + ((size_t)(kd >= 0 ? kd : k) * cells2 + brick2 + tpart);
+    const unsigned long long pol_u = ((bid.own >> (2 * s)) & 1) ? pol_own : pol_str;
+    const unsigned long long pol_d = ((bid.own >> (2 * s + 1)) & 1) ? pol_own : pol_str;
+    constexpr int CH = (NC <= 5) ? NC : (NC % 5 == 0 ? 5 : (NC % 4 == 0 ? 4 : (NC % 3 == 0 ? 3 : 1)));   // planes per batch
+    Unroll<0, NC / CH>::run([&](auto C0) {
+      constexpr int j0 = decltype(C0)::value * CH;
+      double2 gg[CH];
 #pragma unroll
-    for (int j = 0; j < NC; j++) gg[j] = make_double2(dUs * xk[j].x, dUs * xk[j].y);
-    if (ku >= 0) {                                                  // Phi_s W^(n+e_s), CTA-uniform branch
-      const double2* Xu = X2 + ((size_t)ku * cells2 + brick2 + tpart);
-      const unsigned long long pol_u = ((bid.own >> (2 * s)) & 1) ? pol_own : pol_str;
-      double2 v[NC];
-      Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; v[j] = ldg2o<j * PL2>(Xu, pol_u); });
+      for (int j = 0; j < CH; j++) gg[j] = make_double2(dUs * xk[j0 + j].x, dUs * xk[j0 + j].y);
+      if (ku >= 0) {                                                // Phi_s W^(n+e_s), CTA-uniform branch
+        double2 v[CH];
+        Unroll<0, CH>::run([&](auto J) { constexpr int j = decltype(J)::value; v[j] = ldg2o<(j0 + j) * PL2>(Xu, pol_u); });
 #pragma unroll
-      for (int j = 0; j < NC; j++) {
-        const double psa = (s == 0) ? fma((double)j, h1, p1_0) : (s == 1 ? p2 : p3a);
-        const double psb = (s == 2) ? p3b : psa;
-        gg[j] = fma2(cu, v[j], gg[j]);
-        acc[j].x = fma(psa * pu, v[j].x, acc[j].x);
-        acc[j].y = fma(psb * pu, v[j].y, acc[j].y);
-      }
-    }
-    if (kd >= 0) {                                                  // n_s Theta_s W^(n-e_s)
-      const double2* Xd = X2 + ((size_t)kd * cells2 + brick2 + tpart);
-      const unsigned long long pol_d = ((bid.own >> (2 * s + 1)) & 1) ? pol_own : pol_str;
-      double2 v[NC];
-      Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; v[j] = ldg2o<j * PL2>(Xd, pol_d); });
-#pragma unroll
-      for (int j = 0; j < NC; j++) {
-        const double psa = (s == 0) ? fma((double)j, h1, p1_0) : (s == 1 ? p2 : p3a);
-        const double psb = (s == 2) ? p3b : psa;
-        gg[j] = fma2(cd, v[j], gg[j]);
-        acc[j].x = fma(psa * pd, v[j].x, acc[j].x);
-        acc[j].y = fma(psb * pd, v[j].y, acc[j].y);
-      }
-    }
-#pragma unroll
-    for (int j = 0; j < NC; j++) {
-      if (s == 0) {                                                 // D_{p_1} G_1 in scatter form
-        if (j >= 1) acc[j - 1] = fma2(wp8, gg[j], acc[j - 1]);
-        if (j + 1 < NC) acc[j + 1] = fma2(-wp8, gg[j], acc[j + 1]);
-        if (j >= 2) acc[j - 2] = fma2(-wp1, gg[j], acc[j - 2]);
-        if (j + 2 < NC) acc[j + 2] = fma2(wp1, gg[j], acc[j + 2]);
-        if (SPLIT > 1) {                                            // segment edges: hand G_1 to the neighbour segment
-          if (j < 2) *reinterpret_cast<double2*>(xg + (seg * 4 + j) * PLANE + 2 * tid) = gg[j];
-          if (j >= NC - 2) *reinterpret_cast<double2*>(xg + (seg * 4 + 2 + j - (NC - 2)) * PLANE + 2 * tid) = gg[j];
+        for (int j = 0; j < CH; j++) {
+          const double psa = (s == 0) ? fma((double)(j0 + j), h1, p1_0) : (s == 1 ? p2 : p3a);
+          const double psb = (s == 2) ? p3b : psa;
+          gg[j] = fma2(cu, v[j], gg[j]);
+          acc[j0 + j].x = fma(psa * pu, v[j].x, acc[j0 + j].x);
+          acc[j0 + j].y = fma(psb * pu, v[j].y, acc[j0 + j].y);
         }
-      } else if (s == 1) {
-        *reinterpret_cast<double2*>(g2 + (jbase + j) * G2_PLANE + (i2 + 2) * G2_ROW + i3) = gg[j];
-      } else {
-        *reinterpret_cast<double2*>(g3 + (jbase + j) * G3_PLANE + i2 * G3_ROW + i3 + 2) = gg[j];
-        if (KEEP_G3) g3own[j] = gg[j];
       }
-    }
+      if (kd >= 0) {                                                // n_s Theta_s W^(n-e_s)
+        double2 v[CH];
+        Unroll<0, CH>::run([&](auto J) { constexpr int j = decltype(J)::value; v[j] = ldg2o<(j0 + j) * PL2>(Xd, pol_d); });
+#pragma unroll
+        for (int j = 0; j < CH; j++) {
+          const double psa = (s == 0) ? fma((double)(j0 + j), h1, p1_0) : (s == 1 ? p2 : p3a);
+          const double psb = (s == 2) ? p3b : psa;
+          gg[j] = fma2(cd, v[j], gg[j]);
+          acc[j0 + j].x = fma(psa * pd, v[j].x, acc[j0 + j].x);
+          acc[j0 + j].y = fma(psb * pd, v[j].y, acc[j0 + j].y);
+        }
+      }
+#pragma unroll
+      for (int jj = 0; jj < CH; jj++) {
+        const int j = j0 + jj;
+        if (s == 0) {                                               // D_{p_1} G_1 in scatter form
+          if (j >= 1) acc[j - 1] = fma2(wp8, gg[jj], acc[j - 1]);
+          if (j + 1 < NC) acc[j + 1] = fma2(-wp8, gg[jj], acc[j + 1]);
+          if (j >= 2) acc[j - 2] = fma2(-wp1, gg[jj], acc[j - 2]);
+          if (j + 2 < NC) acc[j + 2] = fma2(wp1, gg[jj], acc[j + 2]);
+          if (SPLIT > 1) {                                          // segment edges: hand G_1 to the neighbour segment
+            if (j < 2) *reinterpret_cast<double2*>(xg + (seg * 4 + j) * PLANE + 2 * tid) = gg[jj];
+            if (j >= NC - 2) *reinterpret_cast<double2*>(xg + (seg * 4 + 2 + j - (NC - 2)) * PLANE + 2 * tid) = gg[jj];
+          }
+        } else if (s == 1) {
+          *reinterpret_cast<double2*>(g2 + (jbase + j) * G2_PLANE + (i2 + 2) * G2_ROW + i3) = gg[jj];
+        } else {
+          *reinterpret_cast<double2*>(g3 + (jbase + j) * G3_PLANE + i2 * G3_ROW + i3 + 2) = gg[jj];
+          if (KEEP_G3) g3own[KEEP_G3 ? j : 0] = gg[jj];
+        }
+      }
+    });
   }
   __syncthreads();
   if (SPLIT > 1) {
@@ -309,6 +328,8 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   for (int j = 0; j < NC; j++) acc[j] = make_double2(fma(cc, acc[j].x, a * xk[j].x), fma(cc, acc[j].y, a * xk[j].y));
   double2* O = reinterpret_cast<double2*>(out + boff) + ((size_t)k * cells2 + brick2 + tpart);
   Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; st2o<j * PL2>(O, acc[j], pol_str); });
+  __syncthreads();                                                  // shared bricks free for the next brick
+  }
 }
 
 template <int P1, int P2, int P3, int SPLIT>
@@ -342,7 +363,7 @@ int brick_configure(const BrickPlan& bp, int M) {
 
 int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out, double a,
                        double c, int nb, size_t slot_stride, cudaStream_t s) {
-  dim3 grid((unsigned)((long long)op.K * op.nqc), nb);
+  dim3 grid((unsigned)(((long long)op.K * op.nqc + bp.bpc - 1) / bp.bpc), nb);
   const int y_is_in = (y == in) ? 1 : 0;
 #define X(A, B, C, S, MB)                                                                                  \
   if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                            \

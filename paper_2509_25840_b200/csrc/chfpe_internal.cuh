@@ -38,6 +38,7 @@ struct BrickPlan {
   int n_groups;
   long long blocks_per_full_group;    // g * nqc
   long long rest;                     // q-points per q1 plane
+  int bpc;                            // consecutive bricks per CTA of the brick kernel
   int q2chunk;                        // q_2 rows per sweep chunk (= n_q2 unless five q_1 planes exceed the L2 budget)
   const int* order;                   // [K] element order, groups contiguous (device)
   const int* pos;                     // [K] position of element k in `order`
