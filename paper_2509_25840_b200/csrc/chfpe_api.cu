@@ -64,6 +64,9 @@ static int validate(const chfpe_desc* d, std::string* why) {
     if (!(d->mass[s] > 0) || !(d->gamma[s] > 0) || d->zeta[s] < 0) { *why = "mass, gamma must be > 0 and zeta >= 0"; return CHFPE_ERR_INVALID; }
     if (!(d->qmax[s] > d->qmin[s]) || !(d->pmax[s] > d->pmin[s])) { *why = "empty coordinate range"; return CHFPE_ERR_INVALID; }
   }
+  double cells = 1.0;
+  for (int s = 0; s < d->n_modes; s++) cells *= (double)d->nq[s] * d->np[s];
+  if (cells >= 2147483648.0) { *why = "grid of 2^31 cells or more"; return CHFPE_ERR_INVALID; }
   return CHFPE_OK;
 }
 

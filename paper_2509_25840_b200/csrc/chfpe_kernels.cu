@@ -6,14 +6,20 @@
 
 namespace {
 
+// cell -> per-axis indices; 32-bit arithmetic (chfpe_create rejects grids of 2^31 cells or more): a 64-bit
+// division costs ~80 instructions, and these kernels are instruction-bound
 template <int NAX>
-__device__ __forceinline__ void decode(const DevOp& op, long long cell, int (&idx)[NAX]) {
+__device__ __forceinline__ void decode(const DevOp& op, long long cell64, int (&idx)[NAX]) {
+  unsigned cell = (unsigned)cell64;
 #pragma unroll
   for (int a = NAX - 1; a >= 0; a--) {
-    long long q = cell / op.n[a];
-    idx[a] = (int)(cell - q * op.n[a]);
+    const unsigned q = cell / (unsigned)op.n[a];
+    idx[a] = (int)(cell - q * (unsigned)op.n[a]);
     cell = q;
   }
+}
+__device__ __forceinline__ long long qlinear(const DevOp& op, long long cell) {   // index of the q-point of a cell
+  return (long long)((unsigned)cell / (unsigned)op.pb);
 }
 
 // explicit antisymmetric stencil with zero ghosts (R9): c1 (f[+1]-f[-1]) + c2 (f[+2]-f[-2])
@@ -56,7 +62,7 @@ __device__ __forceinline__ double rhs_value(const DevOp& op, const double* __res
   const double* Xk = X + (size_t)k * op.cells;
   int idx[2 * M];
   decode<2 * M>(op, cell, idx);
-  const long long ql = cell / op.pb;
+  const long long ql = qlinear(op, cell);
   const bool wide = (op.scheme == CHFPE_CENTRAL4);
   double acc = -__ldg(op.Gamma + k) * ldx<COHERENT>(Xk + cell);
 #pragma unroll
@@ -168,7 +174,7 @@ __device__ __forceinline__ double expect_weight(const DevOp& op, const DevObs& o
     for (int r = 0; r < M; r++) O = fma(0.5 * ob.quad[s][r] * q[s], q[r], O);
     if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.ep[s] + idx[M + s]);
   }
-  if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.eU + cell / op.pb);
+  if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.eU + qlinear(op, cell));
   return O * w;
 }
 
@@ -186,7 +192,7 @@ __global__ void __launch_bounds__(256) k_reduce_partial(DevOp op, DevObs ob, int
     const double v = X[c];
     if (mode == RED_SUMSQ) { acc = fma(v, v, acc); continue; }
     if (mode == RED_SUM) { acc += v; continue; }
-    acc = fma(expect_weight<M>(op, ob, c % op.cells), v, acc);
+    acc = fma(expect_weight<M>(op, ob, c), v, acc);   // RED_EXPECT: ncells == op.cells
   }
   const double r = block_sum_256(acc);
   if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = r;
@@ -211,7 +217,7 @@ __global__ void __launch_bounds__(256) k_init_eq(DevOp op, double* __restrict__ 
   if (k == 0) {
     int idx[2 * M];
     decode<2 * M>(op, cell, idx);
-    v = __ldg(op.eU + cell / op.pb);
+    v = __ldg(op.eU + qlinear(op, cell));
 #pragma unroll
     for (int s = 0; s < M; s++) v *= __ldg(op.ep[s] + idx[M + s]);
   }
