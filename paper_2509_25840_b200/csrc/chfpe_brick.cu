@@ -339,7 +339,7 @@ constexpr int brick3_smem_bytes() {
 
 }  // namespace
 
-#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 2, 2) X(16, 16, 16, 2, 1) X(16, 16, 16, 4, 2) X(16, 16, 16, 4, 1) X(20, 20, 20, 2, 1) X(20, 20, 20, 4, 1) X(8, 8, 8, 1, 2) X(8, 8, 8, 2, 2) X(12, 12, 12, 2, 2) X(12, 12, 12, 3, 2)
+#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 4, 1) X(16, 16, 16, 2, 2) X(20, 20, 20, 2, 1) X(12, 12, 12, 2, 2) X(8, 8, 8, 2, 2)
 
 int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {
   if (M != 3) return 0;

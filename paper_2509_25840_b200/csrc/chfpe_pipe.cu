@@ -286,7 +286,7 @@ k_stage_pipe(DevOp op, BrickPlan bp, const double* __restrict__ in, const double
 
 }  // namespace
 
-#define PIPE_SPECIALISATIONS(X) X(16, 16, 16, 4) X(16, 16, 16, 2) X(20, 20, 20, 2) X(8, 8, 8, 4) X(8, 8, 8, 2) X(12, 12, 12, 4)
+#define PIPE_SPECIALISATIONS(X) X(16, 16, 16, 2) X(16, 16, 16, 4) X(8, 8, 8, 2)
 
 int pipe_has_fixed(int M, int P1, int P2, int P3, int stages) {
   if (M != 3) return 0;
