@@ -47,7 +47,6 @@ static int validate(const chfpe_desc* d, std::string* why) {
   if (d->depth < 0 || d->depth > 64) { *why = "depth out of range"; return CHFPE_ERR_INVALID; }
   if (!(d->beta > 0)) { *why = "beta must be > 0"; return CHFPE_ERR_INVALID; }
   if (d->scheme != CHFPE_CENTRAL4 && d->scheme != CHFPE_CENTRAL2 && d->scheme != CHFPE_COMPACT6) { *why = "unknown scheme"; return CHFPE_ERR_INVALID; }
-  if (d->scheme == CHFPE_COMPACT6) { *why = "COMPACT6 (conditional step a9) is not built in this round"; return CHFPE_ERR_INVALID; }
   if (d->gauge != CHFPE_GAUGE_SQRT_EQ && d->gauge != CHFPE_GAUGE_W) { *why = "unknown gauge"; return CHFPE_ERR_INVALID; }
   if (d->batch < 1 || d->batch > 4096) { *why = "batch must be 1..4096"; return CHFPE_ERR_INVALID; }
   if (d->n_terms < 0 || (d->n_terms > 0 && !d->U)) { *why = "bad potential term list"; return CHFPE_ERR_INVALID; }
@@ -61,6 +60,7 @@ static int validate(const chfpe_desc* d, std::string* why) {
   }
   for (int s = 0; s < d->n_modes; s++) {
     if (d->nq[s] < 5 || d->np[s] < 5) { *why = "need >= 5 grid points per axis"; return CHFPE_ERR_INVALID; }
+    if (d->scheme == CHFPE_COMPACT6 && (d->nq[s] > 4096 || d->np[s] > 4096)) { *why = "COMPACT6: at most 4096 points per axis"; return CHFPE_ERR_INVALID; }
     if (!(d->mass[s] > 0) || !(d->gamma[s] > 0) || d->zeta[s] < 0) { *why = "mass, gamma must be > 0 and zeta >= 0"; return CHFPE_ERR_INVALID; }
     if (!(d->qmax[s] > d->qmin[s]) || !(d->pmax[s] > d->pmin[s])) { *why = "empty coordinate range"; return CHFPE_ERR_INVALID; }
   }
@@ -73,7 +73,7 @@ static int validate(const chfpe_desc* d, std::string* why) {
 struct Plan {
   int M, K, batch, n_arrays, red_blocks;
   long long cells, nqc;
-  size_t off_tables, tables_bytes, off_partial, off_results, off_arrays, total;
+  size_t off_tables, tables_bytes, off_partial, off_results, off_arrays, off_scratch, total;
   static const long long RESULTS = 1 << 16;
 };
 
@@ -93,6 +93,7 @@ static Plan make_plan(const chfpe_desc* d) {
   tb += align256(sizeof(double) * sum_n);                      // ep
   tb += align256(sizeof(int) * 3 * p.K) * 3;                   // up, dn, nvec
   tb += align256(sizeof(double) * p.K);                        // Gamma
+  if (d->scheme == CHFPE_COMPACT6) tb += 2 * p.M * 2 * align256(sizeof(double) * 4096);   // Thomas factors per axis
   tb += align256(sizeof(int) * p.K) * 2;                       // brick-kernel element order and its inverse
   tb += align256(sizeof(double) * (p.cells / p.nqc));          // brick of zeros (ghost bricks)
   tb += align256(sizeof(int) * 4 * (size_t)p.K * p.nqc);       // brick-order table of the three-mode kernels
@@ -100,6 +101,8 @@ static Plan make_plan(const chfpe_desc* d) {
   p.off_partial = o; o += align256(sizeof(double) * p.red_blocks * (size_t)p.batch);
   p.off_results = o; o += align256(sizeof(double) * Plan::RESULTS);
   p.off_arrays = o; o += align256(sizeof(double) * (size_t)p.n_arrays * p.K * p.cells);
+  p.off_scratch = o;
+  if (d->scheme == CHFPE_COMPACT6) o += align256(sizeof(double) * 3 * (size_t)p.cells);   // G, D, F of chfpe_compact.cu
   p.total = o;
   return p;
 }
@@ -376,6 +379,21 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
     if (per_sm < 1 || pipe_configure(h->bp) != 0) { cudaGetLastError(); h->bp.pipe = 0; }
     h->bp.pipe_ctas = sms * per_sm;
   }
+  memset(&h->ct, 0, sizeof(h->ct));
+  h->scratch = nullptr;
+  if (desc->scheme == CHFPE_COMPACT6) {                                // elimination factors of tridiag(1/3, 1, 1/3), n rows
+    for (int a = 0; a < 2 * M; a++) {
+      const int n = op.n[a];
+      std::vector<double> bet(n), cf(n);
+      const double al = 1.0 / 3.0;
+      bet[0] = 1.0; cf[0] = 0.0;
+      for (int i = 1; i < n; i++) { cf[i] = al / bet[i - 1]; bet[i] = 1.0 - al * cf[i]; }
+      h->ct.bet[a] = (const double*)put(bet.data(), sizeof(double) * n);
+      h->ct.cfac[a] = (const double*)put(cf.data(), sizeof(double) * n);
+      cudaStreamSynchronize(h->stream);
+    }
+    h->scratch = (double*)(base + pl.off_scratch);
+  }
   h->partial = (double*)(base + pl.off_partial);
   h->results = (double*)(base + pl.off_results);
   h->arrays = (double*)(base + pl.off_arrays);
@@ -429,6 +447,8 @@ static int check_launch(chfpe_handle* h) {
 
 static int run_stage(chfpe_handle* h, const double* in, const double* y, double* out, double a, double c, int nb,
                      size_t ss) {
+  if (h->op.scheme == CHFPE_COMPACT6)
+    return launch_stage_compact(h->op, h->ct, in, y, out, a, c, nb, ss, h->scratch, h->stream);
   if (h->bp.enabled && h->bp.pipe) return launch_stage_pipe(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
   if (h->bp.enabled) return launch_stage_brick(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
   return launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);
@@ -456,7 +476,7 @@ static void stage(chfpe_handle* h, const double* in, const double* y, double* ou
 // CHFPE_COOP=0 forces per-stage launches, CHFPE_COOP=2 lifts the limit to 24 MB (tests).
 static bool coop_eligible(const chfpe_handle* h, int nb) {
   const size_t limit = (h->coop_mode == 2) ? ((size_t)24 << 20) : ((size_t)1 << 20);
-  return nb == 1 && h->coop && h->state_doubles * sizeof(double) <= limit;
+  return nb == 1 && h->coop && h->op.scheme != CHFPE_COMPACT6 && h->state_doubles * sizeof(double) <= limit;
 }
 
 // n RK4 steps (Horner form, R13) on slots [b0, b0+nb)
@@ -504,7 +524,10 @@ extern "C" int chfpe_profile_read(chfpe_handle* h, double* total_ms, int64_t* n_
 static int kick_slots(chfpe_handle* h, int b0, int nb, const chfpe_observable* X) {
   const size_t ss = 3 * h->state_doubles;
   DevObs o = to_dev(X);
-  h->launches += launch_kick(h->op, o, h->y(b0), h->va(b0), nb, ss, h->stream);
+  if (h->op.scheme == CHFPE_COMPACT6)
+    h->launches += launch_kick_compact(h->op, h->ct, o, h->y(b0), h->va(b0), nb, ss, h->scratch, h->stream);
+  else
+    h->launches += launch_kick(h->op, o, h->y(b0), h->va(b0), nb, ss, h->stream);
   for (int b = b0; b < b0 + nb; b++)
     CU(h, cudaMemcpyAsync(h->y(b), h->va(b), sizeof(double) * h->state_doubles, cudaMemcpyDeviceToDevice, h->stream));
   return check_launch(h);

@@ -75,6 +75,12 @@ struct DevObs {                       // observable polynomial, Eq. (13)-(14)
   double c0, lin_q[3], quad[3][3], lin_p[3];
 };
 
+// COMPACT6 (step a9): per-axis elimination factors of tridiag(1/3, 1, 1/3) (device), see chfpe_compact.cu
+struct CompactTables {
+  const double* bet[CHFPE_MAXAX];
+  const double* cfac[CHFPE_MAXAX];
+};
+
 enum ReduceMode { RED_EXPECT = 0, RED_SUMSQ = 1, RED_SUM = 2 };
 
 struct chfpe_handle {
@@ -82,6 +88,8 @@ struct chfpe_handle {
   std::vector<chfpe_monomial> U;
   DevOp op;
   BrickPlan bp;
+  CompactTables ct;
+  double* scratch;                    // COMPACT6 only: three element-sized arrays (G, D, F)
   cudaStream_t stream;
   int K, batch, n_arrays;
   long long cells;
@@ -110,6 +118,11 @@ struct chfpe_handle {
 // out = a*y + c*F(in) for slots [b0, b0+nb); slot stride = 3*state_doubles for all three pointers.
 int launch_stage(const DevOp& op, const double* in, const double* y, double* out, double a, double c,
                  int nb, size_t slot_stride, cudaStream_t s);
+// COMPACT6 path (chfpe_compact.cu): element-by-element assembly from whole-array Pade derivatives
+int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double* in, const double* y, double* out, double a,
+                         double c, int nb, size_t slot_stride, double* scratch, cudaStream_t s);
+int launch_kick_compact(const DevOp& op, const CompactTables& ct, const DevObs& o, const double* in, double* out, int nb,
+                        size_t slot_stride, double* scratch, cudaStream_t s);
 // persistent cooperative kernel for L2-resident states (one replica): n_samples x (stride steps [+ <O> sample]);
 // returns 0 if a cooperative launch is not possible
 int launch_steps_coop(const DevOp& op, const DevObs& o, double* y, double* va, double* vb, double dt,

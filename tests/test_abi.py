@@ -52,11 +52,14 @@ def test_workspace_bytes_and_validation():
     n5 = P.workspace_bytes(ci.config("cfg5"), batch=5)
     assert n5 < 180e9                       # config 5 with 5 slots (trajectory + 4 replicas) fits one B200
     for bad in (dict(nq=[4]), dict(depth=-1), dict(beta=0.0), dict(gamma=[0.0]), dict(U=[(1.0, (5,))]),
-                dict(scheme="compact6")):
+                dict(scheme="compact6", nq=[5000])):
         with pytest.raises(P.ChfpeError):
             P.workspace_bytes(ci.config("cfg1", **bad))
     with pytest.raises(P.ChfpeError):
         P.workspace_bytes(ci.config("cfg1"), batch=0)
+    # COMPACT6 (step a9) needs three element-sized scratch arrays on top of the explicit schemes' workspace
+    extra = P.workspace_bytes(ci.config("cfg1", scheme="compact6")) - P.workspace_bytes(ci.config("cfg1"))
+    assert 3 * 64 * 64 * 8 <= extra <= 3 * 64 * 64 * 8 + (1 << 20)
 
 
 def test_create_rejects_bad_workspace_without_touching_the_gpu():
