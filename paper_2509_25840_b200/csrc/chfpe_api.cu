@@ -95,7 +95,6 @@ static Plan make_plan(const chfpe_desc* d) {
   tb += align256(sizeof(double) * p.K);                        // Gamma
   if (d->scheme == CHFPE_COMPACT6) tb += 2 * p.M * 2 * align256(sizeof(double) * 4096);   // Thomas factors per axis
   tb += align256(sizeof(int) * p.K) * 2;                       // brick-kernel element order and its inverse
-  tb += align256(sizeof(double) * (p.cells / p.nqc));          // brick of zeros (ghost bricks)
   tb += align256(sizeof(int) * 4 * (size_t)p.K * p.nqc);       // brick-order table of the three-mode kernels
   p.tables_bytes = tb; o += tb;
   p.off_partial = o; o += align256(sizeof(double) * p.red_blocks * (size_t)p.batch);
@@ -360,11 +359,6 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
     }
     h->bp.table = (const int4*)put(tab.data(), sizeof(int) * tab.size());
     cudaStreamSynchronize(h->stream);                                  // `tab` goes out of scope
-  }
-  {
-    std::vector<double> zeros((size_t)(pl.cells / pl.nqc), 0.0);
-    h->bp.zero_brick = (const double*)put(zeros.data(), sizeof(double) * zeros.size());
-    cudaStreamSynchronize(h->stream);                                  // `zeros` goes out of scope
   }
   if (h->bp.enabled && brick_configure(h->bp, M) != 0) { cudaGetLastError(); h->bp.enabled = 0; }
   if (h->bp.enabled && h->bp.pipe) {

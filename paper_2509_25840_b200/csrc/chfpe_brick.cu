@@ -76,7 +76,7 @@ constexpr int brick3_maxreg(int nt, int minb) {
 template <int P1, int P2, int P3, int SPLIT, int MINB>
 __global__ void __launch_bounds__(SPLIT * P2 * P3 / 2) __maxnreg__(brick3_maxreg(SPLIT * P2 * P3 / 2, MINB))
 k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const double* y, double* out, double a,
-               double cc, size_t slot_stride, int y_is_in, const double* __restrict__ zero_brick) {
+               double cc, size_t slot_stride, int y_is_in) {
   static_assert(P3 % 2 == 0 && P1 % SPLIT == 0 && (SPLIT == 1 || P1 / SPLIT >= 2), "unsupported brick shape");
   constexpr int PLANE = P2 * P3, PL2 = PLANE / 2, NTT = SPLIT * PL2, NC = P1 / SPLIT;
   constexpr int G2_ROW = P3, G2_PLANE = (P2 + 4) * P3;              // G_2[i1][i2+2][i3]
@@ -118,7 +118,6 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const unsigned tpart = (unsigned)(jbase * PL2 + tid);             // this thread's first pair inside a brick
   const unsigned brick2 = ql * (unsigned)(P1 * PL2);                // brick offset inside an element
   const double2* Xk = X2 + ((size_t)k * cells2 + brick2 + tpart);   // own pairs: Xk[j * PL2]
-  (void)zero_brick;
 
   const double Gam = __ldg(op.Gamma + k);
   int kup[3], kdn[3];
@@ -368,7 +367,7 @@ int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, c
 #define X(A, B, C, S, MB)                                                                                  \
   if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                            \
     k_stage_brick3<A, B, C, S, MB><<<grid, S * B * C / 2, brick3_smem_bytes<A, B, C, S>(), s>>>(           \
-        op, bp, in, y, out, a, c, slot_stride, y_is_in, bp.zero_brick);
+        op, bp, in, y, out, a, c, slot_stride, y_is_in);
   BRICK3_SPECIALISATIONS(X)
 #undef X
   return 1;

@@ -47,7 +47,6 @@ struct BrickPlan {
   int minb;                           // CTAs per SM the specialised kernel is compiled for (register budget)
   int split;                          // p_1 segments (thread groups) per brick in the specialised kernel
   int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3,...>) exists
-  const double* zero_brick;           // pb zeros (device)
   int pipe;                           // use the plane-pipelined kernel (chfpe_pipe.cu)
   int pipe_stages, pipe_ctas;         // shared-memory stages per CTA, persistent CTAs in the grid
 };
