@@ -91,7 +91,7 @@ static Plan make_plan(const chfpe_desc* d) {
   size_t tb = 0;
   tb += align256(sizeof(double) * p.nqc) * (p.M + 1);          // dU[s], eU
   tb += align256(sizeof(double) * sum_n);                      // ep
-  tb += align256(sizeof(int) * 3 * p.K) * 3;                   // up, dn, nvec
+  tb += align256(sizeof(int) * 3 * p.K) * 6;                   // up, dn, nvec (+ their three-mode view for M = 2)
   tb += align256(sizeof(double) * p.K);                        // Gamma
   if (d->scheme == CHFPE_COMPACT6) tb += 2 * p.M * 2 * align256(sizeof(double) * 4096);   // Thomas factors per axis
   tb += align256(sizeof(int) * p.K) * 2;                       // brick-kernel element order and its inverse
@@ -123,9 +123,12 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   order_out->resize(K);
   for (int k = 0; k < K; k++) (*order_out)[k] = k;
   bp.g = 1; bp.n_groups = K;
-  if (M != 3 || d->scheme == CHFPE_COMPACT6 || !env_int("CHFPE_BRICK", 1)) return bp;
-  if (d->nq[0] > 1023 || d->nq[1] > 1023 || d->nq[2] > 1023 || (long long)pl.K * pl.nqc > 0x7fffffffLL) return bp;
-  bp.P1 = d->np[0]; bp.P2 = d->np[1]; bp.P3 = d->np[2];
+  if (M < 2 || d->scheme == CHFPE_COMPACT6 || !env_int("CHFPE_BRICK", 1)) return bp;
+  // two modes run as three with a one-point, uncoupled middle mode (same memory layout)
+  const int vnq[3] = {d->nq[0], M == 3 ? d->nq[1] : 1, M == 3 ? d->nq[2] : d->nq[1]};
+  const int vnp[3] = {d->np[0], M == 3 ? d->np[1] : 1, M == 3 ? d->np[2] : d->np[1]};
+  if (vnq[0] > 1023 || vnq[1] > 1023 || vnq[2] > 1023 || (long long)pl.K * pl.nqc > 0x7fffffffLL) return bp;
+  bp.P1 = vnp[0]; bp.P2 = vnp[1]; bp.P3 = vnp[2];
   bp.PB2 = bp.P2 * bp.P3;
   // threads per CTA = split * P2*P3/2 (128-bit accesses); aim at ~512 threads (one CTA per SM at 128 registers)
   // with >= 4 planes per thread: at 16^3 the 256-thread / 2-CTA variant times the same but its register allocation
@@ -135,31 +138,38 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
          split_default * bp.PB2 / 2 < 384)
     split_default *= 2;
   if (bp.P1 == 12) split_default = 2;
+  if (M == 2) split_default = (bp.P1 == 48) ? 8 : 4;                  // the instantiated two-mode shapes
   bp.split = env_int("CHFPE_BRICK_SPLIT", split_default);
   bp.minb = env_int("CHFPE_BRICK_MINB", (bp.PB2 * bp.split / 2 <= 256) ? 2 : 1);
+  bp.vn[0] = vnq[0]; bp.vn[1] = vnq[1]; bp.vn[2] = vnq[2];
   bp.fixed = brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb);
   if (!bp.fixed) return bp;
   // L2 reuse window = five q_1 planes x (q_2 chunk + 2+2 halo rows) x g elements of the stage input; budget 64 MiB
   // of the 126 MB L2 (the rest serves the once-touched streams).  Pairs of linked elements (g = 2) save one
   // neighbour-brick read per pair if at least 6 q_2 rows per chunk still fit, else one element at a time.
-  const double plane_bytes = 8.0 * (double)pl.cells / d->nq[0];
-  const double row_bytes = plane_bytes / d->nq[1];                 // one q_2 row of one q_1 plane
+  const double plane_bytes = 8.0 * (double)pl.cells / vnq[0];
+  const double row_bytes = plane_bytes / vnq[1];                 // one q_2 row of one q_1 plane
   const double budget = 64.0 * 1024 * 1024;
   auto rows_that_fit = [&](int gg) { return (int)(budget / (5.0 * row_bytes * gg)) - 4; };
   int g = (K >= 2 && rows_that_fit(2) >= 6) ? 2 : 1;
+  if (vnq[1] == 1) {                                                 // no q_2 rows to chunk: as many whole planes as fit
+    g = (int)(budget / (5.0 * plane_bytes));
+    if (g < 1) g = 1;
+    if (g > K) g = K;
+  }
   g = env_int("CHFPE_GROUP", g);
   if (g < 1) g = 1;
   if (g > K) g = K;
   int cs = rows_that_fit(g);
-  if (cs >= d->nq[1]) cs = d->nq[1];
+  if (cs >= vnq[1]) cs = vnq[1];
   else {
     if (cs < 4) cs = 4;
-    const int nch = (d->nq[1] + cs - 1) / cs;                      // equalise the chunks
-    cs = (d->nq[1] + nch - 1) / nch;
+    const int nch = (vnq[1] + cs - 1) / cs;                      // equalise the chunks
+    cs = (vnq[1] + nch - 1) / nch;
   }
   cs = env_int("CHFPE_Q2CHUNK", cs);
   if (cs < 1) cs = 1;
-  if (cs > d->nq[1]) cs = d->nq[1];
+  if (cs > vnq[1]) cs = vnq[1];
   bp.q2chunk = cs;
   // greedy grouping: grow each group by the unassigned element with most hierarchy links into it
   std::vector<int> assigned(K, 0), order;
@@ -184,11 +194,11 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   *order_out = order;
   bp.g = g; bp.n_groups = (K + g - 1) / g;
   bp.blocks_per_full_group = (long long)g * pl.nqc;
-  bp.rest = pl.nqc / d->nq[0];
+  bp.rest = pl.nqc / vnq[0];
   bp.enabled = 1;
   {                                                                  // bricks per CTA: amortises the per-CTA setup
     int bpc = 1;                                                     // (16^6: 4.47 -> 4.17 ms); a divisor of n_q3 so
-    for (int c = 2; c <= 16; c++) if (d->nq[2] % c == 0) bpc = c;    // that a run never straddles two q_3 lines
+    for (int c = 2; c <= 16; c++) if (vnq[2] % c == 0) bpc = c;    // that a run never straddles two q_3 lines
     bp.bpc = env_int("CHFPE_BPC", bpc);
   }
   if (bp.bpc < 1) bp.bpc = 1;
@@ -330,7 +340,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   h->bp.l2mode = env_int("CHFPE_L2MODE", 1);
   if (h->bp.enabled) {                                                 // tabulate the brick order (decode_brick_id)
     const BrickPlan& b = h->bp;
-    const int n1 = desc->nq[0], n2 = desc->nq[1], n3 = desc->nq[2], cs = b.q2chunk;
+    const int n1 = b.vn[0], n2 = b.vn[1], n3 = b.vn[2], cs = b.q2chunk;
     const int nch = (n2 + cs - 1) / cs;
     std::vector<int> tab;
     tab.reserve((size_t)4 * pl.K * pl.nqc);
@@ -342,9 +352,10 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
           for (int kk = 0; kk < gs; kk++) {
             const int k = order[G * b.g + kk];
             int own = 0;
-            for (int s = 0; s < 3; s++) {
-              if (up[3 * k + s] >= 0 && pos[up[3 * k + s]] / b.g == G) own |= 1 << (2 * s);
-              if (dn[3 * k + s] >= 0 && pos[dn[3 * k + s]] / b.g == G) own |= 1 << (2 * s + 1);
+            for (int s = 0; s < M; s++) {
+              const int vs = (M == 2 && s == 1) ? 2 : s;                // mode index in the three-mode view
+              if (up[3 * k + s] >= 0 && pos[up[3 * k + s]] / b.g == G) own |= 1 << (2 * vs);
+              if (dn[3 * k + s] >= 0 && pos[dn[3 * k + s]] / b.g == G) own |= 1 << (2 * vs + 1);
             }
             for (int r2 = 0; r2 < w; r2++)
               for (int i3 = 0; i3 < n3; i3++) {
@@ -359,6 +370,38 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
     }
     h->bp.table = (const int4*)put(tab.data(), sizeof(int) * tab.size());
     cudaStreamSynchronize(h->stream);                                  // `tab` goes out of scope
+    // operator as the three-mode kernels see it
+    h->op3 = op;
+    if (M == 2) {
+      DevOp& v = h->op3;
+      v.M = 3; v.nax = 6;
+      const int map[3] = {0, -1, 1};                                   // view mode -> real mode
+      for (int vs = 0; vs < 3; vs++) {
+        const int r = map[vs];
+        v.n[vs] = r < 0 ? 1 : op.n[r];          v.n[3 + vs] = r < 0 ? 1 : op.n[M + r];
+        v.x0[vs] = r < 0 ? 0.0 : op.x0[r];      v.x0[3 + vs] = r < 0 ? 0.0 : op.x0[M + r];
+        v.h[vs] = r < 0 ? 1.0 : op.h[r];        v.h[3 + vs] = r < 0 ? 1.0 : op.h[M + r];
+        v.c1[vs] = r < 0 ? 0.0 : op.c1[r];      v.c1[3 + vs] = r < 0 ? 0.0 : op.c1[M + r];
+        v.c2[vs] = r < 0 ? 0.0 : op.c2[r];      v.c2[3 + vs] = r < 0 ? 0.0 : op.c2[M + r];
+        v.inv_mass[vs] = r < 0 ? 0.0 : op.inv_mass[r];
+        v.kup[vs] = r < 0 ? 0.0 : op.kup[r];    v.kdn[vs] = r < 0 ? 0.0 : op.kdn[r];
+        v.cdn[vs] = r < 0 ? 0.0 : op.cdn[r];
+        v.VLL[vs] = r < 0 ? 0.0 : op.VLL[r];    v.VSL[vs] = r < 0 ? 0.0 : op.VSL[r];
+        v.dU[vs] = op.dU[r < 0 ? 0 : r];
+      }
+      long long st = 1;
+      for (int a2 = 5; a2 >= 0; a2--) { v.st[a2] = st; st *= v.n[a2]; }
+      std::vector<int> up3(3 * pl.K, -1), dn3(3 * pl.K, -1), nv3(3 * pl.K, 0);
+      for (int k = 0; k < pl.K; k++)
+        for (int vs = 0; vs < 3; vs++)
+          if (map[vs] >= 0) {
+            up3[3 * k + vs] = up[3 * k + map[vs]]; dn3[3 * k + vs] = dn[3 * k + map[vs]]; nv3[3 * k + vs] = nv[3 * k + map[vs]];
+          }
+      v.up = (const int*)put(up3.data(), sizeof(int) * up3.size());
+      v.dn = (const int*)put(dn3.data(), sizeof(int) * dn3.size());
+      v.nvec = (const int*)put(nv3.data(), sizeof(int) * nv3.size());
+      cudaStreamSynchronize(h->stream);
+    }
   }
   if (h->bp.enabled && brick_configure(h->bp, M) != 0) { cudaGetLastError(); h->bp.enabled = 0; }
   if (h->bp.enabled && h->bp.pipe) {
@@ -444,7 +487,7 @@ static int run_stage(chfpe_handle* h, const double* in, const double* y, double*
   if (h->op.scheme == CHFPE_COMPACT6)
     return launch_stage_compact(h->op, h->ct, in, y, out, a, c, nb, ss, h->scratch, h->stream);
   if (h->bp.enabled && h->bp.pipe) return launch_stage_pipe(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
-  if (h->bp.enabled) return launch_stage_brick(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
+  if (h->bp.enabled) return launch_stage_brick(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
   return launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);
 }
 

@@ -79,7 +79,10 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
                double cc, size_t slot_stride, int y_is_in) {
   static_assert(P3 % 2 == 0 && P1 % SPLIT == 0 && (SPLIT == 1 || P1 / SPLIT >= 2), "unsupported brick shape");
   constexpr int PLANE = P2 * P3, PL2 = PLANE / 2, NTT = SPLIT * PL2, NC = P1 / SPLIT;
-  constexpr int G2_ROW = P3, G2_PLANE = (P2 + 4) * P3;              // G_2[i1][i2+2][i3]
+  // P2 == 1: two-mode systems run as a three-mode one whose middle mode has a single q and a single p point and no
+  // couplings (same memory layout); everything that belongs to that mode is compiled out.
+  constexpr bool SKIP1 = (P2 == 1);
+  constexpr int G2_ROW = P3, G2_PLANE = SKIP1 ? 0 : (P2 + 4) * P3;  // G_2[i1][i2+2][i3]
   constexpr int G3_ROW = P3 + 4, G3_PLANE = P2 * (P3 + 4);          // G_3[i1][i2][i3+2]
   extern __shared__ __align__(16) double sm[];
   double* g2 = sm;
@@ -91,7 +94,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const int i2 = tid / (P3 / 2), i3 = 2 * (tid - i2 * (P3 / 2));
 
   // zero the ghost rows / columns of the two shared bricks
-  for (int i = threadIdx.x; i < P1 * 4 * P3; i += NTT) {            // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
+  for (int i = threadIdx.x; i < (SKIP1 ? 0 : P1 * 4 * P3); i += NTT) {   // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
     const int pl = i / (4 * P3), rr = i - pl * (4 * P3), row = rr / P3, col = rr - row * P3;
     g2[pl * G2_PLANE + (row < 2 ? row : P2 + row) * G2_ROW + col] = 0.0;
   }
@@ -135,6 +138,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     if (!y_is_in) bulk_prefetch_l2(y + boff + (size_t)k * op.cells + b0, BB);
 #pragma unroll
     for (int s = 0; s < 3; s++) {
+      if (SKIP1 && s == 1) continue;
       if (kup[s] >= 0) bulk_prefetch_l2(Xd + (size_t)kup[s] * op.cells + b0, BB);
       if (kdn[s] >= 0) bulk_prefetch_l2(Xd + (size_t)kdn[s] * op.cells + b0, BB);
     }
@@ -146,6 +150,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   // ---- -(p_s/m_s) dW/dq_s: same pair of the 4 neighbouring bricks of this element along every q axis ----
 #pragma unroll
   for (int s = 0; s < 3; s++) {
+    if (SKIP1 && s == 1) continue;
     const long long st2 = op.st[s] >> 1;                            // brick stride of q_s in double2 (even)
     const int i = bid.iq[s], n = op.n[s];
     const double wq = -(wide ? -op.c2[s] : op.c1[s]) * op.inv_mass[s];   // -(1/m_s) / (12 h) or / (2 h)
@@ -205,6 +210,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   double2 g3own[KEEP_G3 ? NC : 1];
 #pragma unroll
   for (int s = 0; s < 3; s++) {
+    if (SKIP1 && s == 1) continue;
     const double qs = op.x0[s] + bid.iq[s] * op.h[s];
     const double Vp = fma(op.VSL[s], qs, op.VLL[s]);
     const double dUs = __ldg(op.dU[s] + ql);
@@ -297,21 +303,28 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     for (int j = 0; j < NC; j++) {
       const double* a2 = c2 + j * G2_PLANE;
       const double* a3 = c3 + j * G3_PLANE;
-      const double2 u1 = *reinterpret_cast<const double2*>(a2 + G2_ROW), d1 = *reinterpret_cast<const double2*>(a2 - G2_ROW);
-      double e2x = u1.x - d1.x, e2y = u1.y - d1.y;
+      double e2x = 0.0, e2y = 0.0;
+      if (!SKIP1) {
+        const double2 u1 = *reinterpret_cast<const double2*>(a2 + G2_ROW), d1 = *reinterpret_cast<const double2*>(a2 - G2_ROW);
+        e2x = u1.x - d1.x; e2y = u1.y - d1.y;
+      }
       const double2 lft = *reinterpret_cast<const double2*>(a3 - 2), rgt = *reinterpret_cast<const double2*>(a3 + 2);
       // pair (i3, i3+1): neighbours i3-2..i3+3 = lft.x lft.y [own.x own.y] rgt.x rgt.y
       const double2 own = KEEP_G3 ? g3own[KEEP_G3 ? j : 0] : *reinterpret_cast<const double2*>(a3);
       double e3x = own.y - lft.y, e3y = rgt.x - own.x;
       if (wide) {
-        const double2 u2 = *reinterpret_cast<const double2*>(a2 + 2 * G2_ROW), d2 = *reinterpret_cast<const double2*>(a2 - 2 * G2_ROW);
-        e2x = fma(8.0, e2x, -(u2.x - d2.x));
-        e2y = fma(8.0, e2y, -(u2.y - d2.y));
+        if (!SKIP1) {
+          const double2 u2 = *reinterpret_cast<const double2*>(a2 + 2 * G2_ROW), d2 = *reinterpret_cast<const double2*>(a2 - 2 * G2_ROW);
+          e2x = fma(8.0, e2x, -(u2.x - d2.x));
+          e2y = fma(8.0, e2y, -(u2.y - d2.y));
+        }
         e3x = fma(8.0, e3x, -(rgt.x - lft.x));
         e3y = fma(8.0, e3y, -(rgt.y - lft.y));
       }
-      acc[j].x = fma(w2, e2x, acc[j].x);
-      acc[j].y = fma(w2, e2y, acc[j].y);
+      if (!SKIP1) {
+        acc[j].x = fma(w2, e2x, acc[j].x);
+        acc[j].y = fma(w2, e2y, acc[j].y);
+      }
       acc[j].x = fma(w3, e3x, acc[j].x);
       acc[j].y = fma(w3, e3y, acc[j].y);
     }
@@ -333,15 +346,15 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
 
 template <int P1, int P2, int P3, int SPLIT>
 constexpr int brick3_smem_bytes() {
-  return (int)sizeof(double) * (P1 * (P2 + 4) * P3 + P1 * P2 * (P3 + 4) + (SPLIT > 1 ? SPLIT * 4 * P2 * P3 : 0));
+  return (int)sizeof(double) * ((P2 == 1 ? 0 : P1 * (P2 + 4) * P3) + P1 * P2 * (P3 + 4) + (SPLIT > 1 ? SPLIT * 4 * P2 * P3 : 0));
 }
 
 }  // namespace
 
-#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 4, 1) X(16, 16, 16, 2, 2) X(20, 20, 20, 2, 1) X(12, 12, 12, 2, 2) X(8, 8, 8, 2, 2)
+#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 4, 1) X(16, 16, 16, 2, 2) X(20, 20, 20, 2, 1) X(12, 12, 12, 2, 2) X(8, 8, 8, 2, 2) X(48, 1, 48, 8, 2) X(16, 1, 16, 4, 2)
 
-int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {
-  if (M != 3) return 0;
+int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {   // M = 2 arrives as (P1, 1, P2)
+  if (M != 3 && M != 2) return 0;
 #define X(A, B, C, S, MB) if (P1 == A && P2 == B && P3 == C && split == S && minb == MB) return 1;
   BRICK3_SPECIALISATIONS(X)
 #undef X
@@ -350,7 +363,7 @@ int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {
 
 int brick_configure(const BrickPlan& bp, int M) {
   cudaError_t e = cudaErrorInvalidValue;
-  if (M != 3) return (int)e;
+  if (M != 3 && M != 2) return (int)e;
 #define X(A, B, C, S, MB)                                                                                 \
   if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                           \
     e = cudaFuncSetAttribute(k_stage_brick3<A, B, C, S, MB>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \

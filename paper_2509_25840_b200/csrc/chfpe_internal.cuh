@@ -33,7 +33,8 @@ struct DevOp {
 // Launch plan of the brick kernels (chfpe_brick.cu, chfpe_pipe.cu): one CTA per (element, q-point) p-brick.
 struct BrickPlan {
   int enabled;
-  int P1, P2, P3, PB2;                // p-extents, PB2 = P2*P3
+  int P1, P2, P3, PB2;                // p-extents, PB2 = P2*P3 (two modes: P2 = 1)
+  int vn[3];                          // q-extents as the three-mode kernels see them (two modes: vn[1] = 1)
   int g;                              // elements per lock-step group (L2 window)
   int n_groups;
   long long blocks_per_full_group;    // g * nqc
@@ -86,6 +87,7 @@ struct chfpe_handle {
   chfpe_desc desc;
   std::vector<chfpe_monomial> U;
   DevOp op;
+  DevOp op3;                          // the same operator as a three-mode one (identical for M = 3), brick kernels
   BrickPlan bp;
   CompactTables ct;
   double* scratch;                    // COMPACT6 only: three element-sized arrays (G, D, F)

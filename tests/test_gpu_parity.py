@@ -42,6 +42,8 @@ SMALL = [
     ("m3_sqrt", ci.config("cfg4s8", nq=[7, 8, 6], np=[8, 6, 9], depth=3)),
     ("m3_w_c2", ci.config("cfg4s8", nq=[6, 5, 7], np=[5, 7, 6], depth=2, gauge="w", scheme="central2",
                           mass=[1.0, 0.8, 1.2])),
+    ("m2_16_brick", ci.config("cfg3s", nq=[7, 9])),
+    ("m2_48_brick_w", ci.config("cfg3", nq=[6, 5], depth=2, gauge="w", mass=[1.0, 1.3])),
     ("m3_cube8", ci.config("cfg4s8")),
     ("m3_cube12", ci.config("cfg4s12", nq=[5, 6, 7])),
     ("m3_cube16_w", ci.config("cfg4", nq=[5, 5, 6], gauge="w")),
