@@ -160,11 +160,12 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     if (wide && i >= 2 && i + 2 < n) {                              // interior in q_s: all four neighbours exist
       const double2* bp2 = Xk + 2 * st2;
       const double2* bm2 = Xk - 2 * st2;
-      constexpr int CH = (NC <= 5) ? NC : (NC % 5 == 0 ? 5 : (NC % 4 == 0 ? 4 : (NC % 3 == 0 ? 3 : 1)));   // planes per load batch
-      Unroll<0, NC / CH>::run([&](auto C0) {
+      constexpr int CH = (NC <= 5) ? NC : 4;                        // planes per load batch (<= 20 loads), last one partial
+      Unroll<0, (NC + CH - 1) / CH>::run([&](auto C0) {
         constexpr int j0 = decltype(C0)::value * CH;
-        double2 vp1[CH], vm1[CH], vp2[CH], vm2[CH];
-        Unroll<0, CH>::run([&](auto J) {
+        constexpr int CN = (NC - j0 < CH) ? NC - j0 : CH;
+        double2 vp1[CN], vm1[CN], vp2[CN], vm2[CN];
+        Unroll<0, CN>::run([&](auto J) {
           constexpr int j = decltype(J)::value;
           vp1[j] = ldg2o<(j0 + j) * PL2>(bp1, pol_own);
           vm1[j] = ldg2o<(j0 + j) * PL2>(bm1, pol_own);
@@ -172,7 +173,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
           vm2[j] = ldg2o<(j0 + j) * PL2>(bm2, pol_own);
         });
 #pragma unroll
-        for (int j = 0; j < CH; j++) {
+        for (int j = 0; j < CN; j++) {
           const double ex = fma(8.0, vp1[j].x - vm1[j].x, -(vp2[j].x - vm2[j].x));
           const double ey = fma(8.0, vp1[j].y - vm1[j].y, -(vp2[j].y - vm2[j].y));
           const double c1 = wq * fma((double)(j0 + j), h1, p1_0);
