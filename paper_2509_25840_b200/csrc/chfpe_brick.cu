@@ -1,4 +1,4 @@
-// Brick kernel of the RK stage (steps a1-a3 of DESIGN.md) for three modes on sm_100a.
+// Brick kernel of the RK stage (steps a1-a3 of DESIGN.md) for two and three modes on sm_100a.
 //
 // Internal layout [k][q_1..q_M][p_1..p_M] makes all momenta of one (element, q-point) a contiguous "p-brick".
 // Everything in Eq. (8) :77-80 except the q-derivatives of Eq. (9)-(10) :86-91 is local to the bricks of one
@@ -7,7 +7,8 @@
 //     G_s = (dU/dq_s) X_k + V'_s X_up(k,s) + n_s c_s V'_s X_dn(k,s)                      (per cell, 3 flops)
 // The gauge terms kappa p_s X_{up,dn} are pointwise.  The q-derivatives are pointwise in the brick: coalesced loads
 // of the same cell of the 12 neighbouring bricks of the same element, which the L2 serves (CTAs are ordered q_1-plane
-// by q_1-plane, element group by group).  One CTA = one brick.  Grids without a compile-time specialisation run the
+// by q_1-plane, element group by group).  A CTA walks a short run of bricks; two-mode grids run as three-mode
+// ones with a one-point middle mode (P2 == 1).  Grids without a compile-time specialisation run the
 // generic kernel of chfpe_kernels.cu (a run-time-shaped brick kernel was measured slower than it and removed).
 #include <type_traits>
 #include "chfpe_internal.cuh"
