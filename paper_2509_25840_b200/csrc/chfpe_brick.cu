@@ -74,12 +74,14 @@ constexpr int brick3_maxreg(int nt, int minb) {
   return r > 255 ? 255 : r;
 }
 
-template <int P1, int P2, int P3, int SPLIT, int MINB>
+// NPASS > 1: a brick is processed in NPASS passes over blocks of P1/NPASS consecutive p_1 planes (large bricks: keeps
+// the per-thread state small); G_1 of the two planes beyond a block edge is recomputed from three extra loads.
+template <int P1, int P2, int P3, int SPLIT, int MINB, int NPASS>
 __global__ void __launch_bounds__(SPLIT * P2 * P3 / 2) __maxnreg__(brick3_maxreg(SPLIT * P2 * P3 / 2, MINB))
 k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const double* y, double* out, double a,
                double cc, size_t slot_stride, int y_is_in) {
-  static_assert(P3 % 2 == 0 && P1 % SPLIT == 0 && (SPLIT == 1 || P1 / SPLIT >= 2), "unsupported brick shape");
-  constexpr int PLANE = P2 * P3, PL2 = PLANE / 2, NTT = SPLIT * PL2, NC = P1 / SPLIT;
+  static_assert(P3 % 2 == 0 && P1 % (SPLIT * NPASS) == 0 && P1 / (SPLIT * NPASS) >= 2, "unsupported brick shape");
+  constexpr int PLANE = P2 * P3, PL2 = PLANE / 2, NTT = SPLIT * PL2, P1P = P1 / NPASS, NC = P1P / SPLIT;
   // P2 == 1: two-mode systems run as a three-mode one whose middle mode has a single q and a single p point and no
   // couplings (same memory layout); everything that belongs to that mode is compiled out.
   constexpr bool SKIP1 = (P2 == 1);
@@ -87,19 +89,19 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   constexpr int G3_ROW = P3 + 4, G3_PLANE = P2 * (P3 + 4);          // G_3[i1][i2][i3+2]
   extern __shared__ __align__(16) double sm[];
   double* g2 = sm;
-  double* g3 = sm + P1 * G2_PLANE;
-  double* xg = g3 + P1 * G3_PLANE;                                  // [SPLIT][4][PLANE]: first/last two G_1 planes of a segment
+  double* g3 = sm + P1P * G2_PLANE;
+  double* xg = g3 + P1P * G3_PLANE;                                 // [SPLIT][4][PLANE]: first/last two G_1 planes of a segment
   const int seg = (SPLIT == 1) ? 0 : threadIdx.x / PL2;
   const int tid = threadIdx.x - seg * PL2;                          // pair index inside the plane
   const int jbase = seg * NC;                                       // first p_1 plane of this thread
   const int i2 = tid / (P3 / 2), i3 = 2 * (tid - i2 * (P3 / 2));
 
   // zero the ghost rows / columns of the two shared bricks
-  for (int i = threadIdx.x; i < (SKIP1 ? 0 : P1 * 4 * P3); i += NTT) {   // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
+  for (int i = threadIdx.x; i < (SKIP1 ? 0 : P1P * 4 * P3); i += NTT) {   // G_2: rows i2 = -2,-1,P2,P2+1 of every plane
     const int pl = i / (4 * P3), rr = i - pl * (4 * P3), row = rr / P3, col = rr - row * P3;
     g2[pl * G2_PLANE + (row < 2 ? row : P2 + row) * G2_ROW + col] = 0.0;
   }
-  for (int i = threadIdx.x; i < P1 * P2 * 4; i += NTT) {            // G_3: columns i3 = -2,-1,P3,P3+1 of every row
+  for (int i = threadIdx.x; i < P1P * P2 * 4; i += NTT) {           // G_3: columns i3 = -2,-1,P3,P3+1 of every row
     const int rw = i >> 2, c4 = i & 3;
     g3[rw * G3_ROW + (c4 < 2 ? c4 : P3 + c4)] = 0.0;
   }
@@ -107,7 +109,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const unsigned long long pol_own = l2_policy((bp.l2mode & 2) ? 2 : 0);
   const unsigned long long pol_str = l2_policy((bp.l2mode & 1) ? 1 : 0);
   const bool wide = (op.scheme == CHFPE_CENTRAL4);
-  const double h1 = op.h[3], p1_0 = op.x0[3] + jbase * h1;
+  const double h1 = op.h[3];
   const double p2 = op.x0[4] + i2 * op.h[4];
   const double p3a = op.x0[5] + i3 * op.h[5], p3b = op.x0[5] + (i3 + 1) * op.h[5];
   // ---- bricks of this CTA: bp.bpc consecutive entries of the brick order (setup above is paid once) ----
@@ -119,7 +121,11 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   const size_t boff = (size_t)blockIdx.y * slot_stride;
   const double2* X2 = reinterpret_cast<const double2*>(in + boff);  // replica base
   const unsigned cells2 = (unsigned)(op.cells >> 1);                // element stride in double2
-  const unsigned tpart = (unsigned)(jbase * PL2 + tid);             // this thread's first pair inside a brick
+#pragma unroll 1
+  for (int pass = 0; pass < NPASS; pass++) {
+  const int pofs = pass * P1P;                                      // first p_1 plane of this pass
+  const double p1_0 = op.x0[3] + (pofs + jbase) * h1;
+  const unsigned tpart = (unsigned)((pofs + jbase) * PL2 + tid);    // this thread's first pair inside a brick
   const unsigned brick2 = ql * (unsigned)(P1 * PL2);                // brick offset inside an element
   const double2* Xk = X2 + ((size_t)k * cells2 + brick2 + tpart);   // own pairs: Xk[j * PL2]
 
@@ -131,7 +137,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   // Everything this brick needs from HBM (its own stage input, the bricks of its hierarchy neighbours, y) is
   // requested into L2 now -- one bulk prefetch per array, issued by one thread -- and consumed after the
   // q-derivative part, whose loads are L2 hits on the q_1-plane window and cover the DRAM latency.
-  if (threadIdx.x == 0) {
+  if (threadIdx.x == 0 && pass == 0) {
     constexpr unsigned BB = P1 * PLANE * sizeof(double);
     const double* Xd = in + boff;
     const size_t b0 = (size_t)ql * (P1 * PLANE);
@@ -278,6 +284,33 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
         }
       }
     });
+    if (NPASS > 1 && s == 0) {                                      // G_1 on the two planes beyond a pass edge
+      if (seg == SPLIT - 1 && pass + 1 < NPASS) {
+#pragma unroll
+        for (int hp = 0; hp < 2; hp++) {
+          double2 gg = hp == 0 ? ldg2o<NC * PL2>(Xk, pol_own) : ldg2o<(NC + 1) * PL2>(Xk, pol_own);
+          gg = make_double2(dUs * gg.x, dUs * gg.y);
+          if (ku >= 0) gg = fma2(cu, hp == 0 ? ldg2o<NC * PL2>(Xu, pol_u) : ldg2o<(NC + 1) * PL2>(Xu, pol_u), gg);
+          if (kd >= 0) gg = fma2(cd, hp == 0 ? ldg2o<NC * PL2>(Xd, pol_d) : ldg2o<(NC + 1) * PL2>(Xd, pol_d), gg);
+          if (hp == 0) { acc[NC - 1] = fma2(wp8, gg, acc[NC - 1]); acc[NC - 2] = fma2(-wp1, gg, acc[NC - 2]); }
+          else acc[NC - 1] = fma2(-wp1, gg, acc[NC - 1]);
+        }
+      }
+      if (seg == 0 && pass > 0) {
+        const double2* Xkm = Xk - 2 * PL2;
+        const double2* Xum = Xu - 2 * PL2;
+        const double2* Xdm = Xd - 2 * PL2;
+#pragma unroll
+        for (int hp = 0; hp < 2; hp++) {                            // hp = 0: plane -2, hp = 1: plane -1
+          double2 gg = hp == 0 ? ldg2o<0>(Xkm, pol_own) : ldg2o<PL2>(Xkm, pol_own);
+          gg = make_double2(dUs * gg.x, dUs * gg.y);
+          if (ku >= 0) gg = fma2(cu, hp == 0 ? ldg2o<0>(Xum, pol_u) : ldg2o<PL2>(Xum, pol_u), gg);
+          if (kd >= 0) gg = fma2(cd, hp == 0 ? ldg2o<0>(Xdm, pol_d) : ldg2o<PL2>(Xdm, pol_d), gg);
+          if (hp == 1) { acc[0] = fma2(-wp8, gg, acc[0]); acc[1] = fma2(wp1, gg, acc[1]); }
+          else acc[0] = fma2(wp1, gg, acc[0]);
+        }
+      }
+    }
   }
   __syncthreads();
   if (SPLIT > 1) {
@@ -342,22 +375,24 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   for (int j = 0; j < NC; j++) acc[j] = make_double2(fma(cc, acc[j].x, a * xk[j].x), fma(cc, acc[j].y, a * xk[j].y));
   double2* O = reinterpret_cast<double2*>(out + boff) + ((size_t)k * cells2 + brick2 + tpart);
   Unroll<0, NC>::run([&](auto J) { constexpr int j = decltype(J)::value; st2o<j * PL2>(O, acc[j], pol_str); });
-  __syncthreads();                                                  // shared bricks free for the next brick
-  }
+  __syncthreads();                                                  // shared bricks free for the next pass / brick
+  }  // pass
+  }  // brick
 }
 
-template <int P1, int P2, int P3, int SPLIT>
+template <int P1, int P2, int P3, int SPLIT, int NPASS>
 constexpr int brick3_smem_bytes() {
-  return (int)sizeof(double) * ((P2 == 1 ? 0 : P1 * (P2 + 4) * P3) + P1 * P2 * (P3 + 4) + (SPLIT > 1 ? SPLIT * 4 * P2 * P3 : 0));
+  return (int)sizeof(double) * ((P2 == 1 ? 0 : (P1 / NPASS) * (P2 + 4) * P3) + (P1 / NPASS) * P2 * (P3 + 4) +
+                                (SPLIT > 1 ? SPLIT * 4 * P2 * P3 : 0));
 }
 
 }  // namespace
 
-#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 4, 1) X(16, 16, 16, 2, 2) X(20, 20, 20, 2, 1) X(12, 12, 12, 2, 2) X(8, 8, 8, 2, 2) X(48, 1, 48, 8, 2) X(16, 1, 16, 4, 2)
+#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 4, 1, 1) X(16, 16, 16, 2, 2, 1) X(20, 20, 20, 2, 1, 1) X(20, 20, 20, 2, 1, 2) X(12, 12, 12, 2, 2, 1) X(8, 8, 8, 2, 2, 1) X(48, 1, 48, 8, 2, 1) X(16, 1, 16, 4, 2, 1)
 
-int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {   // M = 2 arrives as (P1, 1, P2)
+int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb, int npass) {   // M = 2 arrives as (P1, 1, P2)
   if (M != 3 && M != 2) return 0;
-#define X(A, B, C, S, MB) if (P1 == A && P2 == B && P3 == C && split == S && minb == MB) return 1;
+#define X(A, B, C, S, MB, NP) if (P1 == A && P2 == B && P3 == C && split == S && minb == MB && npass == NP) return 1;
   BRICK3_SPECIALISATIONS(X)
 #undef X
   return 0;
@@ -366,10 +401,10 @@ int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb) {   // M
 int brick_configure(const BrickPlan& bp, int M) {
   cudaError_t e = cudaErrorInvalidValue;
   if (M != 3 && M != 2) return (int)e;
-#define X(A, B, C, S, MB)                                                                                 \
-  if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                           \
-    e = cudaFuncSetAttribute(k_stage_brick3<A, B, C, S, MB>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
-                             brick3_smem_bytes<A, B, C, S>());
+#define X(A, B, C, S, MB, NP)                                                                             \
+  if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB && bp.npass == NP)         \
+    e = cudaFuncSetAttribute(k_stage_brick3<A, B, C, S, MB, NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                             brick3_smem_bytes<A, B, C, S, NP>());
   BRICK3_SPECIALISATIONS(X)
 #undef X
   return (int)e;
@@ -379,9 +414,9 @@ int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, c
                        double c, int nb, size_t slot_stride, cudaStream_t s) {
   dim3 grid((unsigned)(((long long)op.K * op.nqc + bp.bpc - 1) / bp.bpc), nb);
   const int y_is_in = (y == in) ? 1 : 0;
-#define X(A, B, C, S, MB)                                                                                  \
-  if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB)                            \
-    k_stage_brick3<A, B, C, S, MB><<<grid, S * B * C / 2, brick3_smem_bytes<A, B, C, S>(), s>>>(           \
+#define X(A, B, C, S, MB, NP)                                                                              \
+  if (bp.P1 == A && bp.P2 == B && bp.P3 == C && bp.split == S && bp.minb == MB && bp.npass == NP)          \
+    k_stage_brick3<A, B, C, S, MB, NP><<<grid, S * B * C / 2, brick3_smem_bytes<A, B, C, S, NP>(), s>>>(   \
         op, bp, in, y, out, a, c, slot_stride, y_is_in);
   BRICK3_SPECIALISATIONS(X)
 #undef X

@@ -46,6 +46,7 @@ struct BrickPlan {
   const int4* table;                  // [K * n_q] brick order (device), see decode_brick_id
   int l2mode;                         // bit 0: once-touched data evict_first, bit 1: window data evict_last
   int minb;                           // CTAs per SM the specialised kernel is compiled for (register budget)
+  int npass;                          // passes over blocks of P1/npass planes per brick (large bricks)
   int split;                          // p_1 segments (thread groups) per brick in the specialised kernel
   int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3,...>) exists
   int pipe;                           // use the plane-pipelined kernel (chfpe_pipe.cu)
@@ -134,7 +135,7 @@ int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, c
                        double a, double c, int nb, size_t slot_stride, cudaStream_t s);
 // one-off opt-in to > 48 KB dynamic shared memory for the brick kernels; returns a cudaError_t as int
 int brick_configure(const BrickPlan& bp, int M);
-int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb);
+int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb, int npass);
 // plane-pipelined variant (chfpe_pipe.cu): bulk async copies into a shared-memory ring, persistent CTAs
 int pipe_has_fixed(int M, int P1, int P2, int P3, int stages);
 size_t pipe_smem_bytes(const BrickPlan& bp);
