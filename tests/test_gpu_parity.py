@@ -370,3 +370,18 @@ def test_compact6_closed_form_response():
     gold = [0.0, 0.4704830104, 0.7836581507, 0.8508220546, 0.6713837425]
     assert np.max(np.abs(-R - np.array(gold))) < 2e-7
     g.close()
+
+
+def test_response_2d_shrunken_config5():
+    """Config 5 protocol (A = mu, B = C = alpha, t1 replicas batched) on the 10^6 shrink of its model with 3 slots:
+    as many steps as the oracle affords in about half a minute (3 t1 x 3 t2 delays, 18 oracle steps of 2e7 values)."""
+    cfg = ci.config("cfg4s10")
+    g, o = both(cfg, batch=3)
+    mu_g, mu_o = obs_pair("mu", 3)
+    al_g, al_o = obs_pair("alpha", 3)
+    g.equilibrate(); o.equilibrate()
+    t1, t2 = [0, 1, 3], [0, 2, 5]
+    Rg = g.response_2d(mu_g, al_g, al_g, t1, t2, cfg["dt"])
+    Ro = o.response_2d(mu_o, al_o, al_o, t1, t2, cfg["dt"])
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    g.close()
