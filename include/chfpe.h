@@ -132,6 +132,12 @@ int chfpe_launch_count(const chfpe_handle* h, int64_t* n);
 int chfpe_profile_enable(chfpe_handle* h, int on);
 int chfpe_profile_read(chfpe_handle* h, double* total_ms, int64_t* n_launches);
 
+/* Which kernel family runs the RK stage on this handle (host pointer), so that a test or a benchmark can assert
+   that a configuration did not fall back to the generic kernel.  The cooperative multi-step kernel of tiny
+   states is a property of the step call, not of the handle, and is not reported here. */
+enum { CHFPE_STAGE_GENERIC = 0, CHFPE_STAGE_BRICK = 1, CHFPE_STAGE_PIPE = 2, CHFPE_STAGE_COMPACT = 3 };
+int chfpe_stage_kernel(const chfpe_handle* h, int32_t* kind);
+
 const char* chfpe_last_error(const chfpe_handle* h);   /* h may be NULL: last create-time error */
 
 #ifdef __cplusplus

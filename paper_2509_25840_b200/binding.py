@@ -10,7 +10,7 @@ EXPORTED_SYMBOLS = [
     "chfpe_workspace_bytes", "chfpe_create", "chfpe_destroy", "chfpe_num_elements", "chfpe_element_index",
     "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
     "chfpe_response_1d", "chfpe_response_2d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
-    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_last_error",
+    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_last_error",
 ]
 
 
@@ -75,6 +75,7 @@ def lib():
     L.chfpe_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
     L.chfpe_profile_enable.argtypes = [vp, C.c_int]
     L.chfpe_profile_read.argtypes = [vp, dp, C.POINTER(C.c_int64)]
+    L.chfpe_stage_kernel.argtypes = [vp, C.POINTER(C.c_int32)]
     L.chfpe_last_error.argtypes = [vp]
     L.chfpe_last_error.restype = C.c_char_p
     _lib = L
@@ -272,6 +273,12 @@ class CHFPE:
         ms, n = C.c_double(), C.c_int64()
         self._ck(lib().chfpe_profile_read(self._h, C.byref(ms), C.byref(n)), "chfpe_profile_read")
         return ms.value, n.value
+
+    def stage_kernel(self):
+        """'generic' | 'brick' | 'pipe' | 'compact': the kernel family that runs the RK stage on this handle."""
+        k = C.c_int32()
+        self._ck(lib().chfpe_stage_kernel(self._h, C.byref(k)), "chfpe_stage_kernel")
+        return ("generic", "brick", "pipe", "compact")[k.value]
 
     def launch_count(self):
         n = C.c_int64()

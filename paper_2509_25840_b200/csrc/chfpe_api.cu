@@ -146,6 +146,9 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   // thread at 20^3 (no register spills; measured 25.4 -> 21.6 ms per stage at config 5)
   bp.npass = env_int("CHFPE_BRICK_NPASS", (bp.P1 > 16 && bp.P1 % (2 * bp.split) == 0) ? 2 : 1);
   bp.fixed = brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb, bp.npass);
+  if (!bp.fixed && bp.npass > 1 && brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb, 1)) {
+    bp.npass = 1; bp.fixed = 1;                                      // shapes instantiated single-pass only (48 x 48)
+  }
   if (!bp.fixed) return bp;
   // L2 reuse window = five q_1 planes x (q_2 chunk + 2+2 halo rows) x g elements of the stage input; budget 64 MiB
   // of the 126 MB L2 (the rest serves the once-touched streams).  Pairs of linked elements (g = 2) save one
@@ -470,6 +473,15 @@ extern "C" int chfpe_element_index(const chfpe_handle* h, int32_t k, int32_t n_o
 extern "C" int chfpe_launch_count(const chfpe_handle* h, int64_t* n) {
   if (!h || !n) return CHFPE_ERR_INVALID;
   *n = h->launches; return CHFPE_OK;
+}
+
+extern "C" int chfpe_stage_kernel(const chfpe_handle* h, int32_t* kind) {
+  if (!h || !kind) return CHFPE_ERR_INVALID;
+  *kind = (h->op.scheme == CHFPE_COMPACT6) ? CHFPE_STAGE_COMPACT
+          : (h->bp.enabled && h->bp.pipe)  ? CHFPE_STAGE_PIPE
+          : h->bp.enabled                  ? CHFPE_STAGE_BRICK
+                                           : CHFPE_STAGE_GENERIC;
+  return CHFPE_OK;
 }
 
 static DevObs to_dev(const chfpe_observable* o) {

@@ -219,6 +219,7 @@ def test_full_size_sampled_rhs_and_step_properties(name):
     cfg = ci.config(name)
     P = gpu_mod()
     g = P.CHFPE(cfg, batch=1)
+    assert g.stage_kernel() == "brick"      # the named configurations must not fall back to the generic kernel
     o = oracle.RefCHFPE(cfg)
     levels = [sum(n) for n in o.elements()]
     X = ci.seeded_state(cfg, levels, seed=0)
