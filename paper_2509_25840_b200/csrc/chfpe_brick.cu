@@ -87,6 +87,11 @@ constexpr int brick3_maxreg(int nt, int minb) {
   return r > 255 ? 255 : r;
 }
 
+// true if the P3/2 pairs of a p_3 row are a power-of-two lane group of a warp and warps hold whole rows
+__host__ __device__ constexpr bool brick3_shfl3(int p2, int p3, int split) {
+  return (32 % (p3 / 2) == 0) && ((split * p2 * p3 / 2) % 32 == 0) && ((p2 * p3 / 2) % (p3 / 2) == 0);
+}
+
 // NPASS > 1: a brick is processed in NPASS passes over blocks of P1/NPASS consecutive p_1 planes (large bricks: keeps
 // the per-thread state small); G_1 of the two planes beyond a block edge is recomputed from three extra loads.
 template <int P1, int P2, int P3, int SPLIT, int MINB, int NPASS>
@@ -102,7 +107,10 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   // bricks 0.79 -> 0.75 ms per stage; 16^3 bricks, 160 KB per five, gain nothing and keep L1::no_allocate)
   constexpr int L1Q3 = (5 * P1 * P2 * P3 * (int)sizeof(double) <= 100 * 1024) ? 2 : 0;
   constexpr int G2_ROW = P3, G2_PLANE = SKIP1 ? 0 : (P2 + 4) * P3;  // G_2[i1][i2+2][i3]
-  constexpr int G3_ROW = P3 + 4, G3_PLANE = P2 * (P3 + 4);          // G_3[i1][i2][i3+2]
+  // p_3 rows of P3/2 pairs that tile a warp: the p_3 stencil of G_3 runs on warp shuffles as soon as G_3 is formed
+  // (no shared array, no copy kept in registers); other shapes stage G_3 in shared memory like G_2.
+  constexpr bool SHFL3 = brick3_shfl3(P2, P3, SPLIT);
+  constexpr int G3_ROW = P3 + 4, G3_PLANE = SHFL3 ? 0 : P2 * (P3 + 4);   // G_3[i1][i2][i3+2]
   extern __shared__ __align__(16) double sm[];
   double* g2 = sm;
   double* g3 = sm + P1P * G2_PLANE;
@@ -117,7 +125,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
     const int pl = i / (4 * P3), rr = i - pl * (4 * P3), row = rr / P3, col = rr - row * P3;
     g2[pl * G2_PLANE + (row < 2 ? row : P2 + row) * G2_ROW + col] = 0.0;
   }
-  for (int i = threadIdx.x; i < P1P * P2 * 4; i += NTT) {           // G_3: columns i3 = -2,-1,P3,P3+1 of every row
+  for (int i = threadIdx.x; i < (SHFL3 ? 0 : P1P * P2 * 4); i += NTT) {   // G_3: columns i3 = -2,-1,P3,P3+1 of every row
     const int rw = i >> 2, c4 = i & 3;
     g3[rw * G3_ROW + (c4 < 2 ? c4 : P3 + c4)] = 0.0;
   }
@@ -240,7 +248,7 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
   for (int j = 0; j < NC; j++) acc[j] = fma2(-Gam, xk[j], acc[j]);
 
   double w2 = 0.0, w3 = 0.0;                                        // 1/(12h) or 1/(2h) of p_2, p_3
-  constexpr bool KEEP_G3 = (NC <= 8);                              // else re-read the own G_3 pair from shared memory
+  constexpr bool KEEP_G3 = (NC <= 8) && !SHFL3;                    // else re-read the own G_3 pair from shared memory
   double2 g3own[KEEP_G3 ? NC : 1];
 #pragma unroll
   for (int s = 0; s < 3; s++) {
@@ -304,6 +312,23 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
           }
         } else if (s == 1) {
           *reinterpret_cast<double2*>(g2 + (jbase + j) * G2_PLANE + (i2 + 2) * G2_ROW + i3) = gg[jj];
+        } else if (SHFL3) {                                         // D_{p_3} G_3 from the neighbour lanes of the row
+          constexpr int W = P3 / 2;
+          const int c = tid % W;
+          const double2 own = gg[jj];
+          double ly = __shfl_up_sync(0xffffffffu, own.y, 1, W), rx = __shfl_down_sync(0xffffffffu, own.x, 1, W);
+          if (c == 0) ly = 0.0;
+          if (c == W - 1) rx = 0.0;
+          double e3x = own.y - ly, e3y = rx - own.x;
+          if (wide) {
+            double lx = __shfl_up_sync(0xffffffffu, own.x, 1, W), ry = __shfl_down_sync(0xffffffffu, own.y, 1, W);
+            if (c == 0) lx = 0.0;
+            if (c == W - 1) ry = 0.0;
+            e3x = fma(8.0, e3x, -(rx - lx));
+            e3y = fma(8.0, e3y, -(ry - ly));
+          }
+          acc[j].x = fma(wp, e3x, acc[j].x);
+          acc[j].y = fma(wp, e3y, acc[j].y);
         } else {
           *reinterpret_cast<double2*>(g3 + (jbase + j) * G3_PLANE + i2 * G3_ROW + i3 + 2) = gg[jj];
           if (KEEP_G3) g3own[KEEP_G3 ? j : 0] = gg[jj];
@@ -369,25 +394,33 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
         const double2 u1 = *reinterpret_cast<const double2*>(a2 + G2_ROW), d1 = *reinterpret_cast<const double2*>(a2 - G2_ROW);
         e2x = u1.x - d1.x; e2y = u1.y - d1.y;
       }
-      const double2 lft = *reinterpret_cast<const double2*>(a3 - 2), rgt = *reinterpret_cast<const double2*>(a3 + 2);
-      // pair (i3, i3+1): neighbours i3-2..i3+3 = lft.x lft.y [own.x own.y] rgt.x rgt.y
-      const double2 own = KEEP_G3 ? g3own[KEEP_G3 ? j : 0] : *reinterpret_cast<const double2*>(a3);
-      double e3x = own.y - lft.y, e3y = rgt.x - own.x;
+      double e3x = 0.0, e3y = 0.0;
+      double2 lft = make_double2(0.0, 0.0), rgt = lft;
+      if (!SHFL3) {
+        lft = *reinterpret_cast<const double2*>(a3 - 2); rgt = *reinterpret_cast<const double2*>(a3 + 2);
+        // pair (i3, i3+1): neighbours i3-2..i3+3 = lft.x lft.y [own.x own.y] rgt.x rgt.y
+        const double2 own = KEEP_G3 ? g3own[KEEP_G3 ? j : 0] : *reinterpret_cast<const double2*>(a3);
+        e3x = own.y - lft.y; e3y = rgt.x - own.x;
+      }
       if (wide) {
         if (!SKIP1) {
           const double2 u2 = *reinterpret_cast<const double2*>(a2 + 2 * G2_ROW), d2 = *reinterpret_cast<const double2*>(a2 - 2 * G2_ROW);
           e2x = fma(8.0, e2x, -(u2.x - d2.x));
           e2y = fma(8.0, e2y, -(u2.y - d2.y));
         }
-        e3x = fma(8.0, e3x, -(rgt.x - lft.x));
-        e3y = fma(8.0, e3y, -(rgt.y - lft.y));
+        if (!SHFL3) {
+          e3x = fma(8.0, e3x, -(rgt.x - lft.x));
+          e3y = fma(8.0, e3y, -(rgt.y - lft.y));
+        }
       }
       if (!SKIP1) {
         acc[j].x = fma(w2, e2x, acc[j].x);
         acc[j].y = fma(w2, e2y, acc[j].y);
       }
-      acc[j].x = fma(w3, e3x, acc[j].x);
-      acc[j].y = fma(w3, e3y, acc[j].y);
+      if (!SHFL3) {
+        acc[j].x = fma(w3, e3x, acc[j].x);
+        acc[j].y = fma(w3, e3y, acc[j].y);
+      }
     }
   }
 
@@ -408,7 +441,8 @@ k_stage_brick3(DevOp op, BrickPlan bp, const double* __restrict__ in, const doub
 
 template <int P1, int P2, int P3, int SPLIT, int NPASS>
 constexpr int brick3_smem_bytes() {
-  return (int)sizeof(double) * ((P2 == 1 ? 0 : (P1 / NPASS) * (P2 + 4) * P3) + (P1 / NPASS) * P2 * (P3 + 4) +
+  return (int)sizeof(double) * ((P2 == 1 ? 0 : (P1 / NPASS) * (P2 + 4) * P3) +
+                                (brick3_shfl3(P2, P3, SPLIT) ? 0 : (P1 / NPASS) * P2 * (P3 + 4)) +
                                 (SPLIT > 1 ? SPLIT * 4 * P2 * P3 : 0));
 }
 
