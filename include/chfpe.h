@@ -115,6 +115,18 @@ int chfpe_response_2d(chfpe_handle* h, const chfpe_observable* A, const chfpe_ob
                       const int64_t* t1_steps, int32_t n1, const int64_t* t2_steps, int32_t n2,
                       double dt, double* R);
 
+/* R3[k][j][l] (row f2 of DESIGN.md): T1 <- Kick(A) replica 0, advanced along t1; at t1_steps[k] a copy T2 of T1 gets
+   Kick(B) and is advanced along t2; at t2_steps[j] a copy of T2 gets Kick(C) and is propagated over the t3 grid, <D>
+   recorded after t3_steps[l] steps.  Literal Eq. (17) :126-127 (no sign, like Eq. 15-16).  Step lists: host,
+   ascending, >= 0.  R: host, row-major [n1][n2][n3].  Replicas of different t1 are propagated together per launch:
+   slot 0 = T1; a group of nb t1 samples uses slots [1, 1+nb) for its t2 trajectories and [1+nb, 1+2nb) for the t3
+   replicas, nb = (batch-1)/2; at the last t2 sample C is applied in place, so n2 == 1 (a fixed waiting time, the
+   scan of Eq. 21) runs nb = batch-1 replicas.  CHFPE_ERR_INVALID if nb < 1 or nb*n3 exceeds the 65536-entry results
+   buffer.  On return replica 0 holds T1 at t1_steps[n1-1]. */
+int chfpe_response_3d(chfpe_handle* h, const chfpe_observable* A, const chfpe_observable* B, const chfpe_observable* C,
+                      const chfpe_observable* D, const int64_t* t1_steps, int32_t n1, const int64_t* t2_steps,
+                      int32_t n2, const int64_t* t3_steps, int32_t n3, double dt, double* R);
+
 /* Canonical-layout copy of one replica out of / into the library (K*cells doubles). dst/src: device if *_is_device. */
 int chfpe_export_state(chfpe_handle* h, int32_t replica, double* dst, int dst_is_device);
 int chfpe_import_state(chfpe_handle* h, int32_t replica, const double* src, int src_is_device);

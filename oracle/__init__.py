@@ -84,6 +84,8 @@ def lib():
         L.chfpe_ref_response_2d.argtypes = [C.c_void_p, C.POINTER(Observable), C.POINTER(Observable),
                                             C.POINTER(Observable), C.POINTER(C.c_int64), C.c_int32,
                                             C.POINTER(C.c_int64), C.c_int32, C.c_double, dp]
+        L.chfpe_ref_response_3d.argtypes = [C.c_void_p] + [C.POINTER(Observable)] * 4 + \
+            [C.POINTER(C.c_int64), C.c_int32] * 3 + [C.c_double, dp]
         L.chfpe_ref_export_state.argtypes = [C.c_void_p, dp]
         L.chfpe_ref_import_state.argtypes = [C.c_void_p, dp]
         L.chfpe_ref_scaled_norm2.argtypes = [C.c_void_p, dp]
@@ -231,6 +233,18 @@ class RefCHFPE:
                                          t2.ctypes.data_as(C.POINTER(C.c_int64)), len(t2), dt, _dp(R))
         if rc != 0:
             raise ValueError("response_2d failed: %d" % rc)
+        return R
+
+    def response_3d(self, A, B, Cobs, D, t1_steps, t2_steps, t3_steps, dt):
+        """Eq. (17) PAPER.md:126-127, literal: R[k][j][l]."""
+        ts = [np.ascontiguousarray(t, dtype=np.int64) for t in (t1_steps, t2_steps, t3_steps)]
+        R = np.empty(tuple(len(t) for t in ts))
+        args = []
+        for t in ts:
+            args += [t.ctypes.data_as(C.POINTER(C.c_int64)), len(t)]
+        rc = lib().chfpe_ref_response_3d(self._h, C.byref(A), C.byref(B), C.byref(Cobs), C.byref(D), *args, dt, _dp(R))
+        if rc != 0:
+            raise ValueError("response_3d failed: %d" % rc)
         return R
 
     def export_state(self):

@@ -487,6 +487,44 @@ int chfpe_ref_response_2d(chfpe_ref_handle* h, const chfpe_ref_observable* A, co
   return 0;
 }
 
+/* R3[k][j][l] (row f2 of DESIGN.md): Eq. (17) PAPER.md:126-127 written out, literal like Eq. (15)-(16) (no sign, R3):
+   T1 <- Kick(A) state, advanced to t1[k]; T2 <- Kick(B) T1, advanced to t2[j]; Y <- Kick(C) T2; <D> on Y after
+   t3[l] steps.  Plain triple loop; the two trajectories are kept as copies. */
+int chfpe_ref_response_3d(chfpe_ref_handle* h, const chfpe_ref_observable* A, const chfpe_ref_observable* B,
+                          const chfpe_ref_observable* C, const chfpe_ref_observable* D, const int64_t* t1, int32_t n1,
+                          const int64_t* t2, int32_t n2, const int64_t* t3, int32_t n3, double dt, double* R) {
+  size_t tot = (size_t)h->K * h->cells;
+  double* T1 = malloc(sizeof(double) * tot);
+  double* T2 = malloc(sizeof(double) * tot);
+  if (!T1 || !T2) { free(T1); free(T2); return -2; }
+  int rc = 0;
+  chfpe_ref_kick(h, A);
+  int64_t now1 = 0;
+  for (int k = 0; k < n1 && !rc; k++) {
+    if (t1[k] < now1) { rc = -1; break; }
+    chfpe_ref_step(h, t1[k] - now1, dt); now1 = t1[k];
+    memcpy(T1, h->X, sizeof(double) * tot);                 /* keep the t1 trajectory */
+    chfpe_ref_kick(h, B);
+    int64_t now2 = 0;
+    for (int j = 0; j < n2 && !rc; j++) {
+      if (t2[j] < now2) { rc = -1; break; }
+      chfpe_ref_step(h, t2[j] - now2, dt); now2 = t2[j];
+      memcpy(T2, h->X, sizeof(double) * tot);               /* keep the t2 trajectory */
+      chfpe_ref_kick(h, C);
+      int64_t now3 = 0;
+      for (int l = 0; l < n3; l++) {
+        if (t3[l] < now3) { rc = -1; break; }
+        chfpe_ref_step(h, t3[l] - now3, dt); now3 = t3[l];
+        chfpe_ref_expect(h, D, &R[((size_t)k * n2 + j) * n3 + l]);
+      }
+      memcpy(h->X, T2, sizeof(double) * tot);
+    }
+    memcpy(h->X, T1, sizeof(double) * tot);
+  }
+  free(T1); free(T2);
+  return rc;
+}
+
 int chfpe_ref_export_state(const chfpe_ref_handle* h, double* dst) {
   memcpy(dst, h->X, sizeof(double) * (size_t)h->K * h->cells); return 0;
 }

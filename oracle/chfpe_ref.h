@@ -80,6 +80,12 @@ int     chfpe_ref_response_1d(chfpe_ref_handle*, const chfpe_ref_observable* A, 
 int     chfpe_ref_response_2d(chfpe_ref_handle*, const chfpe_ref_observable* A, const chfpe_ref_observable* B,
                               const chfpe_ref_observable* C, const int64_t* t1_steps, int32_t n1,
                               const int64_t* t2_steps, int32_t n2, double dt, double* R);
+/* Eq. (17): R[k][j][l] = <D> after t3_steps[l] steps of Kick(C) [t2_steps[j] steps of Kick(B) [t1_steps[k] steps of
+   Kick(A) X]]; row-major [n1][n2][n3] */
+int     chfpe_ref_response_3d(chfpe_ref_handle*, const chfpe_ref_observable* A, const chfpe_ref_observable* B,
+                              const chfpe_ref_observable* C, const chfpe_ref_observable* D,
+                              const int64_t* t1_steps, int32_t n1, const int64_t* t2_steps, int32_t n2,
+                              const int64_t* t3_steps, int32_t n3, double dt, double* R);
 int     chfpe_ref_export_state(const chfpe_ref_handle*, double* dst);
 int     chfpe_ref_import_state(chfpe_ref_handle*, const double* src);
 /* sum_n ||X_n||^2 / prod_s [ n_s! (zeta_s gamma_s m_s / beta)^{n_s} ] * dV  (contraction pin P6) */

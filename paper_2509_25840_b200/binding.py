@@ -9,7 +9,7 @@ from . import build as _build
 EXPORTED_SYMBOLS = [
     "chfpe_workspace_bytes", "chfpe_create", "chfpe_destroy", "chfpe_num_elements", "chfpe_element_index",
     "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
-    "chfpe_response_1d", "chfpe_response_2d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
+    "chfpe_response_1d", "chfpe_response_2d", "chfpe_response_3d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
     "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_last_error",
 ]
 
@@ -69,6 +69,7 @@ def lib():
     L.chfpe_expect_element.argtypes = [vp, C.c_int32, C.c_int32, op, dp]
     L.chfpe_response_1d.argtypes = [vp, op, op, C.c_int64, C.c_int64, C.c_double, dp]
     L.chfpe_response_2d.argtypes = [vp, op, op, op, i64p, C.c_int32, i64p, C.c_int32, C.c_double, dp]
+    L.chfpe_response_3d.argtypes = [vp, op, op, op, op, i64p, C.c_int32, i64p, C.c_int32, i64p, C.c_int32, C.c_double, dp]
     L.chfpe_export_state.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_import_state.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_export_rhs.argtypes = [vp, C.c_int32, vp, C.c_int]
@@ -233,6 +234,17 @@ class CHFPE:
                                          t1.ctypes.data_as(C.POINTER(C.c_int64)), len(t1),
                                          t2.ctypes.data_as(C.POINTER(C.c_int64)), len(t2), dt,
                                          R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_response_2d")
+        return R
+
+    def response_3d(self, A, B, Cobs, D, t1_steps, t2_steps, t3_steps, dt):
+        """R[k][j][l] of Eq. (17); needs batch >= 3."""
+        ts = [np.ascontiguousarray(t, dtype=np.int64) for t in (t1_steps, t2_steps, t3_steps)]
+        R = np.empty(tuple(len(t) for t in ts))
+        args = []
+        for t in ts:
+            args += [t.ctypes.data_as(C.POINTER(C.c_int64)), len(t)]
+        self._ck(lib().chfpe_response_3d(self._h, C.byref(A), C.byref(B), C.byref(Cobs), C.byref(D), *args, dt,
+                                         R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_response_3d")
         return R
 
     def export_state(self, replica=0):

@@ -329,6 +329,74 @@ def test_two_dimensional_closed_form_on_gpu():
     g.close()
 
 
+@pytest.mark.parametrize("name,batch", [("m1", 3), ("m2", 4), ("m3", 5)])
+def test_response_3d(name, batch):
+    """Row f2: R3 (Eq. 17) with the replicas of (batch-1)/2 t1 samples propagated together (ragged last group,
+    repeated delays; batch-1 replicas when there is a single waiting time t2) against the oracle's plain triple loop;
+    M = 1, 2, 3."""
+    cfg = {"m1": ci.config("cfg2", nq=[37], np=[41], depth=4),
+           "m2": ci.config("cfg3s", nq=[9, 10], np=[11, 8], depth=2),
+           "m3": ci.config("cfg4s8", nq=[6, 5, 7], np=[5, 7, 6], depth=2)}[name]
+    M = cfg["n_modes"]
+    g, o = both(cfg, batch=batch)
+    mu_g, mu_o = obs_pair("mu", M)
+    al_g, al_o = obs_pair("alpha", M)
+    nl_g, nl_o = obs_pair("mu_nl", M)
+    g.equilibrate(); o.equilibrate()
+    t1, t2, t3 = [0, 2, 5], [0, 1, 1, 4, 6], [0, 3, 4]
+    dt = 10 * cfg["dt"]
+    Rg = g.response_3d(mu_g, al_g, nl_g, al_g, t1, t2, t3, dt)
+    Ro = o.response_3d(mu_o, al_o, nl_o, al_o, t1, t2, t3, dt)
+    assert Rg.shape == (3, 5, 3)
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    assert np.array_equal(Rg[:, 1], Rg[:, 2])
+    # replica 0 holds the t1 trajectory at its last delay; the call can be repeated after equilibrate
+    g.equilibrate()
+    Rg2 = g.response_3d(mu_g, al_g, nl_g, al_g, t1, t2, t3, dt)
+    assert np.array_equal(Rg, Rg2)
+    g.equilibrate()
+    Rw = g.response_3d(mu_g, al_g, nl_g, al_g, t1, [4], t3, dt)      # fixed waiting time: C applied in place
+    assert np.max(np.abs(Rw[:, 0] - Ro[:, 3])) <= 1e-8 * np.max(np.abs(Ro))
+    g.close()
+
+
+def test_response_3d_closed_forms_and_errors():
+    """Pin P4b on the CUDA path: harmonic + LL in the W gauge, c = R_phys:
+    A = D = q, B = C = q^2: -4 c(t1) c(t2) c(t3);  A = B = q, C = D = q^2: -4 c(t3)[c(t2) c(t1+t2+t3) + c(t2+t3) c(t1+t2)]."""
+    cfg = ci.config("cfg1", nq=[48], np=[48], depth=4, gauge="w")
+    P = gpu_mod()
+    g = P.CHFPE(cfg, batch=4)
+    q = P.make_observable(0.0, [1.0], [[0.0]], [0.0])
+    q2 = P.make_observable(0.0, [0.0], [[2.0]], [0.0])
+
+    def c(t, w0=1.0, zeta=0.5, gamma=1.0):          # Brownian-oscillator response (3 x 3 first-moment ODE, pin P3)
+        import scipy.linalg
+        A = np.array([[0, 1, 0], [-w0 ** 2, 0, 1], [0, -zeta * gamma, -gamma]], dtype=float)
+        return float(scipy.linalg.expm(t * A)[0, 1])
+
+    t1, t2, t3 = [500], [300, 700], [400, 900]
+    g.equilibrate()
+    Ra = g.response_3d(q, q2, q2, q, t1, t2, t3, 1e-3)
+    g.equilibrate()
+    Rb = g.response_3d(q, q, q2, q2, t1, t2, t3, 1e-3)
+    for j, b in enumerate(t2):
+        for l, d in enumerate(t3):
+            a_, b_, d_ = 0.5, b * 1e-3, d * 1e-3
+            assert abs(Ra[0, j, l] + 4 * c(a_) * c(b_) * c(d_)) < 3e-5
+            assert abs(Rb[0, j, l] + 4 * c(d_) * (c(b_) * c(a_ + b_ + d_) + c(b_ + d_) * c(a_ + b_))) < 3e-5
+    with pytest.raises(Exception):
+        g.response_3d(q, q2, q2, q, [3, 1], t2, t3, 1e-3)        # descending t1
+    g.close()
+    g2 = P.CHFPE(cfg, batch=2)
+    g2.equilibrate()
+    with pytest.raises(Exception):
+        g2.response_3d(q, q2, q2, q, t1, t2, t3, 1e-3)           # two waiting times need three slots
+    g2.equilibrate()
+    Rw = g2.response_3d(q, q2, q2, q, t1, [700], t3, 1e-3)       # one waiting time runs in two
+    assert np.max(np.abs(Rw[:, 0] - Ra[:, 1])) <= 1e-12
+    g2.close()
+
+
 COMPACT = [
     ("m1", ci.config("cfg2", nq=[37], np=[41], depth=4, scheme="compact6")),
     ("m2_w", ci.config("cfg3s", nq=[9, 10], np=[11, 8], depth=2, scheme="compact6", gauge="w")),

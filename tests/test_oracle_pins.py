@@ -182,6 +182,49 @@ def test_P4_two_dimensional_closed_form():
     assert abs(R0[0, 0]) < 1e-7
 
 
+def test_P4b_third_order_closed_forms():
+    """Eq. (17) PAPER.md:126-127 on the harmonic + LL model, where E[q(t) | q0, p0, Omega0] is linear with
+    d E[q(t)] / d p0 = R_phys(t) =: c(t): integrating each kick by parts (int f X^x W = -int (dX/dq)(df/dp) W) gives
+      A = D = q, B = C = q^2:   R3_lib = -4 c(t1) c(t2) c(t3)
+      A = B = q, C = D = q^2:   R3_lib = -4 c(t3) [ c(t2) c(t1+t2+t3) + c(t2+t3) c(t1+t2) ]
+    (the second is not symmetric in the delays: it pins the order of the operators and of the time arguments), and
+    zero if fewer than two of the four operators are quadratic."""
+    c = bo_response
+    dt = 1e-3
+    t1s, t2s, t3s = [0, 500], [300, 700], [0, 400, 900]
+    mu, al = obs("mu", 1), obs("alpha", 1)
+    o = oracle.RefCHFPE(harmonic_cfg(n=48, depth=4))
+    o.equilibrate()
+    Ra = o.response_3d(mu, al, al, mu, t1s, t2s, t3s, dt)
+    o.equilibrate()
+    Rb = o.response_3d(mu, mu, al, al, t1s, t2s, t3s, dt)
+    o.equilibrate()
+    Rz = o.response_3d(mu, mu, al, mu, t1s, t2s, t3s, dt)
+    for k, a in enumerate(t1s):
+        for j, b in enumerate(t2s):
+            for l, d in enumerate(t3s):
+                a_, b_, d_ = a * dt, b * dt, d * dt
+                assert abs(Ra[k, j, l] + 4 * c(a_) * c(b_) * c(d_)) < 3e-5
+                assert abs(Rb[k, j, l] + 4 * c(d_) * (c(b_) * c(a_ + b_ + d_) + c(b_ + d_) * c(a_ + b_))) < 3e-5
+                assert abs(Rz[k, j, l]) < 3e-5
+    assert abs(Ra[1, 1, 2]) > 0.8 and abs(Rb[1, 1, 2]) > 3.0     # the tolerances above are 1e-5 relative
+
+
+def test_response_3d_equals_manual_protocol():
+    """Eq. (17) order of operations: kick A, t1, kick B, t2, kick C, t3, <D>."""
+    cfg = ci.config("cfg2", nq=[24], np=[24], depth=3)
+    o = oracle.RefCHFPE(cfg)
+    o.equilibrate()
+    t1s, t2s, t3s = [0, 3], [1, 4], [0, 2, 5]
+    R = o.response_3d(obs("mu", 1), obs("alpha", 1), obs("mu_nl", 1), obs("alpha", 1), t1s, t2s, t3s, 1e-2)
+    for k, a in enumerate(t1s):
+        for j, b in enumerate(t2s):
+            for l, d in enumerate(t3s):
+                o.equilibrate(); o.kick(obs("mu", 1)); o.step(a, 1e-2); o.kick(obs("alpha", 1)); o.step(b, 1e-2)
+                o.kick(obs("mu_nl", 1)); o.step(d, 1e-2)
+                assert abs(o.expect(obs("alpha", 1)) - R[k, j, l]) <= 1e-14 * max(1.0, abs(R[k, j, l]))
+
+
 def test_response_2d_equals_manual_protocol():
     """Eq. (16) order of operations: kick A, t1, kick B, t2, <C>."""
     cfg = ci.config("cfg2", nq=[24], np=[24], depth=3)
