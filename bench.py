@@ -332,6 +332,47 @@ def run_2d(args):
     return 0
 
 
+def run_3d(args):
+    """Row f2: third-order response R3(t3, t2, t1) of Eq. (17) at one waiting time t2 -- the scan behind
+    the 2D IR spectrum of Eq. (21) -- on config 4's model.  Times chfpe_response_3d end to end (trajectory, replica
+    copies, three kicks, batched propagation of batch-1 replicas, expectations, D2H of R) on an n1 x 1 x n2 sample
+    of delays (--n2 is the number of t3 delays here) and reports replica-steps per second; not a BASELINE metric."""
+    import numpy as np
+    import torch
+    import paper_2509_25840_b200 as P
+    wl = args.workload
+    cfg = ci.config(wl)
+    M = cfg["n_modes"]
+    g = P.CHFPE(cfg, batch=args.batch)
+    mu = obs(P, "mu_nl", M)
+    g.equilibrate(residual=False)
+    n1, n3, wait = args.n1, args.n2, 4
+    t1, t3 = list(range(n1)), list(range(n3))
+    g.response_3d(mu, mu, mu, mu, t1[:2], [wait], t3[:2], cfg["dt"])   # warm-up
+    g.equilibrate(residual=False)
+    n0 = g.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    R = g.response_3d(mu, mu, mu, mu, t1, [wait], t3, cfg["dt"])
+    e1.record()
+    torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    rsteps = (n1 - 1) + n1 * wait + n1 * (n3 - 1)                   # t1 trajectory + waiting time + t3 scans
+    line = {"metric": "third-order response replica-steps/s", "value": rsteps / sec, "unit": "replica-steps/s",
+            "higher_is_better": True, "n_gpus": 1, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl + " response_3d", "grid": "x".join(str(x) for x in g.shape), "K": g.K,
+                       "batch_slots": args.batch, "workspace_GB": P.workspace_bytes(cfg, args.batch) / 1e9,
+                       "timed_sample": "%d t1 x 1 t2 (%d steps) x %d t3 delays, stride 1, A=B=C=D=mu (nonlinear)"
+                                       % (n1, wait, n3)},
+            "sample_seconds": sec, "replica_steps_timed": rsteps, "ms_per_replica_step": 1e3 * sec / rsteps,
+            "cell_updates_per_s": g.cells * rsteps / sec, "gpu_launches": int(g.launch_count() - n0),
+            "finite": bool(np.all(np.isfinite(R)))}
+    print(json.dumps(line))
+    g.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -340,8 +381,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
-    ap.add_argument("--protocol", default="step", choices=["step", "2d"],
-                    help="'2d': time chfpe_response_2d on config 5 (secondary metric: 2D THz-Raman wall time)")
+    ap.add_argument("--protocol", default="step", choices=["step", "2d", "3d"],
+                    help="'2d': time chfpe_response_2d on config 5 (secondary metric: 2D THz-Raman wall time); "
+                         "'3d': time chfpe_response_3d (row f2) on --workload")
     ap.add_argument("--batch", type=int, default=5, help="replica slots for --protocol 2d (trajectory + t1 replicas)")
     ap.add_argument("--n1", type=int, default=8)
     ap.add_argument("--n2", type=int, default=16)
@@ -350,6 +392,8 @@ def main():
         return run_reference(args)
     if args.protocol == "2d":
         return run_2d(args)
+    if args.protocol == "3d":
+        return run_3d(args)
     return run_ours(args)
 
 

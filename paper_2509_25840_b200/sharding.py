@@ -45,3 +45,19 @@ def response_2d_sharded(engine, A, B, C, t1_steps, t2_steps, dt, group=None, dev
     else:
         local = np.empty((0, len(t2_steps)))
     return gather_rows(local, rows, len(t1), len(t2_steps), group=group, device=device)
+
+
+def response_3d_sharded(engine, A, B, C, D, t1_steps, t2_steps, t3_steps, dt, group=None, device="cpu"):
+    """R3 (Eq. 17) over the full (t1, t2, t3) grid: the (t2, t3) blocks started from different t1 states are
+    independent, so the t1 samples are split across the ranks exactly like the rows of R2 (one all_gather)."""
+    import torch.distributed as dist
+    rank, world = dist.get_rank(group), dist.get_world_size(group)
+    t1 = list(t1_steps)
+    n2, n3 = len(t2_steps), len(t3_steps)
+    rows = rows_for_rank(len(t1), rank, world)
+    if rows:
+        local = engine.response_3d(A, B, C, D, [t1[i] for i in rows], list(t2_steps), list(t3_steps), dt)
+    else:
+        local = np.empty((0, n2, n3))
+    return gather_rows(local.reshape(len(rows), n2 * n3), rows, len(t1), n2 * n3, group=group,
+                       device=device).reshape(len(t1), n2, n3)

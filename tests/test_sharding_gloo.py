@@ -15,6 +15,7 @@ torch = pytest.importorskip("torch")
 CFG = ci.config("cfg3s", nq=[7, 6], np=[6, 7], depth=2)
 T1 = [0, 1, 3, 4, 6]
 T2 = [0, 2, 3]
+T3 = [1, 2]
 
 
 def _obs():
@@ -34,6 +35,9 @@ def _worker(rank, world, port, out):
         A, B, C = _obs()
         R = sharding.response_2d_sharded(o, A, B, C, T1, T2, 10 * CFG["dt"])
         np.save(os.path.join(out, "R%d.npy" % rank), R)
+        o.equilibrate()
+        R3 = sharding.response_3d_sharded(o, A, B, C, A, T1[:3], T2[:2], T3, 10 * CFG["dt"])
+        np.save(os.path.join(out, "R3_%d.npy" % rank), R3)
     finally:
         dist.destroy_process_group()
 
@@ -62,3 +66,9 @@ def test_response_2d_sharded_world2(tmp_path):
         R = np.load(tmp_path / ("R%d.npy" % r))
         assert R.shape == full.shape
         assert np.max(np.abs(R - full)) <= 1e-14 * np.max(np.abs(full))
+    o.equilibrate()
+    full3 = o.response_3d(A, B, C, A, T1[:3], T2[:2], T3, 10 * CFG["dt"])
+    for r in range(2):
+        R3 = np.load(tmp_path / ("R3_%d.npy" % r))
+        assert R3.shape == full3.shape == (3, 2, 2)
+        assert np.max(np.abs(R3 - full3)) <= 1e-14 * np.max(np.abs(full3))
