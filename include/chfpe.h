@@ -144,6 +144,22 @@ int chfpe_launch_count(const chfpe_handle* h, int64_t* n);
 int chfpe_profile_enable(chfpe_handle* h, int on);
 int chfpe_profile_read(chfpe_handle* h, double* total_ms, int64_t* n_launches);
 
+/* Spectra (row f3 of DESIGN.md): half-line Fourier integrals of sampled response functions, Eq. (19)-(21) :138-146,
+   as trapezoid sums over the uniform delay grid t_k = k dt (weights 1/2, 1, ..., 1, 1/2; no window, no padding;
+   reading R22) at the frequencies the caller lists.  No handle: ALL pointers are DEVICE pointers, the kernels are
+   enqueued on `cuda_stream` (asynchronous), nothing is allocated.
+     spectrum_1d, Eq. (19):  I[a] = omega[a] * Im sum_k w_k e^{+i omega[a] t_k} R[k] dt          (R: n, I: n_omega)
+     spectrum_2d, Eq. (20):  I[a][b] = Im sum_k sum_j w_k w_j e^{i sign1 omega1[a] k dt1} e^{i sign2 omega2[b] j dt2}
+                             R[k][j] dt1 dt2       (R row-major [n1][n2], I row-major [n_omega1][n_omega2]);
+                             sign1 = sign2 = -1 is Eq. (20); Eq. (21) at one waiting time is sign1 = -1 (t1),
+                             sign2 = +1 (t3) on R3[:, j, :].  scratch: 2*n1*n_omega2 doubles, 16-byte aligned.
+   CHFPE_ERR_INVALID for null pointers, sizes < 1, dt <= 0, signs other than +-1. */
+int chfpe_spectrum_1d(void* cuda_stream, const double* R, int64_t n, double dt, const double* omega, int32_t n_omega,
+                      double* I);
+int chfpe_spectrum_2d(void* cuda_stream, const double* R, int32_t n1, int32_t n2, double dt1, double dt2,
+                      const double* omega1, int32_t n_omega1, const double* omega2, int32_t n_omega2, int32_t sign1,
+                      int32_t sign2, double* scratch, double* I);
+
 /* Which kernel family runs the RK stage on this handle (host pointer), so that a test or a benchmark can assert
    that a configuration did not fall back to the generic kernel.  The cooperative multi-step kernel of tiny
    states is a property of the step call, not of the handle, and is not reported here. */

@@ -10,7 +10,7 @@ EXPORTED_SYMBOLS = [
     "chfpe_workspace_bytes", "chfpe_create", "chfpe_destroy", "chfpe_num_elements", "chfpe_element_index",
     "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
     "chfpe_response_1d", "chfpe_response_2d", "chfpe_response_3d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
-    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_last_error",
+    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_spectrum_1d", "chfpe_spectrum_2d", "chfpe_last_error",
 ]
 
 
@@ -77,6 +77,9 @@ def lib():
     L.chfpe_profile_enable.argtypes = [vp, C.c_int]
     L.chfpe_profile_read.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.chfpe_stage_kernel.argtypes = [vp, C.POINTER(C.c_int32)]
+    L.chfpe_spectrum_1d.argtypes = [vp, vp, C.c_int64, C.c_double, vp, C.c_int32, vp]
+    L.chfpe_spectrum_2d.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_double, C.c_double, vp, C.c_int32, vp, C.c_int32,
+                                    C.c_int32, C.c_int32, vp, vp]
     L.chfpe_last_error.argtypes = [vp]
     L.chfpe_last_error.restype = C.c_char_p
     _lib = L
@@ -296,3 +299,43 @@ class CHFPE:
         n = C.c_int64()
         self._ck(lib().chfpe_launch_count(self._h, C.byref(n)), "chfpe_launch_count")
         return n.value
+
+
+def _dev(a):
+    import torch
+    if not torch.cuda.is_available():
+        raise ChfpeError("no CUDA device: the spectra run in CUDA kernels only (no CPU fallback)")
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def spectrum_1d(R, dt, omega):
+    """Eq. (19): I(w) = w Im int_0^T e^{iwt} R1(t) dt (trapezoid sum) at the frequencies `omega`; numpy in / out,
+    computed by chfpe_spectrum_1d on the current CUDA stream."""
+    import torch
+    Rd, od = _dev(np.ravel(R)), _dev(np.ravel(omega))
+    out = torch.empty(od.numel(), dtype=torch.float64, device=Rd.device)
+    rc = lib().chfpe_spectrum_1d(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.c_void_p(Rd.data_ptr()),
+                                 Rd.numel(), float(dt), C.c_void_p(od.data_ptr()), od.numel(),
+                                 C.c_void_p(out.data_ptr()))
+    if rc != 0:
+        raise ChfpeError("chfpe_spectrum_1d failed: %d" % rc)
+    return out.cpu().numpy()
+
+
+def spectrum_2d(R, dt1, dt2, omega1, omega2, sign1=-1, sign2=-1):
+    """Eq. (20) (default signs) / Eq. (21) (sign1 = -1, sign2 = +1): I[a][b] = Im of the double half-line transform
+    of R[k][j] (rows = first delay); numpy in / out, computed by chfpe_spectrum_2d on the current CUDA stream."""
+    import torch
+    R = np.asarray(R, dtype=np.float64)
+    if R.ndim != 2:
+        raise ValueError("R must be [n1][n2]")
+    Rd, o1, o2 = _dev(R), _dev(np.ravel(omega1)), _dev(np.ravel(omega2))
+    scratch = torch.empty(2 * R.shape[0] * o2.numel(), dtype=torch.float64, device=Rd.device)
+    out = torch.empty((o1.numel(), o2.numel()), dtype=torch.float64, device=Rd.device)
+    rc = lib().chfpe_spectrum_2d(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.c_void_p(Rd.data_ptr()),
+                                 R.shape[0], R.shape[1], float(dt1), float(dt2), C.c_void_p(o1.data_ptr()), o1.numel(),
+                                 C.c_void_p(o2.data_ptr()), o2.numel(), int(sign1), int(sign2),
+                                 C.c_void_p(scratch.data_ptr()), C.c_void_p(out.data_ptr()))
+    if rc != 0:
+        raise ChfpeError("chfpe_spectrum_2d failed: %d" % rc)
+    return out.cpu().numpy()
