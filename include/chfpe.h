@@ -44,7 +44,7 @@ enum {
   CHFPE_ERR_STATE = -5       /* call sequence error (e.g. response before equilibrate/import) */
 };
 
-enum { CHFPE_CENTRAL4 = 0, CHFPE_CENTRAL2 = 1, CHFPE_COMPACT6 = 2 };   /* derivative scheme; COMPACT6 = Pade scheme Eq. (25)-(31) :177-201 with a = 7/9 (R4), unfused path */
+enum { CHFPE_CENTRAL4 = 0, CHFPE_CENTRAL2 = 1, CHFPE_COMPACT6 = 2 };   /* derivative scheme; COMPACT6 = Pade scheme Eq. (25)-(31) :177-201 with a = 7/9 (R4), one fused line pass per axis */
 enum { CHFPE_GAUGE_SQRT_EQ = 0, CHFPE_GAUGE_W = 1 };                   /* propagated variable (R7) */
 
 /* coef * q1^e1 q2^e2 q3^e3 ; total degree <= 4.  Eq. (3)-(4). */

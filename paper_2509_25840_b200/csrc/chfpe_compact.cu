@@ -6,10 +6,16 @@
 // choice for this step is parallel cyclic reduction on Ampere-class GPUs (section III.C :203-207) -- at line lengths
 // of 16..128 one thread per line is enough to occupy the GPU (a 16^6 grid has 10^6 lines per element and axis).
 //
-// This is the conditional, correctness-first path of SURVEY.md 8(a9): the RHS is assembled element by element from
-// whole-array derivatives (one line solve per (element, axis) on X_k along q_s, one on the combination
-// G_s = (dU/dq_s) X_k + V'_s X_up + n_s c_s V'_s X_dn along p_s), not fused; the explicit CENTRAL4 scheme is the
-// performance path.
+// This is the conditional path of SURVEY.md 8(a9); the explicit CENTRAL4 scheme is the performance path.  A stage is
+// 2M line passes + one pointwise pass, each ONE launch over all elements and replica slots (grid.y, grid.z):
+//   q_s pass: d = A^{-1} B X_k along q_s, accumulated as  out (+)= c * (-(p_s/m_s)) d
+//   p_s pass: d = A^{-1} B G_s along p_s with G_s = (dU/dq_s) X_k + V'_s X_up + n_s c_s V'_s X_dn formed on the fly
+//             (its coefficients are constant along a p-line),  out += c * d
+//   pointwise pass: out += c * [ -Gamma_k X_k + sum_s p_s V'_s (kup_s X_up + n_s c_s kdn_s X_dn) ]
+// The first pass writes out = a*y + c*(...), so no right-hand-side array exists; the forward-elimination values of a
+// line stay in thread-local memory for lines of up to 128 points (all BASELINE configs), longer lines keep
+// them in an element-sized scratch array and run element by element.  (First version: whole-array derivatives,
+// 17 launches per element, 37.4 ms per stage at config 4.)
 #include "chfpe_internal.cuh"
 
 namespace {
@@ -49,57 +55,6 @@ __global__ void __launch_bounds__(128) k_compact_deriv(const double* __restrict_
   }
 }
 
-// G_s = (dU/dq_s) X_k + V'_s X_up + n_s c_s V'_s X_dn  (per cell)
-template <int M>
-__global__ void __launch_bounds__(256) k_compact_G(DevOp op, const double* __restrict__ X, int k, int s, double* __restrict__ G) {
-  const long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (cell >= op.cells) return;
-  int idx[2 * M];
-  cdecode<2 * M>(op, (unsigned)cell, idx);
-  const long long ql = (long long)((unsigned)cell / (unsigned)op.pb);
-  const double q = op.x0[s] + idx[s] * op.h[s];
-  const double Vp = fma(op.VSL[s], q, op.VLL[s]);
-  double g = __ldg(op.dU[s] + ql) * X[(size_t)k * op.cells + cell];
-  const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
-  if (ku >= 0) g = fma(Vp, X[(size_t)ku * op.cells + cell], g);
-  if (kd >= 0) g = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp, X[(size_t)kd * op.cells + cell], g);
-  G[cell] = g;
-}
-
-// F = -Gamma_k X_k + sum_s p_s V'_s (kup_s X_up + n_s c_s kdn_s X_dn)   (damping and the gauge terms, pointwise)
-template <int M>
-__global__ void __launch_bounds__(256) k_compact_init(DevOp op, const double* __restrict__ X, int k, double* __restrict__ F) {
-  const long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (cell >= op.cells) return;
-  int idx[2 * M];
-  cdecode<2 * M>(op, (unsigned)cell, idx);
-  double acc = -__ldg(op.Gamma + k) * X[(size_t)k * op.cells + cell];
-#pragma unroll
-  for (int s = 0; s < M; s++) {
-    const double q = op.x0[s] + idx[s] * op.h[s];
-    const double p = op.x0[M + s] + idx[M + s] * op.h[M + s];
-    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
-    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
-    if (ku >= 0) acc = fma(Vp * op.kup[s] * p, X[(size_t)ku * op.cells + cell], acc);
-    if (kd >= 0) acc = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp * op.kdn[s] * p, X[(size_t)kd * op.cells + cell], acc);
-  }
-  F[cell] = acc;
-}
-
-// F += coef(cell) * D, coef = -(p_s / m_s) (mode 0, the q_s-derivative of X_k) or 1 (mode 1, the p_s-derivative of G_s)
-template <int M>
-__global__ void __launch_bounds__(256) k_compact_accum(DevOp op, const double* __restrict__ D, int s, int mode, double* __restrict__ F) {
-  const long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (cell >= op.cells) return;
-  double c = 1.0;
-  if (mode == 0) {
-    int idx[2 * M];
-    cdecode<2 * M>(op, (unsigned)cell, idx);
-    c = -(op.x0[M + s] + idx[M + s] * op.h[M + s]) * op.inv_mass[s];
-  }
-  F[cell] = fma(c, D[cell], F[cell]);
-}
-
 // kick (Eq. 18): F (+)= dX/dq_s (D + kup_s p_s X_k)
 template <int M>
 __global__ void __launch_bounds__(256) k_compact_kick_accum(DevOp op, DevObs ob, const double* __restrict__ Xk,
@@ -116,10 +71,98 @@ __global__ void __launch_bounds__(256) k_compact_kick_accum(DevOp op, DevObs ob,
   F[cell] = first ? v : F[cell] + v;
 }
 
-__global__ void __launch_bounds__(256) k_compact_combine(const double* __restrict__ F, const double* y, double* out, long long n,
-                                                         double a, double c) {
-  const long long i = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (i < n) out[i] = fma(c, F[i], a * y[i]);
+constexpr int CLINE_MAX = 128;    // longest line whose elimination values stay in thread-local memory
+
+// One Pade line solve per thread, fused with the formation of its operand and with the accumulation into `out`.
+// PAXIS = 0: line along q_s of X_k; PAXIS = 1: line along p_s of G_s.  grid = (line blocks, elements, slots).
+// NF = 0: run-time length <= CLINE_MAX, elimination values in a thread-local array; NF = -1: element-sized scratch D.
+// (NF > 0, a compile-time length with the values in registers, was measured slower at 16 points: 30.4 vs 22.5 ms
+// per stage at config 4 -- 100 registers per thread leave too few warps to hide the line's dependent loads.)
+template <int M, int PAXIS, int NF>
+__global__ void __launch_bounds__(128) k_compact_line(DevOp op, const double* __restrict__ in, const double* y, double* out,
+                                                      double a, double c, int s, int first, int k0, int b0,
+                                                      size_t slot_stride, const double* __restrict__ bet,
+                                                      const double* __restrict__ cfac, double* __restrict__ D) {
+  const int axis = PAXIS ? M + s : s;
+  constexpr bool LOCAL = NF >= 0;
+  const int n = NF > 0 ? NF : op.n[axis];
+  const long long st = op.st[axis];
+  const long long line = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (line >= op.cells / n) return;
+  const int k = k0 + blockIdx.y;
+  const size_t eoff = (size_t)(b0 + blockIdx.z) * slot_stride + (size_t)k * op.cells;
+  const long long outer = line / st, inner = line - outer * st;
+  const long long base = outer * st * n + inner;                   // cell of point 0 of the line
+  int idx[2 * M];
+  cdecode<2 * M>(op, (unsigned)base, idx);
+  const double* Xk = in + eoff + base;
+  const double* Xu = Xk;
+  const double* Xd = Xk;
+  double ck = 1.0, cu = 0.0, cd = 0.0, coef = 1.0;
+  if (PAXIS) {                                                     // G_s: coefficients depend on q only
+    const long long ql = base / op.pb;
+    const double q = op.x0[s] + idx[s] * op.h[s];
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    ck = __ldg(op.dU[s] + ql);
+    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+    if (ku >= 0) { cu = Vp; Xu = Xk + ((long long)ku - k) * op.cells; }
+    if (kd >= 0) { cd = __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp; Xd = Xk + ((long long)kd - k) * op.cells; }
+  } else {
+    coef = -(op.x0[M + s] + idx[M + s] * op.h[M + s]) * op.inv_mass[s];
+  }
+  auto f = [&](int i) -> double {
+    const long long o = (long long)i * st;
+    double v = PAXIS ? ck * Xk[o] : Xk[o];
+    if (PAXIS) { if (cu != 0.0) v = fma(cu, Xu[o], v); if (cd != 0.0) v = fma(cd, Xd[o], v); }
+    return v;
+  };
+  double rl[NF > 0 ? NF : (NF == 0 ? CLINE_MAX : 1)];
+  double* rg = D + base;                                           // element-sized scratch (LOCAL == false)
+  const double al = 1.0 / 3.0, ca = 7.0 / 9.0, cb = 1.0 / 36.0, inv_h = 1.0 / op.h[axis];
+  double fm2 = 0.0, fm1 = 0.0, f0 = f(0), fp1 = (n > 1) ? f(1) : 0.0, prev = 0.0;
+#pragma unroll
+  for (int i = 0; i < n; i++) {                                    // forward elimination
+    const double fp2 = (i + 2 < n) ? f(i + 2) : 0.0;
+    const double r = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
+    prev = (i == 0) ? r / __ldg(bet) : (r - al * prev) / __ldg(bet + i);
+    if (LOCAL) rl[LOCAL ? i : 0] = prev; else rg[(long long)i * st] = prev;
+    fm2 = fm1; fm1 = f0; f0 = fp1; fp1 = fp2;
+  }
+  const double cc = c * coef;
+  const double* Y = y + eoff + base;
+  double* O = out + eoff + base;
+  double next = 0.0;
+#pragma unroll
+  for (int i = n - 1; i >= 0; i--) {                               // back substitution + accumulation
+    const double ri = LOCAL ? rl[LOCAL ? i : 0] : rg[(long long)i * st];
+    next = (i == n - 1) ? ri : ri - __ldg(cfac + i + 1) * next;
+    const long long o = (long long)i * st;
+    O[o] = first ? fma(a, Y[o], cc * next) : fma(cc, next, O[o]);
+  }
+}
+
+// out += c * [ -Gamma_k X_k + sum_s p_s V'_s (kup_s X_up + n_s c_s kdn_s X_dn) ]   (damping and gauge terms)
+template <int M>
+__global__ void __launch_bounds__(256) k_compact_point(DevOp op, const double* __restrict__ in, double* out, double c,
+                                                       size_t slot_stride) {
+  const long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (cell >= op.cells) return;
+  const int k = blockIdx.y;
+  const double* X = in + (size_t)blockIdx.z * slot_stride;
+  int idx[2 * M];
+  cdecode<2 * M>(op, (unsigned)cell, idx);
+  double acc = -__ldg(op.Gamma + k) * X[(size_t)k * op.cells + cell];
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const double q = op.x0[s] + idx[s] * op.h[s];
+    const double p = op.x0[M + s] + idx[M + s] * op.h[M + s];
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+    if (ku >= 0) acc = fma(Vp * op.kup[s] * p, X[(size_t)ku * op.cells + cell], acc);
+    if (kd >= 0) acc = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp * op.kdn[s] * p, X[(size_t)kd * op.cells + cell], acc);
+  }
+  double* o = out + (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells + cell;
+  *o = fma(c, acc, *o);
 }
 
 }  // namespace
@@ -134,39 +177,49 @@ static int compact_deriv(const DevOp& op, const CompactTables& ct, const double*
   return 1;
 }
 
-// out = a*y + c*F(in) for slots [0, nb); scratch: three element-sized arrays (G, D, F)
+// out = a*y + c*F(in) for slots [0, nb); scratch: three element-sized arrays (the second one holds the elimination
+// values of lines longer than CLINE_MAX)
 int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double* in, const double* y, double* out, double a,
                          double c, int nb, size_t slot_stride, double* scratch, cudaStream_t s) {
   int launches = 0;
-  const unsigned blocks = (unsigned)((op.cells + 255) / 256);
-  double *G = scratch, *D = scratch + op.cells, *F = scratch + 2 * op.cells;
-  for (int b = 0; b < nb; b++) {
-    const double* X = in + (size_t)b * slot_stride;
-    for (int k = 0; k < op.K; k++) {
-#define CALL(MM) k_compact_init<MM><<<blocks, 256, 0, s>>>(op, X, k, F)
+  double* D = scratch + op.cells;
+  int first = 1;
+  for (int pa = 0; pa < 2; pa++)
+    for (int sI = 0; sI < op.M; sI++) {
+      const int axis = pa ? op.M + sI : sI;
+      const int n = op.n[axis];
+      const unsigned lb = (unsigned)((op.cells / n + 127) / 128);
+      const bool local = n <= CLINE_MAX;
+#define LINE(MM, PA, NFV, GRID, K0, B0)                                                                               \
+  k_compact_line<MM, PA, NFV><<<GRID, 128, 0, s>>>(op, in, y, out, a, c, sI, first, K0, B0, slot_stride, ct.bet[axis],  \
+                                                   ct.cfac[axis], D)
+#define LINE_PA(MM, NFV, GRID, K0, B0)                                                                                \
+  do { if (pa) LINE(MM, 1, NFV, GRID, K0, B0); else LINE(MM, 0, NFV, GRID, K0, B0); } while (0)
+#define CALL(MM)                                                                                                      \
+  do {                                                                                                                \
+    if (local) {                                                                                                      \
+      const dim3 grid(lb, op.K, nb);                                                                                  \
+      LINE_PA(MM, 0, grid, 0, 0);                                                                                     \
+      launches++;                                                                                                     \
+    } else {                                                                                                          \
+      for (int b = 0; b < nb; b++)                                                                                    \
+        for (int k = 0; k < op.K; k++) {                                                                              \
+          LINE_PA(MM, -1, dim3(lb, 1, 1), k, b);                                                                      \
+          launches++;                                                                                                 \
+        }                                                                                                             \
+    }                                                                                                                 \
+  } while (0)
       CDISPATCH(op.M, CALL);
 #undef CALL
-      launches++;
-      for (int sI = 0; sI < op.M; sI++) {
-        launches += compact_deriv(op, ct, X + (size_t)k * op.cells, sI, D, s);            // d/dq_s of X_k
-#define CALL(MM) k_compact_accum<MM><<<blocks, 256, 0, s>>>(op, D, sI, 0, F)
-        CDISPATCH(op.M, CALL);
-#undef CALL
-#define CALL(MM) k_compact_G<MM><<<blocks, 256, 0, s>>>(op, X, k, sI, G)
-        CDISPATCH(op.M, CALL);
-#undef CALL
-        launches += 2 + compact_deriv(op, ct, G, op.M + sI, D, s);                        // d/dp_s of G_s
-#define CALL(MM) k_compact_accum<MM><<<blocks, 256, 0, s>>>(op, D, sI, 1, F)
-        CDISPATCH(op.M, CALL);
-#undef CALL
-        launches++;
-      }
-      const size_t o = (size_t)b * slot_stride + (size_t)k * op.cells;
-      k_compact_combine<<<blocks, 256, 0, s>>>(F, y + o, out + o, op.cells, a, c);
-      launches++;
+#undef LINE_PA
+#undef LINE
+      first = 0;
     }
-  }
-  return launches;
+  const unsigned blocks = (unsigned)((op.cells + 255) / 256);
+#define CALL(MM) k_compact_point<MM><<<dim3(blocks, op.K, nb), 256, 0, s>>>(op, in, out, c, slot_stride)
+  CDISPATCH(op.M, CALL);
+#undef CALL
+  return launches + 1;
 }
 
 // out_k = Kick_obs(in_k) for every element of slots [0, nb)
