@@ -141,6 +141,67 @@ __global__ void __launch_bounds__(128) k_compact_line(DevOp op, const double* __
   }
 }
 
+// p_M pass (the contiguous axis): one thread per line would read 8 bytes per 128-byte line and request.  A warp
+// therefore takes 32 consecutive lines (32 n contiguous doubles), loads them coalesced, forms G_M on the way and
+// transposes through a padded shared tile [32][n+1]; every lane then runs the Thomas recurrence on its row in place,
+// and the tile is written back coalesced.  Needs n <= 32 and cells % (32 n) == 0.
+template <int M>
+__global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double* __restrict__ in, const double* y,
+                                                          double* out, double a, double c, int first,
+                                                          size_t slot_stride, const double* __restrict__ bet,
+                                                          const double* __restrict__ cfac) {
+  constexpr int s = M - 1, axis = 2 * M - 1;
+  extern __shared__ double tiles[];
+  const int n = op.n[axis], lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long line0 = ((long long)blockIdx.x * 4 + warp) * 32;
+  if (line0 >= op.cells / n) return;
+  double* tile = tiles + warp * 32 * (n + 1);
+  const int k = blockIdx.y;
+  const size_t eoff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells;
+  const long long base = line0 * n;                                // first cell of the tile
+  const double* Xk = in + eoff + base;
+  const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+  const double* Xu = Xk + ((long long)(ku >= 0 ? ku : k) - k) * op.cells;
+  const double* Xd = Xk + ((long long)(kd >= 0 ? kd : k) - k) * op.cells;
+  const double ncd = (kd >= 0) ? __ldg(op.nvec + 3 * k + s) * op.cdn[s] : 0.0;
+  for (int j = 0; j < n; j++) {                                    // coalesced load, G_M formed per cell
+    const int e = j * 32 + lane;
+    const int ln = e / n, i = e - ln * n;
+    const long long ql = (base + e) / op.pb;
+    const double q = op.x0[s] + (double)(ql % op.n[s]) * op.h[s];
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    double v = __ldg(op.dU[s] + ql) * Xk[e];
+    if (ku >= 0) v = fma(Vp, Xu[e], v);
+    if (kd >= 0) v = fma(ncd * Vp, Xd[e], v);
+    tile[ln * (n + 1) + i] = v;
+  }
+  __syncwarp();
+  double* row = tile + lane * (n + 1);
+  const double al = 1.0 / 3.0, ca = 7.0 / 9.0, cb = 1.0 / 36.0, inv_h = 1.0 / op.h[axis];
+  double fm2 = 0.0, fm1 = 0.0, f0 = row[0], fp1 = (n > 1) ? row[1] : 0.0, prev = 0.0;
+  for (int i = 0; i < n; i++) {                                    // forward elimination, in place
+    const double fp2 = (i + 2 < n) ? row[i + 2] : 0.0;
+    const double r = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
+    prev = (i == 0) ? r / __ldg(bet) : (r - al * prev) / __ldg(bet + i);
+    row[i] = prev;
+    fm2 = fm1; fm1 = f0; f0 = fp1; fp1 = fp2;
+  }
+  double next = 0.0;
+  for (int i = n - 1; i >= 0; i--) {                               // back substitution, in place
+    next = (i == n - 1) ? row[i] : row[i] - __ldg(cfac + i + 1) * next;
+    row[i] = next;
+  }
+  __syncwarp();
+  const double* Y = y + eoff + base;
+  double* O = out + eoff + base;
+  for (int j = 0; j < n; j++) {                                    // coalesced accumulation into the stage output
+    const int e = j * 32 + lane;
+    const int ln = e / n, i = e - ln * n;
+    const double d = tile[ln * (n + 1) + i];
+    O[e] = first ? fma(a, Y[e], c * d) : fma(c, d, O[e]);
+  }
+}
+
 // out += c * [ -Gamma_k X_k + sum_s p_s V'_s (kup_s X_up + n_s c_s kdn_s X_dn) ]   (damping and gauge terms)
 template <int M>
 __global__ void __launch_bounds__(256) k_compact_point(DevOp op, const double* __restrict__ in, double* out, double c,
@@ -197,7 +258,12 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
   do { if (pa) LINE(MM, 1, NFV, GRID, K0, B0); else LINE(MM, 0, NFV, GRID, K0, B0); } while (0)
 #define CALL(MM)                                                                                                      \
   do {                                                                                                                \
-    if (local) {                                                                                                      \
+    if (pa && sI == MM - 1 && n <= 32 && op.cells % (32 * n) == 0) {       /* contiguous axis: transposing kernel */    \
+      const unsigned wb = (unsigned)((op.cells / n / 32 + 3) / 4);                                                    \
+      k_compact_pline_s1<MM><<<dim3(wb, op.K, nb), 128, sizeof(double) * 4 * 32 * (n + 1), s>>>(                      \
+          op, in, y, out, a, c, first, slot_stride, ct.bet[axis], ct.cfac[axis]);                                     \
+      launches++;                                                                                                     \
+    } else if (local) {                                                                                               \
       const dim3 grid(lb, op.K, nb);                                                                                  \
       LINE_PA(MM, 0, grid, 0, 0);                                                                                     \
       launches++;                                                                                                     \

@@ -401,6 +401,10 @@ COMPACT = [
     ("m1", ci.config("cfg2", nq=[37], np=[41], depth=4, scheme="compact6")),
     ("m2_w", ci.config("cfg3s", nq=[9, 10], np=[11, 8], depth=2, scheme="compact6", gauge="w")),
     ("m3", ci.config("cfg4s8", nq=[6, 5, 7], np=[5, 7, 6], depth=2, scheme="compact6")),
+    # shapes whose contiguous p axis takes the transposing kernel (n <= 32, cells a multiple of 32 n)
+    ("m1_t", ci.config("cfg2", nq=[32], np=[16], depth=3, scheme="compact6")),
+    ("m2_t", ci.config("cfg3s", nq=[8, 7], np=[8, 16], depth=2, scheme="compact6")),
+    ("m3_t", ci.config("cfg4s8", nq=[8, 5, 6], np=[5, 8, 12], depth=2, scheme="compact6", gauge="w")),
 ]
 
 
