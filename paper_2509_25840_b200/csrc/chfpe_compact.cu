@@ -7,11 +7,12 @@
 // of 16..128 one thread per line is enough to occupy the GPU (a 16^6 grid has 10^6 lines per element and axis).
 //
 // This is the conditional path of SURVEY.md 8(a9); the explicit CENTRAL4 scheme is the performance path.  A stage is
-// 2M line passes + one pointwise pass, each ONE launch over all elements and replica slots (grid.y, grid.z):
+// 2M line passes, each ONE launch over all elements and replica slots (grid.y, grid.z):
 //   q_s pass: d = A^{-1} B X_k along q_s, accumulated as  out (+)= c * (-(p_s/m_s)) d
 //   p_s pass: d = A^{-1} B G_s along p_s with G_s = (dU/dq_s) X_k + V'_s X_up + n_s c_s V'_s X_dn formed on the fly
-//             (its coefficients are constant along a p-line),  out += c * d
-//   pointwise pass: out += c * [ -Gamma_k X_k + sum_s p_s V'_s (kup_s X_up + n_s c_s kdn_s X_dn) ]
+//             (its coefficients are constant along a p-line),  out += c * d; the pass has X_up and X_dn in hand, so
+//             it also adds the pointwise gauge terms c * p_s V'_s (kup_s X_up + n_s c_s kdn_s X_dn) of its mode, and
+//             the last one the damping -c * Gamma_k X_k
 // The first pass writes out = a*y + c*(...), so no right-hand-side array exists; the forward-elimination values of a
 // line stay in thread-local memory for lines of up to 128 points (all BASELINE configs), longer lines keep
 // them in an element-sized scratch array and run element by element.  (First version: whole-array derivatives,
@@ -98,7 +99,7 @@ __global__ void __launch_bounds__(128) k_compact_line(DevOp op, const double* __
   const double* Xk = in + eoff + base;
   const double* Xu = Xk;
   const double* Xd = Xk;
-  double ck = 1.0, cu = 0.0, cd = 0.0, coef = 1.0;
+  double ck = 1.0, cu = 0.0, cd = 0.0, coef = 1.0, gam = 0.0;
   if (PAXIS) {                                                     // G_s: coefficients depend on q only
     const long long ql = base / op.pb;
     const double q = op.x0[s] + idx[s] * op.h[s];
@@ -107,6 +108,7 @@ __global__ void __launch_bounds__(128) k_compact_line(DevOp op, const double* __
     const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
     if (ku >= 0) { cu = Vp; Xu = Xk + ((long long)ku - k) * op.cells; }
     if (kd >= 0) { cd = __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp; Xd = Xk + ((long long)kd - k) * op.cells; }
+    if (s == M - 1) gam = __ldg(op.Gamma + k);                     // the damping term rides on the last p pass
   } else {
     coef = -(op.x0[M + s] + idx[M + s] * op.h[M + s]) * op.inv_mass[s];
   }
@@ -137,7 +139,17 @@ __global__ void __launch_bounds__(128) k_compact_line(DevOp op, const double* __
     const double ri = LOCAL ? rl[LOCAL ? i : 0] : rg[(long long)i * st];
     next = (i == n - 1) ? ri : ri - __ldg(cfac + i + 1) * next;
     const long long o = (long long)i * st;
-    O[o] = first ? fma(a, Y[o], cc * next) : fma(cc, next, O[o]);
+    double t = cc * next;
+    if (PAXIS) {                                                   // pointwise terms of mode s (gauge) and the damping
+      const double p = op.x0[M + s] + i * op.h[M + s];
+      double pw = 0.0;
+      if (cu != 0.0) pw = op.kup[s] * cu * Xu[o];
+      if (cd != 0.0) pw = fma(op.kdn[s] * cd, Xd[o], pw);
+      pw *= p;
+      if (s == M - 1) pw = fma(-gam, Xk[o], pw);
+      t = fma(c, pw, t);
+    }
+    O[o] = first ? fma(a, Y[o], t) : O[o] + t;
   }
 }
 
@@ -155,7 +167,8 @@ __global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double
   const int n = op.n[axis], lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long line0 = ((long long)blockIdx.x * 4 + warp) * 32;
   if (line0 >= op.cells / n) return;
-  double* tile = tiles + warp * 32 * (n + 1);
+  double* tile = tiles + warp * 64 * (n + 1);                      // [32][n+1] G_M, then [32][n+1] pointwise terms
+  double* ptile = tile + 32 * (n + 1);
   const int k = blockIdx.y;
   const size_t eoff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells;
   const long long base = line0 * n;                                // first cell of the tile
@@ -164,16 +177,19 @@ __global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double
   const double* Xu = Xk + ((long long)(ku >= 0 ? ku : k) - k) * op.cells;
   const double* Xd = Xk + ((long long)(kd >= 0 ? kd : k) - k) * op.cells;
   const double ncd = (kd >= 0) ? __ldg(op.nvec + 3 * k + s) * op.cdn[s] : 0.0;
+  const double gam = __ldg(op.Gamma + k);
   for (int j = 0; j < n; j++) {                                    // coalesced load, G_M formed per cell
     const int e = j * 32 + lane;
     const int ln = e / n, i = e - ln * n;
     const long long ql = (base + e) / op.pb;
     const double q = op.x0[s] + (double)(ql % op.n[s]) * op.h[s];
     const double Vp = fma(op.VSL[s], q, op.VLL[s]);
-    double v = __ldg(op.dU[s] + ql) * Xk[e];
-    if (ku >= 0) v = fma(Vp, Xu[e], v);
-    if (kd >= 0) v = fma(ncd * Vp, Xd[e], v);
+    const double xk = Xk[e];
+    double v = __ldg(op.dU[s] + ql) * xk, pw = 0.0;
+    if (ku >= 0) { const double xu = Xu[e]; v = fma(Vp, xu, v); pw = op.kup[s] * Vp * xu; }
+    if (kd >= 0) { const double xd = Xd[e]; v = fma(ncd * Vp, xd, v); pw = fma(op.kdn[s] * ncd * Vp, xd, pw); }
     tile[ln * (n + 1) + i] = v;
+    ptile[ln * (n + 1) + i] = fma(-gam, xk, pw * (op.x0[axis] + i * op.h[axis]));   // gauge terms of mode M, damping
   }
   __syncwarp();
   double* row = tile + lane * (n + 1);
@@ -197,33 +213,9 @@ __global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double
   for (int j = 0; j < n; j++) {                                    // coalesced accumulation into the stage output
     const int e = j * 32 + lane;
     const int ln = e / n, i = e - ln * n;
-    const double d = tile[ln * (n + 1) + i];
+    const double d = tile[ln * (n + 1) + i] + ptile[ln * (n + 1) + i];
     O[e] = first ? fma(a, Y[e], c * d) : fma(c, d, O[e]);
   }
-}
-
-// out += c * [ -Gamma_k X_k + sum_s p_s V'_s (kup_s X_up + n_s c_s kdn_s X_dn) ]   (damping and gauge terms)
-template <int M>
-__global__ void __launch_bounds__(256) k_compact_point(DevOp op, const double* __restrict__ in, double* out, double c,
-                                                       size_t slot_stride) {
-  const long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (cell >= op.cells) return;
-  const int k = blockIdx.y;
-  const double* X = in + (size_t)blockIdx.z * slot_stride;
-  int idx[2 * M];
-  cdecode<2 * M>(op, (unsigned)cell, idx);
-  double acc = -__ldg(op.Gamma + k) * X[(size_t)k * op.cells + cell];
-#pragma unroll
-  for (int s = 0; s < M; s++) {
-    const double q = op.x0[s] + idx[s] * op.h[s];
-    const double p = op.x0[M + s] + idx[M + s] * op.h[M + s];
-    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
-    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
-    if (ku >= 0) acc = fma(Vp * op.kup[s] * p, X[(size_t)ku * op.cells + cell], acc);
-    if (kd >= 0) acc = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp * op.kdn[s] * p, X[(size_t)kd * op.cells + cell], acc);
-  }
-  double* o = out + (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells + cell;
-  *o = fma(c, acc, *o);
 }
 
 }  // namespace
@@ -260,7 +252,7 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
   do {                                                                                                                \
     if (pa && sI == MM - 1 && n <= 32 && op.cells % (32 * n) == 0) {       /* contiguous axis: transposing kernel */    \
       const unsigned wb = (unsigned)((op.cells / n / 32 + 3) / 4);                                                    \
-      k_compact_pline_s1<MM><<<dim3(wb, op.K, nb), 128, sizeof(double) * 4 * 32 * (n + 1), s>>>(                      \
+      k_compact_pline_s1<MM><<<dim3(wb, op.K, nb), 128, sizeof(double) * 4 * 64 * (n + 1), s>>>(                      \
           op, in, y, out, a, c, first, slot_stride, ct.bet[axis], ct.cfac[axis]);                                     \
       launches++;                                                                                                     \
     } else if (local) {                                                                                               \
@@ -281,11 +273,7 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
 #undef LINE
       first = 0;
     }
-  const unsigned blocks = (unsigned)((op.cells + 255) / 256);
-#define CALL(MM) k_compact_point<MM><<<dim3(blocks, op.K, nb), 256, 0, s>>>(op, in, out, c, slot_stride)
-  CDISPATCH(op.M, CALL);
-#undef CALL
-  return launches + 1;
+  return launches;
 }
 
 // out_k = Kick_obs(in_k) for every element of slots [0, nb)
