@@ -148,7 +148,7 @@ def workspace_bytes(cfg, batch=1):
 class CHFPE:
     """One library handle.  The workspace is a torch uint8 CUDA tensor owned by this object."""
 
-    def __init__(self, cfg, batch=1, device="cuda:0", stream=None):
+    def __init__(self, cfg, batch=1, device="cuda:0", stream=None, guard_bytes=0):
         import torch
         if not torch.cuda.is_available():
             raise ChfpeError("CUDA device required: the CHFPE path has no CPU fallback")
@@ -158,10 +158,14 @@ class CHFPE:
         d, keep = make_desc(cfg, batch)
         nbytes = workspace_bytes(cfg, batch)
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            # guard_bytes > 0 (tests): canary bytes on both sides of the workspace, checked by guards_intact()
+            self._guard = int(guard_bytes)
+            self.workspace = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=self.device) \
+                if self._guard else torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            base = self.workspace.data_ptr()
+            base = self.workspace.data_ptr() + self._guard
             aligned = (base + 255) & ~255
+            self._ws_lo, self._ws_hi = aligned - self.workspace.data_ptr(), aligned - self.workspace.data_ptr() + nbytes
             self._h = C.c_void_p()
             rc = L.chfpe_create(C.byref(d), C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream),
                                 C.byref(self._h))
@@ -179,6 +183,12 @@ class CHFPE:
     def _ck(self, rc, what):
         if rc != 0:
             raise ChfpeError("%s: %d %s" % (what, rc, lib().chfpe_last_error(self._h).decode()))
+
+    def guards_intact(self):
+        """True if no byte outside [workspace, workspace + workspace_bytes) was written (needs guard_bytes > 0)."""
+        self._torch.cuda.synchronize(self.device)
+        w = self.workspace
+        return bool((w[: self._ws_lo] == 0xA5).all().item() and (w[self._ws_hi:] == 0xA5).all().item())
 
     def close(self):
         if getattr(self, "_h", None):

@@ -397,6 +397,42 @@ def test_response_3d_closed_forms_and_errors():
     g2.close()
 
 
+GUARDED = [
+    ("m3_cube8", ci.config("cfg4s8"), 2),
+    ("m3_cube16", ci.config("cfg4", nq=[5, 5, 6]), 3),
+    ("m3_cube20_two_pass", ci.config("cfg5", nq=[5, 5, 5], depth=2), 3),
+    ("m2_48", ci.config("cfg3", nq=[6, 5], depth=2), 3),
+    ("m3_generic", ci.config("cfg4s8", nq=[7, 8, 6], np=[8, 6, 9], depth=3), 4),
+    ("m1_coop", ci.config("cfg1"), 2),
+    ("m3_compact_transposing", ci.config("cfg4s8", nq=[8, 5, 6], np=[5, 8, 12], depth=2, scheme="compact6"), 3),
+    ("m2_compact", ci.config("cfg3s", nq=[9, 10], np=[11, 8], depth=2, scheme="compact6"), 3),
+]
+
+
+@pytest.mark.parametrize("name,cfg,batch", GUARDED, ids=[c[0] for c in GUARDED])
+def test_no_write_outside_the_workspace(name, cfg, batch):
+    """Canary bytes on both sides of the caller-owned workspace survive every entry point, for every kernel family
+    (brick single- and two-pass, two-mode view, generic, cooperative, COMPACT6 line and transposing kernels)."""
+    P = gpu_mod()
+    M = cfg["n_modes"]
+    g = P.CHFPE(cfg, batch=batch, guard_bytes=1 << 20)
+    mu, al = make_obs(P, ci.observable("mu", M)), make_obs(P, ci.observable("alpha", M))
+    g.equilibrate(n_steps=2, dt=cfg["dt"])
+    g.kick(mu); g.step(3, cfg["dt"]); g.expect(al)
+    g.equilibrate()
+    g.response_1d(mu, mu, 4, 2, cfg["dt"])
+    g.equilibrate()
+    g.response_2d(mu, al, al, [0, 1, 3], [0, 2], cfg["dt"])
+    if batch >= 3:
+        g.equilibrate()
+        g.response_3d(mu, al, al, mu, [0, 2], [1, 2], [0, 1], cfg["dt"])
+    X = g.export_state(batch - 1)
+    g.import_state(X, replica=batch - 1)
+    g.export_rhs()
+    assert g.guards_intact()
+    g.close()
+
+
 COMPACT = [
     ("m1", ci.config("cfg2", nq=[37], np=[41], depth=4, scheme="compact6")),
     ("m2_w", ci.config("cfg3s", nq=[9, 10], np=[11, 8], depth=2, scheme="compact6", gauge="w")),
