@@ -397,6 +397,42 @@ def test_response_3d_closed_forms_and_errors():
     g2.close()
 
 
+PLAN_ENVS = [
+    {"CHFPE_Q2CHUNK": "3", "CHFPE_GROUP": "3"},                      # ragged q_2 chunks (7 = 3 + 3 + 1 -> equalised), ragged last group
+    {"CHFPE_Q2CHUNK": "2", "CHFPE_GROUP": "1", "CHFPE_BPC": "1"},
+    {"CHFPE_BPC": "5"},                                              # n_q3 = 5: one run per q_3 line
+    {"CHFPE_GROUP": "20"},                                           # all elements in one group
+    {"CHFPE_L2MODE": "0"}, {"CHFPE_L2MODE": "3"},
+    {"CHFPE_BRICK": "0"},                                            # generic kernel on a brick-shaped grid
+]
+
+
+@pytest.mark.parametrize("env", PLAN_ENVS, ids=["-".join("%s%s" % (k[6:], v) for k, v in e.items()) for e in PLAN_ENVS])
+@pytest.mark.parametrize("shape", ["cube8", "cube20_two_pass", "m2_16"])
+def test_brick_plan_variants(monkeypatch, env, shape):
+    """The host-tabulated brick order (element groups, q_2 chunks, runs per CTA) and the L2 policies only change the
+    ORDER and caching of the work: every variant must reproduce the oracle's right-hand side and steps.  (At full
+    size configs 4 and 5 take the chunked / grouped paths that small grids would otherwise never reach.)"""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    cfg = {"cube8": ci.config("cfg4s8", nq=[6, 7, 5]),
+           "cube20_two_pass": ci.config("cfg5", nq=[5, 6, 5], depth=2),
+           "m2_16": ci.config("cfg3s", nq=[7, 10])}[shape]
+    g, o = both(cfg, batch=2)
+    if env.get("CHFPE_BRICK") == "0":
+        assert g.stage_kernel() == "generic"
+    else:
+        assert g.stage_kernel() == "brick"
+    levels = [sum(n) for n in o.elements()]
+    X = ci.seeded_state(cfg, levels, seed=11)
+    g.import_state(X); g.import_state(X, replica=1); o.import_state(X)
+    assert rel_l2(g.export_rhs(1), o.rhs(X)) < 1e-13
+    g.step(2, cfg["dt"]); o.step(2, cfg["dt"])
+    assert rel_l2(g.export_state(0), o.export_state()) < 1e-12
+    assert np.array_equal(g.export_state(0), g.export_state(1))
+    g.close()
+
+
 GUARDED = [
     ("m3_cube8", ci.config("cfg4s8"), 2),
     ("m3_cube16", ci.config("cfg4", nq=[5, 5, 6]), 3),
