@@ -1,0 +1,102 @@
+"""Pins of the Hermite-representation oracle (oracle/hermite.py, row f1): the closed-form Brownian-oscillator response
+with fourth-order convergence in the q mesh, the exact first-moment ODE (incl. <p> from the k = 1 coefficient), and
+cross-validation against the independent phase-space-grid oracle (oracle/chfpe_ref.c) on anharmonic models with LL+SL
+coupling for one and two modes.  CPU only."""
+import numpy as np
+import scipy.linalg
+
+import chfpe_inputs as ci
+import oracle
+from oracle import hermite
+from conftest import make_obs
+
+ONE = {"c0": 1.0, "lin_q": [0.0] * 3, "quad": [[0.0] * 3] * 3, "lin_p": [0.0] * 3}
+
+
+def bo_matrix(w0=1.0, zeta=0.5, gamma=1.0):
+    return np.array([[0, 1, 0], [-w0 ** 2, 0, 1], [0, -zeta * gamma, -gamma]], dtype=float)
+
+
+def harmonic(n, half=9.0, kp=8, depth=3):
+    return ci.config("cfg1", nq=[n], np=[kp], depth=depth, qmin=[-half], qmax=[half])
+
+
+def test_element_order_matches_the_grid_oracle():
+    for M, depth, name in ((1, 5, "cfg1"), (2, 4, "cfg3s"), (3, 3, "cfg4s8")):
+        g = oracle.RefCHFPE(ci.config(name, nq=[5] * M, np=[5] * M, depth=depth))
+        assert hermite.enumerate_elements(M, depth) == [tuple(n) for n in g.elements()]
+
+
+def test_closed_form_response_converges_at_fourth_order():
+    """Literal Eq. (15) = -R_phys(t) = -[e^{At}]_{01}; the only error is the q stencil (h^4): the Hermite and hierarchy
+    truncations are exact for first moments of the harmonic + LL model."""
+    mu = ci.observable("mu", 1)
+    exact = scipy.linalg.expm(0.5 * bo_matrix())[0, 1]
+    errs = []
+    for n in (37, 73):                                           # h = 0.5, 0.25 on [-9, 9]
+        o = hermite.RefHermite(harmonic(n))
+        res = o.equilibrate()
+        assert abs(o.expect(ONE) - 1.0) < 1e-12
+        R = o.response_1d(mu, mu, 2, 500, 1e-3)
+        assert R[0] == 0.0
+        errs.append(abs(-R[1] - exact))
+        assert res < (2e-3 if n == 37 else 2e-4)                 # equilibrium is stationary up to the stencil error
+    assert 12.0 < errs[0] / errs[1] < 20.0 and errs[1] < 3e-5
+
+
+def test_first_moments_and_bath_force():
+    """<q>, <p> (from c_{k=1}) and <Omega> = -int W^(1) (from element 1) obey the 3 x 3 linear ODE of pin P3."""
+    o = hermite.RefHermite(harmonic(73))
+    o.equilibrate()
+    o.kick(ci.observable("mu", 1))
+    o.step(400, 1e-3)
+    y = scipy.linalg.expm(0.4 * bo_matrix()) @ np.array([0.0, -1.0, 0.0])
+    q = {"c0": 0.0, "lin_q": [1.0], "quad": [[0.0]], "lin_p": [0.0]}
+    p = {"c0": 0.0, "lin_q": [0.0], "quad": [[0.0]], "lin_p": [1.0]}
+    got = [o.expect(q), o.expect(p), -o.expect(ONE, element=1)]
+    assert np.max(np.abs(np.array(got) - y)) < 3e-5
+    assert abs(y[1]) > 0.5 and abs(y[2]) > 0.05                  # all three are exercised
+
+
+def test_cross_validation_with_the_grid_oracle_one_mode():
+    """Anharmonic U, LL + SL coupling, nonlinear dipole, kick by alpha = q^2: two independent discretisations of
+    Eq. (8) (Hermite functions vs a momentum mesh, numpy vs C) agree to the stencil error of either."""
+    al, d = ci.observable("alpha", 1), ci.observable("mu_nl", 1)
+    oh = hermite.RefHermite(ci.config("cfg2", nq=[64], np=[20], depth=6))
+    oh.equilibrate()
+    Rh = oh.response_1d(al, d, 2, 500, 1e-3)
+    og = oracle.RefCHFPE(ci.config("cfg2", nq=[64], np=[64], depth=6))
+    og.equilibrate()
+    Rg = og.response_1d(make_obs(oracle, al), make_obs(oracle, d), 2, 500, 1e-3)
+    assert np.max(np.abs(Rh)) > 0.2
+    assert np.max(np.abs(Rh - Rg)) < 1e-4
+
+
+def test_cross_validation_with_the_grid_oracle_two_modes():
+    """Two coupled anharmonic modes (cross term q1^2 q2), both baths: mode indices, couplings and the kick of both
+    modes against the grid oracle (coarse meshes)."""
+    al, d = ci.observable("alpha", 2), ci.observable("mu_nl", 2)
+    oh = hermite.RefHermite(ci.config("cfg3s", nq=[22, 22], np=[7, 7], depth=2))
+    oh.equilibrate()
+    Rh = oh.response_1d(al, d, 2, 60, 5e-3)
+    og = oracle.RefCHFPE(ci.config("cfg3s", nq=[22, 22], np=[22, 22], depth=2))
+    og.equilibrate()
+    Rg = og.response_1d(make_obs(oracle, al), make_obs(oracle, d), 2, 60, 5e-3)
+    assert abs(Rh[1]) > 0.3 and abs(Rh[1] - Rg[1]) < 8e-3 * abs(Rg[1])   # h = 0.57 meshes: 0.4 % apart
+
+
+def test_truncations_are_zero_ghosts():
+    """A state living in the top Hermite index and top hierarchy level only couples downwards."""
+    cfg = ci.config("cfg2", nq=[12], np=[4], depth=2)
+    o = hermite.RefHermite(cfg)
+    c = np.zeros(o.shape)
+    c[2, 3, :] = np.exp(-o.q[0] ** 2)                            # top level, top Hermite index
+    F = o.rhs(c)
+    # element 1 would receive it as c^(n+e)_{k-1} at k = 4 (outside), the level above does not exist
+    assert np.all(F[0] == 0.0) and np.all(F[1] == 0.0)
+    assert np.any(F[2, 2] != 0.0) and np.all(F[2, :2] == 0.0)
+    assert np.allclose(F[2, 3], -2.0 * cfg["gamma"][0] * c[2, 3], rtol=1e-15, atol=0)
+    c[:] = 0.0
+    c[1, 0, :] = np.exp(-o.q[0] ** 2)                            # level 1, k = 0: feeds level 0 at k = 1 only (Phi lowers n, raises k)
+    F = o.rhs(c)
+    assert np.any(F[0, 1] != 0.0) and np.all(F[0, 0] == 0.0) and np.all(F[0, 2:] == 0.0) and np.all(F[2] == 0.0)
