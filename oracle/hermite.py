@@ -175,6 +175,25 @@ class RefHermite:
                 self.step(stride, dt)
         return R
 
+    def response_2d(self, A, B, Cobs, t1_steps, t2_steps, dt):
+        """Literal Eq. (16), the double loop of section IV.C.2 :235-237: the A-kicked state is
+        advanced along t1; at every t1 sample a copy gets the B kick and is advanced along t2, <C> recorded."""
+        self.kick(A)
+        R = np.empty((len(t1_steps), len(t2_steps)))
+        now1 = 0
+        for i, s1 in enumerate(t1_steps):
+            self.step(s1 - now1, dt)
+            now1 = s1
+            saved = self.c.copy()
+            self.kick(B)
+            now2 = 0
+            for j, s2 in enumerate(t2_steps):
+                self.step(s2 - now2, dt)
+                now2 = s2
+                R[i, j] = self.expect(Cobs)
+            self.c = saved
+        return R
+
     def export_state(self):
         return self.c.copy()
 

@@ -58,6 +58,27 @@ def test_first_moments_and_bath_force():
     assert abs(y[1]) > 0.5 and abs(y[2]) > 0.05                  # all three are exercised
 
 
+def test_two_dimensional_closed_form():
+    """Pin P4 on the Hermite oracle: R2_lib(t2, t1) = 2 R_phys(t1) R_phys(t2) for A = C = q, B = q^2 on the harmonic
+    + LL model (tests/golden/r2_closed_form.txt, literal Eq. 16), zero for a linear B; second moments of the
+    harmonic model stay within Hermite index 2 and hierarchy level 2, so only the q stencil limits it."""
+    import os
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "r2_closed_form.txt"))
+    mu, al = ci.observable("mu", 1), ci.observable("alpha", 1)
+    errs = []
+    for n in (37, 73):                                           # h = 0.5, 0.25: the stencil error falls as h^4
+        o = hermite.RefHermite(harmonic(n, kp=6, depth=3))
+        o.equilibrate()
+        R = o.response_2d(mu, al, mu, [0, int(round(gold[0] / 2e-3))], [0, int(round(gold[1] / 2e-3))], 2e-3)
+        errs.append((abs(R[1, 1] - gold[2]), abs(R[0, 1])))
+        assert R[1, 0] == 0.0                                    # the B kick empties k = 0
+    assert errs[1][0] < 2e-4 and 10.0 < errs[0][0] / errs[1][0] < 22.0 and abs(gold[2]) > 1.0
+    assert errs[1][1] < 2e-4 and errs[0][1] / errs[1][1] > 10.0  # R_phys(t1 = 0) = 0 up to the stencil error
+    o.equilibrate()
+    R0 = o.response_2d(mu, mu, mu, [400], [600], 2e-3)
+    assert abs(R0[0, 0]) < 1e-7
+
+
 def test_cross_validation_with_the_grid_oracle_one_mode():
     """Anharmonic U, LL + SL coupling, nonlinear dipole, kick by alpha = q^2: two independent discretisations of
     Eq. (8) (Hermite functions vs a momentum mesh, numpy vs C) agree to the stencil error of either."""
