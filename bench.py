@@ -373,6 +373,90 @@ def run_3d(args):
     return 0
 
 
+def run_hermite(args):
+    """Row f1: the Hermite-in-momentum representation (the paper's production scheme, Eq. 22-23 and A1-A4)
+    on config 4's model: 32^3 q mesh x 8^3 Hermite functions x 20 elements = 3.36e8 values (the value count of
+    config 4).  A step = one RK4 step of the whole hierarchy (4 launches of k_hermite_stage) + <mu>.  Not a BASELINE
+    metric (there are no phase-space cells here): value-updates/s, with the same roofline accounting as the grid
+    path (22 compulsory bytes per value per launch)."""
+    import numpy as np
+    import torch
+    import paper_2509_25840_b200 as P
+    wl = args.workload if args.workload != "cfg4" else "cfg4h"
+    cfg = ci.config(wl)
+    M = cfg["n_modes"]
+    g = P.Hermite(cfg, batch=1)
+    mu = obs(P, "mu", M)
+    dt = cfg["dt"]
+    steps, warm = args.steps, max(args.warmup, 3)
+    g.equilibrate(residual=False)
+    g.kick(mu)
+    g.response_1d(None, mu, warm + 1, 1, dt)
+    sampler = ClockSampler(0)
+    sampler.start()
+    time.sleep(0.3)
+    n0 = g.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    torch.cuda.synchronize()
+    ev[0].record()
+    R = g.response_1d(None, mu, steps + 1, 1, dt)
+    ev[1].record()
+    torch.cuda.synchronize()
+    launches = g.launch_count() - n0
+    ev[2].record()
+    g.step(steps, dt)                                    # stage kernels only: 4 * steps launches
+    ev[3].record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms, ms_stage = ev[0].elapsed_time(ev[1]), ev[2].elapsed_time(ev[3])
+    if not np.all(np.isfinite(R)):
+        raise SystemExit("bench.py: non-finite response")
+    X0 = torch.from_numpy(g.export_state()).pin_memory()
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e2.record()
+    g.import_state(X0.numpy())
+    g.response_1d(None, mu, steps + 1, 1, dt)
+    e3.record()
+    torch.cuda.synchronize()
+    ms_e2e = e2.elapsed_time(e3)
+    peak, peak_src = measured_peaks()
+    values = g.values
+    kern_ms = ms_stage / (4 * steps)
+    achieved = values * 22.0 / (kern_ms * 1e-3) / 1e9
+    line = {"metric": "Hermite-representation value-updates/s (fp64)", "value": values * steps / (ms * 1e-3),
+            "unit": "value-updates/s", "n_gpus": 1, "steps": steps, "warmup": warm, "ms_per_step": ms / steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl + " (Hermite representation, row f1)", "modes": M,
+                       "shape": "x".join(str(x) for x in g.shape), "values": values, "depth": cfg["depth"], "dt": dt,
+                       "scheme": cfg["scheme"], "integrator": "RK4 (Horner form)",
+                       "l2": "inputs larger than L2 (state array %.1f GB vs 126 MB)" % (values * 8 / 1e9)},
+            "e2e": {"value": values * steps / (ms_e2e * 1e-3), "unit": "value-updates/s",
+                    "h2d_bytes_per_step": values * 8.0 / steps, "d2h_bytes_per_step": 8.0 * (steps + 1) / steps},
+            "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "kernel": "k_hermite_stage", "kernel_ms": kern_ms,
+                         "kernel_launches_timed": 4 * steps, "kernel_share_of_step": 4 * kern_ms / (ms / steps),
+                         "algorithmic_bytes_per_launch": values * 22.0}}
+    if not args.no_cpu:
+        from oracle import hermite
+        sub = ci.config(wl, nq=[12] * M) if M == 3 else cfg
+        o = hermite.RefHermite(sub)
+        o.equilibrate()
+        d = ci.observable("mu", M)
+        o.kick(d)
+        t0 = time.perf_counter()
+        o.step(1, dt); o.expect(d)
+        tc = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": float(np.prod(o.shape)) / tc, "unit": "value-updates/s",
+                                "cores": os.cpu_count(), "kind": "oracle",
+                                "sample": "oracle/hermite.py (numpy) on %s with a %s q mesh, 1 RK4 step + <mu> (%.1f s)"
+                                          % (wl, "x".join(str(x) for x in o.nq), tc)}
+    print(json.dumps(line))
+    g.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -384,12 +468,16 @@ def main():
     ap.add_argument("--protocol", default="step", choices=["step", "2d", "3d"],
                     help="'2d': time chfpe_response_2d on config 5 (secondary metric: 2D THz-Raman wall time); "
                          "'3d': time chfpe_response_3d (row f2) on --workload")
+    ap.add_argument("--representation", default="grid", choices=["grid", "hermite"],
+                    help="'hermite': row f1, the Hermite-in-momentum representation on cfg4h (not a BASELINE metric)")
     ap.add_argument("--batch", type=int, default=5, help="replica slots for --protocol 2d (trajectory + t1 replicas)")
     ap.add_argument("--n1", type=int, default=8)
     ap.add_argument("--n2", type=int, default=16)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.representation == "hermite":
+        return run_hermite(args)
     if args.protocol == "2d":
         return run_2d(args)
     if args.protocol == "3d":

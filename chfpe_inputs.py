@@ -45,8 +45,8 @@ def config(name, **over):
         U = _poly_modes([1.0, 0.6], g4=[0.05, 0.05]) + [(0.1 / 6.0, (2, 1))]
         c = dict(n_modes=2, U=U, V_LL=[1.0, 1.0], V_SL=[0.3, 0.3], zeta=[0.5, 0.5], gamma=[1.0, 1.0], beta=1.0,
                  depth=4, dt=1e-3, steps=5000, **_grid(2, n, 6.0))
-    elif name in ("cfg4", "cfg5", "cfg4s8", "cfg4s10", "cfg4s12"):   # 3 intermolecular-like modes
-        n = {"cfg4": 16, "cfg5": 20, "cfg4s8": 8, "cfg4s10": 10, "cfg4s12": 12}[name]
+    elif name in ("cfg4", "cfg5", "cfg4s8", "cfg4s10", "cfg4s12", "cfg4h"):   # 3 intermolecular-like modes
+        n = {"cfg4": 16, "cfg5": 20, "cfg4s8": 8, "cfg4s10": 10, "cfg4s12": 12, "cfg4h": 32}[name]
         U = _poly_modes([1.0, 0.5, 0.25], g4=[0.03, 0.03, 0.03])
         for a in range(3):
             for b in range(3):
@@ -57,6 +57,8 @@ def config(name, **over):
                     U.append((0.05 / 6.0, tuple(e)))
         c = dict(n_modes=3, U=U, V_LL=[1.0] * 3, V_SL=[0.2] * 3, zeta=[1.0, 0.65, 0.3], gamma=[0.5, 1.0, 2.0],
                  beta=1.0, depth=3, dt=1e-3, steps=10000, **_grid(3, n, 6.0))
+        if name == "cfg4h":     # config 4's model in the Hermite representation (row f1): 32^3 q mesh, np = 8 Hermite
+            c["np"] = [8, 8, 8]  # functions per mode -> 20 x 512 x 32768 = 3.36e8 values, the value count of config 4
     else:
         raise KeyError(name)
     c["name"] = name
@@ -108,4 +110,27 @@ def seeded_state(cfg, levels, seed):
     for k, lev in enumerate(levels):
         u = rng.uniform(-1.0, 1.0, size=shape)
         X[k] = env * (0.5 ** lev) * (1.0 + 0.5 * u)
+    return X
+
+
+def seeded_hermite_state(cfg, levels, seed):
+    """Random state for the Hermite representation, shape (K, kp_1..kp_M, nq_1..nq_M) with cfg["np"] = Hermite
+    functions per mode: c = E(q) * 2^-level * prod_s 0.8^k_s * (1 + 0.5 u), u ~ U(-1,1), E the Gaussian envelope
+    exp(-q.q/4).  Exercises every element, every Hermite index and every coupling."""
+    rng = np.random.default_rng(seed)
+    M = cfg["n_modes"]
+    kp, nq = list(cfg["np"][:M]), list(cfg["nq"][:M])
+    shape = tuple(kp) + tuple(nq)
+    env = np.ones(shape)
+    for s in range(M):
+        sh = [1] * (2 * M)
+        sh[s] = kp[s]
+        env = env * (0.8 ** np.arange(kp[s])).reshape(sh)
+        x = np.linspace(cfg["qmin"][s], cfg["qmax"][s], nq[s])
+        sh = [1] * (2 * M)
+        sh[M + s] = nq[s]
+        env = env * np.exp(-0.25 * x * x).reshape(sh)
+    X = np.empty((len(levels),) + shape)
+    for k, lev in enumerate(levels):
+        X[k] = env * (0.5 ** lev) * (1.0 + 0.5 * rng.uniform(-1.0, 1.0, size=shape))
     return X

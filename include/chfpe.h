@@ -168,6 +168,48 @@ int chfpe_stage_kernel(const chfpe_handle* h, int32_t* kind);
 
 const char* chfpe_last_error(const chfpe_handle* h);   /* h may be NULL: last create-time error */
 
+/* ---- Hermite-in-momentum representation (row f1 of DESIGN.md): the paper's production scheme -----------------------
+   Eq. (22)-(23) :156-164: W^(n)(p,q) = prod_s psi_0(p_s) e^{-beta U(q)/2} sum_k c^(n)_k(q) prod_s psi_{k_s}(p_s), psi_j the
+   orthonormal Hermite functions of width sqrt(2 m_s/beta); equations of motion = de-garbled Eq. (A1)-(A4) :343-355
+   (reading R19 of DESIGN.md, with the n_s factor of R1):
+     d/dt c^(n)_k = sum_s [ sqrt(k_s+1) D+_s c^(n)_{k+e_s} - sqrt(k_s) D-_s c^(n)_{k-e_s} ] - Gamma_n c^(n)_k
+                  + sum_s V'_s [ n_s gamma_s zeta_s sqrt(m_s/beta) sqrt(k_s+1) c^(n-e_s)_{k+e_s} - sqrt(k_s beta/m_s) c^(n+e_s)_{k-e_s} ],
+     D+-_s g = (dU/dq_s) / (2 sqrt(m_s/beta)) g -+ (1/sqrt(m_s beta)) dg/dq_s.
+   The same chfpe_desc is used with np[s] = number of Hermite functions of mode s (>= 1); pmin/pmax and gauge are
+   ignored; scheme = CHFPE_CENTRAL4 | CHFPE_CENTRAL2 (q-derivatives, zero ghosts R9).  State layout of one replica
+   (import/export AND device): c[element][k_1]..[k_M][i_q1]..[i_qM], last axis fastest, fp64; element order as above.
+   Same conventions as the grid calls: caller-owned 256-byte aligned device workspace and stream, int return codes,
+   host pointers unless stated, calls returning host data synchronise the stream.  No CPU fallback. */
+typedef struct chfpe_hermite_handle chfpe_hermite_handle;
+int chfpe_hermite_workspace_bytes(const chfpe_desc* desc, size_t* bytes);
+int chfpe_hermite_create(const chfpe_desc* desc, void* dev_workspace, size_t bytes, void* cuda_stream,
+                         chfpe_hermite_handle** out);
+int chfpe_hermite_destroy(chfpe_hermite_handle* h);
+int chfpe_hermite_num_elements(const chfpe_hermite_handle* h, int32_t* K);
+/* All replicas: c^(0)_0 <- e^{-beta U/2} / Z_q (Z_q = dV sum_q e^{-beta U}), all other coefficients 0, then n_steps
+   RK4 steps (section IV.B :221-223).  residual_out (may be NULL) <- ||F(c)||_2 / ||c||_2 of replica 0. */
+int chfpe_hermite_equilibrate(chfpe_hermite_handle* h, int64_t n_steps, double dt, double* residual_out);
+/* n_steps RK4 steps on every replica (Horner form of the degree-4 Taylor polynomial, R13). */
+int chfpe_hermite_step(chfpe_hermite_handle* h, int64_t n_steps, double dt);
+/* Eq. (18) :131 on every element of every replica: c_k <- sum_s (dX/dq_s) (-sqrt(k_s beta/m_s)) c_{k-e_s}. */
+int chfpe_hermite_kick(chfpe_hermite_handle* h, const chfpe_observable* X);
+/* out[b] (length batch) <- int int O W^(element) dp dq = dV sum_q e^{-beta U/2} [ O(q) c_0 + sum_s lin_p[s] sqrt(m_s/beta) c_{e_s} ]
+   of replica b (Eq. 15 :119 for element 0). */
+int chfpe_hermite_expect(chfpe_hermite_handle* h, int32_t element, const chfpe_observable* O, double* out);
+/* Same protocols as chfpe_response_1d / _2d (literal Eq. 15, 16); response_2d needs batch >= 2 (slot 0 carries the
+   t1 trajectory, batch-1 replicas of different t1 advance together per launch). */
+int chfpe_hermite_response_1d(chfpe_hermite_handle* h, const chfpe_observable* A, const chfpe_observable* C,
+                              int64_t n_samples, int64_t stride, double dt, double* R);
+int chfpe_hermite_response_2d(chfpe_hermite_handle* h, const chfpe_observable* A, const chfpe_observable* B,
+                              const chfpe_observable* C, const int64_t* t1_steps, int32_t n1, const int64_t* t2_steps,
+                              int32_t n2, double dt, double* R);
+/* K * prod(np) * prod(nq) doubles; dst/src: device if *_is_device, else host. */
+int chfpe_hermite_export_state(chfpe_hermite_handle* h, int32_t replica, double* dst, int dst_is_device);
+int chfpe_hermite_import_state(chfpe_hermite_handle* h, int32_t replica, const double* src, int src_is_device);
+int chfpe_hermite_export_rhs(chfpe_hermite_handle* h, int32_t replica, double* dst, int dst_is_device);
+int chfpe_hermite_launch_count(const chfpe_hermite_handle* h, int64_t* n);
+const char* chfpe_hermite_last_error(const chfpe_hermite_handle* h);   /* h may be NULL: last create-time error */
+
 #ifdef __cplusplus
 }
 #endif

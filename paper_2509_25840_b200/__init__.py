@@ -4,5 +4,5 @@ Argument marshalling only -- every step of the path runs in the hand-written sm_
 C-ABI of ``include/chfpe.h``.  PyTorch is used for device memory (the workspace tensor) and streams.
 There is no CPU fallback: constructing a ``CHFPE`` without the CUDA library or without a GPU raises.
 """
-from .binding import (CHFPE, ChfpeError, lib, make_observable, workspace_bytes, spectrum_1d, spectrum_2d,  # noqa: F401
+from .binding import (CHFPE, Hermite, hermite_workspace_bytes, ChfpeError, lib, make_observable, workspace_bytes, spectrum_1d, spectrum_2d,  # noqa: F401
                       EXPORTED_SYMBOLS)

@@ -11,6 +11,10 @@ EXPORTED_SYMBOLS = [
     "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
     "chfpe_response_1d", "chfpe_response_2d", "chfpe_response_3d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
     "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_spectrum_1d", "chfpe_spectrum_2d", "chfpe_last_error",
+    "chfpe_hermite_workspace_bytes", "chfpe_hermite_create", "chfpe_hermite_destroy", "chfpe_hermite_num_elements",
+    "chfpe_hermite_equilibrate", "chfpe_hermite_step", "chfpe_hermite_kick", "chfpe_hermite_expect",
+    "chfpe_hermite_response_1d", "chfpe_hermite_response_2d", "chfpe_hermite_export_state",
+    "chfpe_hermite_import_state", "chfpe_hermite_export_rhs", "chfpe_hermite_launch_count", "chfpe_hermite_last_error",
 ]
 
 
@@ -82,6 +86,22 @@ def lib():
                                     C.c_int32, C.c_int32, vp, vp]
     L.chfpe_last_error.argtypes = [vp]
     L.chfpe_last_error.restype = C.c_char_p
+    L.chfpe_hermite_workspace_bytes.argtypes = [C.POINTER(Desc), C.POINTER(C.c_size_t)]
+    L.chfpe_hermite_create.argtypes = [C.POINTER(Desc), vp, C.c_size_t, vp, C.POINTER(vp)]
+    L.chfpe_hermite_destroy.argtypes = [vp]
+    L.chfpe_hermite_num_elements.argtypes = [vp, C.POINTER(C.c_int32)]
+    L.chfpe_hermite_equilibrate.argtypes = [vp, C.c_int64, C.c_double, dp]
+    L.chfpe_hermite_step.argtypes = [vp, C.c_int64, C.c_double]
+    L.chfpe_hermite_kick.argtypes = [vp, op]
+    L.chfpe_hermite_expect.argtypes = [vp, C.c_int32, op, dp]
+    L.chfpe_hermite_response_1d.argtypes = [vp, op, op, C.c_int64, C.c_int64, C.c_double, dp]
+    L.chfpe_hermite_response_2d.argtypes = [vp, op, op, op, i64p, C.c_int32, i64p, C.c_int32, C.c_double, dp]
+    L.chfpe_hermite_export_state.argtypes = [vp, C.c_int32, vp, C.c_int]
+    L.chfpe_hermite_import_state.argtypes = [vp, C.c_int32, vp, C.c_int]
+    L.chfpe_hermite_export_rhs.argtypes = [vp, C.c_int32, vp, C.c_int]
+    L.chfpe_hermite_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.chfpe_hermite_last_error.argtypes = [vp]
+    L.chfpe_hermite_last_error.restype = C.c_char_p
     _lib = L
     return L
 
@@ -308,6 +328,138 @@ class CHFPE:
     def launch_count(self):
         n = C.c_int64()
         self._ck(lib().chfpe_launch_count(self._h, C.byref(n)), "chfpe_launch_count")
+        return n.value
+
+
+def hermite_workspace_bytes(cfg, batch=1):
+    d, _keep = make_desc(_hermite_cfg(cfg), batch)
+    n = C.c_size_t()
+    rc = lib().chfpe_hermite_workspace_bytes(C.byref(d), C.byref(n))
+    if rc != 0:
+        raise ChfpeError("chfpe_hermite_workspace_bytes: %d %s" % (rc, lib().chfpe_hermite_last_error(None).decode()))
+    return n.value
+
+
+def _hermite_cfg(cfg):
+    cfg = dict(cfg)                                   # the momentum range is unused by the Hermite representation
+    cfg.setdefault("pmin", [-1.0] * cfg["n_modes"])
+    cfg.setdefault("pmax", [1.0] * cfg["n_modes"])
+    return cfg
+
+
+class Hermite:
+    """One chfpe_hermite_* handle (row f1: Hermite functions in the momenta, cfg["np"] = functions per mode).
+    State arrays have the shape (K, kp_1..kp_M, nq_1..nq_M).  The workspace is a torch uint8 CUDA tensor."""
+
+    def __init__(self, cfg, batch=1, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise ChfpeError("CUDA device required: the CHFPE path has no CPU fallback")
+        L = lib()
+        self._torch = torch
+        self.device = torch.device(device)
+        cfg = _hermite_cfg(cfg)
+        d, keep = make_desc(cfg, batch)
+        nbytes = hermite_workspace_bytes(cfg, batch)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            aligned = (self.workspace.data_ptr() + 255) & ~255
+            self._h = C.c_void_p()
+            rc = L.chfpe_hermite_create(C.byref(d), C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream),
+                                        C.byref(self._h))
+        if rc != 0:
+            raise ChfpeError("chfpe_hermite_create: %d %s" % (rc, L.chfpe_hermite_last_error(None).decode()))
+        self.cfg, self.batch, self.M = cfg, batch, cfg["n_modes"]
+        k = C.c_int32()
+        L.chfpe_hermite_num_elements(self._h, C.byref(k))
+        self.K = k.value
+        self.shape = (self.K,) + tuple(cfg["np"][: self.M]) + tuple(cfg["nq"][: self.M])
+        self.values = int(np.prod(self.shape))
+
+    def _ck(self, rc, what):
+        if rc != 0:
+            raise ChfpeError("%s: %d %s" % (what, rc, lib().chfpe_hermite_last_error(self._h).decode()))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().chfpe_hermite_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def equilibrate(self, n_steps=0, dt=0.0, residual=True):
+        r = C.c_double()
+        self._ck(lib().chfpe_hermite_equilibrate(self._h, n_steps, dt, C.byref(r) if residual else None),
+                 "chfpe_hermite_equilibrate")
+        return r.value if residual else None
+
+    def step(self, n_steps, dt):
+        self._ck(lib().chfpe_hermite_step(self._h, n_steps, dt), "chfpe_hermite_step")
+
+    def kick(self, obs):
+        self._ck(lib().chfpe_hermite_kick(self._h, C.byref(obs)), "chfpe_hermite_kick")
+
+    def expect(self, obs, element=0):
+        out = np.empty(self.batch)
+        self._ck(lib().chfpe_hermite_expect(self._h, element, C.byref(obs), out.ctypes.data_as(C.POINTER(C.c_double))),
+                 "chfpe_hermite_expect")
+        return out
+
+    def response_1d(self, A, Cobs, n_samples, stride, dt):
+        R = np.empty(n_samples)
+        self._ck(lib().chfpe_hermite_response_1d(self._h, C.byref(A) if A is not None else None, C.byref(Cobs),
+                                                 n_samples, stride, dt, R.ctypes.data_as(C.POINTER(C.c_double))),
+                 "chfpe_hermite_response_1d")
+        return R
+
+    def response_2d(self, A, B, Cobs, t1_steps, t2_steps, dt):
+        t1 = np.ascontiguousarray(t1_steps, dtype=np.int64)
+        t2 = np.ascontiguousarray(t2_steps, dtype=np.int64)
+        R = np.empty((len(t1), len(t2)))
+        self._ck(lib().chfpe_hermite_response_2d(self._h, C.byref(A), C.byref(B), C.byref(Cobs),
+                                                 t1.ctypes.data_as(C.POINTER(C.c_int64)), len(t1),
+                                                 t2.ctypes.data_as(C.POINTER(C.c_int64)), len(t2), dt,
+                                                 R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_hermite_response_2d")
+        return R
+
+    def export_state(self, replica=0):
+        X = np.empty(self.shape)
+        self._ck(lib().chfpe_hermite_export_state(self._h, replica, C.c_void_p(X.ctypes.data), 0),
+                 "chfpe_hermite_export_state")
+        return X
+
+    def import_state(self, X, replica=0):
+        if hasattr(X, "data_ptr"):
+            assert X.is_cuda and X.is_contiguous() and X.numel() == self.values
+            self._ck(lib().chfpe_hermite_import_state(self._h, replica, C.c_void_p(X.data_ptr()), 1),
+                     "chfpe_hermite_import_state")
+            return
+        X = np.ascontiguousarray(X, dtype=np.float64)
+        assert X.size == self.values
+        self._ck(lib().chfpe_hermite_import_state(self._h, replica, C.c_void_p(X.ctypes.data), 0),
+                 "chfpe_hermite_import_state")
+
+    def export_rhs(self, replica=0):
+        F = np.empty(self.shape)
+        self._ck(lib().chfpe_hermite_export_rhs(self._h, replica, C.c_void_p(F.ctypes.data), 0),
+                 "chfpe_hermite_export_rhs")
+        return F
+
+    def export_rhs_device(self, replica=0):
+        t = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device)
+        self._ck(lib().chfpe_hermite_export_rhs(self._h, replica, C.c_void_p(t.data_ptr()), 1),
+                 "chfpe_hermite_export_rhs")
+        return t
+
+    def launch_count(self):
+        n = C.c_int64()
+        self._ck(lib().chfpe_hermite_launch_count(self._h, C.byref(n)), "chfpe_hermite_launch_count")
         return n.value
 
 

@@ -1,0 +1,711 @@
+// Row f1 of DESIGN.md: the paper's production representation, Hermite functions in the momenta (Eq. 22-23
+// PAPER.md:156-164, de-garbled Eq. A1-A4 :343-355, reading R19) -- host side of the chfpe_hermite_* C-ABI and its
+// sm_100a kernels.  State: c[slot][element n][k_1..k_M][q_1..q_M], q_M fastest; one (element, Hermite multi-index)
+// pair owns one contiguous "slab" of Q = prod nq doubles.  The generator couples slab (n, k) to the slabs
+// (n, k +- e_s) through D+-_s (a pointwise dU/dq_s term and a q_s-derivative) and pointwise to (n - e_s, k + e_s),
+// (n + e_s, k - e_s) through Theta, Phi: one fused kernel per RK stage, out = a y + c F(in).
+// Shares nothing with oracle/ and nothing but include/chfpe.h with the phase-space-grid path.
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <cmath>
+#include <cstring>
+#include <string>
+#include <vector>
+#include "../../include/chfpe.h"
+
+namespace {
+
+thread_local std::string g_err;
+
+// Host-tabulated neighbourhood of one slab (setup step a0): every index and square-root factor the kernels need,
+// so that no kernel decodes an element or a Hermite multi-index.
+struct HSlab {
+  int up[3], dn[3];        // slab of (n, k + e_s), (n, k - e_s), -1 outside 0 <= k_s < K_p,s
+  int hdn[3], hup[3];      // slab of (n - e_s, k + e_s), (n + e_s, k - e_s), -1 if absent (R5: zero outside the simplex)
+  double su[3], sd[3];     // sqrt(k_s + 1), sqrt(k_s)
+  double hd[3], hu[3];     // n_s gamma_s zeta_s sqrt(m_s/beta) sqrt(k_s + 1),  -sqrt(k_s beta/m_s)
+  double gam, pad;         // Gamma_n = sum_s n_s gamma_s
+};
+static_assert(sizeof(HSlab) == 160, "HSlab layout");
+
+struct HOp {                // device view of the operator, passed by value
+  int M, K, scheme;
+  int nq[3], kp[3], qst[3], kst[3];   // points, Hermite functions, q strides inside a slab, k strides in slabs
+  int Q, KP, nslab, blocks_per_slab, threads;
+  double q0[3], h[3], c1[3], c2[3];   // stencil weights of +-1, +-2 neighbours (pre-divided by 12h resp. 2h)
+  double a1f[3], a2[3];               // 1 / (2 sqrt(m/beta)),  1 / sqrt(m beta)        (A2)
+  double VLL[3], VSL[3];
+  double kickf[3], pfac[3];           // -sqrt(beta/m),  sqrt(m/beta)
+  double dV;
+  const double* dU[3];                // dU/dq_s on the q grid
+  const double* wq;                   // exp(-beta U / 2)
+  const double* ceq;                  // exp(-beta U / 2) / Z_q, Z_q = dV sum exp(-beta U)
+  const HSlab* slabs;
+};
+
+struct HObs { double c0, lin_q[3], quad[3][3], lin_p[3]; };
+
+constexpr long long RESULTS = 65536;   // doubles in the device results buffer
+constexpr int RED_BLOCKS = 296;        // partial sums per reduction (2 per SM), fixed: results do not depend on the device
+
+__device__ __forceinline__ double dq_stencil(const double* __restrict__ p, int i, int n, int st, double c1, double c2) {
+  const double p1 = (i + 1 < n) ? __ldg(p + st) : 0.0;
+  const double m1 = (i >= 1) ? __ldg(p - st) : 0.0;
+  double d = c1 * (p1 - m1);
+  if (c2 != 0.0) {
+    const double p2 = (i + 2 < n) ? __ldg(p + 2 * st) : 0.0;
+    const double m2 = (i >= 2) ? __ldg(p - 2 * st) : 0.0;
+    d += c2 * (p2 - m2);
+  }
+  return d;
+}
+
+// One RK stage: out = a*y + c*F(in) on every slab of every slot (grid.y).  One thread per (slab, q-point), the q grid
+// of a slab is covered by `blocks_per_slab` consecutive CTAs, so everything about the slab is CTA-uniform.
+template <int M>
+__global__ void __launch_bounds__(256) k_hermite_stage(const HOp op, const double* __restrict__ in,
+                                                      const double* y, double* out,
+                                                      const double a, const double c, const size_t slot_stride) {
+  const int slab = blockIdx.x / op.blocks_per_slab;
+  const int qi = (blockIdx.x - slab * op.blocks_per_slab) * blockDim.x + threadIdx.x;
+  if (qi >= op.Q) return;
+  const size_t soff = (size_t)blockIdx.y * slot_stride;
+  in += soff;
+  const HSlab* __restrict__ S = op.slabs + slab;
+  int iq[3] = {0, 0, 0};
+  {
+    int r = qi;
+#pragma unroll
+    for (int s = M - 1; s > 0; s--) { const int t = r / op.nq[s]; iq[s] = r - t * op.nq[s]; r = t; }
+    iq[0] = r;
+  }
+  const size_t Q = (size_t)op.Q;
+  const size_t self = (size_t)slab * Q + qi;
+  double acc = -S->gam * __ldg(in + self);
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const int st = op.qst[s], n = op.nq[s], i = iq[s];
+    const int up = S->up[s], dn = S->dn[s], hdn = S->hdn[s], hup = S->hup[s];
+    double lin = 0.0, der = 0.0;
+    if (up >= 0) {                                   // sqrt(k+1) D+ c_{k+e_s}
+      const double* p = in + (size_t)up * Q + qi;
+      const double su = S->su[s];
+      lin += su * __ldg(p);
+      der += su * dq_stencil(p, i, n, st, op.c1[s], op.c2[s]);
+    }
+    if (dn >= 0) {                                   // -sqrt(k) D- c_{k-e_s}
+      const double* p = in + (size_t)dn * Q + qi;
+      const double sd = S->sd[s];
+      lin -= sd * __ldg(p);
+      der += sd * dq_stencil(p, i, n, st, op.c1[s], op.c2[s]);
+    }
+    acc += op.a1f[s] * __ldg(op.dU[s] + qi) * lin - op.a2[s] * der;
+    double hh = 0.0;                                 // Theta (from n - e_s) and Phi (from n + e_s), pointwise in q
+    if (hdn >= 0) hh += S->hd[s] * __ldg(in + (size_t)hdn * Q + qi);
+    if (hup >= 0) hh += S->hu[s] * __ldg(in + (size_t)hup * Q + qi);
+    acc += (op.VLL[s] + op.VSL[s] * (op.q0[s] + op.h[s] * (double)i)) * hh;
+  }
+  const double base = (a != 0.0) ? a * y[soff + self] : 0.0;
+  out[soff + self] = base + c * acc;
+}
+
+// Kick, Eq. (18) :131 projected on the Hermite functions: c_k <- sum_s (dX/dq_s) (-sqrt(k_s beta/m_s)) c_{k-e_s}
+template <int M>
+__global__ void __launch_bounds__(256) k_hermite_kick(const HOp op, const HObs o, const double* __restrict__ in,
+                                                     double* __restrict__ out, const size_t slot_stride) {
+  const int slab = blockIdx.x / op.blocks_per_slab;
+  const int qi = (blockIdx.x - slab * op.blocks_per_slab) * blockDim.x + threadIdx.x;
+  if (qi >= op.Q) return;
+  const size_t soff = (size_t)blockIdx.y * slot_stride;
+  const HSlab* __restrict__ S = op.slabs + slab;
+  double q[3] = {0.0, 0.0, 0.0};
+  {
+    int r = qi;
+#pragma unroll
+    for (int s = M - 1; s > 0; s--) { const int t = r / op.nq[s]; q[s] = op.q0[s] + op.h[s] * (double)(r - t * op.nq[s]); r = t; }
+    q[0] = op.q0[0] + op.h[0] * (double)r;
+  }
+  const size_t Q = (size_t)op.Q;
+  double acc = 0.0;
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const int dn = S->dn[s];
+    if (dn < 0) continue;
+    double g = o.lin_q[s];
+#pragma unroll
+    for (int r = 0; r < M; r++) g += 0.5 * (o.quad[s][r] + o.quad[r][s]) * q[r];
+    acc += op.kickf[s] * g * S->sd[s] * __ldg(in + soff + (size_t)dn * Q + qi);
+  }
+  out[soff + (size_t)slab * Q + qi] = acc;
+}
+
+__device__ __forceinline__ double block_sum(double v) {
+  __shared__ double sh[32];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) sh[w] = v;
+  __syncthreads();
+  double t = 0.0;
+  if (w == 0) {
+    t = (l < (int)(blockDim.x >> 5)) ? sh[l] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+  }
+  return t;                                          // valid in thread 0
+}
+
+// Partial sums of a deterministic two-pass reduction: block b owns the fixed chunk [b*chunk, (b+1)*chunk).
+// mode 0: integrand of <O> on element `elem` (int O W^(0) dp dq = int O(q) e^{-beta U/2} c_0(q) dq, <p_s> from c_{e_s});
+// mode 1: sum of squares of n doubles starting at x (+ slot offset).
+template <int M>
+__global__ void __launch_bounds__(256) k_hermite_reduce_partial(const HOp op, const HObs o, const int mode,
+                                                               const double* __restrict__ x, const int elem,
+                                                               const long long n, const size_t slot_stride,
+                                                               double* __restrict__ partial) {
+  x += (size_t)blockIdx.y * slot_stride;
+  const long long chunk = (n + gridDim.x - 1) / gridDim.x;
+  const long long lo = (long long)blockIdx.x * chunk;
+  long long hi = lo + chunk;
+  if (hi > n) hi = n;
+  double v = 0.0;
+  if (mode == 1) {
+    for (long long i = lo + threadIdx.x; i < hi; i += blockDim.x) { const double t = x[i]; v += t * t; }
+  } else {
+    const double* c0 = x + (size_t)elem * op.KP * op.Q;
+    for (long long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+      double q[3] = {0.0, 0.0, 0.0};
+      int r = (int)i;
+#pragma unroll
+      for (int s = M - 1; s > 0; s--) { const int t = r / op.nq[s]; q[s] = op.q0[s] + op.h[s] * (double)(r - t * op.nq[s]); r = t; }
+      q[0] = op.q0[0] + op.h[0] * (double)r;
+      double O = o.c0;
+#pragma unroll
+      for (int s = 0; s < M; s++) {
+        O += o.lin_q[s] * q[s];
+#pragma unroll
+        for (int t = 0; t < M; t++) O += 0.5 * o.quad[s][t] * q[s] * q[t];
+      }
+      double term = O * c0[i];
+#pragma unroll
+      for (int s = 0; s < M; s++)
+        if (o.lin_p[s] != 0.0 && op.kp[s] > 1) term += o.lin_p[s] * op.pfac[s] * c0[(size_t)op.kst[s] * op.Q + i];
+      v += op.wq[i] * term;
+    }
+  }
+  const double t = block_sum(v);
+  if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = t;
+}
+
+// fixed-order second pass: one warp per slot
+__global__ void k_hermite_reduce_final(const double* __restrict__ partial, const int nblocks, const double scale,
+                                       double* __restrict__ results, const long long res_stride) {
+  const double* p = partial + (size_t)blockIdx.x * nblocks;
+  double v = 0.0;
+  for (int i = threadIdx.x; i < nblocks; i += 32) v += p[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if (threadIdx.x == 0) results[(long long)blockIdx.x * res_stride] = scale * v;
+}
+
+// equilibrium (section IV.B :221-223; R18): c^(0)_0 = e^{-beta U/2} / Z_q, every other coefficient zero
+__global__ void __launch_bounds__(256) k_hermite_init_eq(const HOp op, double* __restrict__ x, const size_t slot_stride) {
+  const int slab = blockIdx.x / op.blocks_per_slab;
+  const int qi = (blockIdx.x - slab * op.blocks_per_slab) * blockDim.x + threadIdx.x;
+  if (qi >= op.Q) return;
+  x[(size_t)blockIdx.y * slot_stride + (size_t)slab * op.Q + qi] = (slab == 0) ? op.ceq[qi] : 0.0;
+}
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int count_elements(int M, int depth, std::vector<int>* out) {   // R5, R6: graded, ties by descending lexicographic n
+  int K = 0;
+  for (int lev = 0; lev <= depth; lev++)
+    for (int a = lev; a >= 0; a--) {
+      if (M == 1) { if (a != lev) continue; if (out) { out->push_back(a); out->push_back(0); out->push_back(0); } K++; continue; }
+      for (int b = lev - a; b >= 0; b--) {
+        if (M == 2) { if (b != lev - a) continue; if (out) { out->push_back(a); out->push_back(b); out->push_back(0); } K++; continue; }
+        if (out) { out->push_back(a); out->push_back(b); out->push_back(lev - a - b); }
+        K++;
+      }
+    }
+  return K;
+}
+
+int validate(const chfpe_desc* d, std::string* why) {
+  if (!d) { *why = "null descriptor"; return CHFPE_ERR_INVALID; }
+  if (d->n_modes < 1 || d->n_modes > 3) { *why = "n_modes must be 1..3"; return CHFPE_ERR_INVALID; }
+  if (d->depth < 0 || d->depth > 64) { *why = "depth out of range"; return CHFPE_ERR_INVALID; }
+  if (!(d->beta > 0)) { *why = "beta must be > 0"; return CHFPE_ERR_INVALID; }
+  if (d->scheme != CHFPE_CENTRAL4 && d->scheme != CHFPE_CENTRAL2) { *why = "Hermite path: scheme must be CENTRAL4 or CENTRAL2"; return CHFPE_ERR_INVALID; }
+  if (d->batch < 1 || d->batch > 4096) { *why = "batch must be 1..4096"; return CHFPE_ERR_INVALID; }
+  if (d->n_terms < 0 || (d->n_terms > 0 && !d->U)) { *why = "bad potential term list"; return CHFPE_ERR_INVALID; }
+  for (int t = 0; t < d->n_terms; t++) {
+    int deg = 0;
+    for (int s = 0; s < 3; s++) {
+      if (d->U[t].expo[s] < 0) { *why = "negative exponent"; return CHFPE_ERR_INVALID; }
+      if (s < d->n_modes) deg += d->U[t].expo[s];
+    }
+    if (deg > 4) { *why = "potential degree > 4"; return CHFPE_ERR_INVALID; }
+  }
+  double Q = 1.0, KP = 1.0;
+  for (int s = 0; s < d->n_modes; s++) {
+    if (d->nq[s] < 5) { *why = "need >= 5 grid points per q axis"; return CHFPE_ERR_INVALID; }
+    if (d->np[s] < 1 || d->np[s] > 4096) { *why = "need 1..4096 Hermite functions per mode"; return CHFPE_ERR_INVALID; }
+    if (!(d->mass[s] > 0) || !(d->gamma[s] > 0) || d->zeta[s] < 0) { *why = "mass, gamma must be > 0 and zeta >= 0"; return CHFPE_ERR_INVALID; }
+    if (!(d->qmax[s] > d->qmin[s])) { *why = "empty coordinate range"; return CHFPE_ERR_INVALID; }
+    Q *= d->nq[s];
+    KP *= d->np[s];
+  }
+  if (Q >= 1073741824.0) { *why = "q grid of 2^30 points or more"; return CHFPE_ERR_INVALID; }
+  if ((double)count_elements(d->n_modes, d->depth, nullptr) * KP >= 1073741824.0) { *why = "2^30 slabs or more"; return CHFPE_ERR_INVALID; }
+  return CHFPE_OK;
+}
+
+struct Carve { size_t dU, wq, ceq, slabs, arrays, partial, results, total; };
+
+Carve carve(const chfpe_desc* d) {
+  const int M = d->n_modes;
+  size_t Q = 1, KP = 1;
+  for (int s = 0; s < M; s++) { Q *= d->nq[s]; KP *= d->np[s]; }
+  const size_t K = count_elements(M, d->depth, nullptr);
+  Carve c;
+  size_t off = 0;
+  c.dU = off; off += align256(sizeof(double) * Q * 3);
+  c.wq = off; off += align256(sizeof(double) * Q);
+  c.ceq = off; off += align256(sizeof(double) * Q);
+  c.slabs = off; off += align256(sizeof(HSlab) * K * KP);
+  c.arrays = off; off += align256(sizeof(double) * K * KP * Q * 3 * (size_t)d->batch);
+  c.partial = off; off += align256(sizeof(double) * RED_BLOCKS * (size_t)d->batch);
+  c.results = off; off += align256(sizeof(double) * RESULTS);
+  c.total = off;
+  return c;
+}
+
+double ipow(double x, int e) { double r = 1.0; for (int i = 0; i < e; i++) r *= x; return r; }
+
+}  // namespace
+
+struct chfpe_hermite_handle {
+  chfpe_desc desc;
+  HOp op;
+  cudaStream_t stream;
+  int K, batch;
+  size_t state_doubles;               // K * KP * Q
+  double* arrays;                     // slot b: y = arrays[3b], stage buffers arrays[3b+1], arrays[3b+2]
+  double* partial;
+  double* results;
+  std::vector<int> elem;              // [K][3]
+  bool initialised;
+  int64_t launches;
+  std::string err;
+  double* y(int b) const { return arrays + (size_t)(3 * b) * state_doubles; }
+  double* va(int b) const { return arrays + (size_t)(3 * b + 1) * state_doubles; }
+  double* vb(int b) const { return arrays + (size_t)(3 * b + 2) * state_doubles; }
+};
+
+#define HFAIL(h, code, msg) do { (h)->err = (msg); return (code); } while (0)
+#define HCU(h, call)                                                                                  \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess) { (h)->err = std::string(#call) + ": " + cudaGetErrorString(e_); return CHFPE_ERR_CUDA; } \
+  } while (0)
+
+namespace {
+
+int check_launch(chfpe_hermite_handle* h) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { h->err = std::string("kernel launch: ") + cudaGetErrorString(e); return CHFPE_ERR_CUDA; }
+  return CHFPE_OK;
+}
+
+HObs to_dev(const chfpe_observable* o) {
+  HObs d;
+  memset(&d, 0, sizeof(d));
+  if (o) memcpy(&d, o, sizeof(d));
+  return d;
+}
+
+dim3 slab_grid(const HOp& op, int nb) { return dim3((unsigned)((size_t)op.nslab * op.blocks_per_slab), (unsigned)nb); }
+
+void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* out, double a, double c, int nb) {
+  const HOp& op = h->op;
+  const size_t ss = 3 * h->state_doubles;
+  const dim3 g = slab_grid(op, nb);
+  switch (op.M) {
+    case 1: k_hermite_stage<1><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+    case 2: k_hermite_stage<2><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+    default: k_hermite_stage<3><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+  }
+  h->launches++;
+}
+
+// n RK4 steps in the Horner form of the degree-4 Taylor polynomial (R13; the generator is linear and autonomous)
+int step_slots(chfpe_hermite_handle* h, int b0, int nb, int64_t n_steps, double dt) {
+  if (nb <= 0 || n_steps <= 0) return CHFPE_OK;
+  double *y = h->y(b0), *va = h->va(b0), *vb = h->vb(b0);
+  for (int64_t i = 0; i < n_steps; i++) {
+    stage(h, y, y, va, 1.0, dt / 4.0, nb);
+    stage(h, va, y, vb, 1.0, dt / 3.0, nb);
+    stage(h, vb, y, va, 1.0, dt / 2.0, nb);
+    stage(h, va, y, y, 1.0, dt, nb);
+  }
+  return check_launch(h);
+}
+
+int kick_slots(chfpe_hermite_handle* h, int b0, int nb, const chfpe_observable* X) {
+  const HOp& op = h->op;
+  const size_t ss = 3 * h->state_doubles;
+  const HObs o = to_dev(X);
+  const dim3 g = slab_grid(op, nb);
+  switch (op.M) {
+    case 1: k_hermite_kick<1><<<g, op.threads, 0, h->stream>>>(op, o, h->y(b0), h->va(b0), ss); break;
+    case 2: k_hermite_kick<2><<<g, op.threads, 0, h->stream>>>(op, o, h->y(b0), h->va(b0), ss); break;
+    default: k_hermite_kick<3><<<g, op.threads, 0, h->stream>>>(op, o, h->y(b0), h->va(b0), ss); break;
+  }
+  h->launches++;
+  for (int b = b0; b < b0 + nb; b++)
+    HCU(h, cudaMemcpyAsync(h->y(b), h->va(b), sizeof(double) * h->state_doubles, cudaMemcpyDeviceToDevice, h->stream));
+  return check_launch(h);
+}
+
+int reduce(chfpe_hermite_handle* h, const HObs& o, int mode, const double* x, int elem, long long n, int nb,
+           size_t slot_stride, double scale, double* res, long long res_stride) {
+  const HOp& op = h->op;
+  const dim3 g(RED_BLOCKS, (unsigned)nb);
+  switch (op.M) {
+    case 1: k_hermite_reduce_partial<1><<<g, 256, 0, h->stream>>>(op, o, mode, x, elem, n, slot_stride, h->partial); break;
+    case 2: k_hermite_reduce_partial<2><<<g, 256, 0, h->stream>>>(op, o, mode, x, elem, n, slot_stride, h->partial); break;
+    default: k_hermite_reduce_partial<3><<<g, 256, 0, h->stream>>>(op, o, mode, x, elem, n, slot_stride, h->partial); break;
+  }
+  k_hermite_reduce_final<<<nb, 32, 0, h->stream>>>(h->partial, RED_BLOCKS, scale, res, res_stride);
+  h->launches += 2;
+  return check_launch(h);
+}
+
+int expect_slots(chfpe_hermite_handle* h, int b0, int nb, int elem, const chfpe_observable* O, long long res_off,
+                 long long res_stride) {
+  return reduce(h, to_dev(O), 0, h->y(b0), elem, h->op.Q, nb, 3 * h->state_doubles, h->op.dV, h->results + res_off,
+                res_stride);
+}
+
+int fetch_results(chfpe_hermite_handle* h, long long n, double* host) {
+  HCU(h, cudaMemcpyAsync(host, h->results, sizeof(double) * n, cudaMemcpyDeviceToHost, h->stream));
+  HCU(h, cudaStreamSynchronize(h->stream));
+  for (long long i = 0; i < n; i++)
+    if (!std::isfinite(host[i])) HFAIL(h, CHFPE_ERR_DIVERGED, "non-finite expectation value");
+  return CHFPE_OK;
+}
+
+int check_steps(chfpe_hermite_handle* h, const int64_t* t, int n, const char* name) {
+  for (int i = 0; i < n; i++)
+    if (t[i] < 0 || (i && t[i] < t[i - 1])) HFAIL(h, CHFPE_ERR_INVALID, std::string(name) + " must be ascending and >= 0");
+  return CHFPE_OK;
+}
+
+}  // namespace
+
+extern "C" int chfpe_hermite_workspace_bytes(const chfpe_desc* desc, size_t* bytes) {
+  std::string why;
+  int rc = validate(desc, &why);
+  if (rc) { g_err = why; return rc; }
+  if (!bytes) return CHFPE_ERR_INVALID;
+  *bytes = carve(desc).total;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t bytes, void* cuda_stream,
+                                    chfpe_hermite_handle** out) {
+  if (out) *out = nullptr;
+  std::string why;
+  int rc = validate(desc, &why);
+  if (rc) { g_err = why; return rc; }
+  if (!out) return CHFPE_ERR_INVALID;
+  const Carve cv = carve(desc);
+  if (!ws || bytes < cv.total || ((uintptr_t)ws & 255)) { g_err = "workspace too small or not 256-byte aligned"; return CHFPE_ERR_WORKSPACE; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); g_err = "no CUDA device (there is no CPU fallback)"; return CHFPE_ERR_CUDA; }
+
+  chfpe_hermite_handle* h = new chfpe_hermite_handle();
+  h->desc = *desc;
+  h->desc.U = nullptr;
+  h->stream = (cudaStream_t)cuda_stream;
+  h->batch = desc->batch;
+  h->initialised = false;
+  h->launches = 0;
+  const int M = desc->n_modes;
+  h->K = count_elements(M, desc->depth, &h->elem);
+  HOp& op = h->op;
+  memset(&op, 0, sizeof(op));
+  op.M = M; op.K = h->K; op.scheme = desc->scheme;
+  size_t Q = 1, KP = 1;
+  for (int s = 0; s < 3; s++) { op.nq[s] = 1; op.kp[s] = 1; }
+  for (int s = 0; s < M; s++) { op.nq[s] = desc->nq[s]; op.kp[s] = desc->np[s]; Q *= desc->nq[s]; KP *= desc->np[s]; }
+  for (int s = M - 1, st = 1, kt = 1; s >= 0; s--) { op.qst[s] = st; st *= op.nq[s]; op.kst[s] = kt; kt *= op.kp[s]; }
+  op.Q = (int)Q; op.KP = (int)KP; op.nslab = (int)(h->K * KP);
+  op.threads = (Q >= 256) ? 256 : (int)((Q + 31) / 32 * 32);
+  op.blocks_per_slab = (int)((Q + op.threads - 1) / op.threads);
+  op.dV = 1.0;
+  for (int s = 0; s < M; s++) {
+    const double m = desc->mass[s], beta = desc->beta;
+    op.q0[s] = desc->qmin[s];
+    op.h[s] = (desc->qmax[s] - desc->qmin[s]) / (desc->nq[s] - 1);
+    if (desc->scheme == CHFPE_CENTRAL2) { op.c1[s] = 1.0 / (2.0 * op.h[s]); op.c2[s] = 0.0; }
+    else { op.c1[s] = 8.0 / (12.0 * op.h[s]); op.c2[s] = -1.0 / (12.0 * op.h[s]); }
+    op.a1f[s] = 1.0 / (2.0 * sqrt(m / beta));
+    op.a2[s] = 1.0 / sqrt(m * beta);
+    op.VLL[s] = desc->V_LL[s]; op.VSL[s] = desc->V_SL[s];
+    op.kickf[s] = -sqrt(beta / m);
+    op.pfac[s] = sqrt(m / beta);
+    op.dV *= op.h[s];
+  }
+  h->state_doubles = (size_t)h->K * KP * Q;
+
+  // ---- tables (setup step a0): dU/dq_s, exp(-beta U/2) and the equilibrium coefficient on the q grid ----
+  std::vector<double> dU(3 * Q, 0.0), wq(Q), ceq(Q);
+  double Z = 0.0;
+  for (size_t i = 0; i < Q; i++) {
+    double q[3] = {0, 0, 0};
+    size_t r = i;
+    for (int s = M - 1; s >= 0; s--) { q[s] = op.q0[s] + op.h[s] * (double)(r % op.nq[s]); r /= op.nq[s]; }
+    double U = 0.0;
+    for (int t = 0; t < desc->n_terms; t++) {
+      const chfpe_monomial& mo = desc->U[t];
+      double v = mo.coef;
+      for (int s = 0; s < M; s++) v *= ipow(q[s], mo.expo[s]);
+      U += v;
+      for (int s = 0; s < M; s++) {
+        if (mo.expo[s] == 0) continue;
+        double g = mo.coef * mo.expo[s];
+        for (int s2 = 0; s2 < M; s2++) g *= ipow(q[s2], mo.expo[s2] - (s2 == s ? 1 : 0));
+        dU[(size_t)s * Q + i] += g;
+      }
+    }
+    wq[i] = exp(-0.5 * desc->beta * U);
+    Z += exp(-desc->beta * U);
+  }
+  Z *= op.dV;
+  for (size_t i = 0; i < Q; i++) ceq[i] = wq[i] / Z;
+
+  // ---- slab neighbourhoods ----
+  std::vector<HSlab> slabs((size_t)op.nslab);
+  auto find_elem = [&](const int n[3]) -> int {
+    for (int k = 0; k < h->K; k++)
+      if (h->elem[3 * k] == n[0] && h->elem[3 * k + 1] == n[1] && h->elem[3 * k + 2] == n[2]) return k;
+    return -1;
+  };
+  for (int e = 0; e < h->K; e++) {
+    const int* n = &h->elem[3 * e];
+    int eup[3], edn[3];
+    double gam = 0.0;
+    for (int s = 0; s < 3; s++) {
+      eup[s] = edn[s] = -1;
+      if (s >= M) continue;
+      int t[3] = {n[0], n[1], n[2]};
+      t[s]++; eup[s] = find_elem(t);
+      t[s] -= 2; if (t[s] >= 0) edn[s] = find_elem(t);
+      gam += n[s] * desc->gamma[s];
+    }
+    for (size_t ki = 0; ki < KP; ki++) {
+      HSlab& S = slabs[(size_t)e * KP + ki];
+      memset(&S, 0, sizeof(S));
+      S.gam = gam;
+      for (int s = 0; s < 3; s++) {
+        S.up[s] = S.dn[s] = S.hdn[s] = S.hup[s] = -1;
+        if (s >= M) continue;
+        const int ks = (int)((ki / op.kst[s]) % op.kp[s]);
+        const double m = desc->mass[s], beta = desc->beta;
+        S.su[s] = sqrt((double)ks + 1.0);
+        S.sd[s] = sqrt((double)ks);
+        const bool has_up = ks + 1 < op.kp[s], has_dn = ks >= 1;
+        if (has_up) S.up[s] = (int)((size_t)e * KP + ki + op.kst[s]);
+        if (has_dn) S.dn[s] = (int)((size_t)e * KP + ki - op.kst[s]);
+        if (edn[s] >= 0 && has_up) {
+          S.hdn[s] = (int)((size_t)edn[s] * KP + ki + op.kst[s]);
+          S.hd[s] = n[s] * desc->gamma[s] * desc->zeta[s] * sqrt(m / beta) * S.su[s];
+        }
+        if (eup[s] >= 0 && has_dn) {
+          S.hup[s] = (int)((size_t)eup[s] * KP + ki - op.kst[s]);
+          S.hu[s] = -sqrt(beta / m) * S.sd[s];
+        }
+      }
+    }
+  }
+
+  char* base = (char*)ws;
+  double* d_dU = (double*)(base + cv.dU);
+  for (int s = 0; s < 3; s++) op.dU[s] = d_dU + (size_t)s * Q;
+  op.wq = (double*)(base + cv.wq);
+  op.ceq = (double*)(base + cv.ceq);
+  op.slabs = (HSlab*)(base + cv.slabs);
+  h->arrays = (double*)(base + cv.arrays);
+  h->partial = (double*)(base + cv.partial);
+  h->results = (double*)(base + cv.results);
+  cudaError_t e = cudaMemcpyAsync(d_dU, dU.data(), sizeof(double) * 3 * Q, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.wq, wq.data(), sizeof(double) * Q, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.ceq, ceq.data(), sizeof(double) * Q, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.slabs, slabs.data(), sizeof(HSlab) * slabs.size(), cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(h->arrays, 0, sizeof(double) * h->state_doubles * 3 * (size_t)h->batch, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);      // the host vectors go out of scope
+  if (e != cudaSuccess) { g_err = std::string("create: ") + cudaGetErrorString(e); delete h; return CHFPE_ERR_CUDA; }
+  *out = h;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_destroy(chfpe_hermite_handle* h) {
+  if (!h) return CHFPE_ERR_INVALID;
+  delete h;
+  return CHFPE_OK;
+}
+
+extern "C" const char* chfpe_hermite_last_error(const chfpe_hermite_handle* h) { return h ? h->err.c_str() : g_err.c_str(); }
+
+extern "C" int chfpe_hermite_num_elements(const chfpe_hermite_handle* h, int32_t* K) {
+  if (!h || !K) return CHFPE_ERR_INVALID;
+  *K = h->K;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_launch_count(const chfpe_hermite_handle* h, int64_t* n) {
+  if (!h || !n) return CHFPE_ERR_INVALID;
+  *n = h->launches;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_equilibrate(chfpe_hermite_handle* h, int64_t n_steps, double dt, double* residual_out) {
+  if (!h || n_steps < 0) return CHFPE_ERR_INVALID;
+  k_hermite_init_eq<<<slab_grid(h->op, h->batch), h->op.threads, 0, h->stream>>>(h->op, h->y(0), 3 * h->state_doubles);
+  h->launches++;
+  int rc = check_launch(h);
+  if (rc) return rc;
+  h->initialised = true;
+  rc = step_slots(h, 0, h->batch, n_steps, dt);
+  if (rc) return rc;
+  if (residual_out) {
+    const HObs none = to_dev(nullptr);
+    stage(h, h->y(0), h->y(0), h->va(0), 0.0, 1.0, 1);
+    rc = reduce(h, none, 1, h->va(0), 0, (long long)h->state_doubles, 1, 0, 1.0, h->results, 1);
+    if (rc) return rc;
+    rc = reduce(h, none, 1, h->y(0), 0, (long long)h->state_doubles, 1, 0, 1.0, h->results + 1, 1);
+    if (rc) return rc;
+    double r[2];
+    rc = fetch_results(h, 2, r);
+    if (rc) return rc;
+    *residual_out = sqrt(r[0] / r[1]);
+  }
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_step(chfpe_hermite_handle* h, int64_t n_steps, double dt) {
+  if (!h || n_steps < 0) return CHFPE_ERR_INVALID;
+  return step_slots(h, 0, h->batch, n_steps, dt);
+}
+
+extern "C" int chfpe_hermite_kick(chfpe_hermite_handle* h, const chfpe_observable* X) {
+  if (!h || !X) return CHFPE_ERR_INVALID;
+  return kick_slots(h, 0, h->batch, X);
+}
+
+extern "C" int chfpe_hermite_expect(chfpe_hermite_handle* h, int32_t element, const chfpe_observable* O, double* out) {
+  if (!h || !O || !out || element < 0 || element >= h->K) return CHFPE_ERR_INVALID;
+  int rc = expect_slots(h, 0, h->batch, element, O, 0, 1);
+  if (rc) return rc;
+  return fetch_results(h, h->batch, out);
+}
+
+extern "C" int chfpe_hermite_response_1d(chfpe_hermite_handle* h, const chfpe_observable* A, const chfpe_observable* C,
+                                         int64_t n_samples, int64_t stride, double dt, double* R) {
+  if (!h || !C || !R || n_samples < 0 || stride < 0) return CHFPE_ERR_INVALID;
+  if (!h->initialised) HFAIL(h, CHFPE_ERR_STATE, "response_1d before equilibrate/import");
+  int rc = A ? kick_slots(h, 0, 1, A) : CHFPE_OK;
+  if (rc) return rc;
+  int64_t done = 0;
+  while (done < n_samples) {
+    int64_t chunk = n_samples - done;
+    if (chunk > RESULTS) chunk = RESULTS;
+    for (int64_t i = 0; i < chunk; i++) {
+      rc = expect_slots(h, 0, 1, 0, C, i, 1);
+      if (rc) return rc;
+      if (done + i + 1 < n_samples) { rc = step_slots(h, 0, 1, stride, dt); if (rc) return rc; }
+    }
+    rc = fetch_results(h, chunk, R + done);
+    if (rc) return rc;
+    done += chunk;
+  }
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_response_2d(chfpe_hermite_handle* h, const chfpe_observable* A, const chfpe_observable* B,
+                                         const chfpe_observable* C, const int64_t* t1, int32_t n1, const int64_t* t2,
+                                         int32_t n2, double dt, double* R) {
+  if (!h || !A || !B || !C || !t1 || !t2 || !R || n1 < 1 || n2 < 1) return CHFPE_ERR_INVALID;
+  if (!h->initialised) HFAIL(h, CHFPE_ERR_STATE, "response_2d before equilibrate/import");
+  if (h->batch < 2) HFAIL(h, CHFPE_ERR_INVALID, "response_2d needs batch >= 2 (slot 0 carries the t1 trajectory)");
+  int rc = check_steps(h, t1, n1, "t1_steps");
+  if (rc) return rc;
+  rc = check_steps(h, t2, n2, "t2_steps");
+  if (rc) return rc;
+  const long long rows_per_fetch = RESULTS / n2;
+  if (rows_per_fetch < 1) HFAIL(h, CHFPE_ERR_INVALID, "n2 too large for the results buffer");
+  const size_t sbytes = sizeof(double) * h->state_doubles;
+  rc = kick_slots(h, 0, 1, A);
+  if (rc) return rc;
+  int64_t now1 = 0;
+  const int per_round = h->batch - 1;
+  int k = 0, row0 = 0;                               // rows [row0, k) are in the device results buffer
+  while (k < n1) {
+    int nb = n1 - k;
+    if (nb > per_round) nb = per_round;
+    if (k + nb - row0 > rows_per_fetch) {
+      rc = fetch_results(h, (long long)(k - row0) * n2, R + (size_t)row0 * n2);
+      if (rc) return rc;
+      row0 = k;
+    }
+    for (int b = 0; b < nb; b++) {                   // the t1 trajectory drops a copy into a replica slot per sample
+      rc = step_slots(h, 0, 1, t1[k + b] - now1, dt);
+      if (rc) return rc;
+      now1 = t1[k + b];
+      HCU(h, cudaMemcpyAsync(h->y(1 + b), h->y(0), sbytes, cudaMemcpyDeviceToDevice, h->stream));
+    }
+    rc = kick_slots(h, 1, nb, B);
+    if (rc) return rc;
+    int64_t now2 = 0;
+    for (int j = 0; j < n2; j++) {                   // all replicas of the round advance together (grid.y)
+      rc = step_slots(h, 1, nb, t2[j] - now2, dt);
+      if (rc) return rc;
+      now2 = t2[j];
+      rc = expect_slots(h, 1, nb, 0, C, (long long)(k - row0) * n2 + j, n2);
+      if (rc) return rc;
+    }
+    k += nb;
+  }
+  return fetch_results(h, (long long)(k - row0) * n2, R + (size_t)row0 * n2);
+}
+
+extern "C" int chfpe_hermite_export_state(chfpe_hermite_handle* h, int32_t replica, double* dst, int dst_is_device) {
+  if (!h || !dst || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
+  HCU(h, cudaMemcpyAsync(dst, h->y(replica), sizeof(double) * h->state_doubles,
+                         dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  HCU(h, cudaStreamSynchronize(h->stream));
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_import_state(chfpe_hermite_handle* h, int32_t replica, const double* src, int src_is_device) {
+  if (!h || !src || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
+  HCU(h, cudaMemcpyAsync(h->y(replica), src, sizeof(double) * h->state_doubles,
+                         src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+  HCU(h, cudaStreamSynchronize(h->stream));
+  h->initialised = true;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_export_rhs(chfpe_hermite_handle* h, int32_t replica, double* dst, int dst_is_device) {
+  if (!h || !dst || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
+  stage(h, h->y(replica), h->y(replica), h->va(replica), 0.0, 1.0, 1);
+  int rc = check_launch(h);
+  if (rc) return rc;
+  HCU(h, cudaMemcpyAsync(dst, h->va(replica), sizeof(double) * h->state_doubles,
+                         dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, h->stream));
+  HCU(h, cudaStreamSynchronize(h->stream));
+  return CHFPE_OK;
+}

@@ -1,0 +1,213 @@
+"""Row f1: parity of the CUDA Hermite-representation path (chfpe_hermite_* through the C-ABI binding) with the numpy
+oracle oracle/hermite.py on the same seeded inputs.  Tolerances as for the grid path (BASELINE.json north_star):
+one right-hand side / kick 1e-13 relative L2, per-step 1e-12, response functions 1e-8 relative max."""
+import os
+
+import numpy as np
+import pytest
+
+import chfpe_inputs as ci
+from oracle import hermite
+from conftest import make_obs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def P():
+    import paper_2509_25840_b200 as mod
+    return mod
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+def both(cfg, batch=1):
+    return P().Hermite(cfg, batch=batch), hermite.RefHermite(cfg)
+
+
+def gobs(d):
+    return make_obs(P(), d)
+
+
+def p_obs(M):
+    """an observable with every coefficient non-zero, incl. the linear-momentum part"""
+    return dict(c0=0.3, lin_q=[1.0, -0.7, 0.4][:M], quad=[[0.5, 0.2, -0.1][:M], [0.3, -0.4, 0.25][:M], [0.15, 0.1, 0.6][:M]][:M],
+                lin_p=[0.8, -0.5, 0.3][:M])
+
+
+SMALL = [
+    ("m1", ci.config("cfg2", nq=[37], np=[9], depth=5)),
+    ("m1_c2_mass", ci.config("cfg2", nq=[300], np=[4], depth=3, scheme="central2", mass=[1.3])),   # 2 CTAs per slab, ragged
+    ("m1_kp1", ci.config("cfg2", nq=[21], np=[1], depth=2)),                                      # no Hermite neighbours at all
+    ("m1_depth0", ci.config("cfg2", nq=[21], np=[5], depth=0)),                                   # a single element
+    ("m2", ci.config("cfg3s", nq=[13, 11], np=[4, 5], depth=3)),
+    ("m2_ragged_ctas", ci.config("cfg3s", nq=[40, 37], np=[3, 2], depth=2, mass=[1.0, 1.3])),      # 1480 q-points: 6 CTAs per slab
+    ("m2_c2", ci.config("cfg3s", nq=[9, 10], np=[2, 6], depth=2, scheme="central2")),
+    ("m3", ci.config("cfg4s8", nq=[7, 8, 6], np=[3, 2, 4], depth=3)),
+    ("m3_ragged", ci.config("cfg4s8", nq=[11, 9, 13], np=[3, 4, 2], depth=2, mass=[1.0, 0.8, 1.2])),
+    ("m3_kp1_mid", ci.config("cfg4s8", nq=[6, 5, 7], np=[3, 1, 2], depth=2, scheme="central2")),
+]
+
+
+@pytest.mark.parametrize("name,cfg", SMALL, ids=[c[0] for c in SMALL])
+def test_rhs_step_kick_expect(name, cfg):
+    g, o = both(cfg)
+    M = cfg["n_modes"]
+    assert g.K == o.K and g.shape == o.shape
+    levels = [sum(n) for n in o.elems]
+    X = ci.seeded_hermite_state(cfg, levels, seed=11)
+    g.import_state(X); o.import_state(X)
+    assert np.array_equal(g.export_state(), X)
+    assert rel_l2(g.export_rhs(), o.rhs(o.c)) < 1e-13
+    # expectations: polynomial in q plus <p_s> (from the k = e_s coefficients), on element 0 and on the last element
+    d = p_obs(M)
+    for el in (0, o.K - 1):
+        ref = o.expect(d, element=el)
+        got = g.expect(gobs(d), element=el)[0]
+        assert abs(got - ref) <= 1e-13 * max(abs(ref), 1e-3), (el, got, ref)
+    # RK4: the Horner form of the CUDA path against the textbook k1..k4 form of the oracle
+    g.step(3, cfg["dt"]); o.step(3, cfg["dt"])
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+    # kick with a bilinear observable (every dX/dq_s depends on every q)
+    g.kick(gobs(d)); o.kick(d)
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-13
+
+
+def test_zero_steps_and_batch_slots_are_independent():
+    cfg = ci.config("cfg3s", nq=[12, 9], np=[3, 4], depth=2)
+    g = P().Hermite(cfg, batch=3)
+    o = hermite.RefHermite(cfg)
+    levels = [sum(n) for n in o.elems]
+    Xs = [ci.seeded_hermite_state(cfg, levels, seed=s) for s in (1, 2, 3)]
+    for b, X in enumerate(Xs):
+        g.import_state(X, replica=b)
+    g.step(0, cfg["dt"])
+    for b, X in enumerate(Xs):
+        assert np.array_equal(g.export_state(b), X)
+    g.step(2, cfg["dt"])                             # one launch per stage advances all three slots
+    d = p_obs(2)
+    got = g.expect(gobs(d))
+    for b, X in enumerate(Xs):
+        o.import_state(X); o.step(2, cfg["dt"])
+        assert rel_l2(g.export_state(b), o.export_state()) < 1e-12
+        assert abs(got[b] - o.expect(d)) <= 1e-13 * abs(o.expect(d))
+
+
+def test_equilibrium_state_and_residual():
+    for cfg in (ci.config("cfg2", nq=[64], np=[6], depth=3), ci.config("cfg4s8", nq=[9, 8, 7], np=[2, 3, 2], depth=2)):
+        g, o = both(cfg, batch=2)
+        rg, ro = g.equilibrate(), o.equilibrate()
+        assert rel_l2(g.export_state(0), o.export_state()) < 1e-14
+        assert np.array_equal(g.export_state(1), g.export_state(0))
+        assert abs(rg - ro) <= 1e-10 * ro
+        one = ci.observable("one", cfg["n_modes"])
+        assert abs(g.expect(gobs(one))[0] - 1.0) < 1e-12
+        g.close()
+
+
+def test_response_1d_anharmonic_sl():
+    """config-2 model (anharmonic, LL + SL), nonlinear dipole: 400 steps sampled every 20."""
+    cfg = ci.config("cfg2", nq=[64], np=[12], depth=6)
+    g, o = both(cfg)
+    g.equilibrate(); o.equilibrate()
+    al, d = ci.observable("alpha", 1), ci.observable("mu_nl", 1)
+    Rg = g.response_1d(gobs(al), gobs(d), 21, 20, 1e-3)
+    Ro = o.response_1d(al, d, 21, 20, 1e-3)
+    assert np.max(np.abs(Ro)) > 0.1
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+
+
+def test_response_1d_ten_thousand_steps():
+    """north_star: response functions within 1e-8 relative max after 10^4 steps (harmonic config-1 model, small mesh)."""
+    cfg = ci.config("cfg1", nq=[33], np=[4], depth=3, qmin=[-8.0], qmax=[8.0])
+    g, o = both(cfg)
+    g.equilibrate(); o.equilibrate()
+    mu = ci.observable("mu", 1)
+    Rg = g.response_1d(gobs(mu), gobs(mu), 11, 1000, 1e-3)
+    Ro = o.response_1d(mu, mu, 11, 1000, 1e-3)
+    assert np.max(np.abs(Ro)) > 0.3
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+
+
+def test_response_1d_three_modes():
+    cfg = ci.config("cfg4s8", nq=[10, 9, 8], np=[3, 3, 3], depth=2)
+    g, o = both(cfg)
+    g.equilibrate(); o.equilibrate()
+    mu, al = ci.observable("mu", 3), ci.observable("alpha", 3)
+    Rg = g.response_1d(gobs(al), gobs(al), 6, 10, 2e-3)
+    Ro = o.response_1d(al, al, 6, 10, 2e-3)
+    assert np.max(np.abs(Ro)) > 0.05
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    del mu
+
+
+@pytest.mark.parametrize("batch", [2, 3, 5])
+def test_response_2d_batched_over_t1(batch):
+    """Eq. (16): rounds of batch-1 replicas (full, ragged and single rounds), repeated and zero delays."""
+    cfg = ci.config("cfg3s", nq=[12, 11], np=[4, 3], depth=2)
+    g, o = both(cfg, batch=batch)
+    g.equilibrate(); o.equilibrate()
+    mu, al = ci.observable("mu", 2), ci.observable("alpha", 2)
+    t1, t2 = [0, 3, 3, 7, 12], [0, 4, 9]
+    Rg = g.response_2d(gobs(mu), gobs(al), gobs(al), t1, t2, 5e-3)
+    Ro = o.response_2d(mu, al, al, t1, t2, 5e-3)
+    assert np.max(np.abs(Ro)) > 1e-3
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    assert np.array_equal(Rg[1], Rg[2])              # repeated t1 sample
+
+
+def test_closed_forms_on_the_cuda_path():
+    """The pins of the oracle hold for the CUDA path on its own: Brownian-oscillator R1 (tests/golden/bo_response_cfg1.txt,
+    literal Eq. 15 = -R_phys) and the 2D closed form 2 R_phys(t1) R_phys(t2) (tests/golden/r2_closed_form.txt)."""
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "bo_response_cfg1.txt"))
+    cfg = ci.config("cfg1", nq=[73], np=[6], depth=3, qmin=[-9.0], qmax=[9.0])
+    g = P().Hermite(cfg, batch=2)
+    g.equilibrate()
+    mu, al = gobs(ci.observable("mu", 1)), gobs(ci.observable("alpha", 1))
+    steps = [int(round(t / 1e-3)) for t in gold[:, 0]]
+    assert np.allclose(np.array(steps) * 1e-3, gold[:, 0], atol=1e-12)
+    now, worst = 0, 0.0
+    g.kick(mu)
+    one = np.empty(1)
+    for s, ref in zip(steps, gold[:, 1]):
+        g.step(s - now, 1e-3); now = s
+        worst = max(worst, abs(-g.expect(mu)[0] - ref))
+    assert worst < 1e-4, worst
+    g2 = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "r2_closed_form.txt"))
+    g.equilibrate()
+    R = g.response_2d(mu, al, mu, [int(round(g2[0] / 2e-3))], [int(round(g2[1] / 2e-3))], 2e-3)
+    assert abs(R[0, 0] - g2[2]) < 2e-4
+    del one
+
+
+def test_full_size_rhs_on_an_embedded_block():
+    """The bench workload (cfg4h: 32^3 q mesh, 8^3 Hermite functions, 20 elements = 3.36e8 values, launch configuration
+    of bench.py --representation hermite).  The state is zero outside a 9 x 10 x 11 block of the q mesh; zero ghosts
+    (R9) make the right-hand side inside the block equal to that of the oracle on the block alone (same mesh width,
+    shifted origin), for every element and every Hermite index."""
+    cfg = ci.config("cfg4h")
+    if torch.cuda.mem_get_info()[0] < 12e9:
+        pytest.skip("needs 12 GB of device memory")
+    off, ext = (5, 14, 19), (9, 10, 11)
+    h = [(cfg["qmax"][s] - cfg["qmin"][s]) / (cfg["nq"][s] - 1) for s in range(3)]
+    sub = ci.config("cfg4h", nq=list(ext), qmin=[cfg["qmin"][s] + h[s] * off[s] for s in range(3)],
+                    qmax=[cfg["qmin"][s] + h[s] * (off[s] + ext[s] - 1) for s in range(3)])
+    o = hermite.RefHermite(sub)
+    assert max(abs(o.h[s] - h[s]) for s in range(3)) < 1e-14
+    Xs = ci.seeded_hermite_state(sub, [sum(n) for n in o.elems], seed=5)
+    g = P().Hermite(cfg)
+    X = torch.zeros(g.shape, dtype=torch.float64, device="cuda")
+    blk = (slice(None),) * 4 + tuple(slice(off[s], off[s] + ext[s]) for s in range(3))
+    X[blk] = torch.from_numpy(Xs).cuda()
+    g.import_state(X)
+    del X
+    F = g.export_rhs_device()[blk].cpu().numpy()
+    assert rel_l2(F, o.rhs(Xs)) < 1e-13
+    # one RK4 step at full size is four launches of the stage kernel and nothing else
+    n0 = g.launch_count()
+    g.step(1, cfg["dt"])
+    assert g.launch_count() - n0 == 4
+    g.close()
