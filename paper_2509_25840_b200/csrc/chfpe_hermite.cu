@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -24,9 +25,13 @@ struct HSlab {
   int hdn[3], hup[3];      // slab of (n - e_s, k + e_s), (n + e_s, k - e_s), -1 if absent (R5: zero outside the simplex)
   double su[3], sd[3];     // sqrt(k_s + 1), sqrt(k_s)
   double hd[3], hu[3];     // n_s gamma_s zeta_s sqrt(m_s/beta) sqrt(k_s + 1),  -sqrt(k_s beta/m_s)
-  double gam, pad;         // Gamma_n = sum_s n_s gamma_s
+  double gam;              // Gamma_n = sum_s n_s gamma_s
+  // column kernel (last mode, s = M-1): first slab (k_M = 0) of the columns (n - e_M, k_1..k_{M-1}) and (n + e_M, ..),
+  // -1 if the element is absent, and the coupling constants without their sqrt(k) factors
+  int ednM, eupM;
+  double hdM, huM;         // n_M gamma_M zeta_M sqrt(m_M/beta),  -sqrt(beta/m_M)
 };
-static_assert(sizeof(HSlab) == 160, "HSlab layout");
+static_assert(sizeof(HSlab) == 176, "HSlab layout");
 
 struct HOp {                // device view of the operator, passed by value
   int M, K, scheme;
@@ -41,6 +46,10 @@ struct HOp {                // device view of the operator, passed by value
   const double* wq;                   // exp(-beta U / 2)
   const double* ceq;                  // exp(-beta U / 2) / Z_q, Z_q = dV sum exp(-beta U)
   const HSlab* slabs;
+  const double* sq;                   // sq[i] = sqrt(i), i = 0 .. kp_M
+  int kc, nchunk;                     // column kernel: Hermite indices of the last mode per thread, chunks per column
+  int pa, pb, ntileB, pthreads, pblocks;   // patch kernel: patch extents, q_2 tiles, threads and CTAs per slab
+  int fixed;                          // use the compile-time 32^3 specialisation when the mesh matches (CHFPE_HERMITE_FIXED=0: off)
 };
 
 struct HObs { double c0, lin_q[3], quad[3][3], lin_p[3]; };
@@ -107,6 +116,316 @@ __global__ void __launch_bounds__(256) k_hermite_stage(const HOp op, const doubl
   }
   const double base = (a != 0.0) ? a * y[soff + self] : 0.0;
   out[soff + self] = base + c * acc;
+}
+
+// Column form of the same stage (the default): a thread owns, for one q-point, KC consecutive Hermite indices of the
+// LAST mode (whose slabs are adjacent in memory).  The q-point decode, the dU/dq_s and V'_s factors, the ghost
+// handling and the slab neighbourhood are worked out once per thread instead of once per value; the terms of the
+// last mode come from the thread's own column (KC + 2 centre values, each differentiated once); zero ghosts (R9) are
+// weights of 0 on loads redirected to the centre, so no load is predicated.  CTA-uniform: element, k_1..k_{M-1}, chunk.
+template <int M, int KC>
+__global__ void __launch_bounds__(256) k_hermite_stage_col(const HOp op, const double* __restrict__ in, const double* y,
+                                                          double* out, const double a, const double c,
+                                                          const size_t slot_stride) {
+  const int kpM = op.kp[M - 1];
+  const int col_blocks = op.nchunk * op.blocks_per_slab;
+  const int col = blockIdx.x / col_blocks;                 // column = (element, k_1..k_{M-1})
+  const int rem = blockIdx.x - col * col_blocks;
+  const int chunk = rem / op.blocks_per_slab;
+  const int qi = (rem - chunk * op.blocks_per_slab) * blockDim.x + threadIdx.x;
+  if (qi >= op.Q) return;
+  const int k0 = chunk * KC;
+  const int slab0 = col * kpM;                             // slab of k_M = 0 of this column
+  const size_t soff = (size_t)blockIdx.y * slot_stride;
+  in += soff;
+  const HSlab* __restrict__ S = op.slabs + slab0;          // everything read from it is independent of k_M
+  const size_t Q = (size_t)op.Q;
+  int iq[3] = {0, 0, 0};
+  {
+    int r = qi;
+#pragma unroll
+    for (int s = M - 1; s > 0; s--) { const int t = r / op.nq[s]; iq[s] = r - t * op.nq[s]; r = t; }
+    iq[0] = r;
+  }
+  double acc[KC];
+  // ---- last mode: own column, centre values cc[i] and q_M-derivatives dcc[i] of k_M = k0 - 1 + i ----
+  {
+    const int s = M - 1;
+    const int i = iq[s], n = op.nq[s], st = op.qst[s];
+    const long long o1 = (i + 1 < n) ? st : 0, o2 = (i >= 1) ? -st : 0, o3 = (i + 2 < n) ? 2 * st : 0, o4 = (i >= 2) ? -2 * st : 0;
+    const double w1 = (i + 1 < n) ? op.c1[s] : 0.0, w2 = (i >= 1) ? -op.c1[s] : 0.0;
+    const double w3 = (i + 2 < n) ? op.c2[s] : 0.0, w4 = (i >= 2) ? -op.c2[s] : 0.0;
+    double cc[KC + 2], dcc[KC + 2];
+    const double* p = in + (size_t)(slab0 + k0 - 1) * Q + qi;
+#pragma unroll
+    for (int t = 0; t < KC + 2; t++) {
+      const int k = k0 - 1 + t;
+      if (k >= 0 && k < kpM) {
+        cc[t] = __ldg(p);
+        dcc[t] = w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4);
+      } else {
+        cc[t] = 0.0; dcc[t] = 0.0;
+      }
+      p += Q;
+    }
+    const double a1 = op.a1f[s] * __ldg(op.dU[s] + qi), a2 = op.a2[s], gam = S->gam;
+#pragma unroll
+    for (int j = 0; j < KC; j++) {
+      const int k = (k0 + j < kpM) ? k0 + j : 0;           // clamped: entries beyond the column are never stored
+      const double su = __ldg(op.sq + k + 1), sd = __ldg(op.sq + k);
+      acc[j] = a1 * (su * cc[j + 2] - sd * cc[j]) - a2 * (su * dcc[j + 2] + sd * dcc[j]) - gam * cc[j + 1];
+    }
+    // Theta / Phi of the last mode: columns of the elements n -+ e_M, shifted by one Hermite index
+    const int ednM = S->ednM, eupM = S->eupM;
+    if (ednM >= 0 || eupM >= 0) {
+      const double vp = op.VLL[s] + op.VSL[s] * (op.q0[s] + op.h[s] * (double)i);
+      const double hd = vp * S->hdM, hu = vp * S->huM;
+#pragma unroll
+      for (int j = 0; j < KC; j++) {
+        const int k = k0 + j;
+        if (ednM >= 0 && k + 1 < kpM) acc[j] += hd * __ldg(op.sq + k + 1) * __ldg(in + (size_t)(ednM + k + 1) * Q + qi);
+        if (eupM >= 0 && k >= 1 && k < kpM) acc[j] += hu * __ldg(op.sq + k) * __ldg(in + (size_t)(eupM + k - 1) * Q + qi);
+      }
+    }
+  }
+  // ---- the other modes: neighbour columns k_s +- 1 (same element) and the columns of the elements n -+ e_s ----
+#pragma unroll
+  for (int s = 0; s < M - 1; s++) {
+    const int i = iq[s], n = op.nq[s], st = op.qst[s];
+    const long long o1 = (i + 1 < n) ? st : 0, o2 = (i >= 1) ? -st : 0, o3 = (i + 2 < n) ? 2 * st : 0, o4 = (i >= 2) ? -2 * st : 0;
+    const double w1 = (i + 1 < n) ? op.c1[s] : 0.0, w2 = (i >= 1) ? -op.c1[s] : 0.0;
+    const double w3 = (i + 2 < n) ? op.c2[s] : 0.0, w4 = (i >= 2) ? -op.c2[s] : 0.0;
+    const int up = S->up[s], dn = S->dn[s], hdn = S->hdn[s], hup = S->hup[s];
+    const double a1 = op.a1f[s] * __ldg(op.dU[s] + qi), a2 = op.a2[s];
+    const double vp = op.VLL[s] + op.VSL[s] * (op.q0[s] + op.h[s] * (double)i);
+    if (up >= 0) {                                         // sqrt(k_s+1) D+ c_{k+e_s}
+      const double su = S->su[s], f1 = a1 * su, f2 = -a2 * su;
+      const double* p = in + (size_t)(up + k0) * Q + qi;
+#pragma unroll
+      for (int j = 0; j < KC; j++) {
+        if (k0 + j < kpM)
+          acc[j] += f1 * __ldg(p) + f2 * (w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4));
+        p += Q;
+      }
+    }
+    if (dn >= 0) {                                         // -sqrt(k_s) D- c_{k-e_s}
+      const double sd = S->sd[s], f1 = -a1 * sd, f2 = -a2 * sd;
+      const double* p = in + (size_t)(dn + k0) * Q + qi;
+#pragma unroll
+      for (int j = 0; j < KC; j++) {
+        if (k0 + j < kpM)
+          acc[j] += f1 * __ldg(p) + f2 * (w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4));
+        p += Q;
+      }
+    }
+    if (hdn >= 0) {
+      const double f = vp * S->hd[s];
+      const double* p = in + (size_t)(hdn + k0) * Q + qi;
+#pragma unroll
+      for (int j = 0; j < KC; j++) { if (k0 + j < kpM) acc[j] += f * __ldg(p); p += Q; }
+    }
+    if (hup >= 0) {
+      const double f = vp * S->hu[s];
+      const double* p = in + (size_t)(hup + k0) * Q + qi;
+#pragma unroll
+      for (int j = 0; j < KC; j++) { if (k0 + j < kpM) acc[j] += f * __ldg(p); p += Q; }
+    }
+  }
+  const size_t o = soff + (size_t)(slab0 + k0) * Q + qi;
+#pragma unroll
+  for (int j = 0; j < KC; j++) {
+    if (k0 + j < kpM) {
+      const double base = (a != 0.0) ? a * y[o + (size_t)j * Q] : 0.0;
+      out[o + (size_t)j * Q] = base + c * acc[j];
+    }
+  }
+}
+
+// Patch form of the stage for M >= 2 (the default there): lanes run along the last (contiguous) q axis and a thread
+// owns a PA x PB patch of (q_1, q_2) points (PA points of q_1 for two modes) of ONE slab.  The stencils along the
+// patched axes read a window of PA + 4 (PB + 4) values per line and neighbour slab instead of 5 values per point, so
+// a point costs 2 (PA + 4) / PA + 2 (PB + 4) / PB + 10 stencil loads instead of 30, and the slab neighbourhood, the
+// lane-axis ghost weights and the q decode are worked out once per patch.
+template <int M, int PA, int PB, int FA, int FB, int FL, bool INT>
+__device__ __forceinline__ void hermite_patch_body(const HOp& op, const double* __restrict__ in, const double* y, double* out,
+                                                   const double a, const double c, const size_t soff, const int slab,
+                                                   const int a0, const int b0, const int iL) {
+  // FA, FB, FL: compile-time extents of q_1, q_2 and the lane axis (0 = run time; FB is unused for two modes), which turn
+  // every patch offset into an immediate; INT: the patch and its halo lie inside the mesh along q_1 and q_2 (no ghosts).
+  constexpr int L = M - 1;
+  const int nL = FL ? FL : op.nq[L];
+  const int nA = FA ? FA : op.nq[0], nB = (M == 3) ? (FB ? FB : op.nq[1]) : 1;
+  const int stB = (M == 3) ? nL : 0, stA = (M == 3) ? nB * nL : nL;
+  const int na = INT ? PA : min(PA, nA - a0), nb = (M == 3 && !INT) ? min(PB, nB - b0) : PB;
+  const int qi0 = a0 * stA + b0 * stB + iL;
+  const HSlab* __restrict__ S = op.slabs + slab;
+  const size_t Q = (size_t)op.Q;
+  const double* __restrict__ self = in + (size_t)slab * Q + qi0;
+  double acc[PA][PB];
+  {
+    const double gam = S->gam;
+#pragma unroll
+    for (int ia = 0; ia < PA; ia++)
+#pragma unroll
+      for (int ib = 0; ib < PB; ib++) acc[ia][ib] = (INT || (ia < na && ib < nb)) ? -gam * __ldg(self + ia * stA + ib * stB) : 0.0;
+  }
+  // ---- patched axis A (mode 0): windows of PA + 4 values along q_1 ----
+  {
+    constexpr int s = 0;
+    const int up = S->up[s], dn = S->dn[s];
+    const double su = (up >= 0) ? S->su[s] : 0.0, sd = (dn >= 0) ? S->sd[s] : 0.0;
+    const double* pu = in + (size_t)(up >= 0 ? up : slab) * Q + qi0;
+    const double* pd = in + (size_t)(dn >= 0 ? dn : slab) * Q + qi0;
+    const double c1 = op.c1[s], c2 = op.c2[s], a1f = op.a1f[s], a2 = op.a2[s];
+    if (up >= 0 || dn >= 0) {
+#pragma unroll
+      for (int ib = 0; ib < PB; ib++) {
+        if (INT || ib < nb) {
+          double P[PA + 4], Lc[PA];                        // su*up + sd*dn along the line; su*up - sd*dn at the centres
+#pragma unroll
+          for (int w = 0; w < PA + 4; w++) {
+            const int i = a0 - 2 + w;
+            double vu = 0.0, vd = 0.0;
+            if (INT || (i >= 0 && i < nA)) { const int o = (w - 2) * stA + ib * stB; vu = __ldg(pu + o); vd = __ldg(pd + o); }
+            P[w] = su * vu + sd * vd;
+            if (w >= 2 && w < PA + 2) Lc[w - 2] = su * vu - sd * vd;
+          }
+#pragma unroll
+          for (int ia = 0; ia < PA; ia++)
+            if (INT || ia < na)
+              acc[ia][ib] += a1f * __ldg(op.dU[s] + qi0 + ia * stA + ib * stB) * Lc[ia]
+                             - a2 * (c1 * (P[ia + 3] - P[ia + 1]) + c2 * (P[ia + 4] - P[ia]));
+        }
+      }
+    }
+    const int hdn = S->hdn[s], hup = S->hup[s];
+    if (hdn >= 0 || hup >= 0) {
+      const double hd = (hdn >= 0) ? S->hd[s] : 0.0, hu = (hup >= 0) ? S->hu[s] : 0.0;
+      const double* pdn = in + (size_t)(hdn >= 0 ? hdn : slab) * Q + qi0;
+      const double* pup = in + (size_t)(hup >= 0 ? hup : slab) * Q + qi0;
+#pragma unroll
+      for (int ia = 0; ia < PA; ia++) {
+        const double vp = op.VLL[s] + op.VSL[s] * (op.q0[s] + op.h[s] * (double)(a0 + ia));
+#pragma unroll
+        for (int ib = 0; ib < PB; ib++)
+          if (INT || (ia < na && ib < nb)) { const int o = ia * stA + ib * stB; acc[ia][ib] += vp * (hd * __ldg(pdn + o) + hu * __ldg(pup + o)); }
+      }
+    }
+  }
+  // ---- patched axis B (mode 1 of three): windows of PB + 4 values along q_2 ----
+  if (M == 3) {
+    constexpr int s = 1;
+    const int up = S->up[s], dn = S->dn[s];
+    const double su = (up >= 0) ? S->su[s] : 0.0, sd = (dn >= 0) ? S->sd[s] : 0.0;
+    const double* pu = in + (size_t)(up >= 0 ? up : slab) * Q + qi0;
+    const double* pd = in + (size_t)(dn >= 0 ? dn : slab) * Q + qi0;
+    const double c1 = op.c1[s], c2 = op.c2[s], a1f = op.a1f[s], a2 = op.a2[s];
+    if (up >= 0 || dn >= 0) {
+#pragma unroll
+      for (int ia = 0; ia < PA; ia++) {
+        if (INT || ia < na) {
+          double P[PB + 4], Lc[PB];
+#pragma unroll
+          for (int w = 0; w < PB + 4; w++) {
+            const int i = b0 - 2 + w;
+            double vu = 0.0, vd = 0.0;
+            if (INT || (i >= 0 && i < nB)) { const int o = ia * stA + (w - 2) * stB; vu = __ldg(pu + o); vd = __ldg(pd + o); }
+            P[w] = su * vu + sd * vd;
+            if (w >= 2 && w < PB + 2) Lc[w - 2] = su * vu - sd * vd;
+          }
+#pragma unroll
+          for (int ib = 0; ib < PB; ib++)
+            if (INT || ib < nb)
+              acc[ia][ib] += a1f * __ldg(op.dU[s] + qi0 + ia * stA + ib * stB) * Lc[ib]
+                             - a2 * (c1 * (P[ib + 3] - P[ib + 1]) + c2 * (P[ib + 4] - P[ib]));
+        }
+      }
+    }
+    const int hdn = S->hdn[s], hup = S->hup[s];
+    if (hdn >= 0 || hup >= 0) {
+      const double hd = (hdn >= 0) ? S->hd[s] : 0.0, hu = (hup >= 0) ? S->hu[s] : 0.0;
+      const double* pdn = in + (size_t)(hdn >= 0 ? hdn : slab) * Q + qi0;
+      const double* pup = in + (size_t)(hup >= 0 ? hup : slab) * Q + qi0;
+#pragma unroll
+      for (int ib = 0; ib < PB; ib++) {
+        const double vp = op.VLL[s] + op.VSL[s] * (op.q0[s] + op.h[s] * (double)(b0 + ib));
+#pragma unroll
+        for (int ia = 0; ia < PA; ia++)
+          if (INT || (ia < na && ib < nb)) { const int o = ia * stA + ib * stB; acc[ia][ib] += vp * (hd * __ldg(pdn + o) + hu * __ldg(pup + o)); }
+      }
+    }
+  }
+  // ---- lane axis (last mode): five loads per point and neighbour slab; ghosts are zero weights on the centre ----
+  {
+    constexpr int s = L;
+    const int up = S->up[s], dn = S->dn[s];
+    const double su = (up >= 0) ? S->su[s] : 0.0, sd = (dn >= 0) ? S->sd[s] : 0.0;
+    const double* pu = in + (size_t)(up >= 0 ? up : slab) * Q + qi0;
+    const double* pd = in + (size_t)(dn >= 0 ? dn : slab) * Q + qi0;
+    const int n = nL, i = iL;
+    const int o1 = (i + 1 < n) ? 1 : 0, o2 = (i >= 1) ? -1 : 0, o3 = (i + 2 < n) ? 2 : 0, o4 = (i >= 2) ? -2 : 0;
+    const double a2 = op.a2[s], a1f = op.a1f[s];
+    const double w1 = (i + 1 < n) ? -a2 * op.c1[s] : 0.0, w2 = (i >= 1) ? a2 * op.c1[s] : 0.0;
+    const double w3 = (i + 2 < n) ? -a2 * op.c2[s] : 0.0, w4 = (i >= 2) ? a2 * op.c2[s] : 0.0;
+    if (up >= 0 || dn >= 0) {
+      const double* pu1 = pu + o1; const double* pu2 = pu + o2; const double* pu3 = pu + o3; const double* pu4 = pu + o4;
+      const double* pd1 = pd + o1; const double* pd2 = pd + o2; const double* pd3 = pd + o3; const double* pd4 = pd + o4;
+#pragma unroll
+      for (int ia = 0; ia < PA; ia++)
+#pragma unroll
+        for (int ib = 0; ib < PB; ib++)
+          if (INT || (ia < na && ib < nb)) {
+            const int o = ia * stA + ib * stB;
+            const double lin = su * __ldg(pu + o) - sd * __ldg(pd + o);
+            const double der = w1 * (su * __ldg(pu1 + o) + sd * __ldg(pd1 + o)) + w2 * (su * __ldg(pu2 + o) + sd * __ldg(pd2 + o))
+                             + w3 * (su * __ldg(pu3 + o) + sd * __ldg(pd3 + o)) + w4 * (su * __ldg(pu4 + o) + sd * __ldg(pd4 + o));
+            acc[ia][ib] += a1f * __ldg(op.dU[s] + qi0 + o) * lin + der;
+          }
+    }
+    const int hdn = S->hdn[s], hup = S->hup[s];
+    if (hdn >= 0 || hup >= 0) {
+      const double vp = op.VLL[s] + op.VSL[s] * (op.q0[s] + op.h[s] * (double)i);
+      const double hd = (hdn >= 0) ? vp * S->hd[s] : 0.0, hu = (hup >= 0) ? vp * S->hu[s] : 0.0;
+      const double* pdn = in + (size_t)(hdn >= 0 ? hdn : slab) * Q + qi0;
+      const double* pup = in + (size_t)(hup >= 0 ? hup : slab) * Q + qi0;
+#pragma unroll
+      for (int ia = 0; ia < PA; ia++)
+#pragma unroll
+        for (int ib = 0; ib < PB; ib++)
+          if (INT || (ia < na && ib < nb)) { const int o = ia * stA + ib * stB; acc[ia][ib] += hd * __ldg(pdn + o) + hu * __ldg(pup + o); }
+    }
+  }
+  const size_t o0 = soff + (size_t)slab * Q + qi0;
+#pragma unroll
+  for (int ia = 0; ia < PA; ia++)
+#pragma unroll
+    for (int ib = 0; ib < PB; ib++)
+      if (INT || (ia < na && ib < nb)) {
+        const size_t o = o0 + ia * stA + ib * stB;                 // y and out are touched once per launch: streaming
+        const double base = (a != 0.0) ? a * __ldcs(y + o) : 0.0;  // (evict-first) accesses keep the L2 for the slabs of `in`
+        __stcs(out + o, base + c * acc[ia][ib]);
+      }
+}
+
+template <int M, int PA, int PB, int FA, int FB, int FL>
+__global__ void __launch_bounds__(256, (PA * PB <= 4) ? 4 : 1) k_hermite_stage_patch(const HOp op, const double* __restrict__ in, const double* y,
+                                                            double* out, const double a, const double c,
+                                                            const size_t slot_stride) {
+  static_assert(M == 2 || M == 3, "patch kernel: two or three modes");
+  static_assert(M == 3 || PB == 1, "two modes: one patched axis");
+  const int slab = blockIdx.x / op.pblocks;
+  const int t = (blockIdx.x - slab * op.pblocks) * blockDim.x + threadIdx.x;
+  if (t >= op.pthreads) return;
+  const int nL = FL ? FL : op.nq[M - 1];
+  const int nA = FA ? FA : op.nq[0], nB = (M == 3) ? (FB ? FB : op.nq[1]) : 1;
+  const int ntB = (M == 3) ? (FB ? (FB + PB - 1) / PB : op.ntileB) : 1;
+  const int r = t / nL, iL = t - r * nL;
+  const int tb = (M == 3) ? r % ntB : 0, ta = (M == 3) ? r / ntB : r;
+  const int a0 = ta * PA, b0 = tb * PB;
+  const size_t soff = (size_t)blockIdx.y * slot_stride;
+  const bool interior = a0 >= 2 && a0 + PA + 2 <= nA && (M == 2 || (b0 >= 2 && b0 + PB + 2 <= nB));
+  if (interior) hermite_patch_body<M, PA, PB, FA, FB, FL, true>(op, in + soff, y, out, a, c, soff, slab, a0, b0, iL);
+  else hermite_patch_body<M, PA, PB, FA, FB, FL, false>(op, in + soff, y, out, a, c, soff, slab, a0, b0, iL);
 }
 
 // Kick, Eq. (18) :131 projected on the Hermite functions: c_k <- sum_s (dX/dq_s) (-sqrt(k_s beta/m_s)) c_{k-e_s}
@@ -262,7 +581,7 @@ int validate(const chfpe_desc* d, std::string* why) {
   return CHFPE_OK;
 }
 
-struct Carve { size_t dU, wq, ceq, slabs, arrays, partial, results, total; };
+struct Carve { size_t dU, wq, ceq, sq, slabs, arrays, partial, results, total; };
 
 Carve carve(const chfpe_desc* d) {
   const int M = d->n_modes;
@@ -274,6 +593,7 @@ Carve carve(const chfpe_desc* d) {
   c.dU = off; off += align256(sizeof(double) * Q * 3);
   c.wq = off; off += align256(sizeof(double) * Q);
   c.ceq = off; off += align256(sizeof(double) * Q);
+  c.sq = off; off += align256(sizeof(double) * ((size_t)d->np[M - 1] + 2));
   c.slabs = off; off += align256(sizeof(HSlab) * K * KP);
   c.arrays = off; off += align256(sizeof(double) * K * KP * Q * 3 * (size_t)d->batch);
   c.partial = off; off += align256(sizeof(double) * RED_BLOCKS * (size_t)d->batch);
@@ -331,6 +651,28 @@ dim3 slab_grid(const HOp& op, int nb) { return dim3((unsigned)((size_t)op.nslab 
 void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* out, double a, double c, int nb) {
   const HOp& op = h->op;
   const size_t ss = 3 * h->state_doubles;
+  if (op.pa > 0) {                                   // patch kernel (default for M >= 2)
+    const dim3 g((unsigned)((size_t)op.nslab * op.pblocks), (unsigned)nb);
+#define HPATCH(MM, A, B, FA, FB, FL) k_hermite_stage_patch<MM, A, B, FA, FB, FL><<<g, 256, 0, h->stream>>>(op, in, y, out, a, c, ss)
+    const bool cube32 = op.M == 3 && op.nq[0] == 32 && op.nq[1] == 32 && op.nq[2] == 32 && op.fixed;
+    if (op.M == 2) { if (op.pa == 4) HPATCH(2, 4, 1, 0, 0, 0); else HPATCH(2, 2, 1, 0, 0, 0); }
+    else if (op.pa == 4 && op.pb == 4) { if (cube32) HPATCH(3, 4, 4, 32, 32, 32); else HPATCH(3, 4, 4, 0, 0, 0); }
+    else if (op.pa == 4 && op.pb == 2) { if (cube32) HPATCH(3, 4, 2, 32, 32, 32); else HPATCH(3, 4, 2, 0, 0, 0); }
+    else if (op.pa == 2 && op.pb == 4) HPATCH(3, 2, 4, 0, 0, 0);
+    else { if (cube32) HPATCH(3, 2, 2, 32, 32, 32); else HPATCH(3, 2, 2, 0, 0, 0); }
+#undef HPATCH
+    h->launches++;
+    return;
+  }
+  if (op.kc > 0) {                                   // column kernel (M = 1)
+    const dim3 g((unsigned)((size_t)(op.nslab / op.kp[op.M - 1]) * op.nchunk * op.blocks_per_slab), (unsigned)nb);
+#define HCOL(MM, KK) k_hermite_stage_col<MM, KK><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss)
+    if (op.kc == 8) { if (op.M == 1) HCOL(1, 8); else if (op.M == 2) HCOL(2, 8); else HCOL(3, 8); }
+    else { if (op.M == 1) HCOL(1, 4); else if (op.M == 2) HCOL(2, 4); else HCOL(3, 4); }
+#undef HCOL
+    h->launches++;
+    return;
+  }
   const dim3 g = slab_grid(op, nb);
   switch (op.M) {
     case 1: k_hermite_stage<1><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
@@ -510,6 +852,15 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
       HSlab& S = slabs[(size_t)e * KP + ki];
       memset(&S, 0, sizeof(S));
       S.gam = gam;
+      {                                              // column kernel: the columns of n -+ e_M that hold k_M = 0
+        const int sM = M - 1;
+        const size_t ki0 = ki - (ki % op.kp[sM]);
+        const double m = desc->mass[sM], beta = desc->beta;
+        S.ednM = (edn[sM] >= 0) ? (int)((size_t)edn[sM] * KP + ki0) : -1;
+        S.eupM = (eup[sM] >= 0) ? (int)((size_t)eup[sM] * KP + ki0) : -1;
+        S.hdM = (edn[sM] >= 0) ? n[sM] * desc->gamma[sM] * desc->zeta[sM] * sqrt(m / beta) : 0.0;
+        S.huM = (eup[sM] >= 0) ? -sqrt(beta / m) : 0.0;
+      }
       for (int s = 0; s < 3; s++) {
         S.up[s] = S.dn[s] = S.hdn[s] = S.hup[s] = -1;
         if (s >= M) continue;
@@ -538,12 +889,39 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
   op.wq = (double*)(base + cv.wq);
   op.ceq = (double*)(base + cv.ceq);
   op.slabs = (HSlab*)(base + cv.slabs);
+  op.sq = (double*)(base + cv.sq);
+  std::vector<double> sq((size_t)op.kp[M - 1] + 2);
+  for (size_t i = 0; i < sq.size(); i++) sq[i] = sqrt((double)i);
+  {                                                  // CHFPE_HERMITE_KC = 0 | 4 | 8: per-value kernel or column length
+    const char* e = getenv("CHFPE_HERMITE_KC");
+    int kc = (op.kp[M - 1] >= 6) ? 8 : 4;
+    if (e && *e) { const int v = atoi(e); if (v == 0 || v == 4 || v == 8) kc = v; }
+    op.kc = kc;
+    op.nchunk = kc ? (op.kp[M - 1] + kc - 1) / kc : 0;
+    // CHFPE_HERMITE_PATCH = "AB" (A, B in {2, 4}; "0" = off): patch extents along q_1, q_2 of the patch kernel
+    int pa = (M == 2) ? 4 : (M == 3) ? 2 : 0, pb = (M == 3) ? 2 : 1;
+    const char* pe = getenv("CHFPE_HERMITE_PATCH");
+    if (pe && *pe && M >= 2) {
+      if (pe[0] == '0') pa = 0;
+      else if ((pe[0] == '2' || pe[0] == '4') && (M == 2 || pe[1] == '2' || pe[1] == '4')) { pa = pe[0] - '0'; if (M == 3) pb = pe[1] - '0'; }
+    }
+    if (e && *e) pa = 0;                             // an explicit column / per-value request wins
+    op.pa = pa; op.pb = (M == 3) ? pb : 1;
+    { const char* fe = getenv("CHFPE_HERMITE_FIXED"); op.fixed = !(fe && fe[0] == '0'); }
+    if (pa > 0) {
+      const int ntA = (op.nq[0] + pa - 1) / pa;
+      op.ntileB = (M == 3) ? (op.nq[1] + op.pb - 1) / op.pb : 1;
+      op.pthreads = ntA * op.ntileB * op.nq[M - 1];
+      op.pblocks = (op.pthreads + 255) / 256;
+    }
+  }
   h->arrays = (double*)(base + cv.arrays);
   h->partial = (double*)(base + cv.partial);
   h->results = (double*)(base + cv.results);
   cudaError_t e = cudaMemcpyAsync(d_dU, dU.data(), sizeof(double) * 3 * Q, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.wq, wq.data(), sizeof(double) * Q, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.ceq, ceq.data(), sizeof(double) * Q, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.sq, sq.data(), sizeof(double) * sq.size(), cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.slabs, slabs.data(), sizeof(HSlab) * slabs.size(), cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->arrays, 0, sizeof(double) * h->state_doubles * 3 * (size_t)h->batch, h->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);      // the host vectors go out of scope

@@ -76,6 +76,28 @@ def test_rhs_step_kick_expect(name, cfg):
     assert rel_l2(g.export_state(), o.export_state()) < 1e-13
 
 
+@pytest.mark.parametrize("var,val", [("CHFPE_HERMITE_KC", "0"), ("CHFPE_HERMITE_KC", "4"), ("CHFPE_HERMITE_KC", "8"),
+                                     ("CHFPE_HERMITE_PATCH", "44"), ("CHFPE_HERMITE_PATCH", "42"),
+                                     ("CHFPE_HERMITE_PATCH", "24"), ("CHFPE_HERMITE_PATCH", "22"),
+                                     ("CHFPE_HERMITE_PATCH", "0")])
+def test_every_stage_kernel_variant(var, val, monkeypatch):
+    """CHFPE_HERMITE_KC: 0 = one thread per value, 4 / 8 = column kernel with that many Hermite indices of the last
+    mode per thread (columns longer and shorter than a chunk, ragged last chunks, kp = 1).  CHFPE_HERMITE_PATCH = "AB":
+    patch kernel with A x B points of (q_1, q_2) per thread (ragged patches, axes shorter than a patch + halo)."""
+    monkeypatch.setenv(var, val)
+    for cfg in (ci.config("cfg2", nq=[37], np=[11], depth=4),
+                ci.config("cfg3s", nq=[40, 37], np=[3, 9], depth=2, mass=[1.0, 1.3]),
+                ci.config("cfg4s8", nq=[7, 8, 6], np=[2, 3, 5], depth=3),
+                ci.config("cfg4s8", nq=[6, 5, 7], np=[3, 2, 1], depth=2, scheme="central2")):
+        g, o = both(cfg)
+        X = ci.seeded_hermite_state(cfg, [sum(n) for n in o.elems], seed=4)
+        g.import_state(X); o.import_state(X)
+        assert rel_l2(g.export_rhs(), o.rhs(o.c)) < 1e-13
+        g.step(2, cfg["dt"]); o.step(2, cfg["dt"])
+        assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+        g.close()
+
+
 def test_zero_steps_and_batch_slots_are_independent():
     cfg = ci.config("cfg3s", nq=[12, 9], np=[3, 4], depth=2)
     g = P().Hermite(cfg, batch=3)
