@@ -16,7 +16,8 @@ factors of Theta, Phi are not consistent with Eq. 8-12):
     D+-_s g = (dU/dq_s) / (2 sqrt(m_s/beta)) g  -+  (1/sqrt(m_s beta)) dg/dq_s                      (A2)
 
 with c_k = 0 outside 0 <= k_s < K_p,s and outside the hierarchy simplex (R5), q-derivatives by the CENTRAL4 /
-CENTRAL2 stencil with zero ghosts (R9).  Kick (Eq. 18): c_k <- sum_s (dX/dq_s) (-sqrt(k_s beta/m_s)) c_{k-e_s}.
+CENTRAL2 stencil with zero ghosts (R9) or by the paper's sixth-order compact scheme (scheme "compact6", Eq. 25-31:
+one tridiagonal solve per q-line, here scipy.linalg.solve_banded).  Kick (Eq. 18): c_k <- sum_s (dX/dq_s) (-sqrt(k_s beta/m_s)) c_{k-e_s}.
 Expectations: int int O W^(0) dp dq = int O(q) e^{-beta U/2} c^(0)_0(q) dq;  <p_s> uses c^(0)_{e_s} sqrt(m_s/beta).
 Equilibrium: c^(0)_0 = e^{-beta U/2} / Z_q, everything else zero.  Time stepping: textbook RK4.
 State layout: c[element][k_1]..[k_M][i_q1]..[i_qM].
@@ -24,6 +25,7 @@ State layout: c[element][k_1]..[k_M][i_q1]..[i_qM].
 import itertools
 
 import numpy as np
+import scipy.linalg
 
 
 def enumerate_elements(M, depth):
@@ -75,6 +77,16 @@ class RefHermite:
         sl = lambda o: tuple(slice(2 + o, 2 + o + n) if a == ax else slice(None) for a in range(g.ndim))
         if self.scheme == "central2":
             return (gp[sl(1)] - gp[sl(-1)]) / (2 * h)
+        if self.scheme == "compact6":
+            # Pade scheme of Eq. (25)-(31) PAPER.md:177-201, the paper's q-derivative in this representation:
+            # (1/3) d_{i-1} + d_i + (1/3) d_{i+1} = [a (g_{i+1} - g_{i-1}) + b (g_{i+2} - g_{i-2})] / h, a = 7/9 (reading R4:
+            # the printed 7/18 is not consistent), b = 1/36, both matrices truncated as printed in Eq. (28)-(29) (R9).
+            r = ((7.0 / 9.0) * (gp[sl(1)] - gp[sl(-1)]) + (1.0 / 36.0) * (gp[sl(2)] - gp[sl(-2)])) / h
+            ab = np.ones((3, n))
+            ab[0, :], ab[2, :] = 1.0 / 3.0, 1.0 / 3.0
+            r = np.moveaxis(r, ax, 0)
+            d = scipy.linalg.solve_banded((1, 1), ab, r.reshape(n, -1)).reshape(r.shape)
+            return np.moveaxis(d, 0, ax)
         return (8.0 * (gp[sl(1)] - gp[sl(-1)]) - (gp[sl(2)] - gp[sl(-2)])) / (12 * h)
 
     def shift_k(self, g, s, d):
