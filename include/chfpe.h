@@ -176,7 +176,9 @@ const char* chfpe_last_error(const chfpe_handle* h);   /* h may be NULL: last cr
                   + sum_s V'_s [ n_s gamma_s zeta_s sqrt(m_s/beta) sqrt(k_s+1) c^(n-e_s)_{k+e_s} - sqrt(k_s beta/m_s) c^(n+e_s)_{k-e_s} ],
      D+-_s g = (dU/dq_s) / (2 sqrt(m_s/beta)) g -+ (1/sqrt(m_s beta)) dg/dq_s.
    The same chfpe_desc is used with np[s] = number of Hermite functions of mode s (>= 1); pmin/pmax and gauge are
-   ignored; scheme = CHFPE_CENTRAL4 | CHFPE_CENTRAL2 (q-derivatives, zero ghosts R9).  State layout of one replica
+   ignored; scheme = CHFPE_CENTRAL4 | CHFPE_CENTRAL2 (explicit q-stencils, zero ghosts R9) | CHFPE_COMPACT6 (the paper's
+   Pade q-derivative Eq. (25)-(31) :177-201 with a = 7/9 (R4): one tridiagonal line solve per slab, mode and q-line; at
+   most 256 points per q axis; a stage is 1 + M launches).  State layout of one replica
    (import/export AND device): c[element][k_1]..[k_M][i_q1]..[i_qM], last axis fastest, fp64; element order as above.
    Same conventions as the grid calls: caller-owned 256-byte aligned device workspace and stream, int return codes,
    host pointers unless stated, calls returning host data synchronise the stream.  No CPU fallback. */

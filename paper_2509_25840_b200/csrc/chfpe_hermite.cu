@@ -49,6 +49,9 @@ struct HOp {                // device view of the operator, passed by value
   const double* sq;                   // sq[i] = sqrt(i), i = 0 .. kp_M
   int kc, nchunk;                     // column kernel: Hermite indices of the last mode per thread, chunks per column
   int pa, pb, ntileB, pthreads, pblocks;   // patch kernel: patch extents, q_2 tiles, threads and CTAs per slab
+  double ca[3], cb[3];                // COMPACT6: 7/(9h), 1/(36h)
+  const double* ibet[3];              // COMPACT6: reciprocal pivots and elimination factors of tridiag(1/3, 1, 1/3) per mode
+  const double* cfac[3];
   int fixed;                          // use the compile-time 32^3 specialisation when the mesh matches (CHFPE_HERMITE_FIXED=0: off)
 };
 
@@ -69,9 +72,10 @@ __device__ __forceinline__ double dq_stencil(const double* __restrict__ p, int i
   return d;
 }
 
-// One RK stage: out = a*y + c*F(in) on every slab of every slot (grid.y).  One thread per (slab, q-point), the q grid
+// One RK stage: out = a*y + c*F(in) on every slab of every slot (grid.y); DER = false leaves the q-derivative terms
+// out (COMPACT6: k_hermite_compact_line adds them, one pass per mode).  One thread per (slab, q-point), the q grid
 // of a slab is covered by `blocks_per_slab` consecutive CTAs, so everything about the slab is CTA-uniform.
-template <int M>
+template <int M, bool DER>
 __global__ void __launch_bounds__(256) k_hermite_stage(const HOp op, const double* __restrict__ in,
                                                       const double* y, double* out,
                                                       const double a, const double c, const size_t slot_stride) {
@@ -100,13 +104,13 @@ __global__ void __launch_bounds__(256) k_hermite_stage(const HOp op, const doubl
       const double* p = in + (size_t)up * Q + qi;
       const double su = S->su[s];
       lin += su * __ldg(p);
-      der += su * dq_stencil(p, i, n, st, op.c1[s], op.c2[s]);
+      if (DER) der += su * dq_stencil(p, i, n, st, op.c1[s], op.c2[s]);
     }
     if (dn >= 0) {                                   // -sqrt(k) D- c_{k-e_s}
       const double* p = in + (size_t)dn * Q + qi;
       const double sd = S->sd[s];
       lin -= sd * __ldg(p);
-      der += sd * dq_stencil(p, i, n, st, op.c1[s], op.c2[s]);
+      if (DER) der += sd * dq_stencil(p, i, n, st, op.c1[s], op.c2[s]);
     }
     acc += op.a1f[s] * __ldg(op.dU[s] + qi) * lin - op.a2[s] * der;
     double hh = 0.0;                                 // Theta (from n - e_s) and Phi (from n + e_s), pointwise in q
@@ -428,6 +432,56 @@ __global__ void __launch_bounds__(256, (PA * PB <= 4) ? 4 : 1) k_hermite_stage_p
   else hermite_patch_body<M, PA, PB, FA, FB, FL, false>(op, in + soff, y, out, a, c, soff, slab, a0, b0, iL);
 }
 
+// COMPACT6 (the paper's q-derivative, Eq. 25-31, a = 7/9 by reading R4): for one mode s, every slab
+// and every q_s-line of it, form P = sqrt(k_s+1) c_{k+e_s} + sqrt(k_s) c_{k-e_s} along the line, the right-hand side
+// r = [a (P_{+1} - P_{-1}) + b (P_{+2} - P_{-2})] / h (truncated, R9), solve tridiag(1/3, 1, 1/3) d = r by the Thomas
+// recurrence with host-tabulated elimination factors (one thread per line, forward values in thread-local memory) and
+// add -c / sqrt(m_s beta) d to the stage output.  Lines along a non-contiguous axis are coalesced across the warp.
+constexpr int HMAXLINE = 256;
+template <int M>
+__global__ void __launch_bounds__(128) k_hermite_compact_line(const HOp op, const int s, const double* __restrict__ in,
+                                                             double* out, const double c, const size_t slot_stride) {
+  const int n = op.nq[s], st = op.qst[s];
+  const int nlines = op.Q / n;
+  const int bps = (nlines + blockDim.x - 1) / blockDim.x;
+  const int slab = blockIdx.x / bps;
+  const int line = (blockIdx.x - slab * bps) * blockDim.x + threadIdx.x;
+  if (line >= nlines) return;
+  const HSlab* __restrict__ S = op.slabs + slab;
+  const int up = S->up[s], dn = S->dn[s];
+  if (up < 0 && dn < 0) return;
+  const int outer = line / st, inner = line - outer * st;
+  const size_t base = (size_t)outer * st * n + inner;
+  const size_t soff = (size_t)blockIdx.y * slot_stride, Q = (size_t)op.Q;
+  const double su = (up >= 0) ? S->su[s] : 0.0, sd = (dn >= 0) ? S->sd[s] : 0.0;
+  const double* __restrict__ pu = in + soff + (size_t)(up >= 0 ? up : slab) * Q + base;
+  const double* __restrict__ pd = in + soff + (size_t)(dn >= 0 ? dn : slab) * Q + base;
+  double* po = out + soff + (size_t)slab * Q + base;
+  const double* __restrict__ ibet = op.ibet[s];
+  const double* __restrict__ cfac = op.cfac[s];
+  const double ca = op.ca[s], cb = op.cb[s];
+  double loc[HMAXLINE];
+  double Pm2 = 0.0, Pm1 = 0.0;
+  double P0 = su * __ldg(pu) + sd * __ldg(pd);
+  double P1 = su * __ldg(pu + st) + sd * __ldg(pd + st);       // n >= 5
+  double prev = 0.0;
+  for (int i = 0; i < n; i++) {
+    const double P2 = (i + 2 < n) ? su * __ldg(pu + (size_t)(i + 2) * st) + sd * __ldg(pd + (size_t)(i + 2) * st) : 0.0;
+    const double P1e = (i + 1 < n) ? P1 : 0.0;
+    const double r = ca * (P1e - Pm1) + cb * (P2 - Pm2);
+    prev = (r - (1.0 / 3.0) * prev) * __ldg(ibet + i);
+    loc[i] = prev;
+    Pm2 = Pm1; Pm1 = P0; P0 = P1e; P1 = P2;
+  }
+  const double f = -c * op.a2[s];
+  double x = loc[n - 1];
+  po[(size_t)(n - 1) * st] += f * x;
+  for (int i = n - 2; i >= 0; i--) {
+    x = loc[i] - __ldg(cfac + i + 1) * x;
+    po[(size_t)i * st] += f * x;
+  }
+}
+
 // Kick, Eq. (18) :131 projected on the Hermite functions: c_k <- sum_s (dX/dq_s) (-sqrt(k_s beta/m_s)) c_{k-e_s}
 template <int M>
 __global__ void __launch_bounds__(256) k_hermite_kick(const HOp op, const HObs o, const double* __restrict__ in,
@@ -556,7 +610,7 @@ int validate(const chfpe_desc* d, std::string* why) {
   if (d->n_modes < 1 || d->n_modes > 3) { *why = "n_modes must be 1..3"; return CHFPE_ERR_INVALID; }
   if (d->depth < 0 || d->depth > 64) { *why = "depth out of range"; return CHFPE_ERR_INVALID; }
   if (!(d->beta > 0)) { *why = "beta must be > 0"; return CHFPE_ERR_INVALID; }
-  if (d->scheme != CHFPE_CENTRAL4 && d->scheme != CHFPE_CENTRAL2) { *why = "Hermite path: scheme must be CENTRAL4 or CENTRAL2"; return CHFPE_ERR_INVALID; }
+  if (d->scheme != CHFPE_CENTRAL4 && d->scheme != CHFPE_CENTRAL2 && d->scheme != CHFPE_COMPACT6) { *why = "unknown scheme"; return CHFPE_ERR_INVALID; }
   if (d->batch < 1 || d->batch > 4096) { *why = "batch must be 1..4096"; return CHFPE_ERR_INVALID; }
   if (d->n_terms < 0 || (d->n_terms > 0 && !d->U)) { *why = "bad potential term list"; return CHFPE_ERR_INVALID; }
   for (int t = 0; t < d->n_terms; t++) {
@@ -570,6 +624,7 @@ int validate(const chfpe_desc* d, std::string* why) {
   double Q = 1.0, KP = 1.0;
   for (int s = 0; s < d->n_modes; s++) {
     if (d->nq[s] < 5) { *why = "need >= 5 grid points per q axis"; return CHFPE_ERR_INVALID; }
+    if (d->scheme == CHFPE_COMPACT6 && d->nq[s] > 256) { *why = "Hermite path, COMPACT6: at most 256 points per q axis"; return CHFPE_ERR_INVALID; }
     if (d->np[s] < 1 || d->np[s] > 4096) { *why = "need 1..4096 Hermite functions per mode"; return CHFPE_ERR_INVALID; }
     if (!(d->mass[s] > 0) || !(d->gamma[s] > 0) || d->zeta[s] < 0) { *why = "mass, gamma must be > 0 and zeta >= 0"; return CHFPE_ERR_INVALID; }
     if (!(d->qmax[s] > d->qmin[s])) { *why = "empty coordinate range"; return CHFPE_ERR_INVALID; }
@@ -581,7 +636,7 @@ int validate(const chfpe_desc* d, std::string* why) {
   return CHFPE_OK;
 }
 
-struct Carve { size_t dU, wq, ceq, sq, slabs, arrays, partial, results, total; };
+struct Carve { size_t dU, wq, ceq, sq, thomas, slabs, arrays, partial, results, total; };
 
 Carve carve(const chfpe_desc* d) {
   const int M = d->n_modes;
@@ -594,6 +649,7 @@ Carve carve(const chfpe_desc* d) {
   c.wq = off; off += align256(sizeof(double) * Q);
   c.ceq = off; off += align256(sizeof(double) * Q);
   c.sq = off; off += align256(sizeof(double) * ((size_t)d->np[M - 1] + 2));
+  c.thomas = off; off += align256(sizeof(double) * 6 * 256);
   c.slabs = off; off += align256(sizeof(HSlab) * K * KP);
   c.arrays = off; off += align256(sizeof(double) * K * KP * Q * 3 * (size_t)d->batch);
   c.partial = off; off += align256(sizeof(double) * RED_BLOCKS * (size_t)d->batch);
@@ -651,6 +707,26 @@ dim3 slab_grid(const HOp& op, int nb) { return dim3((unsigned)((size_t)op.nslab 
 void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* out, double a, double c, int nb) {
   const HOp& op = h->op;
   const size_t ss = 3 * h->state_doubles;
+  if (op.scheme == CHFPE_COMPACT6) {                 // pointwise terms, then one line pass per mode
+    const dim3 g0 = slab_grid(op, nb);
+    switch (op.M) {
+      case 1: k_hermite_stage<1, false><<<g0, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+      case 2: k_hermite_stage<2, false><<<g0, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+      default: k_hermite_stage<3, false><<<g0, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+    }
+    for (int s = 0; s < op.M; s++) {
+      const int nlines = op.Q / op.nq[s];
+      const int th = (nlines >= 128) ? 128 : (nlines + 31) / 32 * 32;
+      const dim3 g((unsigned)((size_t)op.nslab * ((nlines + th - 1) / th)), (unsigned)nb);
+      switch (op.M) {
+        case 1: k_hermite_compact_line<1><<<g, th, 0, h->stream>>>(op, s, in, out, c, ss); break;
+        case 2: k_hermite_compact_line<2><<<g, th, 0, h->stream>>>(op, s, in, out, c, ss); break;
+        default: k_hermite_compact_line<3><<<g, th, 0, h->stream>>>(op, s, in, out, c, ss); break;
+      }
+    }
+    h->launches += 1 + op.M;
+    return;
+  }
   if (op.pa > 0) {                                   // patch kernel (default for M >= 2)
     const dim3 g((unsigned)((size_t)op.nslab * op.pblocks), (unsigned)nb);
 #define HPATCH(MM, A, B, FA, FB, FL) k_hermite_stage_patch<MM, A, B, FA, FB, FL><<<g, 256, 0, h->stream>>>(op, in, y, out, a, c, ss)
@@ -675,9 +751,9 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
   }
   const dim3 g = slab_grid(op, nb);
   switch (op.M) {
-    case 1: k_hermite_stage<1><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
-    case 2: k_hermite_stage<2><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
-    default: k_hermite_stage<3><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+    case 1: k_hermite_stage<1, true><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+    case 2: k_hermite_stage<2, true><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
+    default: k_hermite_stage<3, true><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
   }
   h->launches++;
 }
@@ -890,6 +966,18 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
   op.ceq = (double*)(base + cv.ceq);
   op.slabs = (HSlab*)(base + cv.slabs);
   op.sq = (double*)(base + cv.sq);
+  std::vector<double> thomas(6 * 256, 0.0);
+  for (int s = 0; s < M; s++) {
+    op.ca[s] = 7.0 / (9.0 * op.h[s]);
+    op.cb[s] = 1.0 / (36.0 * op.h[s]);
+    op.ibet[s] = (double*)(base + cv.thomas) + (size_t)(2 * s) * 256;
+    op.cfac[s] = (double*)(base + cv.thomas) + (size_t)(2 * s + 1) * 256;
+    double* ib = &thomas[(size_t)(2 * s) * 256];
+    double* cf = &thomas[(size_t)(2 * s + 1) * 256];
+    double bet = 1.0;
+    ib[0] = 1.0; cf[0] = 0.0;
+    for (int i = 1; i < op.nq[s] && i < 256; i++) { cf[i] = (1.0 / 3.0) / bet; bet = 1.0 - (1.0 / 3.0) * cf[i]; ib[i] = 1.0 / bet; }
+  }
   std::vector<double> sq((size_t)op.kp[M - 1] + 2);
   for (size_t i = 0; i < sq.size(); i++) sq[i] = sqrt((double)i);
   {                                                  // CHFPE_HERMITE_KC = 0 | 4 | 8: per-value kernel or column length
@@ -921,6 +1009,7 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
   cudaError_t e = cudaMemcpyAsync(d_dU, dU.data(), sizeof(double) * 3 * Q, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.wq, wq.data(), sizeof(double) * Q, cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.ceq, ceq.data(), sizeof(double) * Q, cudaMemcpyHostToDevice, h->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(base + cv.thomas, thomas.data(), sizeof(double) * thomas.size(), cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.sq, sq.data(), sizeof(double) * sq.size(), cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync((void*)op.slabs, slabs.data(), sizeof(HSlab) * slabs.size(), cudaMemcpyHostToDevice, h->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(h->arrays, 0, sizeof(double) * h->state_doubles * 3 * (size_t)h->batch, h->stream);

@@ -49,6 +49,12 @@ SMALL = [
     ("m3", ci.config("cfg4s8", nq=[7, 8, 6], np=[3, 2, 4], depth=3)),
     ("m3_ragged", ci.config("cfg4s8", nq=[11, 9, 13], np=[3, 4, 2], depth=2, mass=[1.0, 0.8, 1.2])),
     ("m3_kp1_mid", ci.config("cfg4s8", nq=[6, 5, 7], np=[3, 1, 2], depth=2, scheme="central2")),
+    # the paper's compact (Pade) q-derivative: one Thomas line solve per slab, mode and q-line
+    ("m1_compact6", ci.config("cfg2", nq=[67], np=[6], depth=4, scheme="compact6")),
+    ("m1_compact6_256", ci.config("cfg2", nq=[256], np=[3], depth=2, scheme="compact6", mass=[1.3])),   # longest line
+    ("m2_compact6", ci.config("cfg3s", nq=[23, 14], np=[3, 4], depth=2, scheme="compact6", mass=[1.0, 1.3])),
+    ("m3_compact6", ci.config("cfg4s8", nq=[9, 12, 7], np=[3, 2, 3], depth=2, scheme="compact6")),
+    ("m3_compact6_5pt", ci.config("cfg4s8", nq=[5, 6, 5], np=[2, 2, 2], depth=3, scheme="compact6")),  # shortest lines
 ]
 
 
@@ -152,6 +158,28 @@ def test_response_1d_ten_thousand_steps():
     Ro = o.response_1d(mu, mu, 11, 1000, 1e-3)
     assert np.max(np.abs(Ro)) > 0.3
     assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+
+
+def test_response_1d_compact6_and_its_closed_form():
+    """COMPACT6 on the CUDA path: parity of a sampled response with the oracle, and the Brownian-oscillator closed form
+    (tests/golden/bo_response_cfg1.txt) to 1e-5 on a mesh (h = 0.5) where CENTRAL4 is only good to 7e-4."""
+    gold = np.loadtxt(os.path.join(os.path.dirname(__file__), "golden", "bo_response_cfg1.txt"))
+    cfg = ci.config("cfg1", nq=[37], np=[6], depth=3, qmin=[-9.0], qmax=[9.0], scheme="compact6")
+    g, o = both(cfg)
+    g.equilibrate(); o.equilibrate()
+    mu = ci.observable("mu", 1)
+    Rg = g.response_1d(gobs(mu), gobs(mu), 5, 500, 1e-3)
+    Ro = o.response_1d(mu, mu, 5, 500, 1e-3)
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    assert np.allclose(gold[:, 0], 0.5 * np.arange(1, 5))
+    assert np.max(np.abs(-Rg[1:] - gold[:, 1])) < 1e-5
+    cfg2 = ci.config("cfg3s", nq=[14, 12], np=[4, 3], depth=2, scheme="compact6")
+    g2, o2 = both(cfg2, batch=3)
+    g2.equilibrate(); o2.equilibrate()
+    mu2, al2 = ci.observable("mu", 2), ci.observable("alpha", 2)
+    R2g = g2.response_2d(gobs(mu2), gobs(al2), gobs(al2), [0, 4, 6], [0, 5], 5e-3)
+    R2o = o2.response_2d(mu2, al2, al2, [0, 4, 6], [0, 5], 5e-3)
+    assert np.max(np.abs(R2g - R2o)) <= 1e-8 * np.max(np.abs(R2o))
 
 
 def test_response_1d_three_modes():
