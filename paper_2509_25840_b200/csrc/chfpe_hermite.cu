@@ -52,6 +52,7 @@ struct HOp {                // device view of the operator, passed by value
   double ca[3], cb[3];                // COMPACT6: 7/(9h), 1/(36h)
   const double* ibet[3];              // COMPACT6: reciprocal pivots and elimination factors of tridiag(1/3, 1, 1/3) per mode
   const double* cfac[3];
+  int contig;                         // COMPACT6: transposing kernel for the contiguous axis (CHFPE_HERMITE_CONTIG=0: off)
   int fixed;                          // use the compile-time 32^3 specialisation when the mesh matches (CHFPE_HERMITE_FIXED=0: off)
 };
 
@@ -482,6 +483,59 @@ __global__ void __launch_bounds__(128) k_hermite_compact_line(const HOp op, cons
   }
 }
 
+// The same line pass for the CONTIGUOUS q axis (s = M - 1, stride 1), where one thread per line would read 8 bytes per
+// 32-byte sector: a CTA of LPC threads owns LPC consecutive lines = one contiguous run of LPC * n doubles, loads the
+// runs of the two neighbour slabs coalesced and combines them to P in a padded shared tile (row stride n + 1: the
+// per-line accesses of the solve are conflict-free), solves its lines in place and adds the result back coalesced.
+template <int LPC>
+__global__ void __launch_bounds__(LPC) k_hermite_compact_line_contig(const HOp op, const int s, const double* __restrict__ in,
+                                                                    double* out, const double c, const size_t slot_stride) {
+  extern __shared__ double tile[];                    // [LPC][n + 1]
+  const int n = op.nq[s];
+  const int nlines = op.Q / n;
+  const int bps = (nlines + LPC - 1) / LPC;
+  const int slab = blockIdx.x / bps;
+  const int line0 = (blockIdx.x - slab * bps) * LPC;
+  const int nl = min(LPC, nlines - line0);
+  const HSlab* __restrict__ S = op.slabs + slab;
+  const int up = S->up[s], dn = S->dn[s];
+  if (up < 0 && dn < 0) return;                       // CTA-uniform
+  const size_t soff = (size_t)blockIdx.y * slot_stride, Q = (size_t)op.Q;
+  const size_t base = (size_t)line0 * n;
+  const double su = (up >= 0) ? S->su[s] : 0.0, sd = (dn >= 0) ? S->sd[s] : 0.0;
+  const double* __restrict__ pu = in + soff + (size_t)(up >= 0 ? up : slab) * Q + base;
+  const double* __restrict__ pd = in + soff + (size_t)(dn >= 0 ? dn : slab) * Q + base;
+  double* po = out + soff + (size_t)slab * Q + base;
+  const int total = nl * n, ld = n + 1;
+  for (int e = threadIdx.x; e < total; e += LPC) {
+    const int l = e / n, i = e - l * n;
+    tile[l * ld + i] = su * __ldg(pu + e) + sd * __ldg(pd + e);
+  }
+  __syncthreads();
+  if ((int)threadIdx.x < nl) {
+    double* P = tile + threadIdx.x * ld;
+    const double* __restrict__ ibet = op.ibet[s];
+    const double* __restrict__ cfac = op.cfac[s];
+    const double ca = op.ca[s], cb = op.cb[s];
+    double Pm2 = 0.0, Pm1 = 0.0, P0 = P[0], P1 = P[1], prev = 0.0;
+    for (int i = 0; i < n; i++) {
+      const double P2 = (i + 2 < n) ? P[i + 2] : 0.0;
+      const double r = ca * (P1 - Pm1) + cb * (P2 - Pm2);
+      prev = (r - (1.0 / 3.0) * prev) * __ldg(ibet + i);
+      P[i] = prev;                                    // P[i] is not read again: the window holds P_{i-2} .. P_{i+2}
+      Pm2 = Pm1; Pm1 = P0; P0 = P1; P1 = P2;
+    }
+    double x = P[n - 1];
+    for (int i = n - 2; i >= 0; i--) { x = P[i] - __ldg(cfac + i + 1) * x; P[i] = x; }
+  }
+  __syncthreads();
+  const double f = -c * op.a2[s];
+  for (int e = threadIdx.x; e < total; e += LPC) {
+    const int l = e / n, i = e - l * n;
+    po[e] += f * tile[l * ld + i];
+  }
+}
+
 // Kick, Eq. (18) :131 projected on the Hermite functions: c_k <- sum_s (dX/dq_s) (-sqrt(k_s beta/m_s)) c_{k-e_s}
 template <int M>
 __global__ void __launch_bounds__(256) k_hermite_kick(const HOp op, const HObs o, const double* __restrict__ in,
@@ -716,6 +770,16 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
     }
     for (int s = 0; s < op.M; s++) {
       const int nlines = op.Q / op.nq[s];
+      if (s == op.M - 1 && op.nq[s] <= 64 && nlines >= 64 && op.contig) {     // contiguous axis: transposing kernel
+        if (op.nq[s] <= 32) {
+          const dim3 g((unsigned)((size_t)op.nslab * ((nlines + 127) / 128)), (unsigned)nb);
+          k_hermite_compact_line_contig<128><<<g, 128, sizeof(double) * 128 * (op.nq[s] + 1), h->stream>>>(op, s, in, out, c, ss);
+        } else {
+          const dim3 g((unsigned)((size_t)op.nslab * ((nlines + 63) / 64)), (unsigned)nb);
+          k_hermite_compact_line_contig<64><<<g, 64, sizeof(double) * 64 * (op.nq[s] + 1), h->stream>>>(op, s, in, out, c, ss);
+        }
+        continue;
+      }
       const int th = (nlines >= 128) ? 128 : (nlines + 31) / 32 * 32;
       const dim3 g((unsigned)((size_t)op.nslab * ((nlines + th - 1) / th)), (unsigned)nb);
       switch (op.M) {
@@ -996,6 +1060,7 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
     if (e && *e) pa = 0;                             // an explicit column / per-value request wins
     op.pa = pa; op.pb = (M == 3) ? pb : 1;
     { const char* fe = getenv("CHFPE_HERMITE_FIXED"); op.fixed = !(fe && fe[0] == '0'); }
+    { const char* fe = getenv("CHFPE_HERMITE_CONTIG"); op.contig = !(fe && fe[0] == '0'); }
     if (pa > 0) {
       const int ntA = (op.nq[0] + pa - 1) / pa;
       op.ntileB = (M == 3) ? (op.nq[1] + op.pb - 1) / op.pb : 1;

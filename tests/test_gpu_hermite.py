@@ -54,6 +54,7 @@ SMALL = [
     ("m1_compact6_256", ci.config("cfg2", nq=[256], np=[3], depth=2, scheme="compact6", mass=[1.3])),   # longest line
     ("m2_compact6", ci.config("cfg3s", nq=[23, 14], np=[3, 4], depth=2, scheme="compact6", mass=[1.0, 1.3])),
     ("m3_compact6", ci.config("cfg4s8", nq=[9, 12, 7], np=[3, 2, 3], depth=2, scheme="compact6")),
+    ("m2_compact6_contig64", ci.config("cfg3s", nq=[70, 40], np=[2, 3], depth=1, scheme="compact6")),   # 64-line tiles, ragged
     ("m3_compact6_5pt", ci.config("cfg4s8", nq=[5, 6, 5], np=[2, 2, 2], depth=3, scheme="compact6")),  # shortest lines
 ]
 
@@ -102,6 +103,19 @@ def test_every_stage_kernel_variant(var, val, monkeypatch):
         g.step(2, cfg["dt"]); o.step(2, cfg["dt"])
         assert rel_l2(g.export_state(), o.export_state()) < 1e-12
         g.close()
+
+
+def test_compact6_strided_kernel_on_the_contiguous_axis(monkeypatch):
+    """CHFPE_HERMITE_CONTIG=0: the one-thread-per-line kernel also serves the contiguous q axis (the fallback for axes
+    longer than 64 points or fewer than 64 lines)."""
+    monkeypatch.setenv("CHFPE_HERMITE_CONTIG", "0")
+    cfg = ci.config("cfg4s8", nq=[9, 12, 7], np=[3, 2, 3], depth=2, scheme="compact6")
+    g, o = both(cfg)
+    X = ci.seeded_hermite_state(cfg, [sum(n) for n in o.elems], seed=8)
+    g.import_state(X); o.import_state(X)
+    assert rel_l2(g.export_rhs(), o.rhs(o.c)) < 1e-13
+    g.step(2, cfg["dt"]); o.step(2, cfg["dt"])
+    assert rel_l2(g.export_state(), o.export_state()) < 1e-12
 
 
 def test_zero_steps_and_batch_slots_are_independent():
