@@ -38,13 +38,13 @@ BYTES_PER_VALUE_STEP_SURVEY = 128.0        # classical RK4, 4 ar
 HBM_NOMINAL_GBS = 8000.0                   # "about 8 TB/s", BASELINE.json north_star
 
 
-def profiled_traffic():
+def profiled_traffic(pattern="r*_stage_kernel_ncu_full.txt", key="dram_bytes_per_launch"):
     """DRAM bytes per launch of the stage kernel from the committed ncu --set full summary (profiles/), or None."""
     import glob
     import re
     best = None
-    for f in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_stage_kernel_ncu_full.txt"))):
-        m = re.search(r"^dram_bytes_per_launch=([0-9.eE+]+)", open(f).read(), flags=re.M)
+    for f in sorted(glob.glob(os.path.join(ROOT, "profiles", pattern))):
+        m = re.search(r"^%s=([0-9.eE+]+)" % key, open(f).read(), flags=re.M)
         if m:
             best = float(m.group(1))
     return best
@@ -438,7 +438,8 @@ def run_hermite(args):
                     "h2d_bytes_per_step": values * 8.0 / steps, "d2h_bytes_per_step": 8.0 * (steps + 1) / steps},
             "gpu_launches": int(launches), "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src, "kernel": kname, "kernel_ms": kern_ms,
+                         "traffic": profiled_traffic("r*_hermite_stage_ncu_full.txt", "dram_bytes_per_launch_hermite")
+                         if (wl == "cfg4h" and per_stage == 1) else None, "peak_source": peak_src, "kernel": kname, "kernel_ms": kern_ms,
                          "kernel_launches_timed": 4 * steps * per_stage,
                          "kernel_share_of_step": min(1.0, 4 * kern_ms / (ms / steps)),
                          "algorithmic_bytes_per_launch": values * 22.0}}

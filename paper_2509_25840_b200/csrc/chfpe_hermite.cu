@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(256) k_hermite_stage(const HOp op, const doubl
 // handling and the slab neighbourhood are worked out once per thread instead of once per value; the terms of the
 // last mode come from the thread's own column (KC + 2 centre values, each differentiated once); zero ghosts (R9) are
 // weights of 0 on loads redirected to the centre, so no load is predicated.  CTA-uniform: element, k_1..k_{M-1}, chunk.
-template <int M, int KC>
+template <int M, int KC, bool DER>
 __global__ void __launch_bounds__(256) k_hermite_stage_col(const HOp op, const double* __restrict__ in, const double* y,
                                                           double* out, const double a, const double c,
                                                           const size_t slot_stride) {
@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(256) k_hermite_stage_col(const HOp op, const d
       const int k = k0 - 1 + t;
       if (k >= 0 && k < kpM) {
         cc[t] = __ldg(p);
-        dcc[t] = w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4);
+        dcc[t] = DER ? w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4) : 0.0;
       } else {
         cc[t] = 0.0; dcc[t] = 0.0;
       }
@@ -208,8 +208,10 @@ __global__ void __launch_bounds__(256) k_hermite_stage_col(const HOp op, const d
       const double* p = in + (size_t)(up + k0) * Q + qi;
 #pragma unroll
       for (int j = 0; j < KC; j++) {
-        if (k0 + j < kpM)
-          acc[j] += f1 * __ldg(p) + f2 * (w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4));
+        if (k0 + j < kpM) {
+          if (DER) acc[j] += f1 * __ldg(p) + f2 * (w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4));
+          else acc[j] += f1 * __ldg(p);
+        }
         p += Q;
       }
     }
@@ -218,8 +220,10 @@ __global__ void __launch_bounds__(256) k_hermite_stage_col(const HOp op, const d
       const double* p = in + (size_t)(dn + k0) * Q + qi;
 #pragma unroll
       for (int j = 0; j < KC; j++) {
-        if (k0 + j < kpM)
-          acc[j] += f1 * __ldg(p) + f2 * (w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4));
+        if (k0 + j < kpM) {
+          if (DER) acc[j] += f1 * __ldg(p) + f2 * (w1 * __ldg(p + o1) + w2 * __ldg(p + o2) + w3 * __ldg(p + o3) + w4 * __ldg(p + o4));
+          else acc[j] += f1 * __ldg(p);
+        }
         p += Q;
       }
     }
@@ -763,6 +767,15 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
   const size_t ss = 3 * h->state_doubles;
   if (op.scheme == CHFPE_COMPACT6) {                 // pointwise terms, then one line pass per mode
     const dim3 g0 = slab_grid(op, nb);
+    if (op.kc > 0) {                                 // column kernel without the derivative terms (4 Hermite indices per thread)
+      const int nch = (op.kp[op.M - 1] + 3) / 4;
+      HOp o4 = op;
+      o4.nchunk = nch;
+      const dim3 gc((unsigned)((size_t)(op.nslab / op.kp[op.M - 1]) * nch * op.blocks_per_slab), (unsigned)nb);
+      if (op.M == 1) k_hermite_stage_col<1, 4, false><<<gc, op.threads, 0, h->stream>>>(o4, in, y, out, a, c, ss);
+      else if (op.M == 2) k_hermite_stage_col<2, 4, false><<<gc, op.threads, 0, h->stream>>>(o4, in, y, out, a, c, ss);
+      else k_hermite_stage_col<3, 4, false><<<gc, op.threads, 0, h->stream>>>(o4, in, y, out, a, c, ss);
+    } else
     switch (op.M) {
       case 1: k_hermite_stage<1, false><<<g0, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
       case 2: k_hermite_stage<2, false><<<g0, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss); break;
@@ -806,7 +819,7 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
   }
   if (op.kc > 0) {                                   // column kernel (M = 1)
     const dim3 g((unsigned)((size_t)(op.nslab / op.kp[op.M - 1]) * op.nchunk * op.blocks_per_slab), (unsigned)nb);
-#define HCOL(MM, KK) k_hermite_stage_col<MM, KK><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss)
+#define HCOL(MM, KK) k_hermite_stage_col<MM, KK, true><<<g, op.threads, 0, h->stream>>>(op, in, y, out, a, c, ss)
     if (op.kc == 8) { if (op.M == 1) HCOL(1, 8); else if (op.M == 2) HCOL(2, 8); else HCOL(3, 8); }
     else { if (op.M == 1) HCOL(1, 4); else if (op.M == 2) HCOL(2, 4); else HCOL(3, 4); }
 #undef HCOL
