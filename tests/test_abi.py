@@ -69,3 +69,26 @@ def test_create_rejects_bad_workspace_without_touching_the_gpu():
     h = C.c_void_p()
     rc = P.lib().chfpe_create(C.byref(d), None, 0, None, C.byref(h))
     assert rc == -2 and not h.value          # CHFPE_ERR_WORKSPACE
+
+
+def test_hermite_workspace_bytes_and_validation():
+    """Row f1 host logic without a GPU: workspace sizing (three state-sized arrays per slot + tables) and descriptor
+    validation of the chfpe_hermite_* entry points; create refuses a missing workspace before touching CUDA."""
+    import paper_2509_25840_b200 as P
+    from paper_2509_25840_b200 import binding
+    cfg = ci.config("cfg4h")
+    values = 20 * 8 ** 3 * 32 ** 3
+    for batch in (1, 3):
+        n = P.hermite_workspace_bytes(cfg, batch=batch)
+        assert 3 * batch * values * 8 <= n <= 3 * batch * values * 8 + (16 << 20)
+    assert P.hermite_workspace_bytes(ci.config("cfg4h", scheme="compact6")) >= 3 * values * 8
+    for bad in (dict(nq=[4, 32, 32]), dict(np=[0, 8, 8]), dict(depth=-1), dict(beta=0.0), dict(gamma=[0.0, 1.0, 1.0]),
+                dict(scheme="compact6", nq=[300, 32, 32])):
+        with pytest.raises(P.ChfpeError):
+            P.hermite_workspace_bytes(ci.config("cfg4h", **bad))
+    with pytest.raises(P.ChfpeError):
+        P.hermite_workspace_bytes(cfg, batch=0)
+    d, keep = binding.make_desc(binding._hermite_cfg(ci.config("cfg2", nq=[64], np=[8])))
+    h = C.c_void_p()
+    rc = P.lib().chfpe_hermite_create(C.byref(d), None, 0, None, C.byref(h))
+    assert rc == -2 and not h.value          # CHFPE_ERR_WORKSPACE
