@@ -49,6 +49,8 @@ struct HOp {                // device view of the operator, passed by value
   const double* sq;                   // sq[i] = sqrt(i), i = 0 .. kp_M
   int kc, nchunk;                     // column kernel: Hermite indices of the last mode per thread, chunks per column
   int pa, pb, ntileB, pthreads, pblocks;   // patch kernel: patch extents, q_2 tiles, threads and CTAs per slab
+  int tile;                           // 32^3 specialisation: 4 x 8 x 32 CTA tiles (CHFPE_HERMITE_TILE=0: 2 x 16 x 32)
+  int pcol;                           // patch kernel: slabs of one column walked by a CTA (1 or kp_M)
   double ca[3], cb[3];                // COMPACT6: 7/(9h), 1/(36h)
   const double* ibet[3];              // COMPACT6: reciprocal pivots and elimination factors of tridiag(1/3, 1, 1/3) per mode
   const double* cfac[3];
@@ -422,19 +424,31 @@ __global__ void __launch_bounds__(256, (PA * PB <= 4) ? 4 : 1) k_hermite_stage_p
                                                             const size_t slot_stride) {
   static_assert(M == 2 || M == 3, "patch kernel: two or three modes");
   static_assert(M == 3 || PB == 1, "two modes: one patched axis");
-  const int slab = blockIdx.x / op.pblocks;
-  const int t = (blockIdx.x - slab * op.pblocks) * blockDim.x + threadIdx.x;
+  // pcol > 1: a CTA walks the pcol slabs of one column (consecutive Hermite indices of the last mode) on its q tile, so
+  // the dU/dq_s values of the tile and two of the three lane-mode slabs (own, k_M - 1, k_M + 1) are re-read from L1
+  const int slab0 = (blockIdx.x / op.pblocks) * op.pcol;
+  const int slab = slab0;
+  const int t = (blockIdx.x - (blockIdx.x / op.pblocks) * op.pblocks) * blockDim.x + threadIdx.x;
   if (t >= op.pthreads) return;
   const int nL = FL ? FL : op.nq[M - 1];
   const int nA = FA ? FA : op.nq[0], nB = (M == 3) ? (FB ? FB : op.nq[1]) : 1;
   const int ntB = (M == 3) ? (FB ? (FB + PB - 1) / PB : op.ntileB) : 1;
   const int r = t / nL, iL = t - r * nL;
-  const int tb = (M == 3) ? r % ntB : 0, ta = (M == 3) ? r / ntB : r;
+  int tb = (M == 3) ? r % ntB : 0, ta = (M == 3) ? r / ntB : r;
+  if (M == 3 && FL == 32 && FB == 32 && FA == 32 && PA == 2 && PB == 2 && op.tile) {
+    // 32^3 mesh, 2 x 2 patches: the 8 warps of a CTA form a 2 x 4 block of patches = a 4 x 8 x 32 tile of the mesh instead
+    // of 2 x 16 x 32, which costs 4 + 3 instead of 6 + 2.5 slab-units of L2 -> SM traffic for the q_1 / q_2 windows
+    const int cta = blockIdx.x - (blockIdx.x / op.pblocks) * op.pblocks, w = threadIdx.x >> 5;
+    ta = (cta >> 2) * 2 + (w >> 2);
+    tb = (cta & 3) * 4 + (w & 3);
+  }
   const int a0 = ta * PA, b0 = tb * PB;
   const size_t soff = (size_t)blockIdx.y * slot_stride;
   const bool interior = a0 >= 2 && a0 + PA + 2 <= nA && (M == 2 || (b0 >= 2 && b0 + PB + 2 <= nB));
-  if (interior) hermite_patch_body<M, PA, PB, FA, FB, FL, true>(op, in + soff, y, out, a, c, soff, slab, a0, b0, iL);
-  else hermite_patch_body<M, PA, PB, FA, FB, FL, false>(op, in + soff, y, out, a, c, soff, slab, a0, b0, iL);
+  for (int kk = 0; kk < op.pcol; kk++) {
+    if (interior) hermite_patch_body<M, PA, PB, FA, FB, FL, true>(op, in + soff, y, out, a, c, soff, slab + kk, a0, b0, iL);
+    else hermite_patch_body<M, PA, PB, FA, FB, FL, false>(op, in + soff, y, out, a, c, soff, slab + kk, a0, b0, iL);
+  }
 }
 
 // COMPACT6 (the paper's q-derivative, Eq. 25-31, a = 7/9 by reading R4): for one mode s, every slab
@@ -805,7 +819,7 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
     return;
   }
   if (op.pa > 0) {                                   // patch kernel (default for M >= 2)
-    const dim3 g((unsigned)((size_t)op.nslab * op.pblocks), (unsigned)nb);
+    const dim3 g((unsigned)((size_t)(op.nslab / op.pcol) * op.pblocks), (unsigned)nb);
 #define HPATCH(MM, A, B, FA, FB, FL) k_hermite_stage_patch<MM, A, B, FA, FB, FL><<<g, 256, 0, h->stream>>>(op, in, y, out, a, c, ss)
     const bool cube32 = op.M == 3 && op.nq[0] == 32 && op.nq[1] == 32 && op.nq[2] == 32 && op.fixed;
     if (op.M == 2) { if (op.pa == 4) HPATCH(2, 4, 1, 0, 0, 0); else HPATCH(2, 2, 1, 0, 0, 0); }
@@ -1073,6 +1087,8 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
     if (e && *e) pa = 0;                             // an explicit column / per-value request wins
     op.pa = pa; op.pb = (M == 3) ? pb : 1;
     { const char* fe = getenv("CHFPE_HERMITE_FIXED"); op.fixed = !(fe && fe[0] == '0'); }
+    { const char* fe = getenv("CHFPE_HERMITE_TILE"); op.tile = !(fe && fe[0] == '0'); }
+    { const char* fe = getenv("CHFPE_HERMITE_PCOL"); op.pcol = (fe && fe[0] == '0') ? 1 : op.kp[M - 1]; }
     { const char* fe = getenv("CHFPE_HERMITE_CONTIG"); op.contig = !(fe && fe[0] == '0'); }
     if (pa > 0) {
       const int ntA = (op.nq[0] + pa - 1) / pa;

@@ -86,11 +86,12 @@ def test_rhs_step_kick_expect(name, cfg):
 @pytest.mark.parametrize("var,val", [("CHFPE_HERMITE_KC", "0"), ("CHFPE_HERMITE_KC", "4"), ("CHFPE_HERMITE_KC", "8"),
                                      ("CHFPE_HERMITE_PATCH", "44"), ("CHFPE_HERMITE_PATCH", "42"),
                                      ("CHFPE_HERMITE_PATCH", "24"), ("CHFPE_HERMITE_PATCH", "22"),
-                                     ("CHFPE_HERMITE_PATCH", "0")])
+                                     ("CHFPE_HERMITE_PATCH", "0"), ("CHFPE_HERMITE_PCOL", "0")])
 def test_every_stage_kernel_variant(var, val, monkeypatch):
     """CHFPE_HERMITE_KC: 0 = one thread per value, 4 / 8 = column kernel with that many Hermite indices of the last
     mode per thread (columns longer and shorter than a chunk, ragged last chunks, kp = 1).  CHFPE_HERMITE_PATCH = "AB":
-    patch kernel with A x B points of (q_1, q_2) per thread (ragged patches, axes shorter than a patch + halo)."""
+    patch kernel with A x B points of (q_1, q_2) per thread (ragged patches, axes shorter than a patch + halo);
+    CHFPE_HERMITE_PCOL=0: one slab per CTA instead of a walk over the column of the last Hermite index."""
     monkeypatch.setenv(var, val)
     for cfg in (ci.config("cfg2", nq=[37], np=[11], depth=4),
                 ci.config("cfg3s", nq=[40, 37], np=[3, 9], depth=2, mass=[1.0, 1.3]),
@@ -267,9 +268,19 @@ def test_full_size_rhs_on_an_embedded_block():
     blk = (slice(None),) * 4 + tuple(slice(off[s], off[s] + ext[s]) for s in range(3))
     X[blk] = torch.from_numpy(Xs).cuda()
     g.import_state(X)
-    del X
     F = g.export_rhs_device()[blk].cpu().numpy()
-    assert rel_l2(F, o.rhs(Xs)) < 1e-13
+    Fo = o.rhs(Xs)
+    assert rel_l2(F, Fo) < 1e-13
+    for var in ("CHFPE_HERMITE_TILE", "CHFPE_HERMITE_FIXED", "CHFPE_HERMITE_PCOL"):   # the other launch shapes at this size
+        os.environ[var] = "0"
+        try:
+            g2 = P().Hermite(cfg)
+        finally:
+            del os.environ[var]
+        g2.import_state(X)
+        assert rel_l2(g2.export_rhs_device()[blk].cpu().numpy(), Fo) < 1e-13, var
+        g2.close()
+    del X
     # one RK4 step at full size is four launches of the stage kernel and nothing else
     n0 = g.launch_count()
     g.step(1, cfg["dt"])
