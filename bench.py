@@ -298,10 +298,11 @@ def run_2d(args):
     import numpy as np
     import torch
     import paper_2509_25840_b200 as P
-    wl = args.workload if args.workload != "cfg4" else "cfg5"
-    cfg = ci.config(wl)
+    herm = args.representation == "hermite"             # row f1: the same protocol on the Hermite representation (cfg4h)
+    wl = args.workload if args.workload != "cfg4" else ("cfg4h" if herm else "cfg5")
+    cfg = ci.config(wl, scheme=args.scheme) if herm else ci.config(wl)
     M = cfg["n_modes"]
-    g = P.CHFPE(cfg, batch=args.batch)
+    g = P.Hermite(cfg, batch=args.batch) if herm else P.CHFPE(cfg, batch=args.batch)
     mu, al = obs(P, "mu", M), obs(P, "alpha", M)
     g.equilibrate(residual=False)
     n1, n2 = args.n1, args.n2
@@ -320,13 +321,15 @@ def run_2d(args):
     full = 63 + 64 * 255
     line = {"metric": "2D THz-Raman wall time", "value": sec * full / rsteps, "unit": "s", "higher_is_better": False,
             "n_gpus": 1, "dtype": "f64", "data": "synthetic", "extrapolated": True,
-            "config": {"workload": wl + " response_2d", "grid": "x".join(str(x) for x in g.shape), "K": g.K,
-                       "batch_slots": args.batch, "workspace_GB": P.workspace_bytes(cfg, args.batch) / 1e9,
+            "config": {"workload": wl + (" chfpe_hermite_response_2d" if herm else " response_2d"),
+                       "grid": "x".join(str(x) for x in g.shape), "K": g.K, "batch_slots": args.batch,
+                       "workspace_GB": (P.hermite_workspace_bytes(cfg, args.batch) if herm
+                                        else P.workspace_bytes(cfg, args.batch)) / 1e9,
                        "timed_sample": "%d t1 x %d t2 delays, stride 1, A=mu B=alpha C=alpha" % (n1, n2),
                        "full_protocol": "64 t1 x 256 t2 (16383 replica-steps), linear extrapolation in replica-steps"},
             "sample_seconds": sec, "replica_steps_timed": rsteps, "ms_per_replica_step": 1e3 * sec / rsteps,
-            "cell_updates_per_s": g.cells * rsteps / sec, "gpu_launches": int(g.launch_count() - n0),
-            "finite": bool(np.all(np.isfinite(R)))}
+            ("value_updates_per_s" if herm else "cell_updates_per_s"): (g.values if herm else g.cells) * rsteps / sec,
+            "gpu_launches": int(g.launch_count() - n0), "finite": bool(np.all(np.isfinite(R)))}
     print(json.dumps(line))
     g.close()
     return 0
@@ -483,10 +486,10 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
-    if args.representation == "hermite":
-        return run_hermite(args)
     if args.protocol == "2d":
         return run_2d(args)
+    if args.representation == "hermite":
+        return run_hermite(args)
     if args.protocol == "3d":
         return run_3d(args)
     return run_ours(args)
