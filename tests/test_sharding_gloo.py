@@ -72,3 +72,43 @@ def test_response_2d_sharded_world2(tmp_path):
         R3 = np.load(tmp_path / ("R3_%d.npy" % r))
         assert R3.shape == full3.shape == (3, 2, 2)
         assert np.max(np.abs(R3 - full3)) <= 1e-14 * np.max(np.abs(full3))
+
+
+HCFG = ci.config("cfg3s", nq=[9, 8], np=[3, 3], depth=2)
+
+
+def _hermite_worker(rank, world, port, out):
+    """Row f1: the same helper with a Hermite-representation engine (here its numpy oracle; on GPUs
+    paper_2509_25840_b200.Hermite, whose response_2d has the same signature)."""
+    import torch.distributed as dist
+    from oracle import hermite
+    from paper_2509_25840_b200 import sharding
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        o = hermite.RefHermite(HCFG)
+        o.equilibrate()
+        mu, al = ci.observable("mu", 2), ci.observable("alpha", 2)
+        R = sharding.response_2d_sharded(o, mu, al, al, T1, T2, 10 * HCFG["dt"])
+        np.save(os.path.join(out, "H%d.npy" % rank), R)
+    finally:
+        dist.destroy_process_group()
+
+
+def test_hermite_response_2d_sharded_world2(tmp_path):
+    import torch.multiprocessing as mp
+    from oracle import hermite
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mp.spawn(_hermite_worker, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    o = hermite.RefHermite(HCFG)
+    o.equilibrate()
+    mu, al = ci.observable("mu", 2), ci.observable("alpha", 2)
+    full = o.response_2d(mu, al, al, T1, T2, 10 * HCFG["dt"])
+    assert np.max(np.abs(full)) > 0
+    for r in range(2):
+        R = np.load(tmp_path / ("H%d.npy" % r))
+        assert R.shape == full.shape
+        assert np.max(np.abs(R - full)) <= 1e-14 * np.max(np.abs(full))
