@@ -206,6 +206,32 @@ class RefHermite:
             self.c = saved
         return R
 
+    def response_3d(self, A, B, Cobs, D, t1_steps, t2_steps, t3_steps, dt):
+        """Literal Eq. (17) PAPER.md:126-127 (section IV.C.3 :239-241): R[k][j][l] = <D> after kick A, t1_k, kick B, t2_j,
+        kick C, t3_l; plain triple loop with the two trajectories saved and restored."""
+        self.kick(A)
+        R = np.empty((len(t1_steps), len(t2_steps), len(t3_steps)))
+        now1 = 0
+        for k, s1 in enumerate(t1_steps):
+            self.step(s1 - now1, dt)
+            now1 = s1
+            T1 = self.c.copy()
+            self.kick(B)
+            now2 = 0
+            for j, s2 in enumerate(t2_steps):
+                self.step(s2 - now2, dt)
+                now2 = s2
+                T2 = self.c.copy()
+                self.kick(Cobs)
+                now3 = 0
+                for l, s3 in enumerate(t3_steps):
+                    self.step(s3 - now3, dt)
+                    now3 = s3
+                    R[k, j, l] = self.expect(D)
+                self.c = T2
+            self.c = T1
+        return R
+
     def export_state(self):
         return self.c.copy()
 

@@ -166,3 +166,29 @@ def test_compact6_closed_form_response():
         err[(scheme, n)] = abs(-R[1] - exact)
     assert err[("compact6", 37)] < 0.1 * err[("central4", 37)]
     assert err[("compact6", 73)] < err[("compact6", 37)] / 30.0 or err[("compact6", 73)] < 1e-9
+
+
+def test_third_order_closed_forms():
+    """Pin P4b on the Hermite oracle (Eq. 17, harmonic + LL model, c = R_phys): A = D = q, B = C = q^2 gives
+    -4 c(t1) c(t2) c(t3); A = B = q, C = D = q^2 gives -4 c(t3) [c(t2) c(t1+t2+t3) + c(t2+t3) c(t1+t2)] (not symmetric in
+    the delays: pins the operator order and the time arguments).  Compact scheme on the h = 0.5 mesh."""
+    def c(t):
+        return scipy.linalg.expm(t * bo_matrix())[0, 1]
+    dt = 5e-3
+    t1s, t2s, t3s = [0, 100], [60, 140], [0, 80, 180]
+    mu, al = ci.observable("mu", 1), ci.observable("alpha", 1)
+    cfg = dict(harmonic(37, kp=6, depth=4), scheme="compact6")
+    res = {}
+    for name, ops in (("a", (mu, al, al, mu)), ("b", (mu, mu, al, al))):
+        o = hermite.RefHermite(cfg)
+        o.equilibrate()
+        res[name] = o.response_3d(*ops, t1s, t2s, t3s, dt)
+    worst = 0.0
+    for k, a in enumerate(t1s):
+        for j, b in enumerate(t2s):
+            for l, d in enumerate(t3s):
+                a_, b_, d_ = a * dt, b * dt, d * dt
+                worst = max(worst, abs(res["a"][k, j, l] + 4 * c(a_) * c(b_) * c(d_)),
+                            abs(res["b"][k, j, l] + 4 * c(d_) * (c(b_) * c(a_ + b_ + d_) + c(b_ + d_) * c(a_ + b_))))
+    assert worst < 3e-4, worst                                   # 1e-4 of the largest value (3.2) on the h = 0.5 mesh
+    assert abs(res["a"][1, 1, 2]) > 0.8 and abs(res["b"][1, 1, 2]) > 3.0
