@@ -205,6 +205,13 @@ int chfpe_hermite_response_1d(chfpe_hermite_handle* h, const chfpe_observable* A
 int chfpe_hermite_response_2d(chfpe_hermite_handle* h, const chfpe_observable* A, const chfpe_observable* B,
                               const chfpe_observable* C, const int64_t* t1_steps, int32_t n1, const int64_t* t2_steps,
                               int32_t n2, double dt, double* R);
+/* Same protocol as chfpe_response_3d (literal Eq. 17 :126-127; R row-major [n1][n2][n3]): slot 0 = t1 trajectory, a group
+   of nb = (batch-1)/2 t1 samples (batch-1 if n2 == 1) owns nb slots for its t2 trajectories and nb for the t3 replicas.
+   CHFPE_ERR_INVALID if nb < 1 or nb*n3 exceeds the 65536-entry results buffer. */
+int chfpe_hermite_response_3d(chfpe_hermite_handle* h, const chfpe_observable* A, const chfpe_observable* B,
+                              const chfpe_observable* C, const chfpe_observable* D, const int64_t* t1_steps, int32_t n1,
+                              const int64_t* t2_steps, int32_t n2, const int64_t* t3_steps, int32_t n3, double dt,
+                              double* R);
 /* K * prod(np) * prod(nq) doubles; dst/src: device if *_is_device, else host. */
 int chfpe_hermite_export_state(chfpe_hermite_handle* h, int32_t replica, double* dst, int dst_is_device);
 int chfpe_hermite_import_state(chfpe_hermite_handle* h, int32_t replica, const double* src, int src_is_device);

@@ -13,7 +13,7 @@ EXPORTED_SYMBOLS = [
     "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_spectrum_1d", "chfpe_spectrum_2d", "chfpe_last_error",
     "chfpe_hermite_workspace_bytes", "chfpe_hermite_create", "chfpe_hermite_destroy", "chfpe_hermite_num_elements",
     "chfpe_hermite_equilibrate", "chfpe_hermite_step", "chfpe_hermite_kick", "chfpe_hermite_expect",
-    "chfpe_hermite_response_1d", "chfpe_hermite_response_2d", "chfpe_hermite_export_state",
+    "chfpe_hermite_response_1d", "chfpe_hermite_response_2d", "chfpe_hermite_response_3d", "chfpe_hermite_export_state",
     "chfpe_hermite_import_state", "chfpe_hermite_export_rhs", "chfpe_hermite_launch_count", "chfpe_hermite_last_error",
 ]
 
@@ -96,6 +96,8 @@ def lib():
     L.chfpe_hermite_expect.argtypes = [vp, C.c_int32, op, dp]
     L.chfpe_hermite_response_1d.argtypes = [vp, op, op, C.c_int64, C.c_int64, C.c_double, dp]
     L.chfpe_hermite_response_2d.argtypes = [vp, op, op, op, i64p, C.c_int32, i64p, C.c_int32, C.c_double, dp]
+    L.chfpe_hermite_response_3d.argtypes = [vp, op, op, op, op, i64p, C.c_int32, i64p, C.c_int32, i64p, C.c_int32,
+                                            C.c_double, dp]
     L.chfpe_hermite_export_state.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_hermite_import_state.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_hermite_export_rhs.argtypes = [vp, C.c_int32, vp, C.c_int]
@@ -426,6 +428,17 @@ class Hermite:
                                                  t1.ctypes.data_as(C.POINTER(C.c_int64)), len(t1),
                                                  t2.ctypes.data_as(C.POINTER(C.c_int64)), len(t2), dt,
                                                  R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_hermite_response_2d")
+        return R
+
+    def response_3d(self, A, B, Cobs, D, t1_steps, t2_steps, t3_steps, dt):
+        """R[k][j][l] of Eq. (17); needs batch >= 3 (batch >= 2 for a single t2 sample)."""
+        ts = [np.ascontiguousarray(t, dtype=np.int64) for t in (t1_steps, t2_steps, t3_steps)]
+        R = np.empty(tuple(len(t) for t in ts))
+        args = []
+        for t in ts:
+            args += [t.ctypes.data_as(C.POINTER(C.c_int64)), len(t)]
+        self._ck(lib().chfpe_hermite_response_3d(self._h, C.byref(A), C.byref(B), C.byref(Cobs), C.byref(D), *args, dt,
+                                                 R.ctypes.data_as(C.POINTER(C.c_double))), "chfpe_hermite_response_3d")
         return R
 
     def export_state(self, replica=0):

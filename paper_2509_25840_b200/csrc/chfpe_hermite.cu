@@ -1243,6 +1243,71 @@ extern "C" int chfpe_hermite_response_2d(chfpe_hermite_handle* h, const chfpe_ob
   return fetch_results(h, (long long)(k - row0) * n2, R + (size_t)row0 * n2);
 }
 
+// Third-order response, literal Eq. (17) PAPER.md:126-127 (section IV.C.3 :239-241).  Slot 0 carries the t1 trajectory; a
+// group of nb t1 samples owns slots [1, 1+nb) for its t2 trajectories and, unless the t2 sample is the last one (then
+// C is applied in place), slots [1+nb, 1+2nb) for the t3 replicas; all replicas of a group advance together (grid.y).
+extern "C" int chfpe_hermite_response_3d(chfpe_hermite_handle* h, const chfpe_observable* A, const chfpe_observable* B,
+                                         const chfpe_observable* C, const chfpe_observable* D, const int64_t* t1,
+                                         int32_t n1, const int64_t* t2, int32_t n2, const int64_t* t3, int32_t n3,
+                                         double dt, double* R) {
+  if (!h || !A || !B || !C || !D || !t1 || !t2 || !t3 || !R || n1 < 1 || n2 < 1 || n3 < 1) return CHFPE_ERR_INVALID;
+  if (!h->initialised) HFAIL(h, CHFPE_ERR_STATE, "response_3d before equilibrate/import");
+  const int nb_max = (n2 == 1) ? h->batch - 1 : (h->batch - 1) / 2;
+  if (nb_max < 1) HFAIL(h, CHFPE_ERR_INVALID, "response_3d needs batch >= 3 (batch >= 2 if n2 == 1)");
+  int rc = check_steps(h, t1, n1, "t1_steps");
+  if (rc) return rc;
+  rc = check_steps(h, t2, n2, "t2_steps");
+  if (rc) return rc;
+  rc = check_steps(h, t3, n3, "t3_steps");
+  if (rc) return rc;
+  if ((long long)nb_max * n3 > RESULTS) HFAIL(h, CHFPE_ERR_INVALID, "replicas * n3 too large for the results buffer");
+  const size_t sbytes = sizeof(double) * h->state_doubles;
+  std::vector<double> tmp((size_t)nb_max * n3);
+  rc = kick_slots(h, 0, 1, A);
+  if (rc) return rc;
+  int64_t now1 = 0;
+  for (int k = 0; k < n1;) {
+    int nb = n1 - k;
+    if (nb > nb_max) nb = nb_max;
+    for (int b = 0; b < nb; b++) {
+      rc = step_slots(h, 0, 1, t1[k + b] - now1, dt);
+      if (rc) return rc;
+      now1 = t1[k + b];
+      HCU(h, cudaMemcpyAsync(h->y(1 + b), h->y(0), sbytes, cudaMemcpyDeviceToDevice, h->stream));
+    }
+    rc = kick_slots(h, 1, nb, B);
+    if (rc) return rc;
+    int64_t now2 = 0;
+    for (int j = 0; j < n2; j++) {
+      rc = step_slots(h, 1, nb, t2[j] - now2, dt);
+      if (rc) return rc;
+      now2 = t2[j];
+      int rep = 1;                                   // last t2 sample: the t2 trajectories are not needed again
+      if (j + 1 < n2) {
+        rep = 1 + nb;
+        for (int b = 0; b < nb; b++)
+          HCU(h, cudaMemcpyAsync(h->y(rep + b), h->y(1 + b), sbytes, cudaMemcpyDeviceToDevice, h->stream));
+      }
+      rc = kick_slots(h, rep, nb, C);
+      if (rc) return rc;
+      int64_t now3 = 0;
+      for (int l = 0; l < n3; l++) {
+        rc = step_slots(h, rep, nb, t3[l] - now3, dt);
+        if (rc) return rc;
+        now3 = t3[l];
+        rc = expect_slots(h, rep, nb, 0, D, l, n3);
+        if (rc) return rc;
+      }
+      rc = fetch_results(h, (long long)nb * n3, tmp.data());
+      if (rc) return rc;
+      for (int b = 0; b < nb; b++)
+        for (int l = 0; l < n3; l++) R[((size_t)(k + b) * n2 + j) * n3 + l] = tmp[(size_t)b * n3 + l];
+    }
+    k += nb;
+  }
+  return CHFPE_OK;
+}
+
 extern "C" int chfpe_hermite_export_state(chfpe_hermite_handle* h, int32_t replica, double* dst, int dst_is_device) {
   if (!h || !dst || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
   HCU(h, cudaMemcpyAsync(dst, h->y(replica), sizeof(double) * h->state_doubles,

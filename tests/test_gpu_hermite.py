@@ -224,6 +224,30 @@ def test_response_2d_batched_over_t1(batch):
     assert np.array_equal(Rg[1], Rg[2])              # repeated t1 sample
 
 
+@pytest.mark.parametrize("batch,n2", [(3, 2), (5, 3), (4, 1), (2, 1)])
+def test_response_3d_batched(batch, n2):
+    """Eq. (17): groups of (batch-1)/2 t1 samples (batch-1 for a single waiting time), ragged last group, repeated and
+    zero delays, against the plain triple loop of the oracle."""
+    cfg = ci.config("cfg3s", nq=[10, 9], np=[4, 3], depth=2, scheme="compact6" if batch == 5 else "central4")
+    g, o = both(cfg, batch=batch)
+    g.equilibrate(); o.equilibrate()
+    mu, al, nl = ci.observable("mu", 2), ci.observable("alpha", 2), ci.observable("mu_nl", 2)
+    t1, t2, t3 = [0, 2, 5], [1, 3, 3][:n2], [0, 2, 3]
+    Rg = g.response_3d(gobs(mu), gobs(nl), gobs(al), gobs(nl), t1, t2, t3, 5e-2)
+    Ro = o.response_3d(mu, nl, al, nl, t1, t2, t3, 5e-2)
+    assert Rg.shape == (3, n2, 3) and np.max(np.abs(Ro)) > 1e-3
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+
+
+def test_response_3d_needs_slots():
+    cfg = ci.config("cfg2", nq=[16], np=[3], depth=1)
+    g = P().Hermite(cfg, batch=2)
+    g.equilibrate()
+    mu = gobs(ci.observable("mu", 1))
+    with pytest.raises(P().ChfpeError):
+        g.response_3d(mu, mu, mu, mu, [0], [0, 1], [0], 1e-3)
+
+
 def test_closed_forms_on_the_cuda_path():
     """The pins of the oracle hold for the CUDA path on its own: Brownian-oscillator R1 (tests/golden/bo_response_cfg1.txt,
     literal Eq. 15 = -R_phys) and the 2D closed form 2 R_phys(t1) R_phys(t2) (tests/golden/r2_closed_form.txt)."""
