@@ -343,10 +343,11 @@ def run_3d(args):
     import numpy as np
     import torch
     import paper_2509_25840_b200 as P
-    wl = args.workload
-    cfg = ci.config(wl)
+    herm = args.representation == "hermite"             # row f1: chfpe_hermite_response_3d on cfg4h
+    wl = args.workload if not (herm and args.workload == "cfg4") else "cfg4h"
+    cfg = ci.config(wl, scheme=args.scheme) if herm else ci.config(wl)
     M = cfg["n_modes"]
-    g = P.CHFPE(cfg, batch=args.batch)
+    g = P.Hermite(cfg, batch=args.batch) if herm else P.CHFPE(cfg, batch=args.batch)
     mu = obs(P, "mu_nl", M)
     g.equilibrate(residual=False)
     n1, n3, wait = args.n1, args.n2, 4
@@ -365,12 +366,14 @@ def run_3d(args):
     line = {"metric": "third-order response replica-steps/s", "value": rsteps / sec, "unit": "replica-steps/s",
             "higher_is_better": True, "n_gpus": 1, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl + " response_3d", "grid": "x".join(str(x) for x in g.shape), "K": g.K,
-                       "batch_slots": args.batch, "workspace_GB": P.workspace_bytes(cfg, args.batch) / 1e9,
+                       "batch_slots": args.batch,
+                       "workspace_GB": (P.hermite_workspace_bytes(cfg, args.batch) if herm
+                                        else P.workspace_bytes(cfg, args.batch)) / 1e9,
                        "timed_sample": "%d t1 x 1 t2 (%d steps) x %d t3 delays, stride 1, A=B=C=D=mu (nonlinear)"
                                        % (n1, wait, n3)},
             "sample_seconds": sec, "replica_steps_timed": rsteps, "ms_per_replica_step": 1e3 * sec / rsteps,
-            "cell_updates_per_s": g.cells * rsteps / sec, "gpu_launches": int(g.launch_count() - n0),
-            "finite": bool(np.all(np.isfinite(R)))}
+            ("value_updates_per_s" if herm else "cell_updates_per_s"): (g.values if herm else g.cells) * rsteps / sec,
+            "gpu_launches": int(g.launch_count() - n0), "finite": bool(np.all(np.isfinite(R)))}
     print(json.dumps(line))
     g.close()
     return 0
@@ -488,6 +491,8 @@ def main():
         return run_reference(args)
     if args.protocol == "2d":
         return run_2d(args)
+    if args.protocol == "3d":
+        return run_3d(args)
     if args.representation == "hermite":
         return run_hermite(args)
     if args.protocol == "3d":
