@@ -105,3 +105,26 @@ def test_absorption_spectrum_in_the_papers_scheme_end_to_end():
     exact = om * (-chi.imag)
     assert np.max(np.abs(Ig - exact)) < 2e-4 * np.max(np.abs(exact))
     g.close()
+
+
+def test_two_dimensional_spectrum_chain_on_the_hermite_path():
+    """Section IV.C.2 end to end on the CUDA path, two coupled anharmonic modes in the paper's scheme: batched
+    chfpe_hermite_response_2d (Eq. 16, TRT ordering A = mu, B = alpha, C = mu) -> chfpe_spectrum_2d (Eq. 20), against
+    the same chain on the oracles (oracle/hermite.py -> oracle/spectra.py)."""
+    from oracle import hermite
+    P = gpu_mod()
+    cfg = ci.config("cfg3s", nq=[14, 12], np=[4, 4], depth=2, scheme="compact6")
+    g, o = P.Hermite(cfg, batch=4), hermite.RefHermite(cfg)
+    g.equilibrate(); o.equilibrate()
+    mu, al = ci.observable("mu", 2), ci.observable("alpha", 2)
+    stride, dt = 4, 2e-2
+    t1, t2 = [stride * i for i in range(7)], [stride * i for i in range(9)]
+    Rg = g.response_2d(make_obs(P, mu), make_obs(P, al), make_obs(P, mu), t1, t2, dt)
+    Ro = o.response_2d(mu, al, mu, t1, t2, dt)
+    assert np.max(np.abs(Ro)) > 1e-2
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    om1, om2 = _omega(6, 2.0, 1), _omega(8, 2.0, 2)
+    Ig = P.spectrum_2d(Rg, stride * dt, stride * dt, om1, om2)
+    Io = spectra.spectrum_2d(Ro, stride * dt, stride * dt, om1, om2)
+    assert np.max(np.abs(Ig - Io)) <= 1e-8 * np.max(np.abs(Io))
+    g.close()
