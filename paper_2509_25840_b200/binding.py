@@ -353,7 +353,7 @@ class Hermite:
     """One chfpe_hermite_* handle (row f1: Hermite functions in the momenta, cfg["np"] = functions per mode).
     State arrays have the shape (K, kp_1..kp_M, nq_1..nq_M).  The workspace is a torch uint8 CUDA tensor."""
 
-    def __init__(self, cfg, batch=1, device="cuda:0", stream=None):
+    def __init__(self, cfg, batch=1, device="cuda:0", stream=None, guard_bytes=0):
         import torch
         if not torch.cuda.is_available():
             raise ChfpeError("CUDA device required: the CHFPE path has no CPU fallback")
@@ -364,9 +364,14 @@ class Hermite:
         d, keep = make_desc(cfg, batch)
         nbytes = hermite_workspace_bytes(cfg, batch)
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            # guard_bytes > 0 (tests): canary bytes on both sides of the workspace, checked by guards_intact()
+            self._guard = int(guard_bytes)
+            self.workspace = torch.full((nbytes + 256 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=self.device) \
+                if self._guard else torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            aligned = (self.workspace.data_ptr() + 255) & ~255
+            aligned = (self.workspace.data_ptr() + self._guard + 255) & ~255
+            self._ws_lo = aligned - self.workspace.data_ptr()
+            self._ws_hi = self._ws_lo + nbytes
             self._h = C.c_void_p()
             rc = L.chfpe_hermite_create(C.byref(d), C.c_void_p(aligned), nbytes, C.c_void_p(self.stream.cuda_stream),
                                         C.byref(self._h))
@@ -382,6 +387,12 @@ class Hermite:
     def _ck(self, rc, what):
         if rc != 0:
             raise ChfpeError("%s: %d %s" % (what, rc, lib().chfpe_hermite_last_error(self._h).decode()))
+
+    def guards_intact(self):
+        """True if no byte outside [workspace, workspace + workspace_bytes) was written (needs guard_bytes > 0)."""
+        self._torch.cuda.synchronize(self.device)
+        w = self.workspace
+        return bool((w[: self._ws_lo] == 0xA5).all().item() and (w[self._ws_hi:] == 0xA5).all().item())
 
     def close(self):
         if getattr(self, "_h", None):

@@ -248,6 +248,34 @@ def test_response_3d_needs_slots():
         g.response_3d(mu, mu, mu, mu, [0], [0, 1], [0], 1e-3)
 
 
+@pytest.mark.parametrize("scheme", ["central4", "compact6"])
+def test_no_entry_point_writes_outside_the_workspace(scheme, monkeypatch):
+    """Canary bytes on both sides of the caller-owned workspace survive every entry point of every stage-kernel family
+    (ragged meshes, all slots in use)."""
+    for var, val in ((None, None), ("CHFPE_HERMITE_KC", "0"), ("CHFPE_HERMITE_KC", "8"), ("CHFPE_HERMITE_PATCH", "44"),
+                     ("CHFPE_HERMITE_CONTIG", "0")):
+        if var:
+            monkeypatch.setenv(var, val)
+        for cfg in (ci.config("cfg2", nq=[37], np=[5], depth=3, scheme=scheme),
+                    ci.config("cfg4s8", nq=[9, 11, 7], np=[3, 2, 5], depth=2, scheme=scheme)):
+            M = cfg["n_modes"]
+            g = P().Hermite(cfg, batch=3, guard_bytes=1 << 16)
+            mu, al = gobs(ci.observable("mu", M)), gobs(ci.observable("alpha", M))
+            g.equilibrate(2, cfg["dt"])
+            g.kick(mu); g.step(2, cfg["dt"]); g.expect(al); g.export_rhs(2)
+            g.equilibrate()
+            g.response_1d(mu, mu, 3, 2, cfg["dt"])
+            g.equilibrate()
+            g.response_2d(mu, al, al, [0, 1, 2], [0, 2], cfg["dt"])
+            g.equilibrate()
+            g.response_3d(mu, al, al, mu, [0, 1], [1, 2], [0, 1], cfg["dt"])
+            g.import_state(g.export_state(1), replica=2)
+            assert g.guards_intact(), (var, val, cfg["name"])
+            g.close()
+        if var:
+            monkeypatch.delenv(var)
+
+
 def test_closed_forms_on_the_cuda_path():
     """The pins of the oracle hold for the CUDA path on its own: Brownian-oscillator R1 (tests/golden/bo_response_cfg1.txt,
     literal Eq. 15 = -R_phys) and the 2D closed form 2 R_phys(t1) R_phys(t2) (tests/golden/r2_closed_form.txt)."""
