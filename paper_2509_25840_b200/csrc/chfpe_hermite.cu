@@ -378,7 +378,22 @@ __device__ __forceinline__ void hermite_patch_body(const HOp& op, const double* 
     const double a2 = op.a2[s], a1f = op.a1f[s];
     const double w1 = (i + 1 < n) ? -a2 * op.c1[s] : 0.0, w2 = (i >= 1) ? a2 * op.c1[s] : 0.0;
     const double w3 = (i + 2 < n) ? -a2 * op.c2[s] : 0.0, w4 = (i >= 2) ? a2 * op.c2[s] : 0.0;
-    if (up >= 0 || dn >= 0) {
+    if (FL == 32 && (up >= 0 || dn >= 0)) {
+      // 32-point lane axis: a warp is one row, so the four neighbours of P = su*up + sd*dn are the neighbour lanes
+      // (warp shuffles instead of eight more loads; the ghost weights w1..w4 zero what a row end would pick up)
+#pragma unroll
+      for (int ia = 0; ia < PA; ia++)
+#pragma unroll
+        for (int ib = 0; ib < PB; ib++)
+          if (INT || (ia < na && ib < nb)) {                     // warp-uniform: na, nb depend on the patch only
+            const int o = ia * stA + ib * stB;
+            const double u0 = __ldg(pu + o), d0 = __ldg(pd + o);
+            const double Pc = su * u0 + sd * d0;
+            const double p1 = __shfl_down_sync(0xffffffffu, Pc, 1), m1 = __shfl_up_sync(0xffffffffu, Pc, 1);
+            const double p2 = __shfl_down_sync(0xffffffffu, Pc, 2), m2 = __shfl_up_sync(0xffffffffu, Pc, 2);
+            acc[ia][ib] += a1f * __ldg(op.dU[s] + qi0 + o) * (su * u0 - sd * d0) + (w1 * p1 + w2 * m1 + w3 * p2 + w4 * m2);
+          }
+    } else if (up >= 0 || dn >= 0) {
       const double* pu1 = pu + o1; const double* pu2 = pu + o2; const double* pu3 = pu + o3; const double* pu4 = pu + o4;
       const double* pd1 = pd + o1; const double* pd2 = pd + o2; const double* pd3 = pd + o3; const double* pd4 = pd + o4;
 #pragma unroll
