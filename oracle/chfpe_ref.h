@@ -24,9 +24,11 @@
  *
  * Pins (tests/test_oracle_pins.py): closed-form Brownian-oscillator response, exact moment ODEs,
  * Boltzmann stationarity order, 2D closed form, rigid rotation, norm contraction, independent dense
- * (Kronecker) assembly, Pade order.  Unpinned: absolute SL / anharmonic response values (no closed
- * form in this container) -- "parity unpinned" beyond stationarity, contraction, convergence and
- * the dense-assembly check.
+ * (Kronecker) assembly, Pade order; the SL coupling V'_s = V_LL + V_SL q by the short-time
+ * expansion R_phys(t) = t/m - [<U''>/m + zeta gamma <V'^2>_eq] t^3/(6m) (test_short_time_expansion_pins_Vprime).
+ * Unpinned: absolute anharmonic response values at finite times (the analytic results of refs. 58-59 are
+ * not in this container) and the paper's water spectra (figures only) -- "parity unpinned" for those beyond
+ * stationarity, contraction, convergence, the short-time coefficient and the dense-assembly check.
  */
 #ifndef CHFPE_REF_H
 #define CHFPE_REF_H

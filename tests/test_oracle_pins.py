@@ -93,6 +93,50 @@ def test_P1_compact6_sqrt_gauge():
     assert np.max(np.abs(-R - bo_response(np.arange(11) * 0.1))) < 2e-7
 
 
+# ----------------------------------------------------------------------------- SL coupling (V'_s of PAPER.md:65)
+def _short_time_t2_coefficient(R_lib, dt):
+    """Least-squares fit of R_phys(t)/t = c0 + c2 t^2 + c3 t^3 + c4 t^4 + c5 t^5 on the sampled window; returns (c0, c2)."""
+    t = np.arange(1, len(R_lib)) * dt
+    f = -np.asarray(R_lib)[1:] / t
+    A = np.stack([t ** k for k in (0, 2, 3, 4, 5)], axis=1)
+    c = np.linalg.lstsq(A, f, rcond=None)[0]
+    return c[0], c[1]
+
+
+@pytest.mark.parametrize("which", ["grid_w_gauge", "hermite"])
+def test_short_time_expansion_pins_Vprime(which):
+    """V'_s(q) = V_LL + V_SL q (Eq. 11-12 :96-100) pinned by mathematics, not by a copy of itself.
+
+    Generalised Langevin picture behind Eq. (8): q'' = (-U' + V'(q) Omega)/m,
+    Omega' = -gamma Omega - zeta gamma V'(q) p + noise, R_phys(t) = <dq(t)/dp(0)>_eq.  Expanding in t:
+        R_phys(t) = t/m - [ <U''>/m + zeta gamma <V'(q)^2>_eq ] t^3 / (6 m) + O(t^4),
+    and for harmonic U:  <V'^2>_eq = V_LL^2 + V_SL^2 / (beta m w0^2)  (the cross term is odd in q).
+    V_SL = 0 must reproduce the closed form's -(w0^2 + zeta gamma)/6; a slip such as V_SL q / 2 gives
+    -0.2708 instead of -0.3333 at V_SL = 1 and fails (tried: editing Vprime / self.Vp that way fails this test).
+    """
+    from oracle import hermite
+    w0, zeta, gamma, beta, m, vll = 1.0, 0.5, 1.0, 1.0, 1.0, 1.0
+    mu = ci.observable("mu", 1)
+    for vsl in (0.0, 1.0):
+        cfg = dict(n_modes=1, U=[(0.5 * m * w0 * w0, (2,))], V_LL=[vll], V_SL=[vsl], zeta=[zeta], gamma=[gamma],
+                   beta=beta, mass=[m], depth=4, nq=[96], np=[96], qmin=[-8.0], qmax=[8.0], pmin=[-8.0], pmax=[8.0],
+                   scheme="central4", gauge="w")
+        if which == "hermite":
+            cfg.update(np=[12], gauge="sqrt_eq")
+            o = hermite.RefHermite(cfg)
+            o.equilibrate()
+            R = o.response_1d(mu, mu, 201, 1, 1e-3)
+        else:
+            o = oracle.RefCHFPE(cfg)
+            o.equilibrate()
+            R = o.response_1d(obs("mu", 1), obs("mu", 1), 201, 1, 1e-3)
+        c0, c2 = _short_time_t2_coefficient(R, 1e-3)
+        expect = -(w0 ** 2 + zeta * gamma * (vll ** 2 + vsl ** 2 / (beta * m * w0 ** 2))) / (6.0 * m)
+        assert abs(c0 - 1.0 / m) < 5e-5
+        assert abs(c2 - expect) < 1e-3 * abs(expect), (which, vsl, c2, expect)
+    assert abs(expect - (-1.0 / 3.0)) < 1e-12 and abs(-(w0 ** 2 + zeta * gamma) / 6.0 - (-0.25)) < 1e-12
+
+
 # ----------------------------------------------------------------------------- P3
 def test_P3_second_moment_ode_pins_down_coupling_factor():
     """Exact 6x6 second-moment ODE (harmonic + LL); wrong by 3e-2 without the n_s of reading R1."""
