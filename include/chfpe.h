@@ -163,7 +163,7 @@ int chfpe_spectrum_2d(void* cuda_stream, const double* R, int32_t n1, int32_t n2
 /* Which kernel family runs the RK stage on this handle (host pointer), so that a test or a benchmark can assert
    that a configuration did not fall back to the generic kernel.  The cooperative multi-step kernel of tiny
    states is a property of the step call, not of the handle, and is not reported here. */
-enum { CHFPE_STAGE_GENERIC = 0, CHFPE_STAGE_BRICK = 1, CHFPE_STAGE_PIPE = 2, CHFPE_STAGE_COMPACT = 3 };
+enum { CHFPE_STAGE_GENERIC = 0, CHFPE_STAGE_BRICK = 1, CHFPE_STAGE_PIPE = 2, CHFPE_STAGE_COMPACT = 3, CHFPE_STAGE_TMA = 4 };
 int chfpe_stage_kernel(const chfpe_handle* h, int32_t* kind);
 
 const char* chfpe_last_error(const chfpe_handle* h);   /* h may be NULL: last create-time error */

@@ -322,10 +322,10 @@ class CHFPE:
         return ms.value, n.value
 
     def stage_kernel(self):
-        """'generic' | 'brick' | 'pipe' | 'compact': the kernel family that runs the RK stage on this handle."""
+        """'generic' | 'brick' | 'pipe' | 'compact' | 'tma': the kernel family that runs the RK stage on this handle."""
         k = C.c_int32()
         self._ck(lib().chfpe_stage_kernel(self._h, C.byref(k)), "chfpe_stage_kernel")
-        return ("generic", "brick", "pipe", "compact")[k.value]
+        return ("generic", "brick", "pipe", "compact", "tma")[k.value]
 
     def launch_count(self):
         n = C.c_int64()

@@ -96,6 +96,7 @@ static Plan make_plan(const chfpe_desc* d) {
   if (d->scheme == CHFPE_COMPACT6) tb += 2 * p.M * 2 * align256(sizeof(double) * 4096);   // Thomas factors per axis
   tb += align256(sizeof(int) * p.K) * 2;                       // brick-kernel element order and its inverse
   tb += align256(sizeof(int) * 4 * (size_t)p.K * p.nqc);       // brick-order table of the three-mode kernels
+  if (p.M == 3) tb += align256(sizeof(int) * 4 * 4 * (size_t)p.K * d->nq[0] * d->nq[1]);   // line table (chfpe_tma.cu), <= 4 parts
   p.tables_bytes = tb; o += tb;
   p.off_partial = o; o += align256(sizeof(double) * p.red_blocks * (size_t)p.batch);
   p.off_results = o; o += align256(sizeof(double) * Plan::RESULTS);
@@ -149,15 +150,24 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   if (!bp.fixed && bp.npass > 1 && brick_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.split, bp.minb, 1)) {
     bp.npass = 1; bp.fixed = 1;                                      // shapes instantiated single-pass only (48 x 48)
   }
-  if (!bp.fixed) return bp;
+  // bulk-copy fed kernel (chfpe_tma.cu): CENTRAL4, three modes, bricks cut into tma_npart parts along p_1
+  bp.tma_npart = env_int("CHFPE_TMA_NPART", 2);
+  bp.tma_nseg = env_int("CHFPE_TMA_NSEG", bp.tma_npart == 1 ? 4 : (bp.P1 == 12 ? 3 : 2));
+  bp.tma_slots = env_int("CHFPE_TMA_SLOTS", 4);
+  bp.tma_ring = env_int("CHFPE_TMA_RING", 1);
+  bp.tma = (M == 3 && d->scheme == CHFPE_CENTRAL4 && env_int("CHFPE_TMA", 1))
+               ? tma_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.tma_npart, bp.tma_nseg, bp.tma_slots, bp.tma_ring) : 0;
+  if (!bp.fixed && !bp.tma) return bp;
   // L2 reuse window = five q_1 planes x (q_2 chunk + 2+2 halo rows) x g elements of the stage input; budget 64 MiB
   // of the 126 MB L2 (the rest serves the once-touched streams).  Pairs of linked elements (g = 2) save one
   // neighbour-brick read per pair if at least 6 q_2 rows per chunk still fit, else one element at a time.
-  const double plane_bytes = 8.0 * (double)pl.cells / vnq[0];
+  // (a sweep of the bulk-copy kernel covers one p_1 part of the bricks: its window is 1/tma_npart of that)
+  const double plane_bytes = 8.0 * (double)pl.cells / vnq[0] / (bp.tma ? bp.tma_npart : 1);
   const double row_bytes = plane_bytes / vnq[1];                 // one q_2 row of one q_1 plane
-  const double budget = 64.0 * 1024 * 1024;
+  const double budget = env_int("CHFPE_L2_WINDOW_MB", 64) * 1024.0 * 1024.0;
   auto rows_that_fit = [&](int gg) { return (int)(budget / (5.0 * row_bytes * gg)) - 4; };
   int g = (K >= 2 && rows_that_fit(2) >= 6) ? 2 : 1;
+  if (bp.tma && K >= 4 && rows_that_fit(4) >= 6) g = 4;           // squares n, n+e_a, n+e_b, n+e_a+e_b: 4 links inside
   if (vnq[1] == 1) {                                                 // no q_2 rows to chunk: as many whole planes as fit
     g = (int)(budget / (5.0 * plane_bytes));
     if (g < 1) g = 1;
@@ -376,6 +386,35 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
     }
     h->bp.table = (const int4*)put(tab.data(), sizeof(int) * tab.size());
     cudaStreamSynchronize(h->stream);                                  // `tab` goes out of scope
+    if (b.tma) {   // sweep order of the bulk-copy kernel: group -> q_2 chunk -> p_1 part -> q_1 plane -> element -> q_2 row
+      std::vector<int> lt;
+      lt.reserve((size_t)4 * pl.K * n1 * n2 * b.tma_npart);
+      for (int G = 0; G < b.n_groups; G++) {
+        const int gs = std::min(b.g, pl.K - G * b.g);
+        for (int ch = 0; ch < nch; ch++) {
+          const int w = std::min(cs, n2 - ch * cs);
+          for (int part = 0; part < b.tma_npart; part++)
+            for (int i1 = 0; i1 < n1; i1++)
+              for (int kk = 0; kk < gs; kk++) {
+                const int k = order[G * b.g + kk];
+                int own = 0;
+                for (int s = 0; s < M; s++) {
+                  if (up[3 * k + s] >= 0 && pos[up[3 * k + s]] / b.g == G) own |= 1 << (2 * s);
+                  if (dn[3 * k + s] >= 0 && pos[dn[3 * k + s]] / b.g == G) own |= 1 << (2 * s + 1);
+                }
+                for (int r2 = 0; r2 < w; r2++) {
+                  lt.push_back(k);
+                  lt.push_back(i1 | ((ch * cs + r2) << 10) | (part << 20));
+                  lt.push_back(own);
+                  lt.push_back(0);
+                }
+              }
+        }
+      }
+      h->bp.n_lines = (int)(lt.size() / 4);
+      h->bp.lines = (const int4*)put(lt.data(), sizeof(int) * lt.size());
+      cudaStreamSynchronize(h->stream);
+    }
     // operator as the three-mode kernels see it
     h->op3 = op;
     if (M == 2) {
@@ -409,7 +448,9 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
       cudaStreamSynchronize(h->stream);
     }
   }
-  if (h->bp.enabled && brick_configure(h->bp, M) != 0) { cudaGetLastError(); h->bp.enabled = 0; }
+  if (h->bp.enabled && h->bp.tma && tma_configure(h->bp) != 0) { cudaGetLastError(); h->bp.tma = 0; }
+  if (h->bp.enabled && !h->bp.fixed && !h->bp.tma) h->bp.enabled = 0;
+  if (h->bp.enabled && h->bp.fixed && brick_configure(h->bp, M) != 0) { cudaGetLastError(); h->bp.fixed = 0; if (!h->bp.tma) h->bp.enabled = 0; }
   if (h->bp.enabled && h->bp.pipe) {
     int dev = 0, sms = 148, smem_sm = 0;
     cudaGetDevice(&dev);
@@ -478,6 +519,7 @@ extern "C" int chfpe_launch_count(const chfpe_handle* h, int64_t* n) {
 extern "C" int chfpe_stage_kernel(const chfpe_handle* h, int32_t* kind) {
   if (!h || !kind) return CHFPE_ERR_INVALID;
   *kind = (h->op.scheme == CHFPE_COMPACT6) ? CHFPE_STAGE_COMPACT
+          : (h->bp.enabled && h->bp.tma)   ? CHFPE_STAGE_TMA
           : (h->bp.enabled && h->bp.pipe)  ? CHFPE_STAGE_PIPE
           : h->bp.enabled                  ? CHFPE_STAGE_BRICK
                                            : CHFPE_STAGE_GENERIC;
@@ -501,6 +543,7 @@ static int run_stage(chfpe_handle* h, const double* in, const double* y, double*
                      size_t ss) {
   if (h->op.scheme == CHFPE_COMPACT6)
     return launch_stage_compact(h->op, h->ct, in, y, out, a, c, nb, ss, h->scratch, h->stream);
+  if (h->bp.enabled && h->bp.tma) return launch_stage_tma(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
   if (h->bp.enabled && h->bp.pipe) return launch_stage_pipe(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
   if (h->bp.enabled) return launch_stage_brick(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
   return launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);

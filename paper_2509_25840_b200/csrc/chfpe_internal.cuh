@@ -51,6 +51,11 @@ struct BrickPlan {
   int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3,...>) exists
   int pipe;                           // use the plane-pipelined kernel (chfpe_pipe.cu)
   int pipe_stages, pipe_ctas;         // shared-memory stages per CTA, persistent CTAs in the grid
+  // bulk-copy fed kernel (chfpe_tma.cu): a CTA owns one q_3 line of one p_1 part of the bricks
+  int tma;                            // use it (CENTRAL4, three-mode view, a compile-time specialisation exists)
+  int tma_npart, tma_nseg, tma_slots, tma_ring;
+  int n_lines;                        // K * n_q1 * n_q2 * tma_npart
+  const int4* lines;                  // [n_lines] sweep order, see decode_line
 };
 
 #ifdef __CUDACC__
@@ -133,6 +138,11 @@ int launch_steps_coop(const DevOp& op, const DevObs& o, double* y, double* va, d
 // same operation by the brick kernel (chfpe_brick.cu); requires bp.enabled
 int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out,
                        double a, double c, int nb, size_t slot_stride, cudaStream_t s);
+// bulk-copy fed variant (chfpe_tma.cu): one CTA per q_3 line and p_1 part, producer thread + consumer warps
+int tma_has_fixed(int M, int P1, int P2, int P3, int npart, int nseg, int slots, int ring);
+int tma_configure(const BrickPlan& bp);
+int launch_stage_tma(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out, double a,
+                     double c, int nb, size_t slot_stride, cudaStream_t s);
 // one-off opt-in to > 48 KB dynamic shared memory for the brick kernels; returns a cudaError_t as int
 int brick_configure(const BrickPlan& bp, int M);
 int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb, int npass);
