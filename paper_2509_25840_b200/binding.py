@@ -54,10 +54,13 @@ def lib():
         return _lib
     try:
         so = _build.build()
-    except Exception as exc:   # no nvcc and no prebuilt library: fail loudly, never fall back
+    except FileNotFoundError as exc:   # no nvcc on this machine: a prebuilt library is acceptable only if it is not stale
         if not os.path.exists(_build.SO):
-            raise ChfpeError("libchfpe.so is missing and could not be built with nvcc: %s" % exc)
+            raise ChfpeError("libchfpe.so is missing and nvcc is not available to build it: %s" % exc)
+        if _build.stale():
+            raise ChfpeError("libchfpe.so is older than its sources and nvcc is not available to rebuild it")
         so = _build.SO
+    # any other failure (e.g. a compile error in freshly edited sources) propagates: never run a stale binary
     L = C.CDLL(so)
     vp, dp, i64p = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)
     op = C.POINTER(Observable)

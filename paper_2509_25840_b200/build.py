@@ -16,11 +16,20 @@ def _nvcc():
     return "nvcc"
 
 
-def build(force=False, verbose=False):
+def _deps():
     src = [os.path.join(_HERE, "csrc", s) for s in SOURCES]
-    deps = src + [os.path.join(_HERE, "csrc", "chfpe_internal.cuh"),
-                  os.path.join(_HERE, "..", "include", "chfpe.h")]
-    if not force and os.path.exists(SO) and os.path.getmtime(SO) >= max(os.path.getmtime(d) for d in deps):
+    return src, src + [os.path.join(_HERE, "csrc", "chfpe_internal.cuh"), os.path.join(_HERE, "..", "include", "chfpe.h")]
+
+
+def stale():
+    """True if libchfpe.so is missing or older than any of its sources."""
+    _, deps = _deps()
+    return not os.path.exists(SO) or os.path.getmtime(SO) < max(os.path.getmtime(d) for d in deps)
+
+
+def build(force=False, verbose=False):
+    src, deps = _deps()
+    if not force and not stale():
         return SO
     tmp = SO + ".tmp%d" % os.getpid()
     flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
