@@ -353,7 +353,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   std::vector<int> pos(order.size());
   for (size_t i = 0; i < order.size(); i++) pos[order[i]] = (int)i;
   h->bp.pos = (const int*)put(pos.data(), sizeof(int) * pos.size());
-  h->bp.l2mode = env_int("CHFPE_L2MODE", 1);
+  h->bp.l2mode = env_int("CHFPE_L2MODE", h->bp.tma ? 3 : 1);
   if (h->bp.enabled) {                                                 // tabulate the brick order (decode_brick_id)
     const BrickPlan& b = h->bp;
     const int n1 = b.vn[0], n2 = b.vn[1], n3 = b.vn[2], cs = b.q2chunk;
@@ -403,10 +403,14 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
                   if (dn[3 * k + s] >= 0 && pos[dn[3 * k + s]] / b.g == G) own |= 1 << (2 * s + 1);
                 }
                 for (int r2 = 0; r2 < w; r2++) {
+                  const int offs[4] = {1, -1, 2, -2};
+                  int q2out = 0;                                         // q_2 neighbours outside this chunk's rows
+                  for (int dd = 0; dd < 4; dd++)
+                    if (r2 + offs[dd] < 0 || r2 + offs[dd] >= w) q2out |= 1 << dd;
                   lt.push_back(k);
                   lt.push_back(i1 | ((ch * cs + r2) << 10) | (part << 20));
                   lt.push_back(own);
-                  lt.push_back(0);
+                  lt.push_back(q2out);
                 }
               }
         }
@@ -581,7 +585,7 @@ static int step_slots(chfpe_handle* h, int b0, int nb, int64_t n_steps, double d
     DevObs none;
     memset(&none, 0, sizeof(none));
     const int n = launch_steps_coop(h->op, none, h->y(b0), h->va(b0), h->vb(b0), dt, 1, n_steps, 0, h->partial,
-                                    h->results, h->stream);
+                                    h->red_blocks, h->results, h->stream);
     if (n > 0) { h->launches += n; return check_launch(h); }
     h->coop = false;                                   // not launchable on this device: fall through for good
   }
@@ -718,7 +722,7 @@ extern "C" int chfpe_response_1d(chfpe_handle* h, const chfpe_observable* A, con
       int64_t chunk = n_samples - done;
       if (chunk > Plan::RESULTS) chunk = Plan::RESULTS;
       const int n = launch_steps_coop(h->op, o, h->y(0), h->va(0), h->vb(0), dt, chunk, stride, 1, h->partial,
-                                      h->results, h->stream);
+                                      h->red_blocks, h->results, h->stream);
       if (n == 0) { h->coop = false; break; }
       h->launches += n;
       rc = check_launch(h);
@@ -764,6 +768,7 @@ extern "C" int chfpe_response_2d(chfpe_handle* h, const chfpe_observable* A, con
   int k = 0, row0 = 0;                               // rows [row0, k) are in the device results buffer
   while (k < n1) {
     int nb = n1 - k; if (nb > per_round) nb = per_round;
+    if (nb > rows_per_fetch) nb = (int)rows_per_fetch;   // a round never holds more rows than the results buffer
     if (k + nb - row0 > rows_per_fetch) {            // flush before the buffer overflows
       rc = fetch_results(h, (long long)(k - row0) * n2, R + (size_t)row0 * n2); if (rc) return rc;
       row0 = k;

@@ -252,6 +252,12 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
   do {                                                                                                                \
     if (pa && sI == MM - 1 && n <= 32 && op.cells % (32 * n) == 0) {       /* contiguous axis: transposing kernel */    \
       const unsigned wb = (unsigned)((op.cells / n / 32 + 3) / 4);                                                    \
+      static bool optin_##MM = false;                                      /* n >= 24 needs more than 48 KB */          \
+      if (!optin_##MM) {                                                                                              \
+        cudaFuncSetAttribute(k_compact_pline_s1<MM>, cudaFuncAttributeMaxDynamicSharedMemorySize,                     \
+                             (int)(sizeof(double) * 4 * 64 * 33));                                                    \
+        optin_##MM = true;                                                                                            \
+      }                                                                                                               \
       k_compact_pline_s1<MM><<<dim3(wb, op.K, nb), 128, sizeof(double) * 4 * 64 * (n + 1), s>>>(                      \
           op, in, y, out, a, c, first, slot_stride, ct.bet[axis], ct.cfac[axis]);                                     \
       launches++;                                                                                                     \

@@ -1232,6 +1232,7 @@ extern "C" int chfpe_hermite_response_2d(chfpe_hermite_handle* h, const chfpe_ob
   while (k < n1) {
     int nb = n1 - k;
     if (nb > per_round) nb = per_round;
+    if (nb > rows_per_fetch) nb = (int)rows_per_fetch;   // a round never holds more rows than the results buffer
     if (k + nb - row0 > rows_per_fetch) {
       rc = fetch_results(h, (long long)(k - row0) * n2, R + (size_t)row0 * n2);
       if (rc) return rc;

@@ -133,8 +133,8 @@ int launch_kick_compact(const DevOp& op, const CompactTables& ct, const DevObs& 
 // persistent cooperative kernel for L2-resident states (one replica): n_samples x (stride steps [+ <O> sample]);
 // returns 0 if a cooperative launch is not possible
 int launch_steps_coop(const DevOp& op, const DevObs& o, double* y, double* va, double* vb, double dt,
-                      long long n_samples, long long stride, int do_expect, double* partial, double* results,
-                      cudaStream_t s);
+                      long long n_samples, long long stride, int do_expect, double* partial, int max_blocks,
+                      double* results, cudaStream_t s);
 // same operation by the brick kernel (chfpe_brick.cu); requires bp.enabled
 int launch_stage_brick(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out,
                        double a, double c, int nb, size_t slot_stride, cudaStream_t s);

@@ -293,6 +293,7 @@ __global__ void __launch_bounds__(256) k_steps_coop(DevOp op, DevObs ob, double*
         const double r2 = block_sum_256(a2);
         if (threadIdx.x == 0) results[smp] = r2 * op.dV;
       }
+      if (stride == 0) grid.sync();                                // no stage barrier follows: block 0 must be done with `partial`
     }
   }
 }
@@ -362,8 +363,8 @@ int launch_permute(const DevOp& op, const double* src, double* dst, int to_inter
 // n_samples x (stride RK4 steps [+ one expectation sample]) on ONE replica in one cooperative launch.  Returns the
 // number of launches (1) or 0 when the device cannot co-schedule the grid (the caller then uses per-stage launches).
 int launch_steps_coop(const DevOp& op, const DevObs& o, double* y, double* va, double* vb, double dt,
-                      long long n_samples, long long stride, int do_expect, double* partial, double* results,
-                      cudaStream_t s) {
+                      long long n_samples, long long stride, int do_expect, double* partial, int max_blocks,
+                      double* results, cudaStream_t s) {
   int dev = 0, coop = 0, sms = 0, per_sm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return 0;
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
@@ -378,6 +379,7 @@ int launch_steps_coop(const DevOp& op, const DevObs& o, double* y, double* va, d
   const long long total = (long long)op.K * op.cells;
   long long blocks = (total + 255) / 256;
   if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
+  if (blocks > max_blocks) blocks = max_blocks;                    // one partial sum per block: `partial` holds max_blocks
   DevOp opv = op; DevObs ov = o;
   void* args[] = {&opv, &ov, &y, &va, &vb, &dt, &n_samples, &stride, &do_expect, &partial, &results};
   if (cudaLaunchCooperativeKernel(fn, dim3((unsigned)blocks), dim3(256), args, 0, s) != cudaSuccess) {

@@ -164,12 +164,13 @@ struct TmaCfg {
   static constexpr int MINB = (2 * (SMEM + 1024) <= 227 * 1024 && 2 * NT <= 1024) ? 2 : 1;
 };
 
-// one line of the sweep: {element, i_q1 | i_q2 << 10 | part << 20, own-mask (as BrickId::own), unused}
-struct TmaLine { int k, iq1, iq2, part, own; };
+// one line of the sweep: {element, i_q1 | i_q2 << 10 | part << 20, own-mask (as BrickId::own), bit d: the q_2 neighbour
+// d (+1, -1, +2, -2) lies outside the q_2 chunk of the sweep, i.e. outside the L2 window}
+struct TmaLine { int k, iq1, iq2, part, own, q2out; };
 __device__ __forceinline__ TmaLine decode_line(const int4* lines, long long L) {
   const int4 t = __ldg(lines + L);
   TmaLine l;
-  l.k = t.x; l.iq1 = t.y & 1023; l.iq2 = (t.y >> 10) & 1023; l.part = t.y >> 20; l.own = t.z;
+  l.k = t.x; l.iq1 = t.y & 1023; l.iq2 = (t.y >> 10) & 1023; l.part = t.y >> 20; l.own = t.z; l.q2out = t.w;
   return l;
 }
 
@@ -326,7 +327,8 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
   const bool do_hi = NPART > 1 && seg == NSEG - 1 && part + 1 < NPART;
 
   int m = 0;
-  unsigned mask = step_mask(0), maskn = step_mask(1), mpar = 0, pre = 0;
+  // (masks are the same in every thread; the shuffle tells the compiler so: uniform branches, no reconvergence code)
+  unsigned mask = __shfl_sync(0xffffffffu, step_mask(0), 0), maskn = __shfl_sync(0xffffffffu, step_mask(1), 0), mpar = 0, pre = 0;
   // barrier parity of use (step parity mp, kind E) of slot E % SLOTS
   auto parity = [&](int E, unsigned mp) -> unsigned { return ((unsigned)(E / SLOTS) & 1u) ^ ((C::USES & 1) ? mp : 0u); };
   // Refill duty for use (mm, EP): wait until every warp has let go of the slot, then load its next user -- kind
@@ -375,11 +377,19 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
   for (; m < n3; m++) {
     if (t == 0 && m + 1 < n3) {                                     // HBM-sourced data of brick m+1 -> L2
       const size_t bn = (size_t)(m + 1) * BRICK;
-      if ((mask_line >> 10) & 1u) t_prefetch_l2(ent[10] + bn, C::CHUNK);
+      if ((mask_line >> 10) & 1u) t_prefetch_l2(ent[10] + bn, C::CHUNK);       // first touch of the brick two q_1 planes ahead
 #pragma unroll
       for (int e = 1; e < 8; e++)
         if (e != 3 && ((mask_line >> e) & (pol_bits >> e) & 1u)) t_prefetch_l2(ent[e] + bn, C::CHUNK);
+#pragma unroll
+      for (int d = 0; d < 4; d++)
+        if ((mask_line >> (12 + d)) & (ln.q2out >> d) & 1u) t_prefetch_l2(ent[12 + d] + bn, C::CHUNK);
       t_prefetch_l2(ent[NK - 1] + bn, C::CHUNK);
+      if (NPART > 1) {
+#pragma unroll
+        for (int e = 0; e < 3; e++)
+          if ((mask_line >> e) & 1u) t_prefetch_l2(ent[e] + bn + hofs, HB);
+      }
     }
     double2 x[NC];
     chunk(KindC<0>(), [&](unsigned S) {
@@ -561,7 +571,7 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
       else A[0][j] = make_double2(0.0, 0.0);
     }
     mask = maskn;
-    maskn = step_mask(m + 2);
+    maskn = __shfl_sync(0xffffffffu, step_mask(m + 2), 0);
     mpar ^= 1u;
   }
 }

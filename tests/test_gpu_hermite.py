@@ -300,6 +300,47 @@ def test_closed_forms_on_the_cuda_path():
     del one
 
 
+
+@pytest.mark.parametrize("kp,depth", [([2, 2, 2], 2), ([1, 1, 8], 1)], ids=["kp222_depth2", "kp118_depth1"])
+def test_cube32_specialisation_up_to_the_mesh_edges(kp, depth):
+    """The 32^3 compile-time specialisation of the patch kernel (`cube32` branch: lane-axis stencil on warp shuffles
+    with zero row ends, 4 x 8 x 32 CTA tiles, immediate-offset ghost handling) with a state that is non-zero on every
+    mesh face, edge and corner: right-hand side and two RK4 steps against oracle/hermite.py on the whole mesh, for the
+    default launch shape and for CHFPE_HERMITE_TILE / _FIXED / _PCOL = 0.  kp = [1, 1, 8] walks a full column of the last
+    Hermite index (the column walk of the bench configuration), kp = [2, 2, 2] exercises every Hermite neighbour."""
+    cfg = ci.config("cfg4h", np=kp, depth=depth)
+    assert cfg["nq"] == [32, 32, 32]
+    o = hermite.RefHermite(cfg)
+    X = ci.seeded_hermite_state(cfg, [sum(n) for n in o.elems], seed=9)
+    # the seeded envelope exp(-q.q/4) is 1e-4 at the faces; lift the faces to O(1) so that a ghost or wrap-around bug
+    # there cannot hide below the tolerance
+    rng = np.random.default_rng(17)
+    X = X + 0.05 * rng.uniform(-1.0, 1.0, size=X.shape)
+    for i in (0, 1, 30, 31):
+        assert np.abs(X[..., i, :, :]).max() > 1e-2 and np.abs(X[..., :, i, :]).max() > 1e-2 and np.abs(X[..., :, :, i]).max() > 1e-2
+    Fo = o.rhs(X)
+    o.import_state(X)
+    o.step(2, cfg["dt"])
+    Yo = o.export_state()
+    for var in (None, "CHFPE_HERMITE_TILE", "CHFPE_HERMITE_FIXED", "CHFPE_HERMITE_PCOL"):
+        if var:
+            os.environ[var] = "0"
+        try:
+            g = P().Hermite(cfg)
+        finally:
+            if var:
+                del os.environ[var]
+        g.import_state(X)
+        F = g.export_rhs()
+        assert rel_l2(F, Fo) < 1e-13, var
+        for sl in (np.s_[..., 0:2, :, :], np.s_[..., 30:32, :, :], np.s_[..., :, 0:2, :], np.s_[..., :, 30:32, :],
+                   np.s_[..., :, :, 0:2], np.s_[..., :, :, 30:32]):   # the faces on their own
+            assert np.linalg.norm(F[sl] - Fo[sl]) <= 1e-13 * np.linalg.norm(Fo[sl]), (var, sl)
+        g.step(2, cfg["dt"])
+        assert rel_l2(g.export_state(), Yo) < 1e-12, var
+        g.close()
+
+
 def test_full_size_rhs_on_an_embedded_block():
     """The bench workload (cfg4h: 32^3 q mesh, 8^3 Hermite functions, 20 elements = 3.36e8 values, launch configuration
     of bench.py --representation hermite).  The state is zero outside a 9 x 10 x 11 block of the q mesh; zero ghosts
@@ -337,4 +378,21 @@ def test_full_size_rhs_on_an_embedded_block():
     n0 = g.launch_count()
     g.step(1, cfg["dt"])
     assert g.launch_count() - n0 == 4
+    g.close()
+
+
+def test_response_2d_round_larger_than_the_results_buffer():
+    """(batch - 1) * n2 > 65536 results: a round must be clamped to the rows the device results buffer holds (the
+    Hermite results region is the last carve of the workspace: an overflow would land outside it)."""
+    cfg = ci.config("cfg2", nq=[9], np=[3], depth=1)
+    n1, n2 = 300, 256
+    g = P().Hermite(cfg, batch=290, guard_bytes=1 << 20)
+    o = hermite.RefHermite(cfg)
+    g.equilibrate(); o.equilibrate()
+    mu_d, al_d = ci.observable("mu", 1), ci.observable("alpha", 1)
+    t1, t2 = list(range(n1)), list(range(n2))
+    R = g.response_2d(gobs(mu_d), gobs(al_d), gobs(mu_d), t1, t2, cfg["dt"])
+    assert g.guards_intact()
+    Ro = o.response_2d(mu_d, al_d, mu_d, t1, t2, cfg["dt"])
+    assert np.max(np.abs(R - Ro)) <= 1e-8 * np.max(np.abs(Ro))
     g.close()

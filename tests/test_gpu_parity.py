@@ -125,17 +125,20 @@ def test_response_1d_config2_full():
     g.close()
 
 
-@pytest.mark.parametrize("name,cfg,nsteps", [("cfg3s", ci.config("cfg3s"), 200),
-                                             ("cfg4s8", ci.config("cfg4s8"), 100)])
-def test_response_1d_shrunken_multimode(name, cfg, nsteps):
+@pytest.mark.parametrize("name,cfg,steps", [("cfg3s", ci.config("cfg3s"), {"mu": 2000, "alpha": 2000}),
+                                            ("cfg4s8", ci.config("cfg4s8"), {"mu": 2000, "alpha": 400})])
+def test_response_1d_shrunken_multimode(name, cfg, steps):
+    """SURVEY 8(d) parity protocol (ii) on the shrunken multi-mode configurations 3' (16^4, 15 elements) and 4'
+    (8^6, 20 elements): 2000 RK4 steps of the kicked state, sampled every 10 steps, rel-max <= 1e-8 (the step count
+    is what the oracle affords: 40-90 ms per step on the box's cores; alpha on 4' runs 400 steps)."""
     g, o = both(cfg)
     M = cfg["n_modes"]
-    for kind in ("mu", "alpha"):
+    for kind, nsteps in steps.items():
         a_g, a_o = obs_pair(kind, M)
         g.equilibrate(); o.equilibrate()
         Rg = g.response_1d(a_g, a_g, nsteps // 10 + 1, 10, cfg["dt"])
         Ro = o.response_1d(a_o, a_o, nsteps // 10 + 1, 10, cfg["dt"])
-        assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+        assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro)), kind
     g.close()
 
 
@@ -146,7 +149,7 @@ def test_response_2d_batched(batch):
     g, o = both(cfg, batch=batch)
     mu_g, mu_o = obs_pair("mu", 3)
     al_g, al_o = obs_pair("alpha", 3)
-    t1 = [0, 2, 3, 7, 8]; t2 = [0, 1, 4, 6]
+    t1 = [0, 2, 3, 7, 8, 12, 16, 20]; t2 = [0, 1, 4, 6, 9, 13, 18, 24, 30]      # 20 + 8 x 30 = 260 replica-steps
     g.equilibrate(); o.equilibrate()
     Rg = g.response_2d(mu_g, al_g, al_g, t1, t2, cfg["dt"] * 10)
     Ro = o.response_2d(mu_o, al_o, al_o, t1, t2, cfg["dt"] * 10)
@@ -254,6 +257,67 @@ def test_full_size_sampled_rhs_and_step_properties(name):
     assert norm(Y) <= norm(X) * (1 + 1e-12)
     assert np.all(np.isfinite(Y))
     assert abs(g.expect(one_g)[0] - n0) < 1e-2 * abs(n0)
+    g.close()
+
+
+def _per_element_rel_l2(A, B):
+    """Overall rel-L2 and the worst element block, normalised by the block of the reference (SURVEY 8(d) protocol (i))."""
+    K = B.shape[0]
+    num = np.array([float(np.sum((A[k] - B[k]) ** 2)) for k in range(K)])
+    den = np.array([float(np.sum(B[k] ** 2)) for k in range(K)])
+    return float(np.sqrt(num.sum() / den.sum())), float(np.sqrt(np.max(num / den)))
+
+
+@pytest.mark.parametrize("name", ["cfg3", "cfg4"])
+def test_full_size_one_step_parity(name):
+    """SURVEY 8(d) parity protocol (i) at FULL size, in the launch configuration bench.py times: the whole right-hand
+    side and one whole RK4 step of BASELINE configs 3 (48^4 x 15 elements, 8.0e7 values) and 4 (16^6 x 20 elements,
+    3.4e8 values) against the oracle, element-wise: rel-L2 <= 1e-13 / 1e-12 overall AND for every element block."""
+    cfg = ci.config(name)
+    P = gpu_mod()
+    g = P.CHFPE(cfg, batch=1)
+    assert g.stage_kernel() in ("brick", "tma")
+    o = oracle.RefCHFPE(cfg)
+    levels = [sum(n) for n in o.elements()]
+    X = ci.seeded_state(cfg, levels, seed=2)
+    g.import_state(X)
+    F, Fo = g.export_rhs(), o.rhs(X)
+    tot, blk = _per_element_rel_l2(F, Fo)
+    assert tot < 1e-13 and blk < 1e-13, (tot, blk)
+    del F, Fo
+    o.import_state(X)
+    del X
+    g.step(1, cfg["dt"]); o.step(1, cfg["dt"])
+    tot, blk = _per_element_rel_l2(g.export_state(), o.export_state())
+    assert tot < 1e-12 and blk < 1e-12, (tot, blk)
+    g.close()
+
+
+def test_full_size_rhs_parity_config5():
+    """BASELINE config 5 (20^6 x 20 elements = 1.28e9 values, 10.2 GB per array, one replica): the whole right-hand side
+    against the oracle, per element block.  Needs about 60 GB of host memory (state, two right-hand sides, the oracle's
+    copy) and 25 GB on the device; skipped, with the reason, where that is not available -- the sampled-entry test
+    above then remains the full-size check of this configuration."""
+    import psutil
+    import torch
+    cfg = ci.config("cfg5")
+    if psutil.virtual_memory().available < 70e9:
+        pytest.skip("full-array config-5 comparison not run: needs 70 GB of free host memory, %.0f GB available"
+                    % (psutil.virtual_memory().available / 1e9))
+    if torch.cuda.mem_get_info()[0] < 45e9:
+        pytest.skip("full-array config-5 comparison not run: needs 45 GB of device memory")
+    P = gpu_mod()
+    g = P.CHFPE(cfg, batch=1)
+    o = oracle.RefCHFPE(cfg)
+    levels = [sum(n) for n in o.elements()]
+    X = ci.seeded_state(cfg, levels, seed=3)
+    g.import_state(X)
+    Fo = o.rhs(X)
+    del X
+    F = g.export_rhs()
+    tot, blk = _per_element_rel_l2(F, Fo)
+    print("config 5 full-array RHS ran: rel-L2 %.2e overall, %.2e worst element block" % (tot, blk))
+    assert tot < 1e-13 and blk < 1e-13, (tot, blk)
     g.close()
 
 
@@ -477,6 +541,9 @@ COMPACT = [
     ("m1_t", ci.config("cfg2", nq=[32], np=[16], depth=3, scheme="compact6")),
     ("m2_t", ci.config("cfg3s", nq=[8, 7], np=[8, 16], depth=2, scheme="compact6")),
     ("m3_t", ci.config("cfg4s8", nq=[8, 5, 6], np=[5, 8, 12], depth=2, scheme="compact6", gauge="w")),
+    # 24 and 32 points on the contiguous axis: the transposing kernel needs > 48 KB of dynamic shared memory
+    ("m1_t32", ci.config("cfg2", nq=[32], np=[32], depth=3, scheme="compact6")),
+    ("m2_t24", ci.config("cfg3s", nq=[8, 8], np=[8, 24], depth=2, scheme="compact6")),
 ]
 
 
@@ -529,4 +596,22 @@ def test_response_2d_shrunken_config5():
     Rg = g.response_2d(mu_g, al_g, al_g, t1, t2, cfg["dt"])
     Ro = o.response_2d(mu_o, al_o, al_o, t1, t2, cfg["dt"])
     assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    g.close()
+
+
+def test_response_2d_round_larger_than_the_results_buffer():
+    """(batch - 1) * n2 > 65536 results: a round is clamped to the rows the device results buffer holds; without the
+    clamp the overflow lands in the arrays that follow it (the state of slot 0, the t1 trajectory) and R2 is wrong."""
+    cfg = ci.config("cfg2", nq=[8], np=[8], depth=1)
+    n1, n2 = 300, 256
+    P = gpu_mod()
+    g = P.CHFPE(cfg, batch=290, guard_bytes=1 << 20)
+    o = oracle.RefCHFPE(cfg)
+    g.equilibrate(); o.equilibrate()
+    (mu_g, mu_o), (al_g, al_o) = obs_pair("mu", 1), obs_pair("alpha", 1)
+    t1, t2 = list(range(n1)), list(range(n2))
+    R = g.response_2d(mu_g, al_g, mu_g, t1, t2, cfg["dt"])
+    assert g.guards_intact()
+    Ro = o.response_2d(mu_o, al_o, mu_o, t1, t2, cfg["dt"])
+    assert np.max(np.abs(R - Ro)) <= 1e-8 * np.max(np.abs(Ro))
     g.close()
