@@ -42,7 +42,8 @@ class Desc(C.Structure):
                 ("nq", C.c_int32 * 3), ("np", C.c_int32 * 3),
                 ("qmin", C.c_double * 3), ("qmax", C.c_double * 3),
                 ("pmin", C.c_double * 3), ("pmax", C.c_double * 3),
-                ("depth", C.c_int32), ("scheme", C.c_int32), ("gauge", C.c_int32), ("batch", C.c_int32)]
+                ("depth", C.c_int32), ("scheme", C.c_int32), ("gauge", C.c_int32), ("batch", C.c_int32),
+                ("closure", C.c_int32)]
 
 
 class Observable(C.Structure):
@@ -51,6 +52,7 @@ class Observable(C.Structure):
 
 
 SCHEMES = {"central4": 0, "central2": 1, "compact6": 2}
+CLOSURES = {"truncate": 0, "terminator": 1}
 GAUGES = {"sqrt_eq": 0, "w": 1}
 
 _lib = None
@@ -146,6 +148,7 @@ class RefCHFPE:
         d.scheme = SCHEMES[cfg.get("scheme", "central4")]
         d.gauge = GAUGES[cfg.get("gauge", "sqrt_eq")]
         d.batch = 1
+        d.closure = CLOSURES[cfg.get("closure", "truncate")]
         self._h = C.c_void_p()
         rc = L.chfpe_ref_create(C.byref(d), C.byref(self._h))
         if rc != 0:

@@ -105,7 +105,7 @@ int chfpe_ref_set_threads(int32_t n) {
 int chfpe_ref_create(const chfpe_ref_desc* d, chfpe_ref_handle** out) {
   if (!d || !out) return -1;
   if (d->n_modes < 1 || d->n_modes > 3 || d->depth < 0 || d->beta <= 0) return -1;
-  if (d->scheme < 0 || d->scheme > 2 || d->gauge < 0 || d->gauge > 1) return -1;
+  if (d->scheme < 0 || d->scheme > 2 || d->gauge < 0 || d->gauge > 1 || d->closure < 0 || d->closure > 1) return -1;
   H* h = (H*)calloc(1, sizeof(H));
   h->d = *d; h->M = d->n_modes; h->nax = 2 * h->M;
   h->U = (chfpe_ref_monomial*)malloc(sizeof(chfpe_ref_monomial) * (d->n_terms > 0 ? d->n_terms : 1));
@@ -263,13 +263,15 @@ static double rhs_point(const H* h, const double* X, int k, int64_t cell, const 
 }
 
 int chfpe_ref_rhs_at(const chfpe_ref_handle* h, const double* X, int32_t k, int64_t cell, double* out) {
-  if (h->d.scheme == 2 || k < 0 || k >= h->K || cell < 0 || cell >= h->cells) return -1;
+  if (h->d.scheme == 2 || h->d.closure != 0 || k < 0 || k >= h->K || cell < 0 || cell >= h->cells) return -1;
   int idx[MAXAX]; decode(h, cell, idx);
   *out = rhs_point(h, X, k, cell, idx);
   return 0;
 }
 
 static void ensure(double** p, size_t n) { if (!*p) *p = malloc(sizeof(double) * n); }
+
+static void add_terminator(chfpe_ref_handle* h, const double* X, double* F);
 
 /* RHS through whole-array derivatives: valid for every scheme */
 int chfpe_ref_rhs_deriv(chfpe_ref_handle* h, const double* X, double* F) {
@@ -301,10 +303,56 @@ int chfpe_ref_rhs_deriv(chfpe_ref_handle* h, const double* X, double* F) {
       }
     }
   }
+  if (h->d.closure == 1) add_terminator(h, X, F);
   return 0;
 }
 
+/* Terminator closure (reading R23; the paper is silent on the truncation).  For a top-level element
+ * n (|n| = depth) the element n+e_s is not propagated; Eq. (8) for it, with everything but its damping and its
+ * source dropped, 0 = -Gamma_{n+e_s} W^(n+e_s) + (n_s+1) Theta_s W^(n), slaves it to W^(n).  Step by step:
+ *   Y   = (n_s+1) c_s V'_s (D_{p_s} + kappa^dn_s p_s) X_n / (Gamma_n + gamma_s)       the virtual element, whole grid
+ *   F_n += V'_s (D_{p_s} + kappa^up_s p_s) Y                                           its Phi_s coupling, Eq. (11)
+ * with the same discrete D (any scheme) and zero ghosts for X_n and for Y.  For depth 0 this is the Kramers
+ * equation with friction zeta_s V'_s^2. */
+static void add_terminator(chfpe_ref_handle* h, const double* X, double* F) {
+  ensure(&h->D0, h->cells); ensure(&h->D1, h->cells);
+  for (int k = 0; k < h->K; k++) {
+    int lev = 0;
+    for (int s = 0; s < h->M; s++) lev += h->elem[k][s];
+    if (lev != h->d.depth) continue;
+    const double* Xk = X + (size_t)k * h->cells; double* Fk = F + (size_t)k * h->cells;
+    for (int s = 0; s < h->M; s++) {
+      int aq = 2 * s, ap = 2 * s + 1;
+      const double fac = (h->elem[k][s] + 1) * h->cdn[s] / (h->Gamma[k] + h->d.gamma[s]);
+      chfpe_ref_deriv_axis(h, Xk, ap, h->D0);
+      double* Y = h->D1;
+      #pragma omp parallel for
+      for (int64_t c = 0; c < h->cells; c++) {
+        int idx[MAXAX]; decode(h, c, idx);
+        double q = coord(h, aq, idx[aq]), p = coord(h, ap, idx[ap]);
+        Y[c] = fac * Vprime(h, s, q) * (h->D0[c] + h->kdn[s] * p * Xk[c]);
+      }
+      chfpe_ref_deriv_axis(h, Y, ap, h->D0);
+      #pragma omp parallel for
+      for (int64_t c = 0; c < h->cells; c++) {
+        int idx[MAXAX]; decode(h, c, idx);
+        double q = coord(h, aq, idx[aq]), p = coord(h, ap, idx[ap]);
+        Fk[c] += Vprime(h, s, q) * (h->D0[c] + h->kup[s] * p * Y[c]);
+      }
+    }
+  }
+}
+
 int chfpe_ref_rhs(chfpe_ref_handle* h, const double* X, double* F) {
+  if (h->d.closure == 1) {                                  /* plain right-hand side, then the slaved elements */
+    const int32_t keep = h->d.closure;
+    h->d.closure = 0;
+    int rc = chfpe_ref_rhs(h, X, F);
+    h->d.closure = keep;
+    if (rc) return rc;
+    add_terminator(h, X, F);
+    return 0;
+  }
   if (h->d.scheme == 2) return chfpe_ref_rhs_deriv(h, X, F);
   int64_t n0 = h->n[0], rest = h->cells / n0;
   #pragma omp parallel for collapse(2) schedule(static)

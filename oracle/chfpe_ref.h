@@ -51,6 +51,8 @@ typedef struct {
   int32_t scheme;   /* 0 CENTRAL4, 1 CENTRAL2, 2 COMPACT6 */
   int32_t gauge;    /* 0 sqrt(W_eq) gauge, 1 W gauge */
   int32_t batch;    /* ignored by the oracle (always one state) */
+  int32_t closure;  /* 0 plain truncation (reading R5), 1 terminator: at the top level |n| = depth the missing element is
+                       slaved to its source, W^(n+e_s) = (n_s+1) Theta_s W^(n) / Gamma_{n+e_s} (reading R23) */
 } chfpe_ref_desc;
 
 typedef struct { double c0, lin_q[3], quad[3][3], lin_p[3]; } chfpe_ref_observable;

@@ -137,6 +137,47 @@ def test_short_time_expansion_pins_Vprime(which):
     assert abs(expect - (-1.0 / 3.0)) < 1e-12 and abs(-(w0 ** 2 + zeta * gamma) / 6.0 - (-0.25)) < 1e-12
 
 
+# ----------------------------------------------------------------------------- terminator closure (reading R23)
+@pytest.mark.parametrize("gauge,tol", [("w", 1e-7), ("sqrt_eq", 8e-5)])
+def test_terminator_depth0_is_the_kramers_equation(gauge, tol):
+    """Depth 0 with the terminator: W^(e_s) = Theta_s W^(0) / gamma_s turns Phi_s W^(e_s) into the Fokker-Planck term
+    zeta_s V'_s^2 d/dp (p + (m/beta) d/dp): the Markovian Kramers equation with friction zeta V'^2, independent of
+    gamma.  Harmonic U, V' = 1: the damped oscillator s^2 + zeta s + w0^2, R_phys(t) = exp(-zeta t/2) sin(Omega t)/(m Omega)."""
+    w0, zeta = 1.0, 0.5
+    t = np.arange(21) * 0.1
+    Om = math.sqrt(w0 * w0 - zeta * zeta / 4.0)
+    exact = np.exp(-zeta * t / 2.0) * np.sin(Om * t) / Om
+    for gamma in (1.0, 3.0):
+        cfg = harmonic_cfg(depth=0, gauge=gauge, zeta=zeta, gamma=gamma)
+        cfg["closure"] = "terminator"
+        o = oracle.RefCHFPE(cfg)
+        o.equilibrate()
+        R = o.response_1d(obs("mu", 1), obs("mu", 1), 21, 100, 1e-3)
+        assert np.max(np.abs(-R - exact)) < tol, (gauge, gamma)
+    cfg["closure"] = "truncate"                                  # plain truncation at depth 0 has no bath at all
+    o = oracle.RefCHFPE(cfg)
+    o.equilibrate()
+    R = o.response_1d(obs("mu", 1), obs("mu", 1), 21, 100, 1e-3)
+    assert np.max(np.abs(-R - np.sin(w0 * t) / w0)) < 1e-4 and np.max(np.abs(-R - exact)) > 0.1
+
+
+def test_terminator_needs_fewer_levels():
+    """Anharmonic mode with LL+SL coupling and a fast bath (config 2 with gamma = 6): at every depth 0..3 the terminator
+    is closer to the converged hierarchy (depth 10) than plain truncation, and it reaches 1e-4 one level earlier."""
+    def resp(depth, closure):
+        cfg = ci.config("cfg2", depth=depth, nq=[64], np=[64], gamma=[6.0], closure=closure)
+        o = oracle.RefCHFPE(cfg)
+        o.equilibrate()
+        return o.response_1d(obs("mu_nl", 1), obs("mu_nl", 1), 41, 100, cfg["dt"])
+    ref = resp(10, "truncate")
+    assert np.max(np.abs(resp(10, "terminator") - ref)) < 1e-10   # both closures converge to the same hierarchy
+    err = {c: [float(np.max(np.abs(resp(N, c) - ref))) for N in range(4)] for c in ("truncate", "terminator")}
+    for N in range(4):
+        assert err["terminator"][N] < 0.5 * err["truncate"][N], (N, err)
+    first = {c: next(N for N in range(4) if err[c][N] < 1e-4) for c in err}
+    assert first["terminator"] < first["truncate"], (first, err)
+
+
 # ----------------------------------------------------------------------------- P3
 def test_P3_second_moment_ode_pins_down_coupling_factor():
     """Exact 6x6 second-moment ODE (harmonic + LL); wrong by 3e-2 without the n_s of reading R1."""
@@ -500,8 +541,19 @@ def _assemble(cfg, elements):
             if nd[s] >= 0:
                 c = cfg["zeta"][s] * cfg["gamma"][s] * m / beta
                 blocks[k][index[tuple(nd)]] = n[s] * c * (Vp @ (D[2 * s + 1] + kdn * P))
+            if cfg.get("closure") == "terminator" and sum(n) == cfg["depth"]:
+                # reading R23: W^(n+e_s) = (n_s+1) Theta_s W^(n) / Gamma_{n+e_s}, fed back through Phi_s (Eq. 11, 12)
+                c = cfg["zeta"][s] * cfg["gamma"][s] * m / beta
+                gam_up = sum(n[r] * cfg["gamma"][r] for r in range(M)) + cfg["gamma"][s]
+                Lk = Lk + ((n[s] + 1) * c / gam_up) * (Vp @ (D[2 * s + 1] + kup * P)) @ (Vp @ (D[2 * s + 1] + kdn * P))
         blocks[k][k] = Lk
     return sp.bmat(blocks, format="csr"), D, coords
+
+
+def _with(cfg, **over):
+    c = dict(cfg)
+    c.update(over)
+    return c
 
 
 ASSEMBLY_CASES = [
@@ -529,6 +581,9 @@ ASSEMBLY_CASES = [
                         qmax=[3.0, 2.5, 4.0], pmin=[-3.0, -3.5, -2.0], pmax=[3.0, 3.0, 2.5],
                         scheme="central4", gauge="sqrt_eq")),
 ]
+# the same operators with the terminator closure (reading R23), all three schemes, both gauges, M = 1..3
+ASSEMBLY_CASES += [(nm + "_terminator", _with(c, closure="terminator")) for nm, c in
+                   [ASSEMBLY_CASES[0], ASSEMBLY_CASES[1], ASSEMBLY_CASES[2], ASSEMBLY_CASES[3], ASSEMBLY_CASES[5]]]
 
 
 @pytest.mark.parametrize("name,cfg", ASSEMBLY_CASES, ids=[c[0] for c in ASSEMBLY_CASES])
@@ -543,7 +598,7 @@ def test_P10_independent_kronecker_assembly(name, cfg):
     scale = np.max(np.abs(want))
     assert np.max(np.abs(o.rhs(X) - want)) < 1e-12 * scale
     assert np.max(np.abs(o.rhs(X, via_deriv=True) - want)) < 1e-12 * scale
-    if cfg["scheme"] != "compact6":
+    if cfg["scheme"] != "compact6" and cfg.get("closure", "truncate") == "truncate":
         for k, cell in ((0, 0), (o.K - 1, o.cells - 1), (1, o.cells // 3)):
             assert abs(o.rhs_at(X, k, cell) - want.reshape(o.K, -1)[k, cell]) < 1e-12 * scale
     # propagation: many small RK4 steps vs expm action
