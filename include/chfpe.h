@@ -46,6 +46,11 @@ enum {
 
 enum { CHFPE_CENTRAL4 = 0, CHFPE_CENTRAL2 = 1, CHFPE_COMPACT6 = 2 };   /* derivative scheme; COMPACT6 = Pade scheme Eq. (25)-(31) :177-201 with a = 7/9 (R4), one fused line pass per axis */
 enum { CHFPE_GAUGE_SQRT_EQ = 0, CHFPE_GAUGE_W = 1 };                   /* propagated variable (R7) */
+/* Closure of the hierarchy at the top level |n| = depth (the paper is silent; readings R5, R23):
+   TRUNCATE drops W^(n+e_s); TERMINATOR slaves it to its source, W^(n+e_s) = (n_s+1) Theta_s W^(n) / Gamma_{n+e_s},
+   which turns Phi_s W^(n+e_s) (Eq. 11-12 :96-100) into a second-derivative Fokker-Planck term (depth 0: the Kramers
+   equation with friction zeta_s V'_s^2).  Explicit schemes only, phase-space grid representation only. */
+enum { CHFPE_CLOSURE_TRUNCATE = 0, CHFPE_CLOSURE_TERMINATOR = 1 };
 
 /* coef * q1^e1 q2^e2 q3^e3 ; total degree <= 4.  Eq. (3)-(4). */
 typedef struct { double coef; int32_t expo[3]; } chfpe_monomial;
@@ -63,6 +68,7 @@ typedef struct {
   int32_t scheme;                     /* CHFPE_CENTRAL4 (default) | CHFPE_CENTRAL2 | CHFPE_COMPACT6 */
   int32_t gauge;                      /* CHFPE_GAUGE_SQRT_EQ (default) | CHFPE_GAUGE_W (literal Eq. 8) */
   int32_t batch;                      /* B >= 1 independent replicas (state slots) sharing the operator */
+  int32_t closure;                    /* CHFPE_CLOSURE_TRUNCATE (default) | CHFPE_CLOSURE_TERMINATOR */
 } chfpe_desc;
 
 /* X(q,p) = c0 + sum lin_q[s] q_s + 1/2 sum quad[s][s'] q_s q_s' + sum lin_p[s] p_s ; Eq. (13)-(14) :108-113.

@@ -34,7 +34,8 @@ class Desc(C.Structure):
                 ("nq", C.c_int32 * 3), ("np", C.c_int32 * 3),
                 ("qmin", C.c_double * 3), ("qmax", C.c_double * 3),
                 ("pmin", C.c_double * 3), ("pmax", C.c_double * 3),
-                ("depth", C.c_int32), ("scheme", C.c_int32), ("gauge", C.c_int32), ("batch", C.c_int32)]
+                ("depth", C.c_int32), ("scheme", C.c_int32), ("gauge", C.c_int32), ("batch", C.c_int32),
+                ("closure", C.c_int32)]
 
 
 class Observable(C.Structure):
@@ -44,6 +45,7 @@ class Observable(C.Structure):
 
 SCHEMES = {"central4": 0, "central2": 1, "compact6": 2}
 GAUGES = {"sqrt_eq": 0, "w": 1}
+CLOSURES = {"truncate": 0, "terminator": 1}
 _lib = None
 
 
@@ -158,6 +160,7 @@ def make_desc(cfg, batch=1):
     d.scheme = SCHEMES[cfg.get("scheme", "central4")]
     d.gauge = GAUGES[cfg.get("gauge", "sqrt_eq")]
     d.batch = batch
+    d.closure = CLOSURES[cfg.get("closure", "truncate")]
     return d, arr
 
 

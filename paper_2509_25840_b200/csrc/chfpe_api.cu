@@ -49,6 +49,8 @@ static int validate(const chfpe_desc* d, std::string* why) {
   if (d->scheme != CHFPE_CENTRAL4 && d->scheme != CHFPE_CENTRAL2 && d->scheme != CHFPE_COMPACT6) { *why = "unknown scheme"; return CHFPE_ERR_INVALID; }
   if (d->gauge != CHFPE_GAUGE_SQRT_EQ && d->gauge != CHFPE_GAUGE_W) { *why = "unknown gauge"; return CHFPE_ERR_INVALID; }
   if (d->batch < 1 || d->batch > 4096) { *why = "batch must be 1..4096"; return CHFPE_ERR_INVALID; }
+  if (d->closure != CHFPE_CLOSURE_TRUNCATE && d->closure != CHFPE_CLOSURE_TERMINATOR) { *why = "unknown closure"; return CHFPE_ERR_INVALID; }
+  if (d->closure == CHFPE_CLOSURE_TERMINATOR && d->scheme == CHFPE_COMPACT6) { *why = "the terminator closure needs an explicit scheme"; return CHFPE_ERR_INVALID; }
   if (d->n_terms < 0 || (d->n_terms > 0 && !d->U)) { *why = "bad potential term list"; return CHFPE_ERR_INVALID; }
   for (int t = 0; t < d->n_terms; t++) {
     int deg = 0;
@@ -261,6 +263,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   DevOp& op = h->op;
   memset(&op, 0, sizeof(op));
   op.M = M; op.nax = 2 * M; op.K = pl.K; op.scheme = desc->scheme; op.gauge = desc->gauge; op.beta = desc->beta;
+  op.closure = desc->closure; op.depth = desc->depth;
   for (int s = 0; s < M; s++) {
     op.n[s] = desc->nq[s]; op.n[M + s] = desc->np[s];
     op.x0[s] = desc->qmin[s]; op.x0[M + s] = desc->pmin[s];
@@ -271,6 +274,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
     if (desc->gauge == CHFPE_GAUGE_W) { op.kup[s] = 0.0; op.kdn[s] = desc->beta / desc->mass[s]; }
     else { op.kup[s] = -desc->beta / (2 * desc->mass[s]); op.kdn[s] = desc->beta / (2 * desc->mass[s]); }
     op.VLL[s] = desc->V_LL[s]; op.VSL[s] = desc->V_SL[s];
+    op.gam[s] = desc->gamma[s];
   }
   op.cells = pl.cells; op.nqc = pl.nqc; op.pb = pl.cells / pl.nqc;
   op.dV = 1.0;
@@ -547,9 +551,14 @@ static int run_stage(chfpe_handle* h, const double* in, const double* y, double*
                      size_t ss) {
   if (h->op.scheme == CHFPE_COMPACT6)
     return launch_stage_compact(h->op, h->ct, in, y, out, a, c, nb, ss, h->scratch, h->stream);
-  if (h->bp.enabled && h->bp.tma) return launch_stage_tma(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
-  if (h->bp.enabled && h->bp.pipe) return launch_stage_pipe(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
-  if (h->bp.enabled) return launch_stage_brick(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
+  if (h->bp.enabled) {                                // (these kernels evaluate plain truncation: the slaved elements follow)
+    int n = 0;
+    if (h->bp.tma) n = launch_stage_tma(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
+    else if (h->bp.pipe) n = launch_stage_pipe(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
+    else n = launch_stage_brick(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
+    if (h->op.closure == CHFPE_CLOSURE_TERMINATOR) n += launch_terminator_add(h->op, in, out, c, nb, ss, h->stream);
+    return n;
+  }
   return launch_stage(h->op, in, y, out, a, c, nb, ss, h->stream);
 }
 

@@ -699,6 +699,7 @@ int validate(const chfpe_desc* d, std::string* why) {
   if (!(d->beta > 0)) { *why = "beta must be > 0"; return CHFPE_ERR_INVALID; }
   if (d->scheme != CHFPE_CENTRAL4 && d->scheme != CHFPE_CENTRAL2 && d->scheme != CHFPE_COMPACT6) { *why = "unknown scheme"; return CHFPE_ERR_INVALID; }
   if (d->batch < 1 || d->batch > 4096) { *why = "batch must be 1..4096"; return CHFPE_ERR_INVALID; }
+  if (d->closure != CHFPE_CLOSURE_TRUNCATE) { *why = "the Hermite representation implements plain truncation only"; return CHFPE_ERR_INVALID; }
   if (d->n_terms < 0 || (d->n_terms > 0 && !d->U)) { *why = "bad potential term list"; return CHFPE_ERR_INVALID; }
   for (int t = 0; t < d->n_terms; t++) {
     int deg = 0;

@@ -14,12 +14,14 @@
 // last axis fastest, so all momenta of one q-point form one contiguous "p-brick" of pb cells.
 struct DevOp {
   int M, nax, K, scheme, gauge;
+  int closure, depth;                 // CHFPE_CLOSURE_*; N (elements with sum n = N are the top level)
   int n[CHFPE_MAXAX];                 // points per internal axis
   long long st[CHFPE_MAXAX];          // internal strides (doubles)
   long long cells, nqc, pb;           // cells per element, q-points, p-brick size
   double x0[CHFPE_MAXAX], h[CHFPE_MAXAX];
   double c1[CHFPE_MAXAX], c2[CHFPE_MAXAX];   // pre-multiplied stencil coefficients (+-1, +-2 neighbours)
   double inv_mass[3], kup[3], kdn[3], cdn[3], VLL[3], VSL[3], beta;
+  double gam[3];                      // gamma_s (terminator closure: Gamma_{n+e_s} = Gamma_n + gamma_s)
   double dV;
   const double* dU[3];                // dU/dq_s on the q-subgrid, q_1 slowest   (device)
   const double* eU;                   // exp(-beta U/2) (sqrt gauge) or exp(-beta U) (W gauge) on the q-subgrid
@@ -152,6 +154,10 @@ size_t pipe_smem_bytes(const BrickPlan& bp);
 int pipe_configure(const BrickPlan& bp);
 int launch_stage_pipe(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out, double a,
                       double c, int nb, size_t slot_stride, cudaStream_t s);
+// terminator closure on top of a stage kernel that does not know it (brick / bulk-copy kernels):
+// out += c * (slaved-element coupling of every top-level element), see terminator_value in chfpe_kernels.cu
+int launch_terminator_add(const DevOp& op, const double* in, double* out, double c, int nb, size_t slot_stride,
+                          cudaStream_t s);
 // out = Kick_obs(in) on every element, slots [b0, b0+nb)
 int launch_kick(const DevOp& op, const DevObs& o, const double* in, double* out, int nb, size_t slot_stride,
                 cudaStream_t s);

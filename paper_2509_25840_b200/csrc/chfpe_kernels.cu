@@ -55,6 +55,30 @@ __device__ __forceinline__ double dstencil_x(const double* __restrict__ f, long 
   return d;
 }
 
+// Terminator closure (reading R23) for a top-level element k, mode s: the element n+e_s that is not propagated is
+//   Y = (n_s+1) c_s V'_s (D_{p_s} + kappa^dn_s p_s) X_k / (Gamma_k + gamma_s)        (Eq. 12 with its damping only)
+// and feeds back through Phi_s (Eq. 11): V'_s (D_{p_s} + kappa^up_s p_s) Y, with zero ghosts for X_k and for Y (R9).
+// One value: nine points of X_k along p_s.
+template <bool COHERENT>
+__device__ __forceinline__ double terminator_value(const DevOp& op, const double* __restrict__ Xk, long long cell, int ap,
+                                                   int i, double Vp, double fac, double kup, double kdn, bool wide) {
+  const int n = op.n[ap];
+  const long long st = op.st[ap];
+  const double c1 = op.c1[ap], c2 = wide ? op.c2[ap] : 0.0;
+  const double p0 = op.x0[ap], h = op.h[ap];
+  double v[9];
+#pragma unroll
+  for (int j = -4; j <= 4; j++) v[j + 4] = (i + j >= 0 && i + j < n) ? ldx<COHERENT>(Xk + cell + j * st) : 0.0;
+  double A[5];                                                      // (D + kdn p) X at i-2..i+2, zero outside the grid
+#pragma unroll
+  for (int j = -2; j <= 2; j++) {
+    const double d = fma(c2, v[j + 6] - v[j + 2], c1 * (v[j + 5] - v[j + 3]));
+    A[j + 2] = (i + j >= 0 && i + j < n) ? fma(kdn * fma((double)(i + j), h, p0), v[j + 4], d) : 0.0;
+  }
+  const double dA = fma(c2, A[4] - A[0], c1 * (A[3] - A[1]));
+  return fac * Vp * Vp * fma(kup * fma((double)i, h, p0), A[2], dA);
+}
+
 // F_k(X)(cell), right-hand side of Eq. (8) :77-80 for one (element, cell): Liouvillian Eq. (9)-(10), Phi Eq. (11),
 // n_s Theta Eq. (12) + R1, damping.  X points at element 0 of the replica.
 template <int M, bool COHERENT>
@@ -86,8 +110,39 @@ __device__ __forceinline__ double rhs_value(const DevOp& op, const double* __res
       double d = dstencil_x<COHERENT>(Xd, cell, op.st[ap], idx[ap], op.n[ap], op.c1[ap], op.c2[ap], wide);
       acc = fma(__ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp, fma(op.kdn[s] * p, ldx<COHERENT>(Xd + cell), d), acc);
     }
+    if (op.closure == CHFPE_CLOSURE_TERMINATOR && ku < 0) {         // top level: the missing element is slaved (R23)
+      const double fac = (__ldg(op.nvec + 3 * k + s) + 1) * op.cdn[s] / (__ldg(op.Gamma + k) + op.gam[s]);
+      acc += terminator_value<COHERENT>(op, Xk, cell, ap, idx[ap], Vp, fac, op.kup[s], op.kdn[s], wide);
+    }
   }
   return acc;
+}
+
+// out += c * (terminator terms of element k) for the stage kernels that evaluate plain truncation only
+template <int M>
+__global__ void __launch_bounds__(256) k_terminator_add(DevOp op, const double* __restrict__ in, double* out, double c,
+                                                        size_t slot_stride) {
+  long long cell = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (cell >= op.cells) return;
+  const int k = blockIdx.y;
+  int lev = 0;
+#pragma unroll
+  for (int s = 0; s < M; s++) lev += __ldg(op.nvec + 3 * k + s);
+  if (lev != op.depth) return;                                      // (simplex truncation: up(k, s) is missing for every s)
+  const size_t boff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells;
+  const double* Xk = in + boff;
+  int idx[2 * M];
+  decode<2 * M>(op, cell, idx);
+  const bool wide = (op.scheme == CHFPE_CENTRAL4);
+  double acc = 0.0;
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const double q = op.x0[s] + idx[s] * op.h[s];
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    const double fac = (__ldg(op.nvec + 3 * k + s) + 1) * op.cdn[s] / (__ldg(op.Gamma + k) + op.gam[s]);
+    acc += terminator_value<false>(op, Xk, cell, M + s, idx[M + s], Vp, fac, op.kup[s], op.kdn[s], wide);
+  }
+  out[boff + cell] = fma(c, acc, out[boff + cell]);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -311,6 +366,15 @@ int launch_stage(const DevOp& op, const double* in, const double* y, double* out
                  size_t slot_stride, cudaStream_t s) {
   dim3 grid((unsigned)((op.cells + 255) / 256), op.K, nb);
 #define CALL(MM) k_stage_generic<MM><<<grid, 256, 0, s>>>(op, in, y, out, a, c, slot_stride)
+  DISPATCH_M(op.M, CALL);
+#undef CALL
+  return 1;
+}
+
+int launch_terminator_add(const DevOp& op, const double* in, double* out, double c, int nb, size_t slot_stride,
+                          cudaStream_t s) {
+  dim3 grid((unsigned)((op.cells + 255) / 256), op.K, nb);
+#define CALL(MM) k_terminator_add<MM><<<grid, 256, 0, s>>>(op, in, out, c, slot_stride)
   DISPATCH_M(op.M, CALL);
 #undef CALL
   return 1;

@@ -390,7 +390,7 @@ def test_response_2d_round_larger_than_the_results_buffer():
     o = hermite.RefHermite(cfg)
     g.equilibrate(); o.equilibrate()
     mu_d, al_d = ci.observable("mu", 1), ci.observable("alpha", 1)
-    t1, t2 = list(range(n1)), list(range(n2))
+    t1, t2 = list(range(n1)), [0] * 200 + list(range(n2 - 200))      # 256 samples per row, 55 steps (oracle time)
     R = g.response_2d(gobs(mu_d), gobs(al_d), gobs(mu_d), t1, t2, cfg["dt"])
     assert g.guards_intact()
     Ro = o.response_2d(mu_d, al_d, mu_d, t1, t2, cfg["dt"])

@@ -609,9 +609,72 @@ def test_response_2d_round_larger_than_the_results_buffer():
     o = oracle.RefCHFPE(cfg)
     g.equilibrate(); o.equilibrate()
     (mu_g, mu_o), (al_g, al_o) = obs_pair("mu", 1), obs_pair("alpha", 1)
-    t1, t2 = list(range(n1)), list(range(n2))
+    t1, t2 = list(range(n1)), [0] * 200 + list(range(n2 - 200))      # 256 samples per row, 55 steps (oracle time)
     R = g.response_2d(mu_g, al_g, mu_g, t1, t2, cfg["dt"])
     assert g.guards_intact()
     Ro = o.response_2d(mu_o, al_o, mu_o, t1, t2, cfg["dt"])
     assert np.max(np.abs(R - Ro)) <= 1e-8 * np.max(np.abs(Ro))
     g.close()
+
+
+TERMINATOR = [
+    ("m1_generic_w", ci.config("cfg2", nq=[37], np=[41], depth=3, gauge="w", closure="terminator")),
+    ("m1_depth0", ci.config("cfg1", nq=[33], np=[29], depth=0, closure="terminator")),
+    ("m1_c2", ci.config("cfg2", nq=[33], np=[29], depth=2, scheme="central2", closure="terminator")),
+    ("m2_brick", ci.config("cfg3s", nq=[7, 9], depth=2, closure="terminator")),
+    ("m3_generic", ci.config("cfg4s8", nq=[7, 8, 6], np=[8, 6, 9], depth=2, closure="terminator", mass=[1.0, 0.8, 1.2])),
+    ("m3_cube8", ci.config("cfg4s8", nq=[6, 5, 7], closure="terminator")),
+    ("m3_cube16", ci.config("cfg4", nq=[5, 5, 6], depth=2, closure="terminator")),
+]
+
+
+@pytest.mark.parametrize("name,cfg", TERMINATOR, ids=[c[0] for c in TERMINATOR])
+def test_terminator_closure(name, cfg):
+    """Row f4 (first half): terminator closure of the top hierarchy level (reading R23) on every stage-kernel family
+    (cooperative / generic kernels evaluate it inside the right-hand side, the brick and bulk-copy kernels add it with
+    k_terminator_add): right-hand side, steps and a batched 2D response against the oracle."""
+    g, o = both(cfg, batch=2)
+    M = cfg["n_modes"]
+    levels = [sum(n) for n in o.elements()]
+    X = ci.seeded_state(cfg, levels, seed=13)
+    g.import_state(X); g.import_state(X, replica=1); o.import_state(X)
+    Fg, Fo = g.export_rhs(1), o.rhs(X)
+    assert rel_l2(Fg, Fo) < 1e-13
+    for k in range(o.K):
+        assert np.linalg.norm(Fg[k] - Fo[k]) <= 1e-13 * np.linalg.norm(Fo)
+    plain = oracle.RefCHFPE(dict(cfg, closure="truncate"))
+    assert rel_l2(plain.rhs(X), Fo) > 1e-3                       # the closure is not a no-op on this state
+    g.step(3, cfg["dt"]); o.step(3, cfg["dt"])
+    assert rel_l2(g.export_state(0), o.export_state()) < 1e-12
+    assert rel_l2(g.export_state(1), o.export_state()) < 1e-12
+    mu_g, mu_o = obs_pair("mu", M)
+    al_g, al_o = obs_pair("alpha", M)
+    g.equilibrate(); o.equilibrate()
+    Rg = g.response_2d(mu_g, al_g, mu_g, [0, 2, 3], [0, 1, 4], cfg["dt"] * 5)
+    Ro = o.response_2d(mu_o, al_o, mu_o, [0, 2, 3], [0, 1, 4], cfg["dt"] * 5)
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    g.close()
+
+
+def test_terminator_depth0_kramers_closed_form_on_the_cuda_path():
+    """The Kramers limit of the closure on the CUDA path itself: depth 0, harmonic mode, V' = 1 -> damped oscillator."""
+    import math
+    zeta = 0.5
+    cfg = ci.config("cfg1", depth=0, gauge="w", closure="terminator")
+    P = gpu_mod()
+    g = P.CHFPE(cfg)
+    g.equilibrate()
+    mu = make_obs(P, ci.observable("mu", 1))
+    R = g.response_1d(mu, mu, 21, 100, 1e-3)
+    t = np.arange(21) * 0.1
+    Om = math.sqrt(1.0 - zeta * zeta / 4.0)
+    assert np.max(np.abs(-R - np.exp(-zeta * t / 2.0) * np.sin(Om * t) / Om)) < 1e-7
+    g.close()
+
+
+def test_terminator_rejected_where_it_is_not_implemented():
+    P = gpu_mod()
+    with pytest.raises(P.ChfpeError):
+        P.CHFPE(ci.config("cfg1", scheme="compact6", closure="terminator"))
+    with pytest.raises(P.ChfpeError):
+        P.Hermite(ci.config("cfg1", np=[6], closure="terminator"))
