@@ -40,7 +40,7 @@ enum {
   CHFPE_ERR_INVALID = -1,    /* bad descriptor / argument (M not in 1..3, < 5 grid points, degree > 4, ...) */
   CHFPE_ERR_WORKSPACE = -2,  /* workspace too small or not 256-byte aligned */
   CHFPE_ERR_CUDA = -3,       /* CUDA runtime error; message from cudaGetErrorString */
-  CHFPE_ERR_DIVERGED = -4,   /* non-finite expectation value encountered */
+  CHFPE_ERR_DIVERGED = -4,   /* non-finite expectation value, or the norm guard of chfpe_step tripped */
   CHFPE_ERR_STATE = -5       /* call sequence error (e.g. response before equilibrate/import) */
 };
 
@@ -95,7 +95,10 @@ int chfpe_element_index(const chfpe_handle* h, int32_t k, int32_t n_out[3]); /* 
 int chfpe_equilibrate(chfpe_handle* h, int64_t n_steps, double dt, double* residual_out);
 
 /* n_steps fourth-order Runge-Kutta steps of Eq. (8) :77-80 on every replica (R13: evaluated in the
-   Horner form of the same degree-4 polynomial in dt*L, the generator being linear and autonomous). */
+   Horner form of the same degree-4 polynomial in dt*L, the generator being linear and autonomous).
+   Norm guard: returns CHFPE_ERR_DIVERGED if, after the steps, the state of a replica is not finite or its sum of
+   squares exceeds 1e8 times its value at the last equilibrate / import / kick / response call (the literal W gauge
+   is unstable on a phase-space grid, reading R7).  The check is one reduction and synchronises the stream. */
 int chfpe_step(chfpe_handle* h, int64_t n_steps, double dt);
 
 /* Every element of every replica: X_k <- sum_s (dX/dq_s) (d/dp_s) X_k, Eq. (18) :131, literal (no sign; R3, R11). */

@@ -254,7 +254,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   h->K = pl.K; h->batch = pl.batch; h->n_arrays = pl.n_arrays; h->cells = pl.cells;
   h->state_doubles = (size_t)pl.K * pl.cells;
   h->red_blocks = pl.red_blocks;
-  h->initialised = false; h->launches = 0; h->prof = false; h->prof_used = 0;
+  h->initialised = false; h->launches = 0; h->prof = false; h->prof_used = 0; h->norm_ref_valid = false;
   h->coop_mode = env_int("CHFPE_COOP", 1);
   h->coop = h->coop_mode != 0;
   const int M = pl.M;
@@ -632,6 +632,10 @@ extern "C" int chfpe_profile_read(chfpe_handle* h, double* total_ms, int64_t* n_
 static int kick_slots(chfpe_handle* h, int b0, int nb, const chfpe_observable* X) {
   const size_t ss = 3 * h->state_doubles;
   DevObs o = to_dev(X);
+  if (h->op.scheme != CHFPE_COMPACT6 && env_int("CHFPE_KICK_BRICK", 1)) {   // in place on the brick layout where it applies
+    const int n = launch_kick_brick(h->op, o, h->y(b0), nb, ss, h->stream);
+    if (n > 0) { h->launches += n; return check_launch(h); }
+  }
   if (h->op.scheme == CHFPE_COMPACT6)
     h->launches += launch_kick_compact(h->op, h->ct, o, h->y(b0), h->va(b0), nb, ss, h->scratch, h->stream);
   else
@@ -660,6 +664,7 @@ static int fetch_results(chfpe_handle* h, long long n, double* host) {
 
 extern "C" int chfpe_equilibrate(chfpe_handle* h, int64_t n_steps, double dt, double* residual_out) {
   if (!h || n_steps < 0) return CHFPE_ERR_INVALID;
+  h->norm_ref_valid = false;
   DevObs none = to_dev(nullptr);
   h->launches += launch_init_eq(h->op, h->y(0), h->stream);
   const int mode = (h->op.gauge == CHFPE_GAUGE_SQRT_EQ) ? RED_SUMSQ : RED_SUM;   // Z_f = dV sum phi^2, Z_W = dV sum e^{-beta H}
@@ -689,13 +694,45 @@ extern "C" int chfpe_equilibrate(chfpe_handle* h, int64_t n_steps, double dt, do
   return CHFPE_OK;
 }
 
+// sum of squares of every slot's state -> host (synchronises the stream); non-finite values give CHFPE_ERR_DIVERGED
+static int slot_norms(chfpe_handle* h, std::vector<double>* out) {
+  DevObs none = to_dev(nullptr);
+  out->resize(h->batch);
+  h->launches += launch_reduce(h->op, none, RED_SUMSQ, h->y(0), 0, (long long)h->state_doubles, h->batch,
+                               3 * h->state_doubles, 1.0, h->partial, h->red_blocks, h->results, 1, h->stream);
+  int rc = check_launch(h);
+  if (rc) return rc;
+  return fetch_results(h, h->batch, out->data());
+}
+
+// Norm guard (SURVEY 8(b) errors): the literal W gauge of Eq. (8) is semi-discretely unstable on a (q,p) grid (R7;
+// 1e30 by t = 3 on a config-2-like grid), so a propagation reports divergence from the call that diverged: the sum of
+// squares of a slot must stay finite and below NORM_GROWTH times its value at the last equilibrate / import / kick /
+// response call.  One deterministic reduction and one 8-byte read per call (0.5 ms at config 4).
+static const double NORM_GROWTH = 1e8;
+
 extern "C" int chfpe_step(chfpe_handle* h, int64_t n_steps, double dt) {
   if (!h || n_steps < 0) return CHFPE_ERR_INVALID;
-  return step_slots(h, 0, h->batch, n_steps, dt);
+  if (n_steps == 0) return CHFPE_OK;
+  int rc;
+  if (!h->norm_ref_valid) {
+    rc = slot_norms(h, &h->norm_ref);
+    if (rc) return rc;
+    h->norm_ref_valid = true;
+  }
+  rc = step_slots(h, 0, h->batch, n_steps, dt);
+  if (rc) return rc;
+  std::vector<double> now;
+  rc = slot_norms(h, &now);
+  if (rc) return rc;
+  for (int b = 0; b < h->batch; b++)
+    if (h->norm_ref[b] > 0.0 && now[b] > NORM_GROWTH * h->norm_ref[b]) FAIL(h, CHFPE_ERR_DIVERGED, "norm growth guard: the propagation diverges");
+  return CHFPE_OK;
 }
 
 extern "C" int chfpe_kick(chfpe_handle* h, const chfpe_observable* X) {
   if (!h || !X) return CHFPE_ERR_INVALID;
+  h->norm_ref_valid = false;
   return kick_slots(h, 0, h->batch, X);
 }
 
@@ -717,6 +754,7 @@ extern "C" int chfpe_response_1d(chfpe_handle* h, const chfpe_observable* A, con
                                  int64_t n_samples, int64_t stride, double dt, double* R) {
   if (!h || !C || !R || n_samples < 0 || stride < 0) return CHFPE_ERR_INVALID;
   if (!h->initialised) FAIL(h, CHFPE_ERR_STATE, "response_1d before equilibrate/import");
+  h->norm_ref_valid = false;
   int rc = A ? kick_slots(h, 0, 1, A) : CHFPE_OK;
   if (rc) return rc;
   int64_t done = 0;
@@ -765,6 +803,7 @@ extern "C" int chfpe_response_2d(chfpe_handle* h, const chfpe_observable* A, con
                                  int32_t n2, double dt, double* R) {
   if (!h || !A || !B || !C || !t1 || !t2 || !R || n1 < 1 || n2 < 1) return CHFPE_ERR_INVALID;
   if (!h->initialised) FAIL(h, CHFPE_ERR_STATE, "response_2d before equilibrate/import");
+  h->norm_ref_valid = false;
   for (int i = 0; i < n1; i++) if (t1[i] < 0 || (i && t1[i] < t1[i - 1])) FAIL(h, CHFPE_ERR_INVALID, "t1_steps must be ascending and >= 0");
   for (int i = 0; i < n2; i++) if (t2[i] < 0 || (i && t2[i] < t2[i - 1])) FAIL(h, CHFPE_ERR_INVALID, "t2_steps must be ascending and >= 0");
   const size_t sbytes = sizeof(double) * h->state_doubles;
@@ -814,6 +853,7 @@ extern "C" int chfpe_response_3d(chfpe_handle* h, const chfpe_observable* A, con
                                  const int64_t* t2, int32_t n2, const int64_t* t3, int32_t n3, double dt, double* R) {
   if (!h || !A || !B || !C || !D || !t1 || !t2 || !t3 || !R || n1 < 1 || n2 < 1 || n3 < 1) return CHFPE_ERR_INVALID;
   if (!h->initialised) FAIL(h, CHFPE_ERR_STATE, "response_3d before equilibrate/import");
+  h->norm_ref_valid = false;
   // slot 0 carries the t1 trajectory.  A group of nb t1 samples owns slots [1, 1+nb) for its t2 trajectories and,
   // unless the t2 sample is the last one (then C is applied in place), slots [1+nb, 1+2nb) for the t3 replicas.
   const int nb_max = (n2 == 1) ? h->batch - 1 : (h->batch - 1) / 2;
@@ -876,6 +916,7 @@ extern "C" int chfpe_export_state(chfpe_handle* h, int32_t replica, double* dst,
 
 extern "C" int chfpe_import_state(chfpe_handle* h, int32_t replica, const double* src, int src_is_device) {
   if (!h || !src || replica < 0 || replica >= h->batch) return CHFPE_ERR_INVALID;
+  h->norm_ref_valid = false;
   if (src_is_device) {
     h->launches += launch_permute(h->op, src, h->y(replica), 1, h->stream);
   } else {

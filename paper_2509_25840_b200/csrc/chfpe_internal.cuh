@@ -110,6 +110,8 @@ struct chfpe_handle {
   int red_blocks;
   std::vector<int> elem;              // host copy [K][3]
   bool initialised;
+  bool norm_ref_valid;                // norm guard of chfpe_step: reference taken since the last non-propagating change
+  std::vector<double> norm_ref;       // per slot: sum of squares of the state at that point
   int64_t launches;
   int coop_mode;                      // CHFPE_COOP: 0 off, 1 tiny states only, 2 every L2-resident state
   bool coop;                          // persistent cooperative kernel allowed for L2-resident states
@@ -158,6 +160,8 @@ int launch_stage_pipe(const DevOp& op, const BrickPlan& bp, const double* in, co
 // out += c * (slaved-element coupling of every top-level element), see terminator_value in chfpe_kernels.cu
 int launch_terminator_add(const DevOp& op, const double* in, double* out, double c, int nb, size_t slot_stride,
                           cudaStream_t s);
+// x <- Kick_obs(x) in place, one CTA per p-brick (M >= 2, explicit schemes); returns 0 if it does not apply
+int launch_kick_brick(const DevOp& op, const DevObs& o, double* x, int nb, size_t slot_stride, cudaStream_t s);
 // out = Kick_obs(in) on every element, slots [b0, b0+nb)
 int launch_kick(const DevOp& op, const DevObs& o, const double* in, double* out, int nb, size_t slot_stride,
                 cudaStream_t s);

@@ -192,6 +192,56 @@ __global__ void __launch_bounds__(256) k_kick_generic(DevOp op, DevObs ob, const
   out[boff + cell] = acc;
 }
 
+// Kick in place on the brick layout (M >= 2): one CTA per p-brick (all momenta of one (element, q-point), contiguous).
+// The kick is local to the brick -- p-derivatives only, dX/dq_s depends on q alone -- so the brick is staged in shared
+// memory, every cell is formed from it and written back to where it came from: one read and one write of the state,
+// no second array and no copy back (the generic kernel above needs both).
+template <int M>
+__global__ void __launch_bounds__(256) k_kick_brick(DevOp op, DevObs ob, double* x, size_t slot_stride) {
+  extern __shared__ __align__(16) double kb[];
+  const long long ql = blockIdx.x;
+  const int k = blockIdx.y;
+  const int pb = (int)op.pb;
+  double* X = x + (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells + (size_t)ql * pb;
+  for (int i = threadIdx.x; i < pb / 2; i += 256)
+    reinterpret_cast<double2*>(kb)[i] = __ldcs(reinterpret_cast<const double2*>(X) + i);
+  if ((pb & 1) && threadIdx.x == 0) kb[pb - 1] = X[pb - 1];
+  int iq[M];
+  {
+    long long r = ql;
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) { iq[s] = (int)(r % op.n[s]); r /= op.n[s]; }
+  }
+  double g[M];                                                      // dX/dq_s at this q-point, Eq. (13)-(14), (18)
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    g[s] = ob.lin_q[s];
+#pragma unroll
+    for (int r = 0; r < M; r++) g[s] = fma(0.5 * (ob.quad[s][r] + ob.quad[r][s]), op.x0[r] + iq[r] * op.h[r], g[s]);
+  }
+  const bool wide = (op.scheme == CHFPE_CENTRAL4);
+  __syncthreads();
+  for (int c = threadIdx.x; c < pb; c += 256) {
+    int r = c;
+    const double xc = kb[c];
+    double acc = 0.0;
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) {                              // p_M is the fastest axis of the brick
+      const int ap = M + s, n = op.n[ap], st = (int)op.st[ap];
+      const int i = r % n;
+      r /= n;
+      const double fp1 = (i + 1 < n) ? kb[c + st] : 0.0, fm1 = (i >= 1) ? kb[c - st] : 0.0;
+      double d = op.c1[ap] * (fp1 - fm1);
+      if (wide) {
+        const double fp2 = (i + 2 < n) ? kb[c + 2 * st] : 0.0, fm2 = (i >= 2) ? kb[c - 2 * st] : 0.0;
+        d = fma(op.c2[ap], fp2 - fm2, d);
+      }
+      acc = fma(g[s], fma(op.kup[s] * (op.x0[ap] + i * op.h[ap]), xc, d), acc);
+    }
+    X[c] = acc;
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Deterministic reductions: per-block partials (warp shuffle -> shared) then a fixed-order final pass.
 // ------------------------------------------------------------------------------------------------
@@ -368,6 +418,22 @@ int launch_stage(const DevOp& op, const double* in, const double* y, double* out
 #define CALL(MM) k_stage_generic<MM><<<grid, 256, 0, s>>>(op, in, y, out, a, c, slot_stride)
   DISPATCH_M(op.M, CALL);
 #undef CALL
+  return 1;
+}
+
+// in-place kick on the brick layout; returns 0 (nothing launched) where it does not apply
+int launch_kick_brick(const DevOp& op, const DevObs& o, double* x, int nb, size_t slot_stride, cudaStream_t s) {
+  const size_t smem = sizeof(double) * (size_t)op.pb;
+  if (op.M < 2 || op.scheme == CHFPE_COMPACT6 || smem > 200 * 1024 || op.nqc > 0x7fffffffLL) return 0;
+  static bool optin[4] = {false, false, false, false};
+  if (!optin[op.M]) {
+    if (op.M == 2) cudaFuncSetAttribute(k_kick_brick<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    else cudaFuncSetAttribute(k_kick_brick<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    optin[op.M] = true;
+  }
+  dim3 grid((unsigned)op.nqc, op.K, nb);
+  if (op.M == 2) k_kick_brick<2><<<grid, 256, smem, s>>>(op, o, x, slot_stride);
+  else k_kick_brick<3><<<grid, 256, smem, s>>>(op, o, x, slot_stride);
   return 1;
 }
 

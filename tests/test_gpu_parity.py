@@ -678,3 +678,31 @@ def test_terminator_rejected_where_it_is_not_implemented():
         P.CHFPE(ci.config("cfg1", scheme="compact6", closure="terminator"))
     with pytest.raises(P.ChfpeError):
         P.Hermite(ci.config("cfg1", np=[6], closure="terminator"))
+
+
+def test_step_reports_divergence_from_the_call_that_diverged():
+    """Norm guard of chfpe_step (SURVEY 8(b) errors): the literal W gauge is semi-discretely unstable on a (q,p) grid
+    (reading R7; a config-2-like run reaches 1e30 by t = 3), so a propagation must return
+    CHFPE_ERR_DIVERGED from the chfpe_step call in which the norm left its bound -- long before any value is
+    non-finite -- while the default sqrt(W_eq) gauge runs through the same protocol untouched."""
+    P = gpu_mod()
+    base = dict(nq=[64], np=[64], depth=6, qmin=[-8.0], qmax=[8.0], pmin=[-8.0], pmax=[8.0])
+    mu = make_obs(P, ci.observable("mu", 1))
+    g = P.CHFPE(ci.config("cfg2", gauge="w", **base))
+    g.equilibrate(); g.kick(mu)
+    t_div = None
+    for i in range(16):
+        try:
+            g.step(250, 1e-3)
+        except P.ChfpeError as exc:
+            assert "-4" in str(exc) or "diverg" in str(exc).lower(), exc
+            t_div = 0.25 * (i + 1)
+            break
+    assert t_div is not None and t_div <= 3.0, t_div
+    assert np.all(np.isfinite(g.export_state()))                 # caught on the norm, not on a NaN
+    g.close()
+    g = P.CHFPE(ci.config("cfg2", gauge="sqrt_eq", **base))
+    g.equilibrate(); g.kick(mu)
+    for i in range(16):
+        g.step(250, 1e-3)
+    g.close()
