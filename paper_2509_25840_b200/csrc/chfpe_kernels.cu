@@ -242,6 +242,75 @@ __global__ void __launch_bounds__(256) k_kick_brick(DevOp op, DevObs ob, double*
   }
 }
 
+// The same with 128-bit shared accesses (even fastest momentum axis): a thread owns a pair of cells adjacent along
+// the fastest axis and marches along p_1 with a five-deep register window, so a pair costs 1 + 2 (+ 4 for M = 3)
+// LDS.128 instead of 2 x 13 LDS.64, and no index division per cell.
+template <int M>
+__global__ void __launch_bounds__(256) k_kick_brick_pairs(DevOp op, DevObs ob, double* x, size_t slot_stride) {
+  extern __shared__ __align__(16) double kb[];
+  const long long ql = blockIdx.x;
+  const int k = blockIdx.y;
+  const int pb = (int)op.pb;
+  double* X = x + (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells + (size_t)ql * pb;
+  for (int i = threadIdx.x; i < pb / 2; i += 256)
+    reinterpret_cast<double2*>(kb)[i] = __ldcs(reinterpret_cast<const double2*>(X) + i);
+  int iq[M];
+  {
+    long long r = ql;
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) { iq[s] = (int)(r % op.n[s]); r /= op.n[s]; }
+  }
+  double g[M];                                                      // dX/dq_s at this q-point, Eq. (13)-(14), (18)
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    g[s] = ob.lin_q[s];
+#pragma unroll
+    for (int r = 0; r < M; r++) g[s] = fma(0.5 * (ob.quad[s][r] + ob.quad[r][s]), op.x0[r] + iq[r] * op.h[r], g[s]);
+  }
+  const bool wide = (op.scheme == CHFPE_CENTRAL4);
+  const int n1 = op.n[M], nf = op.n[2 * M - 1], nm = (M == 3) ? op.n[M + 1] : 1;   // slowest, fastest, middle momentum axis
+  const int plane = nm * nf, plane2 = plane / 2, nf2 = nf / 2;
+  const int af = 2 * M - 1, am = M + 1;
+  const double c1a = op.c1[M] * g[0], c2a = wide ? op.c2[M] * g[0] : 0.0;            // p_1
+  const double c1f = op.c1[af] * g[M - 1], c2f = wide ? op.c2[af] * g[M - 1] : 0.0;  // fastest axis
+  const double c1m = (M == 3) ? op.c1[am] * g[1] : 0.0, c2m = (M == 3 && wide) ? op.c2[am] * g[1] : 0.0;
+  __syncthreads();
+  const double2* K2 = reinterpret_cast<const double2*>(kb);
+  double2* X2 = reinterpret_cast<double2*>(X);
+  const double2 z = make_double2(0.0, 0.0);
+  for (int pos = threadIdx.x; pos < plane2; pos += 256) {
+    const int im = pos / nf2, jf = pos - im * nf2;                  // middle index, pair index along the fastest axis
+    const double pfa = op.x0[af] + (2 * jf) * op.h[af], pfb = pfa + op.h[af];
+    // pointwise part kappa^up (g_f p_f + g_m p_m) x, and g_1 kappa^up p_1 x per plane
+    double ka = g[M - 1] * op.kup[M - 1] * pfa, kbb = g[M - 1] * op.kup[M - 1] * pfb;
+    if (M == 3) { const double pm = g[1] * op.kup[1] * (op.x0[am] + im * op.h[am]); ka += pm; kbb += pm; }
+    double2 w0 = z, w1 = z, w2 = K2[pos], w3 = (n1 > 1) ? K2[plane2 + pos] : z, w4;   // planes i1-2 .. i1+2
+    for (int i1 = 0; i1 < n1; i1++) {
+      w4 = (i1 + 2 < n1) ? K2[(i1 + 2) * plane2 + pos] : z;
+      const int c = i1 * plane2 + pos;
+      const double p1k = g[0] * op.kup[0] * (op.x0[M] + i1 * op.h[M]);
+      double ax = fma(c2a, w4.x - w0.x, c1a * (w3.x - w1.x)) + (ka + p1k) * w2.x;
+      double ay = fma(c2a, w4.y - w0.y, c1a * (w3.y - w1.y)) + (kbb + p1k) * w2.y;
+      {                                                             // fastest axis: pairs to the left and right
+        const double2 l = (jf >= 1) ? K2[c - 1] : z, r = (jf + 1 < nf2) ? K2[c + 1] : z;
+        // cells (a, b) = (2 jf, 2 jf + 1): neighbours of a: l.y | b ; of b: a | r.x ; second neighbours: l.x | r.x ; l.y | r.y
+        ax = fma(c1f, w2.y - l.y, ax); ay = fma(c1f, r.x - w2.x, ay);
+        ax = fma(c2f, r.x - l.x, ax);  ay = fma(c2f, r.y - l.y, ay);
+      }
+      if (M == 3) {
+        const double2 u1 = (im + 1 < nm) ? K2[c + nf2] : z, d1 = (im >= 1) ? K2[c - nf2] : z;
+        ax = fma(c1m, u1.x - d1.x, ax); ay = fma(c1m, u1.y - d1.y, ay);
+        if (wide) {
+          const double2 u2 = (im + 2 < nm) ? K2[c + 2 * nf2] : z, d2 = (im >= 2) ? K2[c - 2 * nf2] : z;
+          ax = fma(c2m, u2.x - d2.x, ax); ay = fma(c2m, u2.y - d2.y, ay);
+        }
+      }
+      __stcs(X2 + c, make_double2(ax, ay));
+      w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Deterministic reductions: per-block partials (warp shuffle -> shared) then a fixed-order final pass.
 // ------------------------------------------------------------------------------------------------
@@ -432,6 +501,16 @@ int launch_kick_brick(const DevOp& op, const DevObs& o, double* x, int nb, size_
     optin[op.M] = true;
   }
   dim3 grid((unsigned)op.nqc, op.K, nb);
+  if (op.n[2 * op.M - 1] % 2 == 0 && ((op.cells * sizeof(double)) % 16) == 0 && (slot_stride % 2) == 0) {   // 128-bit pairs
+    if (!optin[op.M - 2]) {
+      if (op.M == 2) cudaFuncSetAttribute(k_kick_brick_pairs<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      else cudaFuncSetAttribute(k_kick_brick_pairs<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      optin[op.M - 2] = true;
+    }
+    if (op.M == 2) k_kick_brick_pairs<2><<<grid, 256, smem, s>>>(op, o, x, slot_stride);
+    else k_kick_brick_pairs<3><<<grid, 256, smem, s>>>(op, o, x, slot_stride);
+    return 1;
+  }
   if (op.M == 2) k_kick_brick<2><<<grid, 256, smem, s>>>(op, o, x, slot_stride);
   else k_kick_brick<3><<<grid, 256, smem, s>>>(op, o, x, slot_stride);
   return 1;
