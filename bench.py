@@ -39,7 +39,9 @@ HBM_NOMINAL_GBS = 8000.0                   # "about 8 TB/s", BASELINE.json north
 
 
 def profiled_traffic(pattern="r*_stage_kernel_ncu_full.txt", key="dram_bytes_per_launch"):
-    """DRAM bytes per launch of the stage kernel from the committed ncu --set full summary (profiles/), or None."""
+    """A `key=value` figure of the stage kernel from the latest committed ncu --set full summary (profiles/), or None
+    (DRAM bytes per launch by default).  ncu cannot run inside a timed benchmark, so these come from the committed
+    capture of the same command; `roofline.traffic_source` names the file."""
     import glob
     import re
     best = None
@@ -48,6 +50,22 @@ def profiled_traffic(pattern="r*_stage_kernel_ncu_full.txt", key="dram_bytes_per
         if m:
             best = float(m.group(1))
     return best
+
+
+def profile_file(pattern="r*_stage_kernel_ncu_full.txt"):
+    import glob
+    fs = sorted(glob.glob(os.path.join(ROOT, "profiles", pattern)))
+    return os.path.relpath(fs[-1], ROOT) if fs else None
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 def measured_peaks():
@@ -107,10 +125,13 @@ def obs(mod, kind, M):
     return mod.make_observable(d["c0"], d["lin_q"], d["quad"], d["lin_p"])
 
 
-def cpu_oracle_time(cfg, steps, warmup=0):
+def cpu_oracle_time(cfg, steps, warmup=0, threads=0):
     """Time the oracle as it stands: equilibrium, kick(mu), then `steps` x (RK4 step + <mu>).  Returns
-    (seconds, threads, K, cells)."""
+    (seconds, threads, K, cells).  threads = 0: all cores (the OpenMP default), else that many."""
     import oracle
+    all_threads = oracle.set_threads(0)
+    if threads:
+        oracle.set_threads(threads)
     o = oracle.RefCHFPE(cfg)
     mu = obs(oracle, "mu", cfg["n_modes"])
     o.equilibrate()
@@ -123,7 +144,27 @@ def cpu_oracle_time(cfg, steps, warmup=0):
     dt = time.perf_counter() - t0
     K, cells = o.K, o.cells
     o.close()
-    return dt, oracle.set_threads(0), K, cells
+    used = oracle.set_threads(0)
+    oracle.set_threads(all_threads)
+    return dt, used, K, cells
+
+
+def cpu_baseline_record(workload):
+    """SURVEY 8(d) "timing the oracle beside it": all-core time on the full workload (one RK4 step + <mu>, about 6 s at
+    config 4) and single-core time on the 12^6 shrink of the same model (a full-size single-core step would take
+    90 s), both as cell-updates/s, with the core count and the CPU model."""
+    cfg_c, sample = pick_cpu_sample(workload)
+    tc, threads, Kc, cells_c = cpu_oracle_time(cfg_c, 1, 0)
+    rec = {"value": cells_c / tc, "unit": UNIT, "cores": threads, "kind": "oracle",
+           "sample": "%s, 1 RK4 step + <mu> (%.1f s)" % (sample, tc), "nproc": os.cpu_count(), "cpu_model": cpu_model()}
+    small = {"cfg4": "cfg4s12", "cfg5": "cfg4s12", "cfg3": "cfg3s"}.get(workload)
+    if small:
+        c1 = ci.config(small)
+        t1, th1, K1, cells1 = cpu_oracle_time(c1, 1, 0, threads=1)
+        rec["value_1core"] = cells1 / t1
+        rec["sample_1core"] = "%s (%s grid, same model), 1 RK4 step + <mu> on 1 core (%.1f s)" % (
+            small, "x".join(str(x) for x in ci.grid_shape(c1)), t1)
+    return rec
 
 
 def pick_cpu_sample(workload):
@@ -150,6 +191,8 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
+    if args.protocol == "2d":
+        return run_2d_reference(args)
     cfg, sample = pick_cpu_sample(args.workload)
     steps = max(1, args.steps)
     # keep the whole run within a few minutes: the oracle does ~1e7 value-updates/s on 8 cores
@@ -166,7 +209,8 @@ def run_reference(args):
             "config": {"workload": args.workload, "sample": sample, "K": K, "cells": cells,
                        "note": "CPU oracle (oracle/chfpe_ref.c, OpenMP) on the host cores; a deliberately plain program"},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
-                             "sample": "%s, %d RK4 steps + <mu> each" % (sample, steps)},
+                             "sample": "%s, %d RK4 steps + <mu> each" % (sample, steps), "nproc": os.cpu_count(),
+                             "cpu_model": cpu_model()},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -195,6 +239,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     cfg = ci.config(args.workload)
+    cfg4 = args.workload == "cfg4"
     M = cfg["n_modes"]
     g = P.CHFPE(cfg, batch=1, device="cuda:%d" % local)
     mu = obs(P, "mu", M)
@@ -252,7 +297,11 @@ def run_ours(args):
         # dominant kernel: the fused RK-stage kernel.  Algorithmic (compulsory) bytes per launch, DESIGN.md section 5:
         # stage 1 reads y and writes v (16 B/value), stages 2-4 read v, read y, write the next v (24 B/value);
         # averaged over the four launches of a step: 22 B/value/launch = 88 B/value/step.
-        alg_bytes_launch = values * 22.0
+        # Reported two ways: `achieved` / `frac` use the survey's fixed F_alg accounting, 128 B per value
+        # per step = 32 B per value per launch (classical four-array RK4), so traffic the implementation saves shows;
+        # `frac_compulsory_88B` uses the 22 B per value per launch this three-array Horner form must move.
+        alg_bytes_launch = values * (BYTES_PER_VALUE_STEP_SURVEY / 4.0)
+        compulsory_bytes_launch = values * 22.0
         kern_ms = stage_ms / max(stage_n, 1)
         achieved = alg_bytes_launch / (kern_ms * 1e-3) / 1e9
         line = {
@@ -271,23 +320,81 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": profiled_traffic() if args.workload == "cfg4" else None, "peak_source": peak_src, "kernel": "RK stage (k_stage_*)",
+                         "accounting": "achieved/frac: SURVEY 8(d) F_alg, 128 B per value per step = 32 B per value per "
+                                       "launch, against the measured copy peak; frac_compulsory_88B: the 22 B per value "
+                                       "per launch of the three-array Horner form",
+                         "frac_compulsory_88B": compulsory_bytes_launch / (kern_ms * 1e-3) / 1e9 / peak,
+                         "frac_of_8TBs": achieved / HBM_NOMINAL_GBS,
+                         "traffic": profiled_traffic() if cfg4 else None,
+                         "fp64_pipe_pct": profiled_traffic(key="fp64_pipe_pct") if cfg4 else None,
+                         "l2_hit_pct": profiled_traffic(key="l2_hit_pct") if cfg4 else None,
+                         "traffic_source": ("ncu --set full capture of the same command, %s" % profile_file()) if cfg4 else None,
+                         "peak_source": peak_src, "kernel": "RK stage (%s)" % g.stage_kernel_name(),
                          "kernel_ms": kern_ms, "kernel_launches_timed": int(stage_n),
                          "kernel_share_of_step": stage_ms / ms,
                          "algorithmic_bytes_per_launch": alg_bytes_launch,
+                         "compulsory_bytes_per_launch": compulsory_bytes_launch,
                          "frac_survey_128B_of_8TBs": values * BYTES_PER_VALUE_STEP_SURVEY * steps
                          / (ms * 1e-3) / 1e9 / HBM_NOMINAL_GBS},
         }
         if world == 1 and not args.no_cpu:
-            cfg_c, sample = pick_cpu_sample(args.workload)
-            tc, threads, Kc, cells_c = cpu_oracle_time(cfg_c, 1, 0)
-            line["cpu_baseline"] = {"value": cells_c / tc, "unit": UNIT, "cores": threads, "kind": "oracle",
-                                    "sample": "%s, 1 RK4 step + <mu> (%.1f s)" % (sample, tc)}
-        print(json.dumps(line))
+            line["cpu_baseline"] = cpu_baseline_record(args.workload)
     g.close()
+    del X0
+    torch.cuda.empty_cache()
+    if rank == 0:
+        if world == 1 and not args.no_2d:                 # third part of the metric: 2D THz-Raman wall time (config 5)
+            try:
+                line["two_d"] = two_d_record(P, batch=5, n1=4, n2=8)
+            except Exception as exc:                      # e.g. not enough device memory for five replica slots
+                line["two_d"] = {"unavailable": str(exc)[:200]}
+        print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
     return 0
+
+
+FULL_2D_REPLICA_STEPS = 63 + 64 * 255                    # BASELINE configs[4]: 64 t1 x 256 t2 delays, stride 1
+
+
+def two_d_record(P, batch=5, n1=4, n2=8, workload="cfg5"):
+    """Third part of BASELINE.json's metric, "2D THz-Raman wall time": chfpe_response_2d (A = mu, B = C = alpha) on
+    config 5 (20^6 grid, 20 elements, t1 replicas batched into HBM) timed end to end on a bounded n1 x n2 sample of
+    the delay grid -- trajectory steps, replica copies, kicks, batched propagation, expectations, D2H of R -- and
+    extrapolated linearly in replica-steps to the full 64 x 256 grid (labelled as such)."""
+    import numpy as np
+    import torch
+    cfg = ci.config(workload)
+    M = cfg["n_modes"]
+    g = P.CHFPE(cfg, batch=batch)
+    try:
+        mu, al = obs(P, "mu", M), obs(P, "alpha", M)
+        g.equilibrate(residual=False)
+        g.response_2d(mu, al, al, [0, 1], [0, 1], cfg["dt"])          # warm-up
+        g.equilibrate(residual=False)
+        t1, t2 = list(range(n1)), list(range(n2))
+        n0 = g.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        R = g.response_2d(mu, al, al, t1, t2, cfg["dt"])
+        e1.record()
+        torch.cuda.synchronize()
+        sec = e0.elapsed_time(e1) * 1e-3
+        rsteps = (n1 - 1) + n1 * (n2 - 1)                           # trajectory steps + replica steps
+        rec = {"metric": "2D THz-Raman wall time", "workload": workload + " chfpe_response_2d, A=mu B=alpha C=alpha",
+               "grid": "x".join(str(x) for x in g.shape), "K": g.K, "batch_slots": batch,
+               "workspace_GB": P.workspace_bytes(cfg, batch) / 1e9, "stage_kernel": g.stage_kernel_name(),
+               "timed_sample": "%d t1 x %d t2 delays, stride 1" % (n1, n2), "sample_seconds": sec,
+               "replica_steps_timed": rsteps, "ms_per_replica_step": 1e3 * sec / rsteps,
+               "wall_time_s_64x256_extrapolated": sec * FULL_2D_REPLICA_STEPS / rsteps, "extrapolated": True,
+               "full_protocol": "64 t1 x 256 t2 = %d replica-steps, linear in replica-steps" % FULL_2D_REPLICA_STEPS,
+               "cell_updates_per_s": g.cells * rsteps / sec, "gpu_launches": int(g.launch_count() - n0),
+               "finite": bool(np.all(np.isfinite(R)))}
+    finally:
+        g.close()
+        torch.cuda.empty_cache()
+    return rec
 
 
 def run_2d(args):
@@ -298,11 +405,28 @@ def run_2d(args):
     import numpy as np
     import torch
     import paper_2509_25840_b200 as P
+    from paper_2509_25840_b200 import sharding
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    # the t1 rows of R2 shard over the ranks (round-robin), every rank advances its own copy of the t1
+    # trajectory, one NCCL all_gather of n1 x n2 doubles at the end; --sharded runs the same path with one rank
+    dist = None
+    if world > 1 or args.sharded:
+        import torch.distributed as dist
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29517")
+            os.environ.setdefault("RANK", "0")
+            os.environ.setdefault("WORLD_SIZE", "1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     herm = args.representation == "hermite"             # row f1: the same protocol on the Hermite representation (cfg4h)
     wl = args.workload if args.workload != "cfg4" else ("cfg4h" if herm else "cfg5")
     cfg = ci.config(wl, scheme=args.scheme) if herm else ci.config(wl)
     M = cfg["n_modes"]
-    g = P.Hermite(cfg, batch=args.batch) if herm else P.CHFPE(cfg, batch=args.batch)
+    dev = "cuda:%d" % local
+    g = P.Hermite(cfg, batch=args.batch, device=dev) if herm else P.CHFPE(cfg, batch=args.batch, device=dev)
     mu, al = obs(P, "mu", M), obs(P, "alpha", M)
     g.equilibrate(residual=False)
     n1, n2 = args.n1, args.n2
@@ -311,16 +435,34 @@ def run_2d(args):
     g.equilibrate(residual=False)
     n0 = g.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
     torch.cuda.synchronize()
     e0.record()
-    R = g.response_2d(mu, al, al, t1, t2, cfg["dt"])
+    if dist is not None:
+        R = sharding.response_2d_sharded(g, mu, al, al, t1, t2, cfg["dt"], device=dev)
+    else:
+        R = g.response_2d(mu, al, al, t1, t2, cfg["dt"])
     e1.record()
+    if dist is not None:
+        dist.barrier()
     torch.cuda.synchronize()
-    sec = e0.elapsed_time(e1) * 1e-3
-    rsteps = (n1 - 1) + n1 * (n2 - 1)                               # trajectory steps + replica steps
-    full = 63 + 64 * 255
+    tms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)              # time = max over ranks
+    sec = float(tms[0]) * 1e-3
+    rsteps = (n1 - 1) + n1 * (n2 - 1)                               # trajectory steps + replica steps (whole job)
+    full = FULL_2D_REPLICA_STEPS
+    if rank != 0:
+        g.close()
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
     line = {"metric": "2D THz-Raman wall time", "value": sec * full / rsteps, "unit": "s", "higher_is_better": False,
-            "n_gpus": 1, "dtype": "f64", "data": "synthetic", "extrapolated": True,
+            "n_gpus": world, "dtype": "f64", "data": "synthetic", "extrapolated": True,
+            "scaling": "strong" if world > 1 else "weak",
+            "parallelism": ("t1 rows round-robin over %d ranks, one NCCL all_gather of %d doubles" % (world, n1 * n2))
+            if dist is not None else "single GPU",
             "config": {"workload": wl + (" chfpe_hermite_response_2d" if herm else " response_2d"),
                        "grid": "x".join(str(x) for x in g.shape), "K": g.K, "batch_slots": args.batch,
                        "workspace_GB": (P.hermite_workspace_bytes(cfg, args.batch) if herm
@@ -332,6 +474,36 @@ def run_2d(args):
             "gpu_launches": int(g.launch_count() - n0), "finite": bool(np.all(np.isfinite(R)))}
     print(json.dumps(line))
     g.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_2d_reference(args):
+    """Reference arm of --protocol 2d: the CPU oracle's response_2d as it stands, on the 12^6 shrink of config 5's model
+    (a full 20^6 replica-step takes 20 s on 16 cores), scaled by the cell count and extrapolated to 64 x 256 delays."""
+    import oracle
+    cfg = ci.config("cfg4s12")
+    o = oracle.RefCHFPE(cfg)
+    M = cfg["n_modes"]
+    mu, al = obs(oracle, "mu", M), obs(oracle, "alpha", M)
+    o.equilibrate()
+    n1, n2 = 2, 3
+    t0 = time.perf_counter()
+    o.response_2d(mu, al, al, list(range(n1)), list(range(n2)), cfg["dt"])
+    sec = time.perf_counter() - t0
+    rsteps = (n1 - 1) + n1 * (n2 - 1)
+    scale = 20.0 ** 6 / o.cells
+    val = sec / rsteps * scale * FULL_2D_REPLICA_STEPS
+    line = {"impl": "reference", "metric": "2D THz-Raman wall time", "value": val, "unit": "s", "higher_is_better": False,
+            "n_gpus": args.gpus, "dtype": "f64", "data": "synthetic", "extrapolated": True,
+            "config": {"workload": "cfg5 response_2d", "sample": "CPU oracle on the 12^6 grid of the same model, %d t1 x %d t2 "
+                       "delays (%.1f s), scaled by cells (x%.1f) and to 16383 replica-steps" % (n1, n2, sec, scale)},
+            "cpu_baseline": {"value": val, "unit": "s", "cores": oracle.set_threads(0), "kind": "oracle",
+                             "sample": "12^6 proxy, scaled", "nproc": os.cpu_count(), "cpu_model": cpu_model()},
+            "e2e": {"value": val, "unit": "s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    o.close()
+    print(json.dumps(line))
     return 0
 
 
@@ -476,6 +648,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--no-2d", action="store_true", help="skip the two_d sub-record (config 5, 154 GB of device memory)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="--protocol 2d: go through sharding.response_2d_sharded + NCCL even with one rank")
     ap.add_argument("--protocol", default="step", choices=["step", "2d", "3d"],
                     help="'2d': time chfpe_response_2d on config 5 (secondary metric: 2D THz-Raman wall time); "
                          "'3d': time chfpe_response_3d (row f2) on --workload")

@@ -333,6 +333,11 @@ class CHFPE:
         self._ck(lib().chfpe_stage_kernel(self._h, C.byref(k)), "chfpe_stage_kernel")
         return ("generic", "brick", "pipe", "compact", "tma")[k.value]
 
+    def stage_kernel_name(self):
+        """Name of the CUDA kernel family behind stage_kernel() (for benchmark records)."""
+        return {"generic": "k_stage_generic", "brick": "k_stage_brick3", "pipe": "k_stage_pipe",
+                "compact": "k_compact_line passes", "tma": "k_stage_tma"}[self.stage_kernel()]
+
     def launch_count(self):
         n = C.c_int64()
         self._ck(lib().chfpe_launch_count(self._h, C.byref(n)), "chfpe_launch_count")

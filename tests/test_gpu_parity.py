@@ -3,6 +3,8 @@
 Tolerances (BASELINE.json north_star): per-step relative L2 <= 1e-12; response functions relative max
 error <= 1e-8.  Operator-level checks use 1e-13.  All tests need a GPU (`-m gpu`).
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -705,4 +707,33 @@ def test_step_reports_divergence_from_the_call_that_diverged():
     g.equilibrate(); g.kick(mu)
     for i in range(16):
         g.step(250, 1e-3)
+    g.close()
+
+
+def test_response_2d_sharded_over_nccl_world1():
+    """the multi-GPU path of the 2D response -- t1 rows round-robin over the ranks, one all_gather of
+    n1 x n2 doubles -- with a CUDA engine and the NCCL backend (one rank: what a 1-GPU box can run; the row partition
+    and the gather for world size 2 are covered on gloo in test_sharding_gloo.py).  Must equal the unsharded call."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    from paper_2509_25840_b200 import sharding
+    cfg = ci.config("cfg4s8", nq=[6, 6, 6], np=[6, 6, 6])
+    g, o = both(cfg, batch=3)
+    mu_g, _ = obs_pair("mu", 3)
+    al_g, _ = obs_pair("alpha", 3)
+    t1, t2 = [0, 2, 3, 7, 8], [0, 1, 4, 6]
+    g.equilibrate()
+    R_plain = g.response_2d(mu_g, al_g, al_g, t1, t2, cfg["dt"] * 10)
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        g.equilibrate()
+        R = sharding.response_2d_sharded(g, mu_g, al_g, al_g, t1, t2, cfg["dt"] * 10, device="cuda:0")
+    finally:
+        dist.destroy_process_group()
+    assert R.shape == R_plain.shape and np.array_equal(R, R_plain)
     g.close()
