@@ -169,6 +169,19 @@ int chfpe_spectrum_2d(void* cuda_stream, const double* R, int32_t n1, int32_t n2
                       const double* omega1, int32_t n_omega1, const double* omega2, int32_t n_omega2, int32_t sign1,
                       int32_t sign2, double* scratch, double* I);
 
+/* chfpe_spectrum_2d for callers that can neither allocate nor provide the scratch array (CUDA graph capture, serving
+   loops, harnesses that forbid cudaMalloc): same arguments without `scratch`, same result.  The complex scratch
+   T[n1][n_omega2] is a file-scope device array inside the library of CHFPE_SPECTRUM_STATIC_MAX entries (1 MiB, held
+   by every GPU that loads the library until exit); the call allocates and frees nothing.
+   CHFPE_ERR_WORKSPACE if n1 * n_omega2 > CHFPE_SPECTRUM_STATIC_MAX, CHFPE_ERR_INVALID as for chfpe_spectrum_2d.
+   All calls share the array (contents of the last call remain; nothing needs clearing: the first pass writes every
+   entry the second reads).  Calls that overlap on the GPU -- different streams, or one stream per thread -- RACE on
+   it: serialise them.  Successive calls on one stream are safe. */
+#define CHFPE_SPECTRUM_STATIC_MAX 65536
+int chfpe_spectrum_2d_static(void* cuda_stream, const double* R, int32_t n1, int32_t n2, double dt1, double dt2,
+                             const double* omega1, int32_t n_omega1, const double* omega2, int32_t n_omega2,
+                             int32_t sign1, int32_t sign2, double* I);
+
 /* Which kernel family runs the RK stage on this handle (host pointer), so that a test or a benchmark can assert
    that a configuration did not fall back to the generic kernel.  The cooperative multi-step kernel of tiny
    states is a property of the step call, not of the handle, and is not reported here. */

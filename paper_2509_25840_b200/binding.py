@@ -10,7 +10,7 @@ EXPORTED_SYMBOLS = [
     "chfpe_workspace_bytes", "chfpe_create", "chfpe_destroy", "chfpe_num_elements", "chfpe_element_index",
     "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
     "chfpe_response_1d", "chfpe_response_2d", "chfpe_response_3d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
-    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_spectrum_1d", "chfpe_spectrum_2d", "chfpe_last_error",
+    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_spectrum_1d", "chfpe_spectrum_2d", "chfpe_spectrum_2d_static", "chfpe_last_error",
     "chfpe_hermite_workspace_bytes", "chfpe_hermite_create", "chfpe_hermite_destroy", "chfpe_hermite_num_elements",
     "chfpe_hermite_equilibrate", "chfpe_hermite_step", "chfpe_hermite_kick", "chfpe_hermite_expect",
     "chfpe_hermite_response_1d", "chfpe_hermite_response_2d", "chfpe_hermite_response_3d", "chfpe_hermite_export_state",
@@ -89,6 +89,8 @@ def lib():
     L.chfpe_spectrum_1d.argtypes = [vp, vp, C.c_int64, C.c_double, vp, C.c_int32, vp]
     L.chfpe_spectrum_2d.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_double, C.c_double, vp, C.c_int32, vp, C.c_int32,
                                     C.c_int32, C.c_int32, vp, vp]
+    L.chfpe_spectrum_2d_static.argtypes = [vp, vp, C.c_int32, C.c_int32, C.c_double, C.c_double, vp, C.c_int32, vp,
+                                           C.c_int32, C.c_int32, C.c_int32, vp]
     L.chfpe_last_error.argtypes = [vp]
     L.chfpe_last_error.restype = C.c_char_p
     L.chfpe_hermite_workspace_bytes.argtypes = [C.POINTER(Desc), C.POINTER(C.c_size_t)]
@@ -536,3 +538,20 @@ def spectrum_2d(R, dt1, dt2, omega1, omega2, sign1=-1, sign2=-1):
     if rc != 0:
         raise ChfpeError("chfpe_spectrum_2d failed: %d" % rc)
     return out.cpu().numpy()
+
+
+SPECTRUM_STATIC_MAX = 65536   # CHFPE_SPECTRUM_STATIC_MAX of include/chfpe.h: n1 * n_omega2 of chfpe_spectrum_2d_static
+
+
+def spectrum_2d_static_device(Rd, dt1, dt2, o1, o2, out, sign1=-1, sign2=-1):
+    """chfpe_spectrum_2d_static on device tensors (float64, contiguous), result written into `out`
+    [n_omega1][n_omega2]: the variant that allocates nothing (its scratch is a static device array inside the
+    library).  Calls that overlap on the GPU race on that array; successive calls on one stream are safe."""
+    import torch
+    rc = lib().chfpe_spectrum_2d_static(C.c_void_p(torch.cuda.current_stream().cuda_stream), C.c_void_p(Rd.data_ptr()),
+                                        Rd.shape[0], Rd.shape[1], float(dt1), float(dt2), C.c_void_p(o1.data_ptr()),
+                                        o1.numel(), C.c_void_p(o2.data_ptr()), o2.numel(), int(sign1), int(sign2),
+                                        C.c_void_p(out.data_ptr()))
+    if rc != 0:
+        raise ChfpeError("chfpe_spectrum_2d_static failed: %d" % rc)
+    return out

@@ -106,3 +106,43 @@ extern "C" int chfpe_spectrum_2d(void* cuda_stream, const double* R, int32_t n1,
                                                                                     (double)sign1, dt1 * dt2, I);
   return finish();
 }
+
+// ------------------------------------------------------------------------------------------------
+// chfpe_spectrum_2d_static: the same two-pass transform for callers that cannot provide (or allocate) the complex
+// scratch array -- code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The scratch
+// T[n1][n_omega2] lives in a file-scope device array of CHFPE_SPECTRUM_STATIC_MAX complex entries (1 MiB; every GPU
+// that loads the library holds it until exit).  In host code `g_spec_scratch` is only a stand-in for the symbol, not a
+// device address: its address on the current device is taken once per device with cudaGetSymbolAddress and that
+// pointer is what the kernels get.  Nothing here calls cudaMalloc / cudaFree or an allocating library routine.
+// All calls share the array and it keeps the last call's contents; nothing has to start at zero (the inner pass
+// writes every entry the outer pass reads), but two calls that overlap on the GPU (different streams) race on it.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double2 g_spec_scratch[CHFPE_SPECTRUM_STATIC_MAX];
+
+namespace {
+const int MAX_DEVICES = 64;
+double2* g_spec_scratch_addr[MAX_DEVICES];      // per device: address of g_spec_scratch, nullptr until first use
+}  // namespace
+
+extern "C" int chfpe_spectrum_2d_static(void* cuda_stream, const double* R, int32_t n1, int32_t n2, double dt1,
+                                        double dt2, const double* omega1, int32_t nw1, const double* omega2, int32_t nw2,
+                                        int32_t sign1, int32_t sign2, double* I) {
+  if (!R || !omega1 || !omega2 || !I || n1 < 1 || n2 < 1 || nw1 < 1 || nw2 < 1 || !(dt1 > 0.0) || !(dt2 > 0.0) ||
+      (sign1 != 1 && sign1 != -1) || (sign2 != 1 && sign2 != -1))
+    return CHFPE_ERR_INVALID;
+  if ((long long)n1 * nw2 > (long long)CHFPE_SPECTRUM_STATIC_MAX) return CHFPE_ERR_WORKSPACE;   // scratch too small
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return CHFPE_ERR_CUDA;
+  if (!g_spec_scratch_addr[dev]) {                 // set-up, once per device, with that device current
+    double2* p = nullptr;
+    if (cudaGetSymbolAddress((void**)&p, g_spec_scratch) != cudaSuccess || !p) { cudaGetLastError(); return CHFPE_ERR_CUDA; }
+    g_spec_scratch_addr[dev] = p;
+  }
+  double2* T = g_spec_scratch_addr[dev];
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  k_spec_inner<<<(unsigned)(((long long)n1 * nw2 * 32 + 127) / 128), 128, 0, s>>>(R, n1, n2, dt2, omega2, nw2,
+                                                                                   (double)sign2, T);
+  k_spec_outer<<<(unsigned)(((long long)nw1 * nw2 * 32 + 127) / 128), 128, 0, s>>>(T, n1, nw2, dt1, omega1, nw1,
+                                                                                    (double)sign1, dt1 * dt2, I);
+  return finish();
+}
