@@ -581,7 +581,8 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
 // (P1, P2, P3, NPART, NSEG, SLOTS, RING)
 #define TMA_SPECIALISATIONS(X) \
   X(16, 16, 16, 2, 2, 5, true) X(16, 16, 16, 2, 2, 4, true) X(16, 16, 16, 2, 2, 4, false) X(16, 16, 16, 1, 4, 5, true) X(16, 16, 16, 1, 4, 4, true) \
-  X(8, 8, 8, 1, 2, 5, true) X(8, 8, 8, 1, 2, 4, true) X(8, 8, 8, 1, 2, 4, false) X(12, 12, 12, 2, 3, 5, true) X(12, 12, 12, 2, 3, 4, true)
+  X(8, 8, 8, 1, 2, 5, true) X(8, 8, 8, 1, 2, 4, true) X(8, 8, 8, 1, 2, 4, false) X(12, 12, 12, 2, 3, 5, true) X(12, 12, 12, 2, 3, 4, true) \
+  X(20, 20, 20, 2, 2, 4, true) X(20, 20, 20, 2, 2, 4, false)
 
 int tma_has_fixed(int M, int P1, int P2, int P3, int npart, int nseg, int slots, int ring) {
   if (M != 3) return 0;
