@@ -141,9 +141,11 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
          split_default * bp.PB2 / 2 < 384)
     split_default *= 2;
   if (bp.P1 == 12) split_default = 2;
-  if (M == 2) split_default = (bp.P1 == 48) ? 8 : 4;                  // the instantiated two-mode shapes
+  // the instantiated two-mode shapes; 48 x 48: 16 segments of 3 planes (384 threads, 2 CTAs per SM) measured 0.82 ms per
+  // stage at config 3 against 1.01 ms with 8 segments of 6 planes (192 threads): the kernel is L2-latency bound there
+  if (M == 2) split_default = (bp.P1 == 48) ? 16 : 4;
   bp.split = env_int("CHFPE_BRICK_SPLIT", split_default);
-  bp.minb = env_int("CHFPE_BRICK_MINB", (bp.PB2 * bp.split / 2 <= 256) ? 2 : 1);
+  bp.minb = env_int("CHFPE_BRICK_MINB", (M == 2 || bp.PB2 * bp.split / 2 <= 256) ? 2 : 1);
   bp.vn[0] = vnq[0]; bp.vn[1] = vnq[1]; bp.vn[2] = vnq[2];
   // bricks with more than 16 planes are swept in two passes of P1/2 planes: 5 instead of 10 planes of state per
   // thread at 20^3 (no register spills; measured 25.4 -> 21.6 ms per stage at config 5)

@@ -448,7 +448,7 @@ constexpr int brick3_smem_bytes() {
 
 }  // namespace
 
-#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 4, 1, 1) X(16, 16, 16, 2, 2, 1) X(20, 20, 20, 2, 1, 1) X(20, 20, 20, 2, 1, 2) X(12, 12, 12, 2, 2, 1) X(8, 8, 8, 2, 2, 1) X(48, 1, 48, 8, 2, 1) X(16, 1, 16, 4, 2, 1)
+#define BRICK3_SPECIALISATIONS(X) X(16, 16, 16, 4, 1, 1) X(16, 16, 16, 2, 2, 1) X(20, 20, 20, 2, 1, 1) X(20, 20, 20, 2, 1, 2) X(12, 12, 12, 2, 2, 1) X(8, 8, 8, 2, 2, 1) X(48, 1, 48, 8, 2, 1) X(48, 1, 48, 16, 2, 1) X(16, 1, 16, 4, 2, 1)
 
 int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb, int npass) {   // M = 2 arrives as (P1, 1, P2)
   if (M != 3 && M != 2) return 0;
