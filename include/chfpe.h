@@ -185,7 +185,7 @@ int chfpe_spectrum_2d_static(void* cuda_stream, const double* R, int32_t n1, int
 /* Which kernel family runs the RK stage on this handle (host pointer), so that a test or a benchmark can assert
    that a configuration did not fall back to the generic kernel.  The cooperative multi-step kernel of tiny
    states is a property of the step call, not of the handle, and is not reported here. */
-enum { CHFPE_STAGE_GENERIC = 0, CHFPE_STAGE_BRICK = 1, CHFPE_STAGE_PIPE = 2, CHFPE_STAGE_COMPACT = 3, CHFPE_STAGE_TMA = 4 };
+enum { CHFPE_STAGE_GENERIC = 0, CHFPE_STAGE_BRICK = 1, CHFPE_STAGE_COMPACT = 3, CHFPE_STAGE_TMA = 4 };   /* (2: a removed experiment) */
 int chfpe_stage_kernel(const chfpe_handle* h, int32_t* kind);
 
 const char* chfpe_last_error(const chfpe_handle* h);   /* h may be NULL: last create-time error */
@@ -240,6 +240,36 @@ int chfpe_hermite_import_state(chfpe_hermite_handle* h, int32_t replica, const d
 int chfpe_hermite_export_rhs(chfpe_hermite_handle* h, int32_t replica, double* dst, int dst_is_device);
 int chfpe_hermite_launch_count(const chfpe_hermite_handle* h, int64_t* n);
 const char* chfpe_hermite_last_error(const chfpe_hermite_handle* h);   /* h may be NULL: last create-time error */
+
+/* ---------------------------------------------------------------------------------------------------------------
+   Tunables.  The library reads the following environment variables once per chfpe_create / chfpe_hermite_create.
+   They select among kernel variants and launch plans that compute THE SAME results (every one is covered by a parity
+   test); they exist for measurements and for the tests that force the variants small inputs would not reach.
+   Unset = the measured default.  A value without an instantiated kernel falls back to the next kernel family.
+     Stage kernel family (phase-space grid, M >= 2, explicit schemes)
+       CHFPE_BRICK=0          generic one-thread-per-value stage kernel instead of the brick / bulk-copy kernels
+       CHFPE_TMA=0            three modes, CENTRAL4: k_stage_brick3 (register-staged loads) instead of k_stage_tma
+       CHFPE_TMA_NPART=1|2    p_1 parts per brick of k_stage_tma (default 2 from 12 planes on)
+       CHFPE_TMA_NSEG=n       thread groups (p_1 segments) per part
+       CHFPE_TMA_SLOTS=4|5    ring slots (default 5; 4 for 20^3 bricks)
+       CHFPE_TMA_RING=0       load the q_3 neighbour bricks as chunks instead of carrying them in registers
+       CHFPE_BRICK_SPLIT=n, CHFPE_BRICK_MINB=n, CHFPE_BRICK_NPASS=n   thread decomposition of k_stage_brick3
+       CHFPE_BPC=n            consecutive bricks per CTA of k_stage_brick3
+     Sweep order and L2 policy (both brick kernels)
+       CHFPE_GROUP=g          hierarchy elements swept in lock-step (default: 4 with k_stage_tma, else 2, if they fit)
+       CHFPE_Q2CHUNK=r        q_2 rows per sweep chunk
+       CHFPE_L2_WINDOW_MB=m   L2 budget of the reuse window (default 64)
+       CHFPE_L2MODE=bits      bit 0: once-touched data evict_first, bit 1: window data evict_last (default 3 / 1)
+     Other kernels
+       CHFPE_COOP=0|1|2       persistent cooperative step kernel: off | states <= 1 MB (default) | states <= 24 MB
+       CHFPE_KICK_BRICK=0     generic kick kernel + copy back instead of the in-place brick kick
+     Hermite representation
+       CHFPE_HERMITE_KC=0|4|8 per-value kernel | column kernel with 4 / 8 Hermite indices per thread
+       CHFPE_HERMITE_PATCH=AB patch kernel with A x B points of (q_1, q_2) per thread (0: off)
+       CHFPE_HERMITE_FIXED=0, CHFPE_HERMITE_TILE=0, CHFPE_HERMITE_PCOL=0   32^3 specialisation / CTA tile remap / column
+                              walk off
+       CHFPE_HERMITE_CONTIG=0 strided instead of transposing COMPACT6 line kernel on the contiguous axis
+   --------------------------------------------------------------------------------------------------------------- */
 
 #ifdef __cplusplus
 }

@@ -330,14 +330,14 @@ class CHFPE:
         return ms.value, n.value
 
     def stage_kernel(self):
-        """'generic' | 'brick' | 'pipe' | 'compact' | 'tma': the kernel family that runs the RK stage on this handle."""
+        """'generic' | 'brick' | 'compact' | 'tma': the kernel family that runs the RK stage on this handle."""
         k = C.c_int32()
         self._ck(lib().chfpe_stage_kernel(self._h, C.byref(k)), "chfpe_stage_kernel")
-        return ("generic", "brick", "pipe", "compact", "tma")[k.value]
+        return ("generic", "brick", None, "compact", "tma")[k.value]
 
     def stage_kernel_name(self):
         """Name of the CUDA kernel family behind stage_kernel() (for benchmark records)."""
-        return {"generic": "k_stage_generic", "brick": "k_stage_brick3", "pipe": "k_stage_pipe",
+        return {"generic": "k_stage_generic", "brick": "k_stage_brick3",
                 "compact": "k_compact_line passes", "tma": "k_stage_tma"}[self.stage_kernel()]
 
     def launch_count(self):

@@ -4,7 +4,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(_HERE, "libchfpe.so")
-SOURCES = ["chfpe_api.cu", "chfpe_kernels.cu", "chfpe_brick.cu", "chfpe_tma.cu", "chfpe_pipe.cu", "chfpe_compact.cu", "chfpe_spectra.cu", "chfpe_hermite.cu"]
+SOURCES = ["chfpe_api.cu", "chfpe_kernels.cu", "chfpe_brick.cu", "chfpe_tma.cu", "chfpe_compact.cu", "chfpe_spectra.cu", "chfpe_hermite.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--use_fast_math=false", "-Xcompiler", "-fPIC", "-shared"]
 

@@ -114,10 +114,9 @@ static int env_int(const char* name, int dflt) {
   return (v && *v) ? atoi(v) : dflt;
 }
 
-// Choose the brick-kernel variant (chfpe_brick.cu) and the element groups that sweep q_1 in lock-step.
-// order_out: elements with the groups contiguous.  Tunables (experiments only): CHFPE_BRICK=0 disables the brick
-// kernels, CHFPE_GROUP the group size, CHFPE_BRICK_SPLIT / CHFPE_BRICK_MINB the thread decomposition,
-// CHFPE_PIPE=1 the plane-pipelined variant.
+// Choose the stage-kernel family (chfpe_brick.cu, chfpe_tma.cu) and the element groups that sweep q_1 in lock-step.
+// order_out: elements with the groups contiguous.  The CHFPE_* environment variables read here are debugging and
+// measurement tunables, documented in include/chfpe.h ("Tunables"); none of them changes a result.
 static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std::vector<int>& up, const std::vector<int>& dn,
                                  std::vector<int>* order_out) {
   BrickPlan bp;
@@ -222,8 +221,6 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
     bp.bpc = env_int("CHFPE_BPC", bpc);
   }
   if (bp.bpc < 1) bp.bpc = 1;
-  bp.pipe_stages = env_int("CHFPE_PIPE_STAGES", 2);
-  bp.pipe = env_int("CHFPE_PIPE", 0) ? pipe_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.pipe_stages) : 0;
   return bp;
 }
 
@@ -461,18 +458,6 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   if (h->bp.enabled && h->bp.tma && tma_configure(h->bp) != 0) { cudaGetLastError(); h->bp.tma = 0; }
   if (h->bp.enabled && !h->bp.fixed && !h->bp.tma) h->bp.enabled = 0;
   if (h->bp.enabled && h->bp.fixed && brick_configure(h->bp, M) != 0) { cudaGetLastError(); h->bp.fixed = 0; if (!h->bp.tma) h->bp.enabled = 0; }
-  if (h->bp.enabled && h->bp.pipe) {
-    int dev = 0, sms = 148, smem_sm = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
-    const size_t need = pipe_smem_bytes(h->bp) + 1024;                  // + per-CTA reservation
-    int per_sm = need ? (int)((size_t)smem_sm / need) : 0;
-    if (per_sm > 2) per_sm = 2;
-    per_sm = env_int("CHFPE_PIPE_PER_SM", per_sm);
-    if (per_sm < 1 || pipe_configure(h->bp) != 0) { cudaGetLastError(); h->bp.pipe = 0; }
-    h->bp.pipe_ctas = sms * per_sm;
-  }
   memset(&h->ct, 0, sizeof(h->ct));
   h->scratch = nullptr;
   if (desc->scheme == CHFPE_COMPACT6) {                                // elimination factors of tridiag(1/3, 1, 1/3), n rows
@@ -530,7 +515,6 @@ extern "C" int chfpe_stage_kernel(const chfpe_handle* h, int32_t* kind) {
   if (!h || !kind) return CHFPE_ERR_INVALID;
   *kind = (h->op.scheme == CHFPE_COMPACT6) ? CHFPE_STAGE_COMPACT
           : (h->bp.enabled && h->bp.tma)   ? CHFPE_STAGE_TMA
-          : (h->bp.enabled && h->bp.pipe)  ? CHFPE_STAGE_PIPE
           : h->bp.enabled                  ? CHFPE_STAGE_BRICK
                                            : CHFPE_STAGE_GENERIC;
   return CHFPE_OK;
@@ -556,7 +540,6 @@ static int run_stage(chfpe_handle* h, const double* in, const double* y, double*
   if (h->bp.enabled) {                                // (these kernels evaluate plain truncation: the slaved elements follow)
     int n = 0;
     if (h->bp.tma) n = launch_stage_tma(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
-    else if (h->bp.pipe) n = launch_stage_pipe(h->op, h->bp, in, y, out, a, c, nb, ss, h->stream);
     else n = launch_stage_brick(h->op3, h->bp, in, y, out, a, c, nb, ss, h->stream);
     if (h->op.closure == CHFPE_CLOSURE_TERMINATOR) n += launch_terminator_add(h->op, in, out, c, nb, ss, h->stream);
     return n;

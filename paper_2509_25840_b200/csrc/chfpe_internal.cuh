@@ -32,7 +32,7 @@ struct DevOp {
   const double* Gamma;                // [K] sum_s n_s gamma_s
 };
 
-// Launch plan of the brick kernels (chfpe_brick.cu, chfpe_pipe.cu): one CTA per (element, q-point) p-brick.
+// Launch plan of the brick kernels (chfpe_brick.cu, chfpe_tma.cu): bricks = all momenta of one (element, q-point).
 struct BrickPlan {
   int enabled;
   int P1, P2, P3, PB2;                // p-extents, PB2 = P2*P3 (two modes: P2 = 1)
@@ -51,8 +51,6 @@ struct BrickPlan {
   int npass;                          // passes over blocks of P1/npass planes per brick (large bricks)
   int split;                          // p_1 segments (thread groups) per brick in the specialised kernel
   int fixed;                          // a compile-time specialisation (k_stage_brick3<P1,P2,P3,...>) exists
-  int pipe;                           // use the plane-pipelined kernel (chfpe_pipe.cu)
-  int pipe_stages, pipe_ctas;         // shared-memory stages per CTA, persistent CTAs in the grid
   // bulk-copy fed kernel (chfpe_tma.cu): a CTA owns one q_3 line of one p_1 part of the bricks
   int tma;                            // use it (CENTRAL4, three-mode view, a compile-time specialisation exists)
   int tma_npart, tma_nseg, tma_slots, tma_ring;
@@ -150,12 +148,6 @@ int launch_stage_tma(const DevOp& op, const BrickPlan& bp, const double* in, con
 // one-off opt-in to > 48 KB dynamic shared memory for the brick kernels; returns a cudaError_t as int
 int brick_configure(const BrickPlan& bp, int M);
 int brick_has_fixed(int M, int P1, int P2, int P3, int split, int minb, int npass);
-// plane-pipelined variant (chfpe_pipe.cu): bulk async copies into a shared-memory ring, persistent CTAs
-int pipe_has_fixed(int M, int P1, int P2, int P3, int stages);
-size_t pipe_smem_bytes(const BrickPlan& bp);
-int pipe_configure(const BrickPlan& bp);
-int launch_stage_pipe(const DevOp& op, const BrickPlan& bp, const double* in, const double* y, double* out, double a,
-                      double c, int nb, size_t slot_stride, cudaStream_t s);
 // terminator closure on top of a stage kernel that does not know it (brick / bulk-copy kernels):
 // out += c * (slaved-element coupling of every top-level element), see terminator_value in chfpe_kernels.cu
 int launch_terminator_add(const DevOp& op, const double* in, double* out, double c, int nb, size_t slot_stride,

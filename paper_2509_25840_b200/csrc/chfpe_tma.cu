@@ -6,15 +6,13 @@
 // two parts).  A CTA owns one q_3 line of one part.  Every chunk the line needs -- the part of the own brick, of the
 // hierarchy neighbours, of the q_1 / q_2 neighbour bricks, of y -- is streamed with 1-D bulk async copies
 // (cp.async.bulk, completion on an mbarrier) into a ring of shared-memory slots, in a fixed order that every thread
-// can enumerate; the LAST warp to release a slot refills it at once with the chunk SLOTS places ahead, so there is no
-// producer warp (it would be the ninth warp of the CTA and cost 32 registers per thread: warps are allocated in
-// fours).  All threads read each chunk exactly once with LDS.128 and fold it into their accumulators, so no load
+// can enumerate (one ring slot per chunk kind, so slot, barrier parity and shared address are compile-time constants);
+// the warps take turns to refill a slot, one kind late, with the chunk SLOTS places ahead, so there is no producer
+// warp (it would be the ninth warp of the CTA and cost 32 registers per thread: warps are allocated in fours).  All threads read each chunk exactly once with LDS.128 and fold it into their accumulators, so no load
 // latency is exposed and no
-// register is pinned by a load in flight (measured: the bulk-copy engine delivers 71 B/clk/SM = 20 TB/s from L2 while
-// the consumers read and use everything, profiles/r02_probe_bulk_copy.md).  The q_3 derivative runs in scatter form
-// along the line the CTA marches (RING): the own chunk of brick i_3 is added to the accumulators of bricks i_3-2,
-// i_3-1, i_3+1, i_3+2, which live in registers, so no q_3 neighbour is ever loaded (12.7 instead of 16.7 chunk loads per
-// brick).  Cutting bricks along p_1 halves the L2 window a lock-step group of elements needs,
+// register is pinned by a load in flight.  Half of the q_3 derivative runs in scatter form along the line the CTA
+// marches (RING): the own chunk of brick i_3 is added to the accumulators of bricks i_3+1 and i_3+2, which live in
+// registers, so the neighbours i_3-1, i_3-2 are never loaded (14.7 instead of 16.7 chunk loads per brick).  Cutting bricks along p_1 halves the L2 window a lock-step group of elements needs,
 // which pays for groups of four linked elements; the p_1 stencil needs G_1 on two planes beyond a part edge, and
 // those planes (of the own brick and its up_1 / down_1 neighbours) arrive by three small bulk copies one brick ahead.
 #include <type_traits>

@@ -203,17 +203,42 @@ def test_cooperative_and_per_stage_paths_agree(monkeypatch, coop):
         g.close()
 
 
-def test_pipelined_kernel_variant(monkeypatch):
-    """The plane-pipelined stage kernel (cp.async.bulk + mbarrier ring, CHFPE_PIPE=1) computes the same step."""
-    monkeypatch.setenv("CHFPE_PIPE", "1")
-    for cfg in (ci.config("cfg4s8"), ci.config("cfg4", nq=[5, 6, 5], depth=2)):
-        g, o = both(cfg)
+FAMILY_ENVS = [
+    ({}, "tma"),                                                       # default for three modes with CENTRAL4
+    ({"CHFPE_TMA": "0"}, "brick"),                                     # the register-staged brick kernel of round 1
+    ({"CHFPE_TMA_RING": "0", "CHFPE_TMA_SLOTS": "4"}, None),           # q_3 neighbours as chunks instead of the ring
+    ({"CHFPE_TMA_NPART": "1"}, None),                                  # whole bricks per chunk (no halo-plane kind)
+    ({"CHFPE_TMA_SLOTS": "4"}, None),                                  # four ring slots
+]
+
+
+@pytest.mark.parametrize("env,family", FAMILY_ENVS, ids=["-".join("%s%s" % (k[6:], v) for k, v in e.items()) or "default"
+                                                         for e, _ in FAMILY_ENVS])
+def test_stage_kernel_families(monkeypatch, env, family):
+    """Every stage-kernel family and variant of the three-mode CENTRAL4 path computes the same right-hand side and steps:
+    the bulk-copy fed kernel (k_stage_tma: ring / no ring along q_3, bricks cut in two parts or whole, 4 / 5 slots) and the
+    brick kernel (k_stage_brick3), on all four instantiated brick shapes, with ragged q grids so that every edge case of
+    the chunk stream occurs (ghost bricks on all axes, lines shorter than the ring depth + 2)."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    for cfg in (ci.config("cfg4s8", nq=[6, 5, 7]), ci.config("cfg4", nq=[5, 6, 5], depth=2),
+                ci.config("cfg4s12", nq=[5, 5, 6], depth=2), ci.config("cfg5", nq=[5, 5, 6], depth=1),
+                ci.config("cfg4", nq=[5, 5, 19], depth=1)):
+        g, o = both(cfg, batch=2)
+        if family is not None:
+            assert g.stage_kernel() == family, (cfg["name"], g.stage_kernel())
+        else:
+            assert g.stage_kernel() in ("tma", "brick")                # (a variant without an instantiation: brick kernel)
         levels = [sum(n) for n in o.elements()]
         X = ci.seeded_state(cfg, levels, seed=4)
-        g.import_state(X); o.import_state(X)
-        assert rel_l2(g.export_rhs(), o.rhs(X)) < 1e-13
+        g.import_state(X); g.import_state(X, replica=1); o.import_state(X)
+        Fg, Fo = g.export_rhs(1), o.rhs(X)
+        assert rel_l2(Fg, Fo) < 1e-13
+        for k in range(o.K):
+            assert np.linalg.norm(Fg[k] - Fo[k]) <= 1e-13 * np.linalg.norm(Fo)
         g.step(3, cfg["dt"]); o.step(3, cfg["dt"])
-        assert rel_l2(g.export_state(), o.export_state()) < 1e-12
+        assert rel_l2(g.export_state(0), o.export_state()) < 1e-12
+        assert rel_l2(g.export_state(1), o.export_state()) < 1e-12
         g.close()
 
 
