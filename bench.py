@@ -238,8 +238,8 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    cfg = ci.config(args.workload)
-    cfg4 = args.workload == "cfg4"
+    cfg = ci.config(args.workload, scheme=args.scheme)
+    cfg4 = args.workload == "cfg4" and args.scheme == "central4"
     M = cfg["n_modes"]
     g = P.CHFPE(cfg, batch=1, device="cuda:%d" % local)
     mu = obs(P, "mu", M)
@@ -657,7 +657,7 @@ def main():
     ap.add_argument("--representation", default="grid", choices=["grid", "hermite"],
                     help="'hermite': row f1, the Hermite-in-momentum representation on cfg4h (not a BASELINE metric)")
     ap.add_argument("--scheme", default="central4", choices=["central4", "central2", "compact6"],
-                    help="q-derivative of --representation hermite (compact6 = the paper's Pade scheme)")
+                    help="derivative scheme (compact6 = the paper's Pade scheme, step a9 / row f1)")
     ap.add_argument("--batch", type=int, default=5, help="replica slots for --protocol 2d (trajectory + t1 replicas)")
     ap.add_argument("--n1", type=int, default=8)
     ap.add_argument("--n2", type=int, default=16)

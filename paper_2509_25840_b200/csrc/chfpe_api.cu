@@ -95,7 +95,7 @@ static Plan make_plan(const chfpe_desc* d) {
   tb += align256(sizeof(double) * sum_n);                      // ep
   tb += align256(sizeof(int) * 3 * p.K) * 6;                   // up, dn, nvec (+ their three-mode view for M = 2)
   tb += align256(sizeof(double) * p.K);                        // Gamma
-  if (d->scheme == CHFPE_COMPACT6) tb += 2 * p.M * 2 * align256(sizeof(double) * 4096);   // Thomas factors per axis
+  if (d->scheme == CHFPE_COMPACT6) tb += 2 * p.M * 3 * align256(sizeof(double) * 4096);   // Thomas factors per axis
   tb += align256(sizeof(int) * p.K) * 2;                       // brick-kernel element order and its inverse
   tb += align256(sizeof(int) * 4 * (size_t)p.K * p.nqc);       // brick-order table of the three-mode kernels
   if (p.M == 3) tb += align256(sizeof(int) * 4 * 4 * (size_t)p.K * d->nq[0] * d->nq[1]);   // line table (chfpe_tma.cu), <= 4 parts
@@ -469,6 +469,9 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
       for (int i = 1; i < n; i++) { cf[i] = al / bet[i - 1]; bet[i] = 1.0 - al * cf[i]; }
       h->ct.bet[a] = (const double*)put(bet.data(), sizeof(double) * n);
       h->ct.cfac[a] = (const double*)put(cf.data(), sizeof(double) * n);
+      std::vector<double> ib(n);
+      for (int i = 0; i < n; i++) ib[i] = 1.0 / bet[i];
+      h->ct.ibet[a] = (const double*)put(ib.data(), sizeof(double) * n);
       cudaStreamSynchronize(h->stream);
     }
     h->scratch = (double*)(base + pl.off_scratch);

@@ -17,6 +17,7 @@
 // line stay in thread-local memory for lines of up to 128 points (all BASELINE configs), longer lines keep
 // them in an element-sized scratch array and run element by element.  (First version: whole-array derivatives,
 // 17 launches per element, 37.4 ms per stage at config 4.)
+#include <cstdlib>
 #include "chfpe_internal.cuh"
 
 namespace {
@@ -218,6 +219,124 @@ __global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double
   }
 }
 
+// All p-derivative terms of one (element, q-point) in ONE pass over its p-brick (M >= 2; second solver design of step
+// a9).  Everything that needs a p_s-derivative is local to the brick: for every mode s the operand
+//   G_s = (dU/dq_s) X_k + V'_s X_up(k,s) + n_s c_s V'_s X_dn(k,s)
+// is formed from coalesced loads into a shared tile (brick layout with the rows of the contiguous axis padded to n + 1,
+// so that lines along every axis are bank-conflict free); the right-hand side B G_s / h of Eq. (29) is taken by all
+// threads in parallel into a second tile, and only the two Thomas recurrences of tridiag(1/3, 1, 1/3) run one thread
+// per line, in place, one dependent FMA per point (elimination factors and reciprocal pivots tabulated by the host:
+// no division, no thread-local array).  Every thread collects the result for the cells it owns in registers together
+// with the pointwise gauge terms and the damping: one read of X_k, X_up, X_dn and one read-modify-write of `out` per
+// stage instead of one such pass per momentum axis.  The K elements of a q-point run in consecutive CTAs, so the bricks
+// of hierarchy neighbours are served by L2.  CPT cells per thread: pb <= CPT * blockDim.x.
+template <int M, int PBRICK_CPT>
+__global__ void __launch_bounds__(512, (PBRICK_CPT == 8) ? 2 : 1) k_compact_pbrick(DevOp op, CompactTables ct, const double* __restrict__ in,
+                                                         double* out, double c, size_t slot_stride) {
+  extern __shared__ double ptile_s[];
+  const int NT = blockDim.x, t = threadIdx.x;
+  const int pb = (int)op.pb, nl = op.n[2 * M - 1];
+  double* tile = ptile_s;                                           // G_s
+  double* rt = ptile_s + (pb + pb / nl);                            // B G_s / h, then d = A^{-1} B G_s
+  const long long ql = blockIdx.x / op.K;
+  const int k = (int)(blockIdx.x - ql * op.K);
+  const size_t eoff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells + (size_t)ql * pb;
+  const double* Xk = in + eoff;
+  int iq[M];
+  {
+    long long r = ql;
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) { iq[s] = (int)(r % op.n[s]); r /= op.n[s]; }
+  }
+  const double gam = __ldg(op.Gamma + k);
+  double acc[PBRICK_CPT];                                           // (X_k is re-read per mode: L1 / L2 hits, 16 registers less)
+  int pcs[PBRICK_CPT], pidx[PBRICK_CPT];                            // padded tile index, packed momentum indices (10 bits each)
+#pragma unroll
+  for (int j = 0; j < PBRICK_CPT; j++) {
+    const int cell = t + j * NT;
+    acc[j] = (cell < pb) ? -gam * Xk[cell] : 0.0;                   // damping -Gamma_k X_k
+    pcs[j] = cell + cell / nl;
+    int r = cell, pk = 0;
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) { const int n = op.n[M + s]; const int q = r / n; pk |= (r - q * n) << (10 * s); r = q; }
+    pidx[j] = pk;
+  }
+  const double al = 1.0 / 3.0, ca = 7.0 / 9.0, cb = 1.0 / 36.0;
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const int ap = M + s, n = op.n[ap], stb = (int)op.st[ap];       // stride of p_s inside the brick
+    const double q = op.x0[s] + iq[s] * op.h[s];
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    const double ck = __ldg(op.dU[s] + ql);
+    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+    const double cu = (ku >= 0) ? Vp : 0.0;
+    const double cd = (kd >= 0) ? __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp : 0.0;
+    const double* Xu = Xk + ((long long)(ku >= 0 ? ku : k) - k) * op.cells;
+    const double* Xd = Xk + ((long long)(kd >= 0 ? kd : k) - k) * op.cells;
+    const int pitch = (stb == 1) ? 1 : stb + stb / nl;              // padded stride of p_s
+    const double inv_h = 1.0 / op.h[ap];
+#pragma unroll
+    for (int j = 0; j < PBRICK_CPT; j++) {
+      const int cell = t + j * NT;
+      if (cell < pb) {
+        double v = ck * Xk[cell], pw = 0.0;
+        if (ku >= 0) { const double xu = Xu[cell]; v = fma(cu, xu, v); pw = op.kup[s] * cu * xu; }
+        if (kd >= 0) { const double xd = Xd[cell]; v = fma(cd, xd, v); pw = fma(op.kdn[s] * cd, xd, pw); }
+        const int i = (pidx[j] >> (10 * s)) & 1023;
+        acc[j] = fma(op.x0[ap] + i * op.h[ap], pw, acc[j]);         // gauge terms p_s V'_s (kup X_up + n c kdn X_dn)
+        tile[pcs[j]] = v;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < PBRICK_CPT; j++) {                          // right-hand side of Eq. (29), zero ghosts (R9)
+      const int cell = t + j * NT;
+      if (cell < pb) {
+        const int i = (pidx[j] >> (10 * s)) & 1023, pc = pcs[j];
+        const double fp1 = (i + 1 < n) ? tile[pc + pitch] : 0.0, fm1 = (i >= 1) ? tile[pc - pitch] : 0.0;
+        const double fp2 = (i + 2 < n) ? tile[pc + 2 * pitch] : 0.0, fm2 = (i >= 2) ? tile[pc - 2 * pitch] : 0.0;
+        rt[pc] = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
+      }
+    }
+    __syncthreads();
+    {                                                               // A d = r along p_s, in place in rt
+      const double* ibet = ct.ibet[ap];
+      const double* cfac = ct.cfac[ap];
+      const int nlines = pb / n;
+      for (int L = t; L < nlines; L += NT) {
+        const int outer = L / stb, inner = L - outer * stb;
+        const int base = outer * stb * n + inner;
+        double* row = rt + base + base / nl;
+        double prev = row[0] * __ldg(ibet);
+        row[0] = prev;
+#pragma unroll 4
+        for (int i = 1; i < n; i++) {                               // forward elimination: r'_i = (r_i - r'_{i-1}/3) / bet_i
+          const double ib = __ldg(ibet + i);
+          prev = fma(-al * ib, prev, row[i * pitch] * ib);
+          row[i * pitch] = prev;
+        }
+#pragma unroll 4
+        for (int i = n - 2; i >= 0; i--) {                          // back substitution
+          prev = fma(-__ldg(cfac + i + 1), prev, row[i * pitch]);
+          row[i * pitch] = prev;
+        }
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < PBRICK_CPT; j++) {
+      const int cell = t + j * NT;
+      if (cell < pb) acc[j] += rt[pcs[j]];
+    }
+  }
+  double* O = out + eoff;
+#pragma unroll
+  for (int j = 0; j < PBRICK_CPT; j++) {
+    const int cell = t + j * NT;
+    if (cell < pb) O[cell] = fma(c, acc[j], O[cell]);
+  }
+}
+
 }  // namespace
 
 #define CDISPATCH(M, CALL) do { if ((M) == 1) { CALL(1); } else if ((M) == 2) { CALL(2); } else { CALL(3); } } while (0)
@@ -237,7 +356,17 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
   int launches = 0;
   double* D = scratch + op.cells;
   int first = 1;
-  for (int pa = 0; pa < 2; pa++)
+  // p part in one brick pass (M >= 2, brick <= 16 cells per thread of a 512-thread CTA and <= 200 KB padded);
+  // CHFPE_COMPACT_PBRICK=0 keeps one line pass per momentum axis (the first design; profiles/r02_compact_*.txt)
+  static const bool pbrick_on = []() { const char* e = getenv("CHFPE_COMPACT_PBRICK"); return !(e && e[0] == '0'); }();
+  const int nl = op.n[2 * op.M - 1];
+  const size_t tile_bytes = 2 * sizeof(double) * (size_t)(op.pb + op.pb / nl);   // operand tile + right-hand-side tile
+  // (measured per stage, brick pass vs line passes: config 4 16.8 vs 18.3 ms, config 3 3.56 vs 4.58 ms; 20^3 bricks with
+  // 16 cells per thread lose, 83.3 vs 74.9 ms, so they stay on the line passes unless CHFPE_COMPACT_PBRICK=2)
+  static const bool pbrick_big = []() { const char* e = getenv("CHFPE_COMPACT_PBRICK"); return e && e[0] == '2'; }();
+  bool pbrick = pbrick_on && op.M >= 2 && op.pb <= (pbrick_big ? 16 : 8) * 512 && tile_bytes <= 200 * 1024 && op.nqc * op.K <= 0x7fffffffLL;
+  for (int s2 = 0; s2 < op.M; s2++) if (op.n[op.M + s2] > 1023) pbrick = false;
+  for (int pa = 0; pa < (pbrick ? 1 : 2); pa++)
     for (int sI = 0; sI < op.M; sI++) {
       const int axis = pa ? op.M + sI : sI;
       const int n = op.n[axis];
@@ -279,6 +408,26 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
 #undef LINE
       first = 0;
     }
+  if (pbrick) {
+    const int cpt = (op.pb <= 8 * 512) ? 8 : 16;                      // cells per thread
+    int nt = (int)((op.pb + cpt - 1) / cpt);
+    nt = (nt + 31) / 32 * 32;
+    if (nt < 64) nt = 64;
+    static bool optin = false;
+    if (!optin) {
+      cudaFuncSetAttribute(k_compact_pbrick<2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<2, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<3, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<3, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      optin = true;
+    }
+    const dim3 grid((unsigned)(op.nqc * op.K), 1, nb);                // element fastest: hierarchy neighbours meet in L2
+    if (op.M == 2 && cpt == 8) k_compact_pbrick<2, 8><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else if (op.M == 2) k_compact_pbrick<2, 16><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else if (cpt == 8) k_compact_pbrick<3, 8><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else k_compact_pbrick<3, 16><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    launches++;
+  }
   return launches;
 }
 

@@ -85,6 +85,7 @@ struct DevObs {                       // observable polynomial, Eq. (13)-(14)
 struct CompactTables {
   const double* bet[CHFPE_MAXAX];
   const double* cfac[CHFPE_MAXAX];
+  const double* ibet[CHFPE_MAXAX];    // 1 / bet (recurrence as two FMAs in k_compact_pbrick)
 };
 
 enum ReduceMode { RED_EXPECT = 0, RED_SUMSQ = 1, RED_SUM = 2 };
