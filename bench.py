@@ -479,6 +479,60 @@ def run_2d(args):
     return 0
 
 
+def run_slab(args):
+    """Row f4: ONE propagation of --workload cut along q_1 into WORLD_SIZE slabs (sharding.SlabPropagator): every rank
+    steps its slab with chfpe_rk4_stage and refreshes two halo planes per inner face of the stage input over NCCL
+    point-to-point before every stage.  value = global cell-updates/s (strong scaling; time = max over ranks).  With one
+    rank it measures the stage-by-stage path without exchange."""
+    import torch
+    import torch.distributed as dist
+    import paper_2509_25840_b200 as P
+    from paper_2509_25840_b200 import sharding
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world == 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29519")
+        os.environ.setdefault("RANK", "0")
+        os.environ.setdefault("WORLD_SIZE", "1")
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = ci.config(args.workload)
+    loc, geo = sharding.slab_config(cfg, rank, world)
+    g = P.CHFPE(loc, batch=1, device="cuda:%d" % local)
+    g.equilibrate(residual=False)                           # (slab-local normalisation: a timing state, not a physical one)
+    g.kick(obs(P, "mu", cfg["n_modes"]))
+    prop = sharding.SlabPropagator(g, geo, sharding.DistExchange())
+    steps, warm = args.steps, max(args.warmup, 3)
+    prop.step(warm, cfg["dt"])
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier(); torch.cuda.synchronize()
+    e0.record()
+    prop.step(steps, cfg["dt"])
+    e1.record()
+    dist.barrier(); torch.cuda.synchronize()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t[0])
+    cells = 1
+    for s_ in range(cfg["n_modes"]):
+        cells *= cfg["nq"][s_] * cfg["np"][s_]
+    if rank == 0:
+        plane = g.cells // loc["nq"][0]
+        print(json.dumps({"metric": METRIC, "value": cells * steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                          "steps": steps, "warmup": warm, "ms_per_step": ms / steps, "higher_is_better": True,
+                          "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": args.workload + " single propagation, slab-decomposed along q_1",
+                                     "parallelism": "%d slabs, halo 2 planes x %d elements per inner face and stage "
+                                                    "(%.0f MB), NCCL point-to-point" % (world, g.K, 2 * g.K * plane * 8 / 1e6),
+                                     "local_grid": "x".join(str(x) for x in g.shape), "stage_kernel": g.stage_kernel_name()},
+                          "gpu_launches": int(g.launch_count())}))
+    g.close()
+    dist.destroy_process_group()
+    return 0
+
+
 def run_2d_reference(args):
     """Reference arm of --protocol 2d: the CPU oracle's response_2d as it stands, on the 12^6 shrink of config 5's model
     (a full 20^6 replica-step takes 20 s on 16 cores), scaled by the cell count and extrapolated to 64 x 256 delays."""
@@ -651,7 +705,7 @@ def main():
     ap.add_argument("--no-2d", action="store_true", help="skip the two_d sub-record (config 5, 154 GB of device memory)")
     ap.add_argument("--sharded", action="store_true",
                     help="--protocol 2d: go through sharding.response_2d_sharded + NCCL even with one rank")
-    ap.add_argument("--protocol", default="step", choices=["step", "2d", "3d"],
+    ap.add_argument("--protocol", default="step", choices=["step", "2d", "3d", "slab"],
                     help="'2d': time chfpe_response_2d on config 5 (secondary metric: 2D THz-Raman wall time); "
                          "'3d': time chfpe_response_3d (row f2) on --workload")
     ap.add_argument("--representation", default="grid", choices=["grid", "hermite"],
@@ -666,6 +720,8 @@ def main():
         return run_reference(args)
     if args.protocol == "2d":
         return run_2d(args)
+    if args.protocol == "slab":
+        return run_slab(args)
     if args.protocol == "3d":
         return run_3d(args)
     if args.representation == "hermite":

@@ -143,6 +143,19 @@ int chfpe_import_state(chfpe_handle* h, int32_t replica, const double* src, int 
 /* F(X) of replica `replica` (right-hand side of Eq. (8)), canonical layout, for operator-level parity tests. */
 int chfpe_export_rhs(chfpe_handle* h, int32_t replica, double* dst, int dst_is_device);
 
+/* Stage-level access for a slab-decomposed propagation (row f4: one propagation split along q_1 over
+   several GPUs needs the two boundary planes of every element of the STAGE INPUT from its neighbours before every
+   stage).  chfpe_rk4_stage runs stage `stage` = 0..3 of one RK4 step (Horner form, R13) on every replica:
+     0: v_a = y + dt/4 F(y)   1: v_b = y + dt/3 F(v_a)   2: v_a = y + dt/2 F(v_b)   3: y = y + dt F(v_a)
+   so four calls with stage = 0, 1, 2, 3 are exactly chfpe_step(h, 1, dt) without its norm guard.
+   chfpe_stage_input returns the DEVICE pointer of the array that stage `stage` reads (y, v_a, v_b, v_a) for one replica,
+   in the library's internal layout X[k][i_q1][i_q2..i_qM][i_p1..i_pM] (q-major / p-minor, last axis fastest): the q_1
+   plane i of element k is the contiguous run of *plane_doubles doubles at dev + (k * nq_1 + i) * plane_doubles.  The
+   caller may overwrite such planes (halo planes of a slab) on the handle's stream between stages; the pointer stays
+   valid for the life of the handle. */
+int chfpe_rk4_stage(chfpe_handle* h, int32_t stage, double dt);
+int chfpe_stage_input(chfpe_handle* h, int32_t replica, int32_t stage, double** dev, int64_t* plane_doubles);
+
 /* Number of kernels the library has launched on this handle since create (bench.py's gpu_launches). */
 int chfpe_launch_count(const chfpe_handle* h, int64_t* n);
 

@@ -10,7 +10,7 @@ EXPORTED_SYMBOLS = [
     "chfpe_workspace_bytes", "chfpe_create", "chfpe_destroy", "chfpe_num_elements", "chfpe_element_index",
     "chfpe_equilibrate", "chfpe_step", "chfpe_kick", "chfpe_expect", "chfpe_expect_element",
     "chfpe_response_1d", "chfpe_response_2d", "chfpe_response_3d", "chfpe_export_state", "chfpe_import_state", "chfpe_export_rhs",
-    "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_spectrum_1d", "chfpe_spectrum_2d", "chfpe_spectrum_2d_static", "chfpe_last_error",
+    "chfpe_rk4_stage", "chfpe_stage_input", "chfpe_launch_count", "chfpe_profile_enable", "chfpe_profile_read", "chfpe_stage_kernel", "chfpe_spectrum_1d", "chfpe_spectrum_2d", "chfpe_spectrum_2d_static", "chfpe_last_error",
     "chfpe_hermite_workspace_bytes", "chfpe_hermite_create", "chfpe_hermite_destroy", "chfpe_hermite_num_elements",
     "chfpe_hermite_equilibrate", "chfpe_hermite_step", "chfpe_hermite_kick", "chfpe_hermite_expect",
     "chfpe_hermite_response_1d", "chfpe_hermite_response_2d", "chfpe_hermite_response_3d", "chfpe_hermite_export_state",
@@ -83,6 +83,8 @@ def lib():
     L.chfpe_import_state.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_export_rhs.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.chfpe_rk4_stage.argtypes = [vp, C.c_int32, C.c_double]
+    L.chfpe_stage_input.argtypes = [vp, C.c_int32, C.c_int32, C.POINTER(vp), C.POINTER(C.c_int64)]
     L.chfpe_profile_enable.argtypes = [vp, C.c_int]
     L.chfpe_profile_read.argtypes = [vp, dp, C.POINTER(C.c_int64)]
     L.chfpe_stage_kernel.argtypes = [vp, C.POINTER(C.c_int32)]
@@ -319,6 +321,20 @@ class CHFPE:
         t = self._torch.empty((self.K,) + self.shape, dtype=self._torch.float64, device=self.device)
         self._ck(lib().chfpe_export_rhs(self._h, replica, C.c_void_p(t.data_ptr()), 1), "chfpe_export_rhs")
         return t
+
+    def rk4_stage(self, stage, dt):
+        """Stage 0..3 of one RK4 step (chfpe_rk4_stage); four calls = step(1, dt) without the norm guard."""
+        self._ck(lib().chfpe_rk4_stage(self._h, int(stage), float(dt)), "chfpe_rk4_stage")
+
+    def stage_input(self, stage, replica=0):
+        """Torch view [K, nq_1, plane] (float64, device memory inside the workspace, no copy) of the array that RK4
+        stage `stage` reads, internal layout (chfpe_stage_input): index [k, i] is the q_1 plane i of element k."""
+        dev, pd = C.c_void_p(), C.c_int64()
+        self._ck(lib().chfpe_stage_input(self._h, replica, int(stage), C.byref(dev), C.byref(pd)), "chfpe_stage_input")
+        off = dev.value - self.workspace.data_ptr()
+        n = self.K * self.cells
+        flat = self.workspace[off: off + 8 * n].view(self._torch.float64)
+        return flat.view(self.K, self.shape[0], pd.value)
 
     def profile_enable(self, on=True):
         self._ck(lib().chfpe_profile_enable(self._h, 1 if on else 0), "chfpe_profile_enable")

@@ -718,6 +718,24 @@ extern "C" int chfpe_step(chfpe_handle* h, int64_t n_steps, double dt) {
   return CHFPE_OK;
 }
 
+extern "C" int chfpe_rk4_stage(chfpe_handle* h, int32_t stg, double dt) {
+  if (!h || stg < 0 || stg > 3) return CHFPE_ERR_INVALID;
+  const size_t ss = 3 * h->state_doubles;
+  double *y = h->y(0), *va = h->va(0), *vb = h->vb(0);
+  if (stg == 0) stage(h, y, y, va, 1.0, dt / 4.0, h->batch, ss);
+  else if (stg == 1) stage(h, va, y, vb, 1.0, dt / 3.0, h->batch, ss);
+  else if (stg == 2) stage(h, vb, y, va, 1.0, dt / 2.0, h->batch, ss);
+  else stage(h, va, y, y, 1.0, dt, h->batch, ss);
+  return check_launch(h);
+}
+
+extern "C" int chfpe_stage_input(chfpe_handle* h, int32_t replica, int32_t stg, double** dev, int64_t* plane_doubles) {
+  if (!h || !dev || !plane_doubles || replica < 0 || replica >= h->batch || stg < 0 || stg > 3) return CHFPE_ERR_INVALID;
+  *dev = (stg == 0) ? h->y(replica) : (stg == 2 ? h->vb(replica) : h->va(replica));
+  *plane_doubles = (int64_t)(h->cells / h->desc.nq[0]);
+  return CHFPE_OK;
+}
+
 extern "C" int chfpe_kick(chfpe_handle* h, const chfpe_observable* X) {
   if (!h || !X) return CHFPE_ERR_INVALID;
   h->norm_ref_valid = false;

@@ -762,3 +762,98 @@ def test_response_2d_sharded_over_nccl_world1():
         dist.destroy_process_group()
     assert R.shape == R_plain.shape and np.array_equal(R, R_plain)
     g.close()
+
+
+class _LocalExchange:
+    """Halo exchange between slab engines that live in ONE process (test only): plain device copies on the current
+    stream, one slab after the other -- nothing waits on anything, so this is not a stand-in for several GPUs, only a
+    check of the halo logic with the CUDA kernels."""
+
+    def __init__(self, engines, geos):
+        self.engines, self.geos = engines, geos
+
+    def run_all(self, stage):
+        from paper_2509_25840_b200 import sharding
+        H = sharding.HALO
+        views = [e.stage_input(stage) for e in self.engines]
+        for r, (X, (lo, hi, hl, hh)) in enumerate(zip(views, self.geos)):
+            n = X.shape[1]
+            if hl:
+                Y, (_, _, hl2, hh2) = views[r - 1], self.geos[r - 1]
+                X[:, :hl] = Y[:, Y.shape[1] - hh2 - H:Y.shape[1] - hh2]
+            if hh:
+                Y, (_, _, hl2, hh2) = views[r + 1], self.geos[r + 1]
+                X[:, n - hh:] = Y[:, hl2:hl2 + H]
+
+
+@pytest.mark.parametrize("name,cfg,world", [("m3_tma", ci.config("cfg4s8", nq=[11, 5, 6]), 2),
+                                            ("m3_tma_3slabs", ci.config("cfg4", nq=[13, 5, 5], depth=1), 3),
+                                            ("m2_brick", ci.config("cfg3s", nq=[10, 7], depth=2), 2)])
+def test_slab_decomposition_on_the_cuda_path(name, cfg, world):
+    """Row f4 (second half), CUDA path: the grid is cut along q_1 into `world` slabs with two halo planes per inner face
+    (sharding.slab_config); each slab is an ordinary CHFPE handle stepped stage by stage (chfpe_rk4_stage) with the
+    halo planes of the stage input (chfpe_stage_input views) refreshed before every stage.  Owned planes must equal
+    the undecomposed propagation and the oracle.  All slabs run in one process on one stream, one after the other."""
+    from paper_2509_25840_b200 import sharding
+    P = gpu_mod()
+    g, o = both(cfg)
+    X = ci.seeded_state(cfg, [sum(n) for n in o.elements()], seed=31)
+    g.import_state(X); o.import_state(X)
+    g.step(2, cfg["dt"]); o.step(2, cfg["dt"])
+    want = g.export_state()
+    assert rel_l2(want, o.export_state()) < 1e-12
+    locs = [sharding.slab_config(cfg, r, world) for r in range(world)]
+    engines = [P.CHFPE(lc, batch=1) for lc, _ in locs]
+    geos = [ge for _, ge in locs]
+    for e, (lo, hi, hl, hh) in zip(engines, geos):
+        e.import_state(np.ascontiguousarray(X[:, lo - hl:hi + hh]))
+    ex = _LocalExchange(engines, geos)
+    for _ in range(2):
+        for stage in range(4):
+            ex.run_all(stage)
+            for e in engines:
+                e.rk4_stage(stage, cfg["dt"])
+    got = np.concatenate([e.export_state()[:, hl:e.shape[0] - hh] for e, (lo, hi, hl, hh) in zip(engines, geos)], axis=1)
+    assert got.shape == want.shape
+    assert rel_l2(got, want) < 1e-13
+    assert rel_l2(got, o.export_state()) < 1e-12
+    # partial expectations over the owned planes add up to the global one
+    al_g, al_o = obs_pair("alpha", cfg["n_modes"])
+    props = [sharding.SlabPropagator(e, ge, None) for e, ge in zip(engines, geos)]
+    tot = sum(p.expect_partial(al_g) for p in props)
+    assert abs(tot - o.expect(al_o)) <= 1e-12 * max(1.0, abs(o.expect(al_o)))
+    for e in engines:
+        e.close()
+    g.close()
+
+
+def test_slab_propagator_over_nccl_world1_and_stage_api():
+    """chfpe_rk4_stage x 4 == chfpe_step, and SlabPropagator + DistExchange on NCCL with one rank (the whole domain is
+    one slab, no neighbours) equals the plain step bit for bit."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    from paper_2509_25840_b200 import sharding
+    cfg = ci.config("cfg4s8", nq=[6, 5, 7])
+    P = gpu_mod()
+    g, o = both(cfg)
+    X = ci.seeded_state(cfg, [sum(n) for n in o.elements()], seed=5)
+    g.import_state(X)
+    g.step(2, cfg["dt"])
+    want = g.export_state()
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    os.environ["MASTER_ADDR"], os.environ["MASTER_PORT"] = "127.0.0.1", str(port)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        loc, geo = sharding.slab_config(cfg, 0, 1)
+        assert loc["nq"] == cfg["nq"] and geo == (0, cfg["nq"][0], 0, 0)
+        e = P.CHFPE(loc)
+        e.import_state(X)
+        sharding.SlabPropagator(e, geo, sharding.DistExchange()).step(2, cfg["dt"])
+        assert np.array_equal(e.export_state(), want)
+        e.close()
+    finally:
+        dist.destroy_process_group()
+    g.close()
