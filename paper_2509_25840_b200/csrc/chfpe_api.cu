@@ -284,6 +284,10 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
     else { op.c1[a] = 1.0 / (2.0 * op.h[a]); op.c2[a] = 0.0; }
   }
 
+  for (int s = 0; s < M; s++) {
+    const double w[4] = {8.0, -8.0, -1.0, 1.0};
+    for (int dd = 0; dd < 4; dd++) op.cqw[s][dd] = op.c2[s] * op.inv_mass[s] * w[dd];
+  }
   // ---- host tables (setup step a0) ----
   std::vector<double> dU[3], eU(pl.nqc);
   for (int s = 0; s < M; s++) dU[s].resize(pl.nqc);
@@ -438,6 +442,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
         v.inv_mass[vs] = r < 0 ? 0.0 : op.inv_mass[r];
         v.kup[vs] = r < 0 ? 0.0 : op.kup[r];    v.kdn[vs] = r < 0 ? 0.0 : op.kdn[r];
         v.cdn[vs] = r < 0 ? 0.0 : op.cdn[r];
+        for (int dd = 0; dd < 4; dd++) v.cqw[vs][dd] = r < 0 ? 0.0 : op.cqw[r][dd];
         v.VLL[vs] = r < 0 ? 0.0 : op.VLL[r];    v.VSL[vs] = r < 0 ? 0.0 : op.VSL[r];
         v.dU[vs] = op.dU[r < 0 ? 0 : r];
       }

@@ -22,6 +22,7 @@ struct DevOp {
   double c1[CHFPE_MAXAX], c2[CHFPE_MAXAX];   // pre-multiplied stencil coefficients (+-1, +-2 neighbours)
   double inv_mass[3], kup[3], kdn[3], cdn[3], VLL[3], VSL[3], beta;
   double gam[3];                      // gamma_s (terminator closure: Gamma_{n+e_s} = Gamma_n + gamma_s)
+  double cqw[3][4];                   // CENTRAL4: -(1/m_s)/(12 h_qs) x stencil weight of the q_s neighbour +1, -1, +2, -2
   double dV;
   const double* dU[3];                // dU/dq_s on the q-subgrid, q_1 slowest   (device)
   const double* eU;                   // exp(-beta U/2) (sqrt gauge) or exp(-beta U) (W gauge) on the q-subgrid

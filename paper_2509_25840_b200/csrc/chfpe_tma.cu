@@ -502,7 +502,7 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
     Unroll<0, (RING ? 10 : 12)>::run([&](auto SD) {
       constexpr int sd = decltype(SD)::value, s = sd / 4;
       constexpr int d = (RING && s == 2) ? 2 * (sd % 4) : sd % 4;   // ring: kinds 16, 17 are the +1 and +2 neighbours
-      const double wd = op.c2[s] * op.inv_mass[s] * ((d == 0) ? 8.0 : (d == 1 ? -8.0 : (d == 2 ? -1.0 : 1.0)));
+      const double wd = op.cqw[s][d];                               // host-tabulated: one multiply per coefficient here
       chunk(KindC<8 + sd>(), [&](unsigned S) {
 #pragma unroll
         for (int j = 0; j < NC; j++) {
