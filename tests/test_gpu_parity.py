@@ -857,3 +857,23 @@ def test_slab_propagator_over_nccl_world1_and_stage_api():
     finally:
         dist.destroy_process_group()
     g.close()
+
+
+def test_long_q3_line_falls_back_to_the_brick_kernel():
+    """k_stage_tma tabulates dU/dq_s of a q_3 line in shared memory for lines of up to 64 bricks; longer lines must
+    take the brick kernel (and still match the oracle)."""
+    cfg = ci.config("cfg4s8", nq=[5, 5, 70], depth=1)
+    g, o = both(cfg)
+    assert g.stage_kernel() == "brick"
+    X = ci.seeded_state(cfg, [sum(n) for n in o.elements()], seed=8)
+    g.import_state(X); o.import_state(X)
+    assert rel_l2(g.export_rhs(), o.rhs(X)) < 1e-13
+    g.close()
+    g64, o64 = both(ci.config("cfg4s8", nq=[5, 5, 64], depth=1))
+    assert g64.stage_kernel() == "tma"
+    X = ci.seeded_state(g64.cfg if hasattr(g64, "cfg") else ci.config("cfg4s8", nq=[5, 5, 64], depth=1), [sum(n) for n in o64.elements()], seed=8)
+    g64.import_state(X); o64.import_state(X)
+    assert rel_l2(g64.export_rhs(), o64.rhs(X)) < 1e-13
+    g64.step(2, 1e-3); o64.step(2, 1e-3)
+    assert rel_l2(g64.export_state(), o64.export_state()) < 1e-12
+    g64.close()
