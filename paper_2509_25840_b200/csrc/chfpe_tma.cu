@@ -158,7 +158,7 @@ struct TmaCfg {
   static_assert(NK % SLOTS == 0, "the slot of a kind must not depend on the step");
   static constexpr int MAXQ3 = 64;                                 // longest q_3 line (dU/dq_s table of the line)
   static constexpr size_t SMEM = (size_t)SLOTS * CHUNK + sizeof(double) * (PP * G2_PLANE + PP * G3_PLANE + XG) +
-                                 16 * SLOTS + 8 * NK + 8 * 3 * MAXQ3 + 16;
+                                 16 * SLOTS + 16 + 8 * NK + 8 * 3 * MAXQ3 + 16;
   static constexpr int MINB = (2 * (SMEM + 1024) <= 227 * 1024 && 2 * NT <= 1024) ? 2 : 1;
 };
 
@@ -189,9 +189,10 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
   double* xg = g3 + PP * C::G3_PLANE;
   unsigned long long* full = reinterpret_cast<unsigned long long*>(xg + C::XG);       // data of a slot has landed
   unsigned long long* empty = full + SLOTS;                                           // all warps have released a slot
-  const double** ent = reinterpret_cast<const double**>(empty + SLOTS);               // source of every kind at step 0
+  unsigned long long* xbar = empty + SLOTS;                                           // exchange planes: [0] written, [1] read
+  const double** ent = reinterpret_cast<const double**>(xbar + 2);                    // source of every kind at step 0
   double* sdu = reinterpret_cast<double*>(ent + NK);                                  // dU/dq_s at the q-points of the line
-  const unsigned ring_a = t_smem_u32(ring), full_a = t_smem_u32(full), empty_a = t_smem_u32(empty);
+  const unsigned ring_a = t_smem_u32(ring), full_a = t_smem_u32(full), empty_a = t_smem_u32(empty), xbar_a = t_smem_u32(xbar);
 
   const int t = threadIdx.x;
   const TmaLine ln = decode_line(bp.lines, blockIdx.x);
@@ -262,6 +263,7 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
 
   if (t == 0) {
     for (int s = 0; s < SLOTS; s++) { t_mbar_init(full + s, 1); t_mbar_init(empty + s, C::NW); }
+    t_mbar_init(xbar, C::NW); t_mbar_init(xbar + 1, C::NW);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     const double* Xk = X + (size_t)k * op.cells + pofs + (size_t)ql0 * BRICK;
     for (int e = 0; e < NK; e++) ent[e] = Xk;
@@ -463,7 +465,9 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
             acc[NC - 1] = t_fma2(-wp1, gh[1], acc[NC - 1]);
           }
         });
-        asm volatile("bar.sync 1, %0;" ::"r"(C::NT) : "memory");    // exchange planes of the previous brick are free
+        // exchange planes of the previous brick are free: split-phase barrier, every warp arrived on it when it had read
+        // them (end of the previous brick), four chunk kinds ago
+        if (m > 0) a_mbar_wait(xbar_a + 8, (unsigned)(m - 1) & 1u);
         if (NSEG > 1 && active) {                                   // planes next to a segment edge -> neighbour segment
 #pragma unroll
           for (int j = 0; j < NC; j++) {
@@ -498,6 +502,8 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
           *reinterpret_cast<double2*>(g3 + (jbase + j) * C::G3_PLANE + i2 * C::G3_ROW + i3 + 2) = g[j];
       }
     }
+    __syncwarp();
+    a_mbar_arrive_if(xbar_a, lane == 0);                            // this warp's G_2 / G_3 / segment-edge G_1 are written
     // ---- -(p_s/m_s) dW/dq_s: one chunk per existing neighbour brick (q_3: only x_{m+1}, x_{m+2} with the ring) ----
     Unroll<0, (RING ? 10 : 12)>::run([&](auto SD) {
       constexpr int sd = decltype(SD)::value, s = sd / 4;
@@ -516,7 +522,7 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
     });
     if (RING) { chunk(KindC<18>(), [&](unsigned) {}); }             // (unused kind: keeps NK a multiple of SLOTS)
     else { chunk(KindC<20>(), [&](unsigned) {}); chunk(KindC<21>(), [&](unsigned) {}); chunk(KindC<22>(), [&](unsigned) {}); }
-    asm volatile("bar.sync 1, %0;" ::"r"(C::NT) : "memory");        // G_2 / G_3 / segment-edge G_1 complete
+    a_mbar_wait(xbar_a, (unsigned)m & 1u);                          // G_2 / G_3 / segment-edge G_1 of every warp complete
     if (NSEG > 1) {
       if (seg > 0) {                                                // G_1 at planes jbase-2, jbase-1
         const double2 gm2 = *reinterpret_cast<const double2*>(xg + ((seg - 1) * 4 + 0) * PLANE + 2 * tid);
@@ -555,6 +561,8 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
         }
       }
     }
+    __syncwarp();
+    a_mbar_arrive_if(xbar_a + 8, lane == 0);                        // this warp has read the exchange planes
     chunk(KindC<NK - 1>(), [&](unsigned S) {                        // stage combine: out = a y + c F
       double2* O = Ob + (size_t)m * (BRICK / 2);
 #pragma unroll
