@@ -306,7 +306,8 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
   const int jbase = seg * NC;                                       // first plane (inside the part) of this thread
   const int i2 = tid / (P3 / 2), i3 = 2 * (tid - i2 * (P3 / 2));
   const int lane = t & 31, warp = __shfl_sync(0xffffffffu, t >> 5, 0);   // (warp-uniform by construction)
-  const unsigned my_a = ring_a + (unsigned)(jbase * PL2 + tid) * 16;   // this thread's first pair inside slot 0
+  unsigned my_a = ring_a + (unsigned)(jbase * PL2 + tid) * 16;         // this thread's first pair inside slot 0
+  asm volatile("" : "+r"(my_a));                                     // (kept in a register: not rematerialised per chunk)
   const double h1 = op.h[3];
   const double p1_0 = op.x0[3] + (part * PP + jbase) * h1;
   const double p2 = op.x0[4] + i2 * op.h[4];
