@@ -329,7 +329,7 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
 
   int m = 0;
   // (masks are the same in every thread; the shuffle tells the compiler so: uniform branches, no reconvergence code)
-  unsigned mask = __shfl_sync(0xffffffffu, step_mask(0), 0), maskn = __shfl_sync(0xffffffffu, step_mask(1), 0), mpar = 0, pre = 0;
+  unsigned mask = __shfl_sync(0xffffffffu, step_mask(0), 0), maskn = __shfl_sync(0xffffffffu, step_mask(1), 0), mpar = 0;
   // barrier parity of use (step parity mp, kind E) of slot E % SLOTS
   auto parity = [&](int E, unsigned mp) -> unsigned { return ((unsigned)(E / SLOTS) & 1u) ^ ((C::USES & 1) ? mp : 0u); };
   // Refill duty for use (mm, EP): wait until every warp has let go of the slot, then load its next user -- kind
@@ -350,7 +350,7 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
     constexpr int E = decltype(KE)::value;
     // (an absent kind is waited for as well: its barrier is completed, without data, only after every warp has
     // released the slot's previous user, which keeps a fast warp from arriving twice in one phase of `empty`)
-    if (!pre) a_mbar_wait(full_a + 8 * (E % SLOTS), parity(E, mpar));
+    a_mbar_wait(full_a + 8 * (E % SLOTS), parity(E, mpar));
     if ((mask >> E) & 1u) body(my_a + (E % SLOTS) * C::CHUNK);
     __syncwarp();
     a_mbar_arrive_if(empty_a + 8 * (E % SLOTS), lane == 0);
@@ -359,8 +359,6 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
       if (E == 0) duty(KindC<EP>(), m - 1, mpar ^ 1u, 0u, mask);    // last kind of the previous brick
       else duty(KindC<EP>(), m, mpar, mask, maskn);
     }
-    constexpr int EN = (E + 1) % NK;                                // early, non-blocking look at the next kind's barrier
-    pre = a_mbar_test(full_a + 8 * (EN % SLOTS), parity(EN, E + 1 == NK ? (mpar ^ 1u) : mpar));
   };
 
   // RING: accumulators of bricks m, m+1, m+2 (the last one only while brick m is processed)
