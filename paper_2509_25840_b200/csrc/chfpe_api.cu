@@ -6,6 +6,7 @@
 #include <cstdlib>
 #include <cstring>
 #include "chfpe_internal.cuh"
+#include "chfpe_poly.h"
 
 static thread_local std::string g_create_err;
 
@@ -232,8 +233,6 @@ extern "C" int chfpe_workspace_bytes(const chfpe_desc* desc, size_t* bytes) {
   return CHFPE_OK;
 }
 
-static double ipow(double x, int e) { double r = 1.0; for (int i = 0; i < e; i++) r *= x; return r; }
-
 extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void* cuda_stream, chfpe_handle** out) {
   std::string why;
   int rc = validate(desc, &why);
@@ -292,25 +291,15 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   std::vector<double> dU[3], eU(pl.nqc);
   for (int s = 0; s < M; s++) dU[s].resize(pl.nqc);
   const double wfac = (desc->gauge == CHFPE_GAUGE_W) ? 1.0 : 0.5;     // weight exponent: e^{-beta H} or e^{-beta H/2}
+  ChfpePoly poly;
+  poly.build(h->U.data(), (int)h->U.size(), M);
   for (long long l = 0; l < pl.nqc; l++) {
     int iq[3] = {0, 0, 0}; long long r = l;
     for (int s = M - 1; s >= 0; s--) { iq[s] = (int)(r % op.n[s]); r /= op.n[s]; }
     double q[3] = {0, 0, 0};
     for (int s = 0; s < M; s++) q[s] = op.x0[s] + iq[s] * op.h[s];
-    double u = 0.0, du[3] = {0, 0, 0};
-    for (const chfpe_monomial& t : h->U) {
-      double v = t.coef;
-      for (int s = 0; s < M; s++) v *= ipow(q[s], t.expo[s]);
-      u += v;
-      for (int s = 0; s < M; s++) {
-        if (t.expo[s] == 0) continue;
-        double w = t.coef * t.expo[s] * ipow(q[s], t.expo[s] - 1);
-        for (int r2 = 0; r2 < M; r2++) if (r2 != s) w *= ipow(q[r2], t.expo[r2]);
-        du[s] += w;
-      }
-    }
-    eU[l] = exp(-wfac * desc->beta * u);
-    for (int s = 0; s < M; s++) dU[s][l] = du[s];
+    eU[l] = exp(-wfac * desc->beta * poly.value(q));
+    for (int s = 0; s < M; s++) dU[s][l] = poly.grad(s, q);
   }
   std::vector<double> ep;
   size_t ep_off[3] = {0, 0, 0};

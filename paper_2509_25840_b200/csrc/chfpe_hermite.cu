@@ -13,6 +13,7 @@
 #include <string>
 #include <vector>
 #include "../../include/chfpe.h"
+#include "chfpe_poly.h"
 
 namespace {
 
@@ -746,7 +747,6 @@ Carve carve(const chfpe_desc* d) {
   return c;
 }
 
-double ipow(double x, int e) { double r = 1.0; for (int i = 0; i < e; i++) r *= x; return r; }
 
 }  // namespace
 
@@ -989,23 +989,14 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
   // ---- tables (setup step a0): dU/dq_s, exp(-beta U/2) and the equilibrium coefficient on the q grid ----
   std::vector<double> dU(3 * Q, 0.0), wq(Q), ceq(Q);
   double Z = 0.0;
+  ChfpePoly poly;
+  poly.build(desc->U, desc->n_terms, M);
   for (size_t i = 0; i < Q; i++) {
     double q[3] = {0, 0, 0};
     size_t r = i;
     for (int s = M - 1; s >= 0; s--) { q[s] = op.q0[s] + op.h[s] * (double)(r % op.nq[s]); r /= op.nq[s]; }
-    double U = 0.0;
-    for (int t = 0; t < desc->n_terms; t++) {
-      const chfpe_monomial& mo = desc->U[t];
-      double v = mo.coef;
-      for (int s = 0; s < M; s++) v *= ipow(q[s], mo.expo[s]);
-      U += v;
-      for (int s = 0; s < M; s++) {
-        if (mo.expo[s] == 0) continue;
-        double g = mo.coef * mo.expo[s];
-        for (int s2 = 0; s2 < M; s2++) g *= ipow(q[s2], mo.expo[s2] - (s2 == s ? 1 : 0));
-        dU[(size_t)s * Q + i] += g;
-      }
-    }
+    const double U = poly.value(q);
+    for (int s = 0; s < M; s++) dU[(size_t)s * Q + i] = poly.grad(s, q);
     wq[i] = exp(-0.5 * desc->beta * U);
     Z += exp(-desc->beta * U);
   }
