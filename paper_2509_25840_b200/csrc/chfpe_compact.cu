@@ -33,7 +33,8 @@ __device__ __forceinline__ void cdecode(const DevOp& op, unsigned cell, int (&id
 }
 
 // d = A^{-1} B f along `axis` for every grid line of one element array; one thread per line.
-// bet[i], cfac[i]: elimination factors of tridiag(1/3,1,1/3) with n rows (host-tabulated per axis).
+// bet[i], cfac[i]: RECIPROCAL pivots and elimination factors of tridiag(1/3,1,1/3) with n rows (host-tabulated per
+// axis; multiplying by the tabulated reciprocal replaces a division per point: q passes 2.33 -> see DESIGN.md).
 __global__ void __launch_bounds__(128) k_compact_deriv(const double* __restrict__ f, double* __restrict__ d, long long nlines,
                                                        int n, long long st, double inv_h, const double* __restrict__ bet,
                                                        const double* __restrict__ cfac) {
@@ -46,7 +47,7 @@ __global__ void __launch_bounds__(128) k_compact_deriv(const double* __restrict_
   for (int i = 0; i < n; i++) {                                    // forward elimination, r'_i stored in d
     const double fp2 = (i + 2 < n) ? f[base + (long long)(i + 2) * st] : 0.0;
     const double r = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
-    prev = (i == 0) ? r / __ldg(bet) : (r - al * prev) / __ldg(bet + i);
+    prev = (i == 0) ? r * __ldg(bet) : (r - al * prev) * __ldg(bet + i);   // bet[]: reciprocal pivots
     d[base + (long long)i * st] = prev;
     fm2 = fm1; fm1 = f0; f0 = fp1; fp1 = fp2;
   }
@@ -127,7 +128,7 @@ __global__ void __launch_bounds__(128) k_compact_line(DevOp op, const double* __
   for (int i = 0; i < n; i++) {                                    // forward elimination
     const double fp2 = (i + 2 < n) ? f(i + 2) : 0.0;
     const double r = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
-    prev = (i == 0) ? r / __ldg(bet) : (r - al * prev) / __ldg(bet + i);
+    prev = (i == 0) ? r * __ldg(bet) : (r - al * prev) * __ldg(bet + i);   // bet[]: reciprocal pivots
     if (LOCAL) rl[LOCAL ? i : 0] = prev; else rg[(long long)i * st] = prev;
     fm2 = fm1; fm1 = f0; f0 = fp1; fp1 = fp2;
   }
@@ -199,7 +200,7 @@ __global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double
   for (int i = 0; i < n; i++) {                                    // forward elimination, in place
     const double fp2 = (i + 2 < n) ? row[i + 2] : 0.0;
     const double r = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
-    prev = (i == 0) ? r / __ldg(bet) : (r - al * prev) / __ldg(bet + i);
+    prev = (i == 0) ? r * __ldg(bet) : (r - al * prev) * __ldg(bet + i);   // bet[]: reciprocal pivots
     row[i] = prev;
     fm2 = fm1; fm1 = f0; f0 = fp1; fp1 = fp2;
   }
@@ -345,7 +346,7 @@ static int compact_deriv(const DevOp& op, const CompactTables& ct, const double*
   const int n = op.n[axis];
   const long long nlines = op.cells / n;
   k_compact_deriv<<<(unsigned)((nlines + 127) / 128), 128, 0, s>>>(f, d, nlines, n, op.st[axis], 1.0 / op.h[axis],
-                                                                   ct.bet[axis], ct.cfac[axis]);
+                                                                   ct.ibet[axis], ct.cfac[axis]);
   return 1;
 }
 
@@ -373,7 +374,7 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
       const unsigned lb = (unsigned)((op.cells / n + 127) / 128);
       const bool local = n <= CLINE_MAX;
 #define LINE(MM, PA, NFV, GRID, K0, B0)                                                                               \
-  k_compact_line<MM, PA, NFV><<<GRID, 128, 0, s>>>(op, in, y, out, a, c, sI, first, K0, B0, slot_stride, ct.bet[axis],  \
+  k_compact_line<MM, PA, NFV><<<GRID, 128, 0, s>>>(op, in, y, out, a, c, sI, first, K0, B0, slot_stride, ct.ibet[axis],  \
                                                    ct.cfac[axis], D)
 #define LINE_PA(MM, NFV, GRID, K0, B0)                                                                                \
   do { if (pa) LINE(MM, 1, NFV, GRID, K0, B0); else LINE(MM, 0, NFV, GRID, K0, B0); } while (0)
@@ -388,7 +389,7 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
         optin_##MM = true;                                                                                            \
       }                                                                                                               \
       k_compact_pline_s1<MM><<<dim3(wb, op.K, nb), 128, sizeof(double) * 4 * 64 * (n + 1), s>>>(                      \
-          op, in, y, out, a, c, first, slot_stride, ct.bet[axis], ct.cfac[axis]);                                     \
+          op, in, y, out, a, c, first, slot_stride, ct.ibet[axis], ct.cfac[axis]);                                     \
       launches++;                                                                                                     \
     } else if (local) {                                                                                               \
       const dim3 grid(lb, op.K, nb);                                                                                  \
