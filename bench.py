@@ -657,7 +657,7 @@ def run_hermite(args):
     values = g.values
     kern_ms = ms_stage / (4 * steps)                     # one RK stage (per_stage launches)
     achieved = values * 22.0 / (kern_ms * 1e-3) / 1e9
-    kname = "k_hermite_stage_patch" if per_stage == 1 else \
+    kname = g.stage_kernel_name() if per_stage == 1 else \
         "RK stage = k_hermite_stage<DER=false> + %d x k_hermite_compact_line" % M
     line = {"metric": "Hermite-representation value-updates/s (fp64)", "value": values * steps / (ms * 1e-3),
             "unit": "value-updates/s", "n_gpus": 1, "steps": steps, "warmup": warm, "ms_per_step": ms / steps,

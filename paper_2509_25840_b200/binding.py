@@ -14,7 +14,7 @@ EXPORTED_SYMBOLS = [
     "chfpe_hermite_workspace_bytes", "chfpe_hermite_create", "chfpe_hermite_destroy", "chfpe_hermite_num_elements",
     "chfpe_hermite_equilibrate", "chfpe_hermite_step", "chfpe_hermite_kick", "chfpe_hermite_expect",
     "chfpe_hermite_response_1d", "chfpe_hermite_response_2d", "chfpe_hermite_response_3d", "chfpe_hermite_export_state",
-    "chfpe_hermite_import_state", "chfpe_hermite_export_rhs", "chfpe_hermite_launch_count", "chfpe_hermite_last_error",
+    "chfpe_hermite_import_state", "chfpe_hermite_export_rhs", "chfpe_hermite_launch_count", "chfpe_hermite_stage_kernel", "chfpe_hermite_last_error",
 ]
 
 
@@ -111,6 +111,7 @@ def lib():
     L.chfpe_hermite_import_state.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_hermite_export_rhs.argtypes = [vp, C.c_int32, vp, C.c_int]
     L.chfpe_hermite_launch_count.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.chfpe_hermite_stage_kernel.argtypes = [vp, C.POINTER(C.c_int32)]
     L.chfpe_hermite_last_error.argtypes = [vp]
     L.chfpe_hermite_last_error.restype = C.c_char_p
     _lib = L
@@ -514,6 +515,17 @@ class Hermite:
         n = C.c_int64()
         self._ck(lib().chfpe_hermite_launch_count(self._h, C.byref(n)), "chfpe_hermite_launch_count")
         return n.value
+
+    def stage_kernel(self):
+        """'value' | 'column' | 'patch' | 'compact' | 'tma': the kernel family that runs the RK stage on this handle."""
+        k = C.c_int32()
+        self._ck(lib().chfpe_hermite_stage_kernel(self._h, C.byref(k)), "chfpe_hermite_stage_kernel")
+        return ("value", "column", "patch", "compact", "tma")[k.value]
+
+    def stage_kernel_name(self):
+        """Name of the CUDA kernel family behind stage_kernel() (for benchmark records)."""
+        return {"value": "k_hermite_stage", "column": "k_hermite_stage_col", "patch": "k_hermite_stage_patch",
+                "compact": "k_hermite_stage<DER=false> + k_hermite_compact_line", "tma": "k_hermite_stage_tma"}[self.stage_kernel()]
 
 
 def _dev(a):

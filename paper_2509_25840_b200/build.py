@@ -18,7 +18,7 @@ def _nvcc():
 
 def _deps():
     src = [os.path.join(_HERE, "csrc", s) for s in SOURCES]
-    return src, src + [os.path.join(_HERE, "csrc", "chfpe_internal.cuh"), os.path.join(_HERE, "csrc", "chfpe_poly.h"), os.path.join(_HERE, "..", "include", "chfpe.h")]
+    return src, src + [os.path.join(_HERE, "csrc", "chfpe_internal.cuh"), os.path.join(_HERE, "csrc", "chfpe_poly.h"), os.path.join(_HERE, "csrc", "chfpe_hermite_tma.cuh"), os.path.join(_HERE, "..", "include", "chfpe.h")]
 
 
 def stale():

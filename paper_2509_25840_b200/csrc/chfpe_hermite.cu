@@ -57,6 +57,7 @@ struct HOp {                // device view of the operator, passed by value
   const double* cfac[3];
   int contig;                         // COMPACT6: transposing kernel for the contiguous axis (CHFPE_HERMITE_CONTIG=0: off)
   int fixed;                          // use the compile-time 32^3 specialisation when the mesh matches (CHFPE_HERMITE_FIXED=0: off)
+  int tma;                            // bulk-copy march kernel (three modes, n_1 x 32 x 32, explicit stencils; CHFPE_HERMITE_TMA=0: off)
 };
 
 struct HObs { double c0, lin_q[3], quad[3][3], lin_p[3]; };
@@ -467,6 +468,8 @@ __global__ void __launch_bounds__(256, (PA * PB <= 4) ? 4 : 1) k_hermite_stage_p
   }
 }
 
+#include "chfpe_hermite_tma.cuh"
+
 // COMPACT6 (the paper's q-derivative, Eq. 25-31, a = 7/9 by reading R4): for one mode s, every slab
 // and every q_s-line of it, form P = sqrt(k_s+1) c_{k+e_s} + sqrt(k_s) c_{k-e_s} along the line, the right-hand side
 // r = [a (P_{+1} - P_{-1}) + b (P_{+2} - P_{-2})] / h (truncated, R9), solve tridiag(1/3, 1, 1/3) d = r by the Thomas
@@ -834,6 +837,11 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
     h->launches += 1 + op.M;
     return;
   }
+  if (op.tma) {                                      // bulk-copy march kernel (n_1 x 32 x 32 meshes of three modes)
+    k_hermite_stage_tma<<<dim3((unsigned)op.nslab, (unsigned)nb), HtCfg::NT, HtCfg::SMEM, h->stream>>>(op, in, y, out, a, c, ss);
+    h->launches++;
+    return;
+  }
   if (op.pa > 0) {                                   // patch kernel (default for M >= 2)
     const dim3 g((unsigned)((size_t)(op.nslab / op.pcol) * op.pblocks), (unsigned)nb);
 #define HPATCH(MM, A, B, FA, FB, FL) k_hermite_stage_patch<MM, A, B, FA, FB, FL><<<g, 256, 0, h->stream>>>(op, in, y, out, a, c, ss)
@@ -1097,6 +1105,15 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
     { const char* fe = getenv("CHFPE_HERMITE_TILE"); op.tile = !(fe && fe[0] == '0'); }
     { const char* fe = getenv("CHFPE_HERMITE_PCOL"); op.pcol = (fe && fe[0] == '0') ? 1 : op.kp[M - 1]; }
     { const char* fe = getenv("CHFPE_HERMITE_CONTIG"); op.contig = !(fe && fe[0] == '0'); }
+    {
+      const char* fe = getenv("CHFPE_HERMITE_TMA");
+      op.tma = !(fe && fe[0] == '0') && !(e && *e) && !(pe && *pe) && M == 3 && op.nq[1] == 32 && op.nq[2] == 32 && op.nq[0] >= 2 && op.nq[0] % 2 == 0 &&
+               op.scheme != CHFPE_COMPACT6;
+      if (op.tma && cudaFuncSetAttribute(k_hermite_stage_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HtCfg::SMEM) != cudaSuccess) {
+        cudaGetLastError();
+        op.tma = 0;
+      }
+    }
     if (pa > 0) {
       const int ntA = (op.nq[0] + pa - 1) / pa;
       op.ntileB = (M == 3) ? (op.nq[1] + op.pb - 1) / op.pb : 1;
@@ -1137,6 +1154,17 @@ extern "C" int chfpe_hermite_num_elements(const chfpe_hermite_handle* h, int32_t
 extern "C" int chfpe_hermite_launch_count(const chfpe_hermite_handle* h, int64_t* n) {
   if (!h || !n) return CHFPE_ERR_INVALID;
   *n = h->launches;
+  return CHFPE_OK;
+}
+
+extern "C" int chfpe_hermite_stage_kernel(const chfpe_hermite_handle* h, int32_t* kind) {
+  if (!h || !kind) return CHFPE_ERR_INVALID;
+  const HOp& op = h->op;
+  *kind = (op.scheme == CHFPE_COMPACT6) ? CHFPE_HERMITE_STAGE_COMPACT
+          : op.tma                      ? CHFPE_HERMITE_STAGE_TMA
+          : (op.pa > 0)                 ? CHFPE_HERMITE_STAGE_PATCH
+          : (op.kc > 0)                 ? CHFPE_HERMITE_STAGE_COLUMN
+                                        : CHFPE_HERMITE_STAGE_VALUE;
   return CHFPE_OK;
 }
 

@@ -1,0 +1,317 @@
+// Bulk-copy fed RK-stage kernel of the Hermite representation (row f1; included by chfpe_hermite.cu inside its anonymous
+// namespace, after HOp / HSlab).  Same arithmetic as hermite_patch_body (de-garbled Eq. A1-A4, reading
+// R19), the data movement of k_stage_tma (chfpe_tma.cu): three modes on an n_1 x 32 x 32 mesh, explicit stencils.
+//
+// A CTA owns one slab (element n, Hermite multi-index k) and marches along q_1 in bands of two planes: a band of a slab
+// is a contiguous 16 KB chunk, so every operand arrives by a 1-D bulk copy (cp.async.bulk + mbarrier) into a ring of
+// shared-memory slots and is read exactly once with LDS.128.  Chunk kinds per band, consumed in this order (kind e always
+// uses slot e mod SLOTS; a kind that is absent moves no data but still flips its barriers):
+//   0 own slab | per mode s = 1..3: up (n, k+e_s), down (n, k-e_s), dU/dq_s on the band | six hierarchy neighbours
+//   (n-e_s, k+e_s), (n+e_s, k-e_s) | y of the PREVIOUS band | three unused kinds (20 kinds = 4 x 5 slots).
+// A thread owns four pairs of q_3-adjacent points: both planes of the band on rows r and r + 16.  Per mode the ladder
+// combination P_s = sqrt(k_s+1) c_up + sqrt(k_s) c_dn is formed in registers; its derivative runs along q_3 on warp
+// shuffles (a row is 16 lanes), along q_2 through one zero-padded shared plane pair, and along q_1 in scatter form over
+// the march: P_1 of band m is added to the accumulators of bands m-1, m and m+1, which live in registers (the halo of
+// two planes is exactly one band), so band m-1 is finished, combined with y and written while band m is in flight.
+// No q_1 halo is ever loaded: 13 chunks per band on average against 16.5 slab-units per value in the patch kernel.
+
+__device__ __forceinline__ unsigned ht_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void ht_mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void ht_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void ht_arrive_if(unsigned bar, bool on) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.u32 p, %1, 0;\n\t"
+      "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n\t}" ::"r"(bar), "r"((unsigned)on)
+      : "memory");
+}
+__device__ __forceinline__ void ht_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void ht_wait(unsigned bar, unsigned parity) {
+  unsigned done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.b32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void ht_bulk(unsigned dst, const void* src, unsigned bytes, unsigned bar, unsigned long long pol) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+      "l"(src), "r"(bytes), "r"(bar), "l"(pol)
+      : "memory");
+}
+__device__ __forceinline__ void ht_prefetch(const void* src, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ double2 ht_lds2(unsigned addr) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ unsigned long long ht_policy(int kind) {   // 0 normal, 1 evict_first
+  unsigned long long p;
+  if (kind == 1) asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  else asm("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void ht_st2(double2* p, double2 v, unsigned long long pol) {
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ double2 ht_fma2(double c, double2 a, double2 b) { return make_double2(fma(c, a.x, b.x), fma(c, a.y, b.y)); }
+
+template <int J, int N> struct HtUnroll {
+  template <typename F> __device__ __forceinline__ static void run(F&& f) { f(std::integral_constant<int, J>()); HtUnroll<J + 1, N>::run(f); }
+};
+template <int N> struct HtUnroll<N, N> {
+  template <typename F> __device__ __forceinline__ static void run(F&&) {}
+};
+template <int E> using HtKind = std::integral_constant<int, E>;
+
+struct HtCfg {
+  static constexpr int NROW = 32, NCOL = 32, PLANE = NROW * NCOL, BAND = 2 * PLANE;   // two q_1 planes per band
+  static constexpr unsigned CHUNK = BAND * sizeof(double);                            // 16 KB
+  static constexpr int SLOTS = 5, NK = 20, NT = 256, NW = NT / 32, NI = 4;            // NI pairs per thread
+  static constexpr int G2_PLANE = (NROW + 4) * NCOL;                                  // P_2[plane][row + 2][col]
+  static constexpr size_t SMEM = (size_t)SLOTS * CHUNK + sizeof(double) * 2 * G2_PLANE + 16 * SLOTS + 16 + 8 * NK + 16;
+};
+
+__global__ void __launch_bounds__(HtCfg::NT, 2) k_hermite_stage_tma(const HOp op, const double* __restrict__ in, const double* y,
+                                                                   double* out, const double a, const double c,
+                                                                   const size_t slot_stride) {
+  using C = HtCfg;
+  constexpr int NK = C::NK, SLOTS = C::SLOTS, NI = C::NI;
+  extern __shared__ __align__(128) unsigned char ht_smem[];
+  double* g2 = reinterpret_cast<double*>(ht_smem + (size_t)SLOTS * C::CHUNK);
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(g2 + 2 * C::G2_PLANE);
+  unsigned long long* empty = full + SLOTS;
+  unsigned long long* xbar = empty + SLOTS;                         // [0]: P_2 planes written, [1]: read
+  const double** ent = reinterpret_cast<const double**>(xbar + 2);  // source of every kind at band 0
+  const unsigned ring_a = ht_smem_u32(ht_smem), full_a = ht_smem_u32(full), empty_a = ht_smem_u32(empty), xbar_a = ht_smem_u32(xbar);
+
+  const int t = threadIdx.x, lane = t & 31, warp = __shfl_sync(0xffffffffu, t >> 5, 0);
+  const int slab = blockIdx.x;
+  const size_t soff = (size_t)blockIdx.y * slot_stride, Q = (size_t)op.Q;
+  const HSlab* __restrict__ S = op.slabs + slab;
+  const int nbands = op.nq[0] / 2;
+  int up[3], dn[3], hdn[3], hup[3];
+#pragma unroll
+  for (int s = 0; s < 3; s++) { up[s] = S->up[s]; dn[s] = S->dn[s]; hdn[s] = S->hdn[s]; hup[s] = S->hup[s]; }
+  // kinds: 0 self | 1+3s up_s, 2+3s dn_s, 3+3s dU_s | 10+2s hdn_s, 11+2s hup_s | 16 y of the previous band
+  unsigned mask_line = 1u;
+#pragma unroll
+  for (int s = 0; s < 3; s++) {
+    if (up[s] >= 0) mask_line |= 1u << (1 + 3 * s);
+    if (dn[s] >= 0) mask_line |= 1u << (2 + 3 * s);
+    if (up[s] >= 0 || dn[s] >= 0) mask_line |= 1u << (3 + 3 * s);
+    if (hdn[s] >= 0) mask_line |= 1u << (10 + 2 * s);
+    if (hup[s] >= 0) mask_line |= 1u << (11 + 2 * s);
+  }
+  auto step_mask = [&](int m) -> unsigned { return (m < nbands ? mask_line : 0u) | ((m >= 1 && m <= nbands) ? (1u << 16) : 0u); };
+  // own slab, Hermite neighbours, dU: re-read by the CTAs of the neighbouring slabs -> normal L2 policy; hierarchy neighbours
+  // (other elements: 512 slabs away in launch order) and y are used once per launch -> evict_first, as are the stores
+  const unsigned long long pol_in = ht_policy(0), pol_str = ht_policy(1);
+  auto issue = [&](int m, int e, unsigned mk) {                      // one thread: load kind e of band m, or just flip its barrier
+    const unsigned fb = full_a + 8 * (e % SLOTS);
+    if ((mk >> e) & 1u) {
+      ht_expect_tx(fb, C::CHUNK);
+      ht_bulk(ring_a + (e % SLOTS) * C::CHUNK, ent[e] + (size_t)m * C::BAND, C::CHUNK, fb, e >= 10 ? pol_str : pol_in);
+    } else {
+      ht_arrive(fb);
+    }
+  };
+  if (t == 0) {
+    for (int s = 0; s < SLOTS; s++) { ht_mbar_init(full_a + 8 * s, 1); ht_mbar_init(empty_a + 8 * s, C::NW); }
+    ht_mbar_init(xbar_a, C::NW); ht_mbar_init(xbar_a + 8, C::NW);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    const double* X = in + soff;
+    for (int e = 0; e < NK; e++) ent[e] = X + (size_t)slab * Q;
+#pragma unroll
+    for (int s = 0; s < 3; s++) {
+      ent[1 + 3 * s] = X + (size_t)(up[s] >= 0 ? up[s] : slab) * Q;
+      ent[2 + 3 * s] = X + (size_t)(dn[s] >= 0 ? dn[s] : slab) * Q;
+      ent[3 + 3 * s] = op.dU[s];
+      ent[10 + 2 * s] = X + (size_t)(hdn[s] >= 0 ? hdn[s] : slab) * Q;
+      ent[11 + 2 * s] = X + (size_t)(hup[s] >= 0 ? hup[s] : slab) * Q;
+    }
+    ent[16] = (a != 0.0 ? y + soff : X) + (size_t)slab * Q - C::BAND;   // (band m - 1 at step m; a = 0: y is not to be read)
+    const unsigned mk0 = step_mask(0);
+    for (int e = 0; e < SLOTS; e++) issue(0, e, mk0);
+  }
+  for (int i = t; i < 2 * 4 * C::NCOL; i += C::NT) {                 // ghost rows -2, -1, 32, 33 of both P_2 planes stay zero
+    const int pl = i / (4 * C::NCOL), rr = i - pl * (4 * C::NCOL), row = rr / C::NCOL, col = rr - row * C::NCOL;
+    g2[pl * C::G2_PLANE + (row < 2 ? row : C::NROW + row) * C::NCOL + col] = 0.0;
+  }
+  __syncthreads();
+
+  const int cp = t & 15, r0 = t >> 4;                               // pair column, first row (the second one is r0 + 16)
+  // item j = 0..3: plane j >> 1, row r0 + 16 (j & 1); byte offset of the pair inside a chunk
+  unsigned my_a = ring_a + (unsigned)(r0 * C::NCOL + 2 * cp) * 8;
+  asm volatile("" : "+r"(my_a));
+  auto item_off = [](int j) { return (unsigned)(((j >> 1) * HtCfg::PLANE + (j & 1) * 16 * HtCfg::NCOL) * 8); };
+  const double gam = S->gam;
+  int m = 0;
+  unsigned mask = __shfl_sync(0xffffffffu, step_mask(0), 0), maskn = __shfl_sync(0xffffffffu, step_mask(1), 0), mpar = 0;
+  auto parity = [&](int E, unsigned mp) -> unsigned { return ((unsigned)(E / SLOTS) & 1u) ^ (((NK / SLOTS) & 1) ? mp : 0u); };
+  auto duty = [&](auto KEP, int mm, unsigned mp, unsigned mk_same, unsigned mk_next) {
+    constexpr int EP = decltype(KEP)::value;
+    constexpr int E2 = (EP + SLOTS < NK) ? EP + SLOTS : EP + SLOTS - NK;
+    const int m2 = (EP + SLOTS < NK) ? mm : mm + 1;
+    if (mm < 0 || m2 > nbands) return;
+    ht_wait(empty_a + 8 * (EP % SLOTS), parity(EP, mp));
+    if (lane == 0) issue(m2, E2, (EP + SLOTS < NK) ? mk_same : mk_next);
+  };
+  auto chunk = [&](auto KE, auto&& body) {
+    constexpr int E = decltype(KE)::value;
+    ht_wait(full_a + 8 * (E % SLOTS), parity(E, mpar));
+    if ((mask >> E) & 1u) body(my_a + (E % SLOTS) * C::CHUNK);
+    __syncwarp();
+    ht_arrive_if(empty_a + 8 * (E % SLOTS), lane == 0);
+    constexpr int EP = (E + NK - 1) % NK;
+    if (warp == EP % C::NW) {
+      if (E == 0) duty(HtKind<EP>(), m - 1, mpar ^ 1u, 0u, mask);
+      else duty(HtKind<EP>(), m, mpar, mask, maskn);
+    }
+  };
+  // accumulators: A[0] band m-1 (complete after this step), A[1] band m, A[2] band m+1
+  double2 A[3][NI];
+#pragma unroll
+  for (int q = 0; q < 3; q++)
+#pragma unroll
+    for (int j = 0; j < NI; j++) A[q][j] = make_double2(0.0, 0.0);
+  double2* Ob = reinterpret_cast<double2*>(out + soff + (size_t)slab * Q) + (r0 * C::NCOL + 2 * cp) / 2;
+  const double q3a = op.q0[2] + op.h[2] * (double)(2 * cp), q3b = q3a + op.h[2];
+
+#pragma unroll 1
+  for (; m <= nbands; m++) {
+    const bool have = m < nbands;
+    if (t == 0 && m + 1 < nbands) {                                  // hierarchy neighbours and y come from HBM: ask L2 one band
+      const size_t bn = (size_t)(m + 1) * C::BAND;                   // early (two bands early measured slower: 3.43 vs 3.15 ms)
+#pragma unroll
+      for (int e = 10; e < 16; e++)
+        if ((mask_line >> e) & 1u) ht_prefetch(ent[e] + bn, C::CHUNK);
+      ht_prefetch(ent[16] + bn + C::BAND, C::CHUNK);
+    }
+    double2(&acc)[NI] = A[1];
+    chunk(HtKind<0>(), [&](unsigned Sa) {                           // -Gamma_n c
+#pragma unroll
+      for (int j = 0; j < NI; j++) acc[j] = ht_fma2(-gam, ht_lds2(Sa + item_off(j)), acc[j]);
+    });
+    HtUnroll<0, 3>::run([&](auto SS) {
+      constexpr int s = decltype(SS)::value;
+      const double su = (up[s] >= 0) ? S->su[s] : 0.0, sd = (dn[s] >= 0) ? S->sd[s] : 0.0;
+      double2 P[NI], Lc[NI];                                        // su c_up + sd c_dn,  su c_up - sd c_dn
+#pragma unroll
+      for (int j = 0; j < NI; j++) { P[j] = make_double2(0.0, 0.0); Lc[j] = make_double2(0.0, 0.0); }
+      chunk(HtKind<1 + 3 * s>(), [&](unsigned Sa) {
+#pragma unroll
+        for (int j = 0; j < NI; j++) { const double2 v = ht_lds2(Sa + item_off(j)); P[j] = ht_fma2(su, v, P[j]); Lc[j] = ht_fma2(su, v, Lc[j]); }
+      });
+      chunk(HtKind<2 + 3 * s>(), [&](unsigned Sa) {
+#pragma unroll
+        for (int j = 0; j < NI; j++) { const double2 v = ht_lds2(Sa + item_off(j)); P[j] = ht_fma2(sd, v, P[j]); Lc[j] = ht_fma2(-sd, v, Lc[j]); }
+      });
+      const double a1f = op.a1f[s];
+      chunk(HtKind<3 + 3 * s>(), [&](unsigned Sa) {                 // a1f dU/dq_s (su c_up - sd c_dn)
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
+          const double2 v = ht_lds2(Sa + item_off(j));
+          acc[j].x = fma(a1f * v.x, Lc[j].x, acc[j].x);
+          acc[j].y = fma(a1f * v.y, Lc[j].y, acc[j].y);
+        }
+      });
+      const double w1 = -op.a2[s] * op.c1[s], w2 = -op.a2[s] * op.c2[s];   // -a2 D_q P, D f = c1 (f+1 - f-1) + c2 (f+2 - f-2)
+      if (have && ((mask_line >> (3 + 3 * s)) & 1u)) {
+        if (s == 0) {                                               // q_1: planes i0 = 2m (items 0, 1) and i0 + 1 (items 2, 3)
+#pragma unroll
+          for (int rr = 0; rr < 2; rr++) {
+            const double2 f0 = P[rr], f1 = P[2 + rr];
+            A[0][rr] = ht_fma2(w2, f0, A[0][rr]);                                   // row 2m-2 sees f(2m) at +2
+            A[0][2 + rr] = ht_fma2(w1, f0, ht_fma2(w2, f1, A[0][2 + rr]));          // row 2m-1: +1 and +2
+            A[1][rr] = ht_fma2(w1, f1, A[1][rr]);                                   // row 2m sees f(2m+1) at +1
+            A[1][2 + rr] = ht_fma2(-w1, f0, A[1][2 + rr]);                          // row 2m+1 sees f(2m) at -1
+            A[2][rr] = ht_fma2(-w1, f1, ht_fma2(-w2, f0, A[2][rr]));                // row 2m+2: -1 and -2
+            A[2][2 + rr] = ht_fma2(-w2, f1, A[2][2 + rr]);                          // row 2m+3 sees f(2m+1) at -2
+          }
+        } else if (s == 1) {                                        // q_2: through the shared plane pair
+          if (m > 0) ht_wait(xbar_a + 8, (unsigned)(m - 1) & 1u);   // the planes of the previous band have been read
+#pragma unroll
+          for (int j = 0; j < NI; j++)
+            *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1) + 2) * C::NCOL + 2 * cp) = P[j];
+        } else {                                                    // q_3: the 16 lanes of a row
+#pragma unroll
+          for (int j = 0; j < NI; j++) {
+            const double2 own = P[j];
+            double ly = __shfl_up_sync(0xffffffffu, own.y, 1, 16), rx = __shfl_down_sync(0xffffffffu, own.x, 1, 16);
+            double lx = __shfl_up_sync(0xffffffffu, own.x, 1, 16), ry = __shfl_down_sync(0xffffffffu, own.y, 1, 16);
+            if (cp == 0) { ly = 0.0; lx = 0.0; }
+            if (cp == 15) { rx = 0.0; ry = 0.0; }
+            // pair (i, i+1): neighbours i-2 .. i+3 = lx ly [own.x own.y] rx ry
+            acc[j].x = fma(w1, own.y - ly, fma(w2, rx - lx, acc[j].x));
+            acc[j].y = fma(w1, rx - own.x, fma(w2, ry - ly, acc[j].y));
+          }
+        }
+      } else if (s == 1 && have) {                                  // nothing to exchange for this slab: keep the barriers in step
+        if (m > 0) ht_wait(xbar_a + 8, (unsigned)(m - 1) & 1u);
+#pragma unroll
+        for (int j = 0; j < NI; j++)
+          *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1) + 2) * C::NCOL + 2 * cp) = make_double2(0.0, 0.0);
+      }
+      if (s == 1 && have) { __syncwarp(); ht_arrive_if(xbar_a, lane == 0); }     // this warp's P_2 values are written
+    });
+    HtUnroll<0, 6>::run([&](auto HH) {                              // V'_s (hd c(n-e_s, k+e_s) + hu c(n+e_s, k-e_s))
+      constexpr int hh = decltype(HH)::value, s = hh / 2;
+      const double hc = (hh & 1) ? S->hu[s] : S->hd[s];
+      chunk(HtKind<10 + hh>(), [&](unsigned Sa) {
+#pragma unroll
+        for (int j = 0; j < NI; j++) {
+          const double2 v = ht_lds2(Sa + item_off(j));
+          const double qa = (s == 0) ? op.q0[0] + op.h[0] * (double)(2 * m + (j >> 1))
+                          : (s == 1 ? op.q0[1] + op.h[1] * (double)(r0 + 16 * (j & 1)) : q3a);
+          const double qb = (s == 2) ? q3b : qa;
+          acc[j].x = fma(hc * fma(op.VSL[s], qa, op.VLL[s]), v.x, acc[j].x);
+          acc[j].y = fma(hc * fma(op.VSL[s], qb, op.VLL[s]), v.y, acc[j].y);
+        }
+      });
+    });
+    if (have) {                                                     // q_2 stencil of P_2
+      ht_wait(xbar_a, (unsigned)m & 1u);
+      const double w1 = -op.a2[1] * op.c1[1], w2 = -op.a2[1] * op.c2[1];
+#pragma unroll
+      for (int j = 0; j < NI; j++) {
+        const double* g = g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1) + 2) * C::NCOL + 2 * cp;
+        const double2 u1 = *reinterpret_cast<const double2*>(g + C::NCOL), d1 = *reinterpret_cast<const double2*>(g - C::NCOL);
+        const double2 u2 = *reinterpret_cast<const double2*>(g + 2 * C::NCOL), d2 = *reinterpret_cast<const double2*>(g - 2 * C::NCOL);
+        acc[j].x = fma(w1, u1.x - d1.x, fma(w2, u2.x - d2.x, acc[j].x));
+        acc[j].y = fma(w1, u1.y - d1.y, fma(w2, u2.y - d2.y, acc[j].y));
+      }
+      __syncwarp();
+      ht_arrive_if(xbar_a + 8, lane == 0);
+    }
+    chunk(HtKind<16>(), [&](unsigned Sa) {                          // band m-1 is complete: out = a y + c F
+      double2* O = Ob + (size_t)(m - 1) * (C::BAND / 2);
+#pragma unroll
+      for (int j = 0; j < NI; j++) {
+        const double2 yv = ht_lds2(Sa + item_off(j));
+        ht_st2(O + item_off(j) / 16, make_double2(fma(c, A[0][j].x, a * yv.x), fma(c, A[0][j].y, a * yv.y)), pol_str);
+      }
+    });
+    chunk(HtKind<17>(), [&](unsigned) {});
+    chunk(HtKind<18>(), [&](unsigned) {});
+    chunk(HtKind<19>(), [&](unsigned) {});
+#pragma unroll
+    for (int j = 0; j < NI; j++) { A[0][j] = A[1][j]; A[1][j] = A[2][j]; A[2][j] = make_double2(0.0, 0.0); }
+    mask = maskn;
+    maskn = __shfl_sync(0xffffffffu, step_mask(m + 2), 0);
+    mpar ^= 1u;
+  }
+}

@@ -322,14 +322,20 @@ def test_cube32_specialisation_up_to_the_mesh_edges(kp, depth):
     o.import_state(X)
     o.step(2, cfg["dt"])
     Yo = o.export_state()
-    for var in (None, "CHFPE_HERMITE_TILE", "CHFPE_HERMITE_FIXED", "CHFPE_HERMITE_PCOL"):
-        if var:
-            os.environ[var] = "0"
+    for var in ("tma", None, "CHFPE_HERMITE_TILE", "CHFPE_HERMITE_FIXED", "CHFPE_HERMITE_PCOL"):
+        # "tma": the default on this mesh, the bulk-copy march kernel; the others: the patch kernel and its launch shapes
+        if var != "tma":
+            os.environ["CHFPE_HERMITE_TMA"] = "0"
+            if var:
+                os.environ[var] = "0"
         try:
             g = P().Hermite(cfg)
         finally:
-            if var:
-                del os.environ[var]
+            if var != "tma":
+                del os.environ["CHFPE_HERMITE_TMA"]
+                if var:
+                    del os.environ[var]
+        assert g.stage_kernel() == ("tma" if var == "tma" else "patch")
         g.import_state(X)
         F = g.export_rhs()
         assert rel_l2(F, Fo) < 1e-13, var
@@ -339,6 +345,41 @@ def test_cube32_specialisation_up_to_the_mesh_edges(kp, depth):
         g.step(2, cfg["dt"])
         assert rel_l2(g.export_state(), Yo) < 1e-12, var
         g.close()
+
+
+MARCH = [
+    ("ten_planes", dict(nq=[10, 32, 32], np=[2, 2, 2], depth=2)),                 # an odd number of bands, every neighbour kind
+    ("six_planes_c2", dict(nq=[6, 32, 32], np=[2, 1, 3], depth=2, scheme="central2", mass=[1.0, 0.8, 1.2])),
+    ("depth0_long", dict(nq=[70, 32, 32], np=[1, 2, 2], depth=0)),                # no hierarchy neighbours, 35 bands
+    ("kp1", dict(nq=[8, 32, 32], np=[1, 1, 1], depth=3)),                         # no Hermite neighbours: couplings only
+]
+
+
+@pytest.mark.parametrize("name,kw", MARCH, ids=[c[0] for c in MARCH])
+def test_march_kernel_on_other_mesh_lengths(name, kw, monkeypatch):
+    """k_hermite_stage_tma (bulk-copy march along q_1 in bands of two planes) on n_1 x 32 x 32 meshes: three bands (the
+    shortest mesh the path accepts has six planes), an odd number of bands, more bands than the ring has parities, absent kinds of every sort.  The state is O(1) on every
+    mesh face.  Right-hand side (a = 0: y is not read), three RK4 steps (the last stage writes y in place) and two
+    batch slots against the oracle; CHFPE_HERMITE_TMA=0 must give the patch kernel's result on the same input."""
+    cfg = ci.config("cfg4h", **kw)
+    g, o = both(cfg, batch=2)
+    assert g.stage_kernel() == "tma"
+    X = ci.seeded_hermite_state(cfg, [sum(n) for n in o.elems], seed=21)
+    X = X + 0.05 * np.random.default_rng(3).uniform(-1.0, 1.0, size=X.shape)
+    g.import_state(X); g.import_state(2.0 * X, replica=1); o.import_state(X)
+    Fo = o.rhs(o.c)
+    assert rel_l2(g.export_rhs(), Fo) < 1e-13
+    assert rel_l2(g.export_rhs(replica=1), 2.0 * Fo) < 1e-13
+    g.step(3, cfg["dt"]); o.step(3, cfg["dt"])
+    Yo = o.export_state()
+    assert rel_l2(g.export_state(), Yo) < 1e-12
+    assert rel_l2(g.export_state(replica=1), 2.0 * Yo) < 1e-12
+    monkeypatch.setenv("CHFPE_HERMITE_TMA", "0")
+    p = P().Hermite(cfg)
+    assert p.stage_kernel() == "patch"
+    p.import_state(X)
+    assert rel_l2(p.export_rhs(), Fo) < 1e-13
+    p.close(); g.close()
 
 
 def test_full_size_rhs_on_an_embedded_block():
@@ -364,12 +405,17 @@ def test_full_size_rhs_on_an_embedded_block():
     F = g.export_rhs_device()[blk].cpu().numpy()
     Fo = o.rhs(Xs)
     assert rel_l2(F, Fo) < 1e-13
-    for var in ("CHFPE_HERMITE_TILE", "CHFPE_HERMITE_FIXED", "CHFPE_HERMITE_PCOL"):   # the other launch shapes at this size
+    assert g.stage_kernel() == "tma"
+    for var in ("CHFPE_HERMITE_TMA", "CHFPE_HERMITE_TILE", "CHFPE_HERMITE_FIXED", "CHFPE_HERMITE_PCOL"):   # the patch kernel's launch shapes at this size
         os.environ[var] = "0"
+        os.environ["CHFPE_HERMITE_TMA"] = "0"
         try:
             g2 = P().Hermite(cfg)
         finally:
-            del os.environ[var]
+            del os.environ["CHFPE_HERMITE_TMA"]
+            if var != "CHFPE_HERMITE_TMA":
+                del os.environ[var]
+        assert g2.stage_kernel() == "patch"
         g2.import_state(X)
         assert rel_l2(g2.export_rhs_device()[blk].cpu().numpy(), Fo) < 1e-13, var
         g2.close()
