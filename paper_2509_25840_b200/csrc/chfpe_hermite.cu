@@ -800,7 +800,15 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
   const size_t ss = 3 * h->state_doubles;
   if (op.scheme == CHFPE_COMPACT6) {                 // pointwise terms, then one line pass per mode
     const dim3 g0 = slab_grid(op, nb);
-    if (op.kc > 0) {                                 // column kernel without the derivative terms (4 Hermite indices per thread)
+    if (op.tma) {                                    // march kernel: pointwise terms and the q_2, q_3 line solves; then the q_1 pass
+      k_hermite_stage_tma<true><<<dim3((unsigned)op.nslab, (unsigned)nb), HtCfgT<true>::NT, HtCfgT<true>::SMEM, h->stream>>>(op, in, y, out, a, c, ss);
+      const int nlines = op.Q / op.nq[0];
+      const dim3 g((unsigned)((size_t)op.nslab * ((nlines + 127) / 128)), (unsigned)nb);
+      k_hermite_compact_line<3><<<g, 128, 0, h->stream>>>(op, 0, in, out, c, ss);
+      h->launches += 2;
+      return;
+    }
+    if (op.kc > 0) {                          // column kernel without the derivative terms (4 Hermite indices per thread)
       const int nch = (op.kp[op.M - 1] + 3) / 4;
       HOp o4 = op;
       o4.nchunk = nch;
@@ -838,7 +846,7 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
     return;
   }
   if (op.tma) {                                      // bulk-copy march kernel (n_1 x 32 x 32 meshes of three modes)
-    k_hermite_stage_tma<<<dim3((unsigned)op.nslab, (unsigned)nb), HtCfg::NT, HtCfg::SMEM, h->stream>>>(op, in, y, out, a, c, ss);
+    k_hermite_stage_tma<false><<<dim3((unsigned)op.nslab, (unsigned)nb), HtCfg::NT, HtCfg::SMEM, h->stream>>>(op, in, y, out, a, c, ss);
     h->launches++;
     return;
   }
@@ -1107,9 +1115,9 @@ extern "C" int chfpe_hermite_create(const chfpe_desc* desc, void* ws, size_t byt
     { const char* fe = getenv("CHFPE_HERMITE_CONTIG"); op.contig = !(fe && fe[0] == '0'); }
     {
       const char* fe = getenv("CHFPE_HERMITE_TMA");
-      op.tma = !(fe && fe[0] == '0') && !(e && *e) && !(pe && *pe) && M == 3 && op.nq[1] == 32 && op.nq[2] == 32 && op.nq[0] >= 2 && op.nq[0] % 2 == 0 &&
-               op.scheme != CHFPE_COMPACT6;
-      if (op.tma && cudaFuncSetAttribute(k_hermite_stage_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HtCfg::SMEM) != cudaSuccess) {
+      op.tma = !(fe && fe[0] == '0') && !(e && *e) && !(pe && *pe) && M == 3 && op.nq[1] == 32 && op.nq[2] == 32 && op.nq[0] >= 2 && op.nq[0] % 2 == 0;
+      if (op.tma && (cudaFuncSetAttribute(k_hermite_stage_tma<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HtCfg::SMEM) != cudaSuccess ||
+                     cudaFuncSetAttribute(k_hermite_stage_tma<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HtCfgT<true>::SMEM) != cudaSuccess)) {
         cudaGetLastError();
         op.tma = 0;
       }

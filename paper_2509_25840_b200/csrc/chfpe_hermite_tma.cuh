@@ -14,6 +14,9 @@
 // the march: P_1 of band m is added to the accumulators of bands m-1, m and m+1, which live in registers (the halo of
 // two planes is exactly one band), so band m-1 is finished, combined with y and written while band m is in flight.
 // No q_1 halo is ever loaded: 13 chunks per band on average against 16.5 slab-units per value in the patch kernel.
+// COMPACT6 (template flag CMP): the compact (Pade) derivative along q_2 and q_3 is solved inside the kernel on shared
+// memory (Eq. 25-31 :177-201 with a = 7/9, R4; Thomas as in k_hermite_compact_line); only the q_1 lines, which run along
+// the march, keep their line pass, so a stage is 2 launches instead of 4.
 
 __device__ __forceinline__ unsigned ht_smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void ht_mbar_init(unsigned bar, unsigned count) {
@@ -77,25 +80,34 @@ template <int N> struct HtUnroll<N, N> {
 };
 template <int E> using HtKind = std::integral_constant<int, E>;
 
-struct HtCfg {
+// CMP = false: explicit stencils (CENTRAL4 / CENTRAL2).  CMP = true: COMPACT6, the Pade derivative along q_2 and q_3 is solved
+// inside the kernel (one Thomas solve per line of the band, 128 lines of 32 points: 16 lanes of every warp own one line each,
+// the recurrence of k_hermite_compact_line on shared memory); the q_1 lines run along the march and keep their own line pass.
+template <bool CMP> struct HtCfgT {
   static constexpr int NROW = 32, NCOL = 32, PLANE = NROW * NCOL, BAND = 2 * PLANE;   // two q_1 planes per band
   static constexpr unsigned CHUNK = BAND * sizeof(double);                            // 16 KB
-  static constexpr int SLOTS = 5, NK = 20, NT = 256, NW = NT / 32, NI = 4;            // NI pairs per thread
+  static constexpr int SLOTS = CMP ? 4 : 5, NK = 20, NT = 256, NW = NT / 32, NI = 4;  // NI pairs per thread
   static constexpr int G2_PLANE = (NROW + 4) * NCOL;                                  // P_2[plane][row + 2][col]
-  static constexpr size_t SMEM = (size_t)SLOTS * CHUNK + sizeof(double) * 2 * G2_PLANE + 16 * SLOTS + 16 + 8 * NK + 16;
+  static constexpr int G3_LD = NCOL + 1, G3_PLANE = NROW * G3_LD;                     // CMP: P_3[plane][row][col], padded rows
+  static constexpr size_t SMEM = (size_t)SLOTS * CHUNK + sizeof(double) * 2 * (G2_PLANE + (CMP ? G3_PLANE : 0)) + 16 * SLOTS + 32 +
+                                 8 * NK + (CMP ? 512 : 0) + 16;
 };
+using HtCfg = HtCfgT<false>;
 
-__global__ void __launch_bounds__(HtCfg::NT, 2) k_hermite_stage_tma(const HOp op, const double* __restrict__ in, const double* y,
-                                                                   double* out, const double a, const double c,
-                                                                   const size_t slot_stride) {
-  using C = HtCfg;
+template <bool CMP>
+__global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const HOp op, const double* __restrict__ in, const double* y,
+                                                                         double* out, const double a, const double c,
+                                                                         const size_t slot_stride) {
+  using C = HtCfgT<CMP>;
   constexpr int NK = C::NK, SLOTS = C::SLOTS, NI = C::NI;
   extern __shared__ __align__(128) unsigned char ht_smem[];
   double* g2 = reinterpret_cast<double*>(ht_smem + (size_t)SLOTS * C::CHUNK);
-  unsigned long long* full = reinterpret_cast<unsigned long long*>(g2 + 2 * C::G2_PLANE);
+  double* g3 = g2 + 2 * C::G2_PLANE;                                // CMP only
+  unsigned long long* full = reinterpret_cast<unsigned long long*>(g3 + (CMP ? 2 * C::G3_PLANE : 0));
   unsigned long long* empty = full + SLOTS;
-  unsigned long long* xbar = empty + SLOTS;                         // [0]: P_2 planes written, [1]: read
-  const double** ent = reinterpret_cast<const double**>(xbar + 2);  // source of every kind at band 0
+  unsigned long long* xbar = empty + SLOTS;                         // [0]: P planes written, [1]: read, [2]: solved (CMP)
+  const double** ent = reinterpret_cast<const double**>(xbar + 4);  // source of every kind at band 0
+  double* tab = reinterpret_cast<double*>(ent + NK);                // CMP: reciprocal pivots [0, 32) and elimination factors [32, 64)
   const unsigned ring_a = ht_smem_u32(ht_smem), full_a = ht_smem_u32(full), empty_a = ht_smem_u32(empty), xbar_a = ht_smem_u32(xbar);
 
   const int t = threadIdx.x, lane = t & 31, warp = __shfl_sync(0xffffffffu, t >> 5, 0);
@@ -131,7 +143,9 @@ __global__ void __launch_bounds__(HtCfg::NT, 2) k_hermite_stage_tma(const HOp op
   };
   if (t == 0) {
     for (int s = 0; s < SLOTS; s++) { ht_mbar_init(full_a + 8 * s, 1); ht_mbar_init(empty_a + 8 * s, C::NW); }
-    ht_mbar_init(xbar_a, C::NW); ht_mbar_init(xbar_a + 8, C::NW);
+    ht_mbar_init(xbar_a, C::NW); ht_mbar_init(xbar_a + 8, C::NW); ht_mbar_init(xbar_a + 16, C::NW);
+    if (CMP)                                                        // both axes have 32 points: one table (it depends on n only)
+      for (int i = 0; i < 32; i++) { tab[i] = op.ibet[1][i]; tab[32 + i] = op.cfac[1][i]; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     const double* X = in + soff;
     for (int e = 0; e < NK; e++) ent[e] = X + (size_t)slab * Q;
@@ -157,7 +171,7 @@ __global__ void __launch_bounds__(HtCfg::NT, 2) k_hermite_stage_tma(const HOp op
   // item j = 0..3: plane j >> 1, row r0 + 16 (j & 1); byte offset of the pair inside a chunk
   unsigned my_a = ring_a + (unsigned)(r0 * C::NCOL + 2 * cp) * 8;
   asm volatile("" : "+r"(my_a));
-  auto item_off = [](int j) { return (unsigned)(((j >> 1) * HtCfg::PLANE + (j & 1) * 16 * HtCfg::NCOL) * 8); };
+  auto item_off = [](int j) { return (unsigned)(((j >> 1) * C::PLANE + (j & 1) * 16 * C::NCOL) * 8); };
   const double gam = S->gam;
   int m = 0;
   unsigned mask = __shfl_sync(0xffffffffu, step_mask(0), 0), maskn = __shfl_sync(0xffffffffu, step_mask(1), 0), mpar = 0;
@@ -230,6 +244,23 @@ __global__ void __launch_bounds__(HtCfg::NT, 2) k_hermite_stage_tma(const HOp op
         }
       });
       const double w1 = -op.a2[s] * op.c1[s], w2 = -op.a2[s] * op.c2[s];   // -a2 D_q P, D f = c1 (f+1 - f-1) + c2 (f+2 - f-2)
+      if (CMP) {                                                    // P_2, P_3 go to shared memory for the line solves
+        if (have && s == 1) {
+          if (m > 0) ht_wait(xbar_a + 8, (unsigned)(m - 1) & 1u);   // the results of the previous band have been read
+#pragma unroll
+          for (int j = 0; j < NI; j++)
+            *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1)) * C::NCOL + 2 * cp) = P[j];
+        }
+        if (have && s == 2) {
+#pragma unroll
+          for (int j = 0; j < NI; j++) {
+            double* g = g3 + (j >> 1) * C::G3_PLANE + (r0 + 16 * (j & 1)) * C::G3_LD + 2 * cp;
+            g[0] = P[j].x; g[1] = P[j].y;
+          }
+          __syncwarp();
+          ht_arrive_if(xbar_a, lane == 0);                          // this warp's P_2 and P_3 values are written
+        }
+      } else
       if (have && ((mask_line >> (3 + 3 * s)) & 1u)) {
         if (s == 0) {                                               // q_1: planes i0 = 2m (items 0, 1) and i0 + 1 (items 2, 3)
 #pragma unroll
@@ -260,13 +291,13 @@ __global__ void __launch_bounds__(HtCfg::NT, 2) k_hermite_stage_tma(const HOp op
             acc[j].y = fma(w1, rx - own.x, fma(w2, ry - ly, acc[j].y));
           }
         }
-      } else if (s == 1 && have) {                                  // nothing to exchange for this slab: keep the barriers in step
+      } else if (!CMP && s == 1 && have) {                          // nothing to exchange for this slab: keep the barriers in step
         if (m > 0) ht_wait(xbar_a + 8, (unsigned)(m - 1) & 1u);
 #pragma unroll
         for (int j = 0; j < NI; j++)
           *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1) + 2) * C::NCOL + 2 * cp) = make_double2(0.0, 0.0);
       }
-      if (s == 1 && have) { __syncwarp(); ht_arrive_if(xbar_a, lane == 0); }     // this warp's P_2 values are written
+      if (!CMP && s == 1 && have) { __syncwarp(); ht_arrive_if(xbar_a, lane == 0); }     // this warp's P_2 values are written
     });
     HtUnroll<0, 6>::run([&](auto HH) {                              // V'_s (hd c(n-e_s, k+e_s) + hu c(n+e_s, k-e_s))
       constexpr int hh = decltype(HH)::value, s = hh / 2;
@@ -283,7 +314,45 @@ __global__ void __launch_bounds__(HtCfg::NT, 2) k_hermite_stage_tma(const HOp op
         }
       });
     });
-    if (have) {                                                     // q_2 stencil of P_2
+    if (CMP && have) {
+      // 128 lines per band (2 planes x 32 columns along q_2, 2 planes x 32 rows along q_3), 16 per warp: lanes 0-7 take q_2 lines,
+      // lanes 8-15 q_3 lines.  T d = r, T = tridiag(1/3, 1, 1/3), r_i = ca (P_{i+1} - P_{i-1}) + cb (P_{i+2} - P_{i-2}) with zero
+      // ghosts (R9), by the Thomas recurrence with the host-tabulated reciprocal pivots of k_hermite_compact_line, in place.
+      ht_wait(xbar_a, (unsigned)m & 1u);
+      if (lane < 16) {
+        const int ax = lane >> 3, ln = warp * 8 + (lane & 7), pl = ln >> 5, i0 = ln & 31;   // ax 0: q_2 line (plane, column); 1: q_3 line (plane, row)
+        double* B = ax ? g3 + pl * C::G3_PLANE + i0 * C::G3_LD : g2 + pl * C::G2_PLANE + i0;
+        const int st = ax ? 1 : C::NCOL;
+        const double ca = op.ca[1 + ax], cb = op.cb[1 + ax];
+        double Pm2 = 0.0, Pm1 = 0.0, P0 = B[0], P1 = B[st], prev = 0.0;
+#pragma unroll
+        for (int i = 0; i < 32; i++) {                              // one dependent FMA per point: everything else is off the chain
+          const double P2 = (i + 2 < 32) ? B[(i + 2) * st] : 0.0;
+          const double r = ca * (P1 - Pm1) + cb * (P2 - Pm2);
+          const double ib = tab[i];
+          prev = fma((-1.0 / 3.0) * ib, prev, r * ib);
+          B[i * st] = prev;                                         // P_i is not read again: the window holds P_{i-2} .. P_{i+2}
+          Pm2 = Pm1; Pm1 = P0; P0 = P1; P1 = P2;
+        }
+        double x = prev;
+#pragma unroll
+        for (int i = 30; i >= 0; i--) { x = fma(-tab[32 + i + 1], x, B[i * st]); B[i * st] = x; }
+      }
+      __syncwarp();
+      ht_arrive_if(xbar_a + 16, lane == 0);
+      ht_wait(xbar_a + 16, (unsigned)m & 1u);
+      const double f2 = -op.a2[1], f3 = -op.a2[2];
+#pragma unroll
+      for (int j = 0; j < NI; j++) {
+        const double2 d2 = *reinterpret_cast<const double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1)) * C::NCOL + 2 * cp);
+        const double* g = g3 + (j >> 1) * C::G3_PLANE + (r0 + 16 * (j & 1)) * C::G3_LD + 2 * cp;
+        acc[j].x = fma(f2, d2.x, fma(f3, g[0], acc[j].x));
+        acc[j].y = fma(f2, d2.y, fma(f3, g[1], acc[j].y));
+      }
+      __syncwarp();
+      ht_arrive_if(xbar_a + 8, lane == 0);
+    }
+    if (!CMP && have) {                                             // q_2 stencil of P_2
       ht_wait(xbar_a, (unsigned)m & 1u);
       const double w1 = -op.a2[1] * op.c1[1], w2 = -op.a2[1] * op.c2[1];
 #pragma unroll

@@ -352,6 +352,8 @@ MARCH = [
     ("six_planes_c2", dict(nq=[6, 32, 32], np=[2, 1, 3], depth=2, scheme="central2", mass=[1.0, 0.8, 1.2])),
     ("depth0_long", dict(nq=[70, 32, 32], np=[1, 2, 2], depth=0)),                # no hierarchy neighbours, 35 bands
     ("kp1", dict(nq=[8, 32, 32], np=[1, 1, 1], depth=3)),                         # no Hermite neighbours: couplings only
+    # COMPACT6: the march kernel solves the Pade derivative along q_2 and q_3 itself, a line pass adds the q_1 part
+    ("compact6", dict(nq=[8, 32, 32], np=[2, 2, 2], depth=2, scheme="compact6", mass=[1.0, 0.8, 1.2])),
 ]
 
 
@@ -363,7 +365,8 @@ def test_march_kernel_on_other_mesh_lengths(name, kw, monkeypatch):
     batch slots against the oracle; CHFPE_HERMITE_TMA=0 must give the patch kernel's result on the same input."""
     cfg = ci.config("cfg4h", **kw)
     g, o = both(cfg, batch=2)
-    assert g.stage_kernel() == "tma"
+    compact = cfg["scheme"] == "compact6"
+    assert g.stage_kernel() == ("compact" if compact else "tma")
     X = ci.seeded_hermite_state(cfg, [sum(n) for n in o.elems], seed=21)
     X = X + 0.05 * np.random.default_rng(3).uniform(-1.0, 1.0, size=X.shape)
     g.import_state(X); g.import_state(2.0 * X, replica=1); o.import_state(X)
@@ -376,9 +379,13 @@ def test_march_kernel_on_other_mesh_lengths(name, kw, monkeypatch):
     assert rel_l2(g.export_state(replica=1), 2.0 * Yo) < 1e-12
     monkeypatch.setenv("CHFPE_HERMITE_TMA", "0")
     p = P().Hermite(cfg)
-    assert p.stage_kernel() == "patch"
+    assert p.stage_kernel() == ("compact" if compact else "patch")
     p.import_state(X)
     assert rel_l2(p.export_rhs(), Fo) < 1e-13
+    n0 = p.launch_count(); p.step(1, cfg["dt"])
+    assert p.launch_count() - n0 == (16 if compact else 4)   # COMPACT6 without the march kernel: pointwise pass + three line passes
+    n0 = g.launch_count(); g.step(1, cfg["dt"])
+    assert g.launch_count() - n0 == (8 if compact else 4)    # with it: fused kernel + the q_1 line pass
     p.close(); g.close()
 
 
