@@ -10,7 +10,7 @@
 //   (n-e_s, k+e_s), (n+e_s, k-e_s) | y of the PREVIOUS band | three unused kinds (20 kinds = 4 x 5 slots).
 // A thread owns four pairs of q_3-adjacent points: both planes of the band on rows r and r + 16.  Per mode the ladder
 // combination P_s = sqrt(k_s+1) c_up + sqrt(k_s) c_dn is formed in registers; its derivative runs along q_3 on warp
-// shuffles (a row is 16 lanes), along q_2 through one zero-padded shared plane pair, and along q_1 in scatter form over
+// shuffles (a row is 16 lanes), along q_2 through one shared plane pair (ghost rows by predicate), and along q_1 in scatter form over
 // the march: P_1 of band m is added to the accumulators of bands m-1, m and m+1, which live in registers (the halo of
 // two planes is exactly one band), so band m-1 is finished, combined with y and written while band m is in flight.
 // No q_1 halo is ever loaded: 13 chunks per band on average against 16.5 slab-units per value in the patch kernel.
@@ -80,15 +80,48 @@ template <int N> struct HtUnroll<N, N> {
 };
 template <int E> using HtKind = std::integral_constant<int, E>;
 
+// One compact-derivative line of 32 points in shared memory, in place: point i holds P_i on entry and d_i on exit, where
+// tridiag(1/3, 1, 1/3) d = r, r_i = ca (P_{i+1} - P_{i-1}) + cb (P_{i+2} - P_{i-2}), zero ghosts.  tab: reciprocal pivots
+// [0, 32) and elimination factors [32, 64) (read-only after the kernel's setup: loaded through asm the compiler may hoist).
+// ST is a compile-time stride so that the window loads are provably distinct from the stores and leave the dependency chain,
+// which is one FMA per point in either sweep.
+__device__ __forceinline__ double ht_lds_const(unsigned addr) {
+  double v;
+  asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+  return v;
+}
+template <int ST, bool SWZ>
+__device__ __forceinline__ void ht_thomas32(double* __restrict__ B0, const int l, const unsigned tab_a, const double ca, const double cb) {
+  // point i of line l lives at B0[i * ST + (SWZ ? l ^ (i >> 1) : l)]
+  auto at = [&](int i) -> double& { return B0[i * ST + (SWZ ? (l ^ (i >> 1)) : l)]; };
+  double Pm2 = 0.0, Pm1 = 0.0, P0 = at(0), P1 = at(1), prev = 0.0;
+#pragma unroll
+  for (int i = 0; i < 32; i++) {
+    const double P2 = (i + 2 < 32) ? at(i + 2) : 0.0;
+    const double r = ca * (P1 - Pm1) + cb * (P2 - Pm2);
+    const double ib = ht_lds_const(tab_a + 8 * i);
+    prev = fma((-1.0 / 3.0) * ib, prev, r * ib);
+    at(i) = prev;                                                   // P_i is not read again: the window holds P_{i-2} .. P_{i+2}
+    Pm2 = Pm1; Pm1 = P0; P0 = P1; P1 = P2;
+  }
+  double x = prev;
+#pragma unroll
+  for (int i = 30; i >= 0; i--) { x = fma(-ht_lds_const(tab_a + 8 * (32 + i + 1)), x, at(i)); at(i) = x; }
+}
+
 // CMP = false: explicit stencils (CENTRAL4 / CENTRAL2).  CMP = true: COMPACT6, the Pade derivative along q_2 and q_3 is solved
 // inside the kernel (one Thomas solve per line of the band, 128 lines of 32 points: 16 lanes of every warp own one line each,
 // the recurrence of k_hermite_compact_line on shared memory); the q_1 lines run along the march and keep their own line pass.
 template <bool CMP> struct HtCfgT {
   static constexpr int NROW = 32, NCOL = 32, PLANE = NROW * NCOL, BAND = 2 * PLANE;   // two q_1 planes per band
   static constexpr unsigned CHUNK = BAND * sizeof(double);                            // 16 KB
-  static constexpr int SLOTS = CMP ? 4 : 5, NK = 20, NT = 256, NW = NT / 32, NI = 4;  // NI pairs per thread
-  static constexpr int G2_PLANE = (NROW + 4) * NCOL;                                  // P_2[plane][row + 2][col]
-  static constexpr int G3_LD = NCOL + 1, G3_PLANE = NROW * G3_LD;                     // CMP: P_3[plane][row][col], padded rows
+  // ring depth: 2 CTAs x (SLOTS x 16 KB + planes) must fit the SM's 228 KB; the kernel waits for data, so depth is speed
+  // (explicit scheme at cfg4h: 4 slots 3.92 ms, 5 slots 3.15 ms); NK = kinds per band, padded to a multiple of SLOTS
+  static constexpr int SLOTS = CMP ? 5 : 6, NK = CMP ? 20 : 18, NT = 256, NW = NT / 32, NI = 4;   // NI pairs per thread
+  static constexpr int G2_PLANE = NROW * NCOL;                                        // P_2[plane][row][col]
+  // CMP: P_3[plane][col][row ^ (col >> 1)]: transposed, so that the q_3 solve walks the same stride as the q_2 solve, and
+  // swizzled, so that both the solver (16 consecutive rows per warp) and the owners (16 pair columns of a row) are conflict-free
+  static constexpr int G3_PLANE = NROW * NCOL;
   static constexpr size_t SMEM = (size_t)SLOTS * CHUNK + sizeof(double) * 2 * (G2_PLANE + (CMP ? G3_PLANE : 0)) + 16 * SLOTS + 32 +
                                  8 * NK + (CMP ? 512 : 0) + 16;
 };
@@ -108,6 +141,7 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
   unsigned long long* xbar = empty + SLOTS;                         // [0]: P planes written, [1]: read, [2]: solved (CMP)
   const double** ent = reinterpret_cast<const double**>(xbar + 4);  // source of every kind at band 0
   double* tab = reinterpret_cast<double*>(ent + NK);                // CMP: reciprocal pivots [0, 32) and elimination factors [32, 64)
+  const unsigned tab_a = ht_smem_u32(tab);
   const unsigned ring_a = ht_smem_u32(ht_smem), full_a = ht_smem_u32(full), empty_a = ht_smem_u32(empty), xbar_a = ht_smem_u32(xbar);
 
   const int t = threadIdx.x, lane = t & 31, warp = __shfl_sync(0xffffffffu, t >> 5, 0);
@@ -160,10 +194,6 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
     ent[16] = (a != 0.0 ? y + soff : X) + (size_t)slab * Q - C::BAND;   // (band m - 1 at step m; a = 0: y is not to be read)
     const unsigned mk0 = step_mask(0);
     for (int e = 0; e < SLOTS; e++) issue(0, e, mk0);
-  }
-  for (int i = t; i < 2 * 4 * C::NCOL; i += C::NT) {                 // ghost rows -2, -1, 32, 33 of both P_2 planes stay zero
-    const int pl = i / (4 * C::NCOL), rr = i - pl * (4 * C::NCOL), row = rr / C::NCOL, col = rr - row * C::NCOL;
-    g2[pl * C::G2_PLANE + (row < 2 ? row : C::NROW + row) * C::NCOL + col] = 0.0;
   }
   __syncthreads();
 
@@ -254,8 +284,8 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
         if (have && s == 2) {
 #pragma unroll
           for (int j = 0; j < NI; j++) {
-            double* g = g3 + (j >> 1) * C::G3_PLANE + (r0 + 16 * (j & 1)) * C::G3_LD + 2 * cp;
-            g[0] = P[j].x; g[1] = P[j].y;
+            double* g = g3 + (j >> 1) * C::G3_PLANE + 2 * cp * C::NROW + ((r0 + 16 * (j & 1)) ^ cp);
+            g[0] = P[j].x; g[C::NROW] = P[j].y;
           }
           __syncwarp();
           ht_arrive_if(xbar_a, lane == 0);                          // this warp's P_2 and P_3 values are written
@@ -277,7 +307,7 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
           if (m > 0) ht_wait(xbar_a + 8, (unsigned)(m - 1) & 1u);   // the planes of the previous band have been read
 #pragma unroll
           for (int j = 0; j < NI; j++)
-            *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1) + 2) * C::NCOL + 2 * cp) = P[j];
+            *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1)) * C::NCOL + 2 * cp) = P[j];
         } else {                                                    // q_3: the 16 lanes of a row
 #pragma unroll
           for (int j = 0; j < NI; j++) {
@@ -295,7 +325,7 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
         if (m > 0) ht_wait(xbar_a + 8, (unsigned)(m - 1) & 1u);
 #pragma unroll
         for (int j = 0; j < NI; j++)
-          *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1) + 2) * C::NCOL + 2 * cp) = make_double2(0.0, 0.0);
+          *reinterpret_cast<double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1)) * C::NCOL + 2 * cp) = make_double2(0.0, 0.0);
       }
       if (!CMP && s == 1 && have) { __syncwarp(); ht_arrive_if(xbar_a, lane == 0); }     // this warp's P_2 values are written
     });
@@ -315,28 +345,13 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
       });
     });
     if (CMP && have) {
-      // 128 lines per band (2 planes x 32 columns along q_2, 2 planes x 32 rows along q_3), 16 per warp: lanes 0-7 take q_2 lines,
-      // lanes 8-15 q_3 lines.  T d = r, T = tridiag(1/3, 1, 1/3), r_i = ca (P_{i+1} - P_{i-1}) + cb (P_{i+2} - P_{i-2}) with zero
+      // 128 lines per band (2 planes x 32 columns along q_2, 2 planes x 32 rows along q_3), 16 per warp.  T d = r, T = tridiag(1/3, 1, 1/3), r_i = ca (P_{i+1} - P_{i-1}) + cb (P_{i+2} - P_{i-2}) with zero
       // ghosts (R9), by the Thomas recurrence with the host-tabulated reciprocal pivots of k_hermite_compact_line, in place.
       ht_wait(xbar_a, (unsigned)m & 1u);
-      if (lane < 16) {
-        const int ax = lane >> 3, ln = warp * 8 + (lane & 7), pl = ln >> 5, i0 = ln & 31;   // ax 0: q_2 line (plane, column); 1: q_3 line (plane, row)
-        double* B = ax ? g3 + pl * C::G3_PLANE + i0 * C::G3_LD : g2 + pl * C::G2_PLANE + i0;
-        const int st = ax ? 1 : C::NCOL;
-        const double ca = op.ca[1 + ax], cb = op.cb[1 + ax];
-        double Pm2 = 0.0, Pm1 = 0.0, P0 = B[0], P1 = B[st], prev = 0.0;
-#pragma unroll
-        for (int i = 0; i < 32; i++) {                              // one dependent FMA per point: everything else is off the chain
-          const double P2 = (i + 2 < 32) ? B[(i + 2) * st] : 0.0;
-          const double r = ca * (P1 - Pm1) + cb * (P2 - Pm2);
-          const double ib = tab[i];
-          prev = fma((-1.0 / 3.0) * ib, prev, r * ib);
-          B[i * st] = prev;                                         // P_i is not read again: the window holds P_{i-2} .. P_{i+2}
-          Pm2 = Pm1; Pm1 = P0; P0 = P1; P1 = P2;
-        }
-        double x = prev;
-#pragma unroll
-        for (int i = 30; i >= 0; i--) { x = fma(-tab[32 + i + 1], x, B[i * st]); B[i * st] = x; }
+      if (lane < 16) {                                              // warps 0-3: q_2 lines (plane, column); warps 4-7: q_3 lines (plane, row)
+        const int ln = (warp & 3) * 16 + lane, pl = ln >> 5, i0 = ln & 31;
+        if (warp < 4) ht_thomas32<C::NCOL, false>(g2 + pl * C::G2_PLANE, i0, tab_a, op.ca[1], op.cb[1]);
+        else ht_thomas32<C::NROW, true>(g3 + pl * C::G3_PLANE, i0, tab_a, op.ca[2], op.cb[2]);
       }
       __syncwarp();
       ht_arrive_if(xbar_a + 16, lane == 0);
@@ -345,9 +360,9 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
 #pragma unroll
       for (int j = 0; j < NI; j++) {
         const double2 d2 = *reinterpret_cast<const double2*>(g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1)) * C::NCOL + 2 * cp);
-        const double* g = g3 + (j >> 1) * C::G3_PLANE + (r0 + 16 * (j & 1)) * C::G3_LD + 2 * cp;
+        const double* g = g3 + (j >> 1) * C::G3_PLANE + 2 * cp * C::NROW + ((r0 + 16 * (j & 1)) ^ cp);
         acc[j].x = fma(f2, d2.x, fma(f3, g[0], acc[j].x));
-        acc[j].y = fma(f2, d2.y, fma(f3, g[1], acc[j].y));
+        acc[j].y = fma(f2, d2.y, fma(f3, g[C::NROW], acc[j].y));
       }
       __syncwarp();
       ht_arrive_if(xbar_a + 8, lane == 0);
@@ -357,9 +372,14 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
       const double w1 = -op.a2[1] * op.c1[1], w2 = -op.a2[1] * op.c2[1];
 #pragma unroll
       for (int j = 0; j < NI; j++) {
-        const double* g = g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1) + 2) * C::NCOL + 2 * cp;
-        const double2 u1 = *reinterpret_cast<const double2*>(g + C::NCOL), d1 = *reinterpret_cast<const double2*>(g - C::NCOL);
-        const double2 u2 = *reinterpret_cast<const double2*>(g + 2 * C::NCOL), d2 = *reinterpret_cast<const double2*>(g - 2 * C::NCOL);
+        // rows r0 (j even) and r0 + 16 (j odd): the lower neighbours of the first and the upper ones of the second may be ghosts
+        const double* g = g2 + (j >> 1) * C::G2_PLANE + (r0 + 16 * (j & 1)) * C::NCOL + 2 * cp;
+        const bool v1 = (j & 1) ? r0 <= 14 : r0 >= 1, v2 = (j & 1) ? r0 <= 13 : r0 >= 2;   // the +-1 / +-2 neighbour on the ghost side exists
+        const int o1 = (j & 1) ? C::NCOL : -C::NCOL;
+        const double2 z = make_double2(0.0, 0.0);
+        const double2 e1 = v1 ? *reinterpret_cast<const double2*>(g + o1) : z, e2 = v2 ? *reinterpret_cast<const double2*>(g + 2 * o1) : z;
+        const double2 i1 = *reinterpret_cast<const double2*>(g - o1), i2 = *reinterpret_cast<const double2*>(g - 2 * o1);
+        const double2 u1 = (j & 1) ? e1 : i1, d1 = (j & 1) ? i1 : e1, u2 = (j & 1) ? e2 : i2, d2 = (j & 1) ? i2 : e2;
         acc[j].x = fma(w1, u1.x - d1.x, fma(w2, u2.x - d2.x, acc[j].x));
         acc[j].y = fma(w1, u1.y - d1.y, fma(w2, u2.y - d2.y, acc[j].y));
       }
@@ -374,9 +394,7 @@ __global__ void __launch_bounds__(HtCfgT<CMP>::NT, 2) k_hermite_stage_tma(const 
         ht_st2(O + item_off(j) / 16, make_double2(fma(c, A[0][j].x, a * yv.x), fma(c, A[0][j].y, a * yv.y)), pol_str);
       }
     });
-    chunk(HtKind<17>(), [&](unsigned) {});
-    chunk(HtKind<18>(), [&](unsigned) {});
-    chunk(HtKind<19>(), [&](unsigned) {});
+    HtUnroll<17, NK>::run([&](auto KP) { chunk(KP, [&](unsigned) {}); });   // padding kinds: barriers only
 #pragma unroll
     for (int j = 0; j < NI; j++) { A[0][j] = A[1][j]; A[1][j] = A[2][j]; A[2][j] = make_double2(0.0, 0.0); }
     mask = maskn;
