@@ -520,6 +520,54 @@ __global__ void __launch_bounds__(128) k_hermite_compact_line(const HOp op, cons
   }
 }
 
+// The same line pass for lines of a compile-time length N along a non-contiguous axis: the forward values stay in
+// registers (the generic kernel keeps them in thread-local memory) and both sweeps are fully unrolled, so the loads
+// leave the recurrence.  Same arithmetic, same order.
+template <int N>
+__global__ void __launch_bounds__(128) k_hermite_compact_line_fixed(const HOp op, const int s, const double* __restrict__ in,
+                                                                   double* out, const double c, const size_t slot_stride) {
+  const int st = op.qst[s];
+  const int nlines = op.Q / N;
+  const int bps = (nlines + blockDim.x - 1) / blockDim.x;
+  const int slab = blockIdx.x / bps;
+  const int line = (blockIdx.x - slab * bps) * blockDim.x + threadIdx.x;
+  if (line >= nlines) return;
+  const HSlab* __restrict__ S = op.slabs + slab;
+  const int up = S->up[s], dn = S->dn[s];
+  if (up < 0 && dn < 0) return;
+  const int outer = line / st, inner = line - outer * st;
+  const size_t base = (size_t)outer * st * N + inner;
+  const size_t soff = (size_t)blockIdx.y * slot_stride, Q = (size_t)op.Q;
+  const double su = (up >= 0) ? S->su[s] : 0.0, sd = (dn >= 0) ? S->sd[s] : 0.0;
+  const double* __restrict__ pu = in + soff + (size_t)(up >= 0 ? up : slab) * Q + base;
+  const double* __restrict__ pd = in + soff + (size_t)(dn >= 0 ? dn : slab) * Q + base;
+  double* po = out + soff + (size_t)slab * Q + base;
+  const double* __restrict__ ibet = op.ibet[s];
+  const double* __restrict__ cfac = op.cfac[s];
+  const double ca = op.ca[s], cb = op.cb[s];
+  double fwd[N];
+  double Pm2 = 0.0, Pm1 = 0.0;
+  double P0 = su * __ldg(pu) + sd * __ldg(pd);
+  double P1 = su * __ldg(pu + st) + sd * __ldg(pd + st);
+  double prev = 0.0;
+#pragma unroll
+  for (int i = 0; i < N; i++) {
+    const double P2 = (i + 2 < N) ? su * __ldg(pu + (size_t)(i + 2) * st) + sd * __ldg(pd + (size_t)(i + 2) * st) : 0.0;
+    const double r = ca * (P1 - Pm1) + cb * (P2 - Pm2);
+    prev = (r - (1.0 / 3.0) * prev) * __ldg(ibet + i);
+    fwd[i] = prev;
+    Pm2 = Pm1; Pm1 = P0; P0 = P1; P1 = P2;
+  }
+  const double f = -c * op.a2[s];
+  double x = fwd[N - 1];
+  po[(size_t)(N - 1) * st] += f * x;
+#pragma unroll
+  for (int i = N - 2; i >= 0; i--) {
+    x = fwd[i] - __ldg(cfac + i + 1) * x;
+    po[(size_t)i * st] += f * x;
+  }
+}
+
 // The same line pass for the CONTIGUOUS q axis (s = M - 1, stride 1), where one thread per line would read 8 bytes per
 // 32-byte sector: a CTA of LPC threads owns LPC consecutive lines = one contiguous run of LPC * n doubles, loads the
 // runs of the two neighbour slabs coalesced and combines them to P in a padded shared tile (row stride n + 1: the
@@ -804,7 +852,8 @@ void stage(chfpe_hermite_handle* h, const double* in, const double* y, double* o
       k_hermite_stage_tma<true><<<dim3((unsigned)op.nslab, (unsigned)nb), HtCfgT<true>::NT, HtCfgT<true>::SMEM, h->stream>>>(op, in, y, out, a, c, ss);
       const int nlines = op.Q / op.nq[0];
       const dim3 g((unsigned)((size_t)op.nslab * ((nlines + 127) / 128)), (unsigned)nb);
-      k_hermite_compact_line<3><<<g, 128, 0, h->stream>>>(op, 0, in, out, c, ss);
+      if (op.nq[0] == 32) k_hermite_compact_line_fixed<32><<<g, 128, 0, h->stream>>>(op, 0, in, out, c, ss);
+      else k_hermite_compact_line<3><<<g, 128, 0, h->stream>>>(op, 0, in, out, c, ss);
       h->launches += 2;
       return;
     }

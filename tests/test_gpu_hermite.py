@@ -354,6 +354,7 @@ MARCH = [
     ("kp1", dict(nq=[8, 32, 32], np=[1, 1, 1], depth=3)),                         # no Hermite neighbours: couplings only
     # COMPACT6: the march kernel solves the Pade derivative along q_2 and q_3 itself, a line pass adds the q_1 part
     ("compact6", dict(nq=[8, 32, 32], np=[2, 2, 2], depth=2, scheme="compact6", mass=[1.0, 0.8, 1.2])),
+    ("compact6_cube32", dict(nq=[32, 32, 32], np=[2, 1, 2], depth=1, scheme="compact6")),   # q_1 pass with the line in registers
 ]
 
 
