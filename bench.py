@@ -617,8 +617,9 @@ def run_hermite(args):
     wl = args.workload if args.workload != "cfg4" else "cfg4h"
     cfg = ci.config(wl, scheme=args.scheme)
     M = cfg["n_modes"]
-    per_stage = 1 + M if args.scheme == "compact6" else 1   # COMPACT6: pointwise pass + one line pass per mode
     g = P.Hermite(cfg, batch=1)
+    # launches per RK stage: 1 (explicit stencils) | 2 (COMPACT6, march kernel + q_1 line pass) | 1 + M (COMPACT6 otherwise)
+    per_stage = {"compact": 1 + M, "compact_tma": 2}.get(g.stage_kernel(), 1)
     mu = obs(P, "mu", M)
     dt = cfg["dt"]
     steps, warm = args.steps, max(args.warmup, 3)
@@ -657,8 +658,7 @@ def run_hermite(args):
     values = g.values
     kern_ms = ms_stage / (4 * steps)                     # one RK stage (per_stage launches)
     achieved = values * 22.0 / (kern_ms * 1e-3) / 1e9
-    kname = g.stage_kernel_name() if per_stage == 1 else \
-        "RK stage = k_hermite_stage<DER=false> + %d x k_hermite_compact_line" % M
+    kname = g.stage_kernel_name()
     line = {"metric": "Hermite-representation value-updates/s (fp64)", "value": values * steps / (ms * 1e-3),
             "unit": "value-updates/s", "n_gpus": 1, "steps": steps, "warmup": warm, "ms_per_step": ms / steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",

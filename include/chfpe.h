@@ -254,9 +254,10 @@ int chfpe_hermite_export_rhs(chfpe_hermite_handle* h, int32_t replica, double* d
 int chfpe_hermite_launch_count(const chfpe_hermite_handle* h, int64_t* n);
 /* Which kernel family runs the RK stage on this handle (benchmark records and tests; the results do not depend on it):
    per-value kernel | column kernel (one mode) | patch kernel | COMPACT6 pointwise + line passes | bulk-copy march kernel
-   (three modes on an n_1 x 32 x 32 mesh with n_1 even, explicit stencils: the default there). */
+   (three modes on an n_1 x 32 x 32 mesh with n_1 even: the default there, for the explicit stencils and for COMPACT6). */
 enum { CHFPE_HERMITE_STAGE_VALUE = 0, CHFPE_HERMITE_STAGE_COLUMN = 1, CHFPE_HERMITE_STAGE_PATCH = 2,
-       CHFPE_HERMITE_STAGE_COMPACT = 3, CHFPE_HERMITE_STAGE_TMA = 4 };
+       CHFPE_HERMITE_STAGE_COMPACT = 3, CHFPE_HERMITE_STAGE_TMA = 4,
+       CHFPE_HERMITE_STAGE_COMPACT_TMA = 5 };   /* COMPACT6 on such a mesh: march kernel with the q_2, q_3 line solves inside + q_1 line pass */
 int chfpe_hermite_stage_kernel(const chfpe_hermite_handle* h, int32_t* kind);
 const char* chfpe_hermite_last_error(const chfpe_hermite_handle* h);   /* h may be NULL: last create-time error */
 
@@ -290,8 +291,9 @@ const char* chfpe_hermite_last_error(const chfpe_hermite_handle* h);   /* h may 
        CHFPE_HERMITE_FIXED=0, CHFPE_HERMITE_TILE=0, CHFPE_HERMITE_PCOL=0   32^3 specialisation / CTA tile remap / column
                               walk off
        CHFPE_HERMITE_CONTIG=0 strided instead of transposing COMPACT6 line kernel on the contiguous axis
-       CHFPE_HERMITE_TMA=0    patch kernel instead of the bulk-copy march kernel (n_1 x 32 x 32 meshes of three modes;
-                              an explicit CHFPE_HERMITE_KC / CHFPE_HERMITE_PATCH request also turns it off)
+       CHFPE_HERMITE_TMA=0    patch kernel (COMPACT6: pointwise pass + three line passes) instead of the bulk-copy march
+                              kernel (n_1 x 32 x 32 meshes of three modes; an explicit CHFPE_HERMITE_KC / CHFPE_HERMITE_PATCH
+                              request also turns it off)
    --------------------------------------------------------------------------------------------------------------- */
 
 #ifdef __cplusplus

@@ -517,15 +517,17 @@ class Hermite:
         return n.value
 
     def stage_kernel(self):
-        """'value' | 'column' | 'patch' | 'compact' | 'tma': the kernel family that runs the RK stage on this handle."""
+        """'value' | 'column' | 'patch' | 'compact' | 'tma' | 'compact_tma': the kernel family that runs the RK stage."""
         k = C.c_int32()
         self._ck(lib().chfpe_hermite_stage_kernel(self._h, C.byref(k)), "chfpe_hermite_stage_kernel")
-        return ("value", "column", "patch", "compact", "tma")[k.value]
+        return ("value", "column", "patch", "compact", "tma", "compact_tma")[k.value]
 
     def stage_kernel_name(self):
         """Name of the CUDA kernel family behind stage_kernel() (for benchmark records)."""
         return {"value": "k_hermite_stage", "column": "k_hermite_stage_col", "patch": "k_hermite_stage_patch",
-                "compact": "k_hermite_stage<DER=false> + k_hermite_compact_line", "tma": "k_hermite_stage_tma"}[self.stage_kernel()]
+                "compact": "RK stage = k_hermite_stage<DER=false> + one k_hermite_compact_line per mode",
+                "tma": "k_hermite_stage_tma<CMP=false>",
+                "compact_tma": "RK stage = k_hermite_stage_tma<CMP=true> (q_2, q_3 solves inside) + k_hermite_compact_line (q_1)"}[self.stage_kernel()]
 
 
 def _dev(a):

@@ -1217,7 +1217,7 @@ extern "C" int chfpe_hermite_launch_count(const chfpe_hermite_handle* h, int64_t
 extern "C" int chfpe_hermite_stage_kernel(const chfpe_hermite_handle* h, int32_t* kind) {
   if (!h || !kind) return CHFPE_ERR_INVALID;
   const HOp& op = h->op;
-  *kind = (op.scheme == CHFPE_COMPACT6) ? CHFPE_HERMITE_STAGE_COMPACT
+  *kind = (op.scheme == CHFPE_COMPACT6) ? (op.tma ? CHFPE_HERMITE_STAGE_COMPACT_TMA : CHFPE_HERMITE_STAGE_COMPACT)
           : op.tma                      ? CHFPE_HERMITE_STAGE_TMA
           : (op.pa > 0)                 ? CHFPE_HERMITE_STAGE_PATCH
           : (op.kc > 0)                 ? CHFPE_HERMITE_STAGE_COLUMN

@@ -367,7 +367,7 @@ def test_march_kernel_on_other_mesh_lengths(name, kw, monkeypatch):
     cfg = ci.config("cfg4h", **kw)
     g, o = both(cfg, batch=2)
     compact = cfg["scheme"] == "compact6"
-    assert g.stage_kernel() == ("compact" if compact else "tma")
+    assert g.stage_kernel() == ("compact_tma" if compact else "tma")
     X = ci.seeded_hermite_state(cfg, [sum(n) for n in o.elems], seed=21)
     X = X + 0.05 * np.random.default_rng(3).uniform(-1.0, 1.0, size=X.shape)
     g.import_state(X); g.import_state(2.0 * X, replica=1); o.import_state(X)
