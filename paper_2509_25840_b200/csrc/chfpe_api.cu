@@ -157,7 +157,7 @@ static BrickPlan make_brick_plan(const chfpe_desc* d, const Plan& pl, const std:
   // bulk-copy fed kernel (chfpe_tma.cu): CENTRAL4, three modes, bricks cut into tma_npart parts along p_1
   bp.tma_npart = env_int("CHFPE_TMA_NPART", bp.P1 >= 12 ? 2 : 1);   // (the halo planes of a part must fit one slot)
   bp.tma_nseg = env_int("CHFPE_TMA_NSEG", bp.P1 == 8 ? 2 : (bp.tma_npart == 1 ? 4 : (bp.P1 == 12 ? 3 : 2)));
-  bp.tma_slots = env_int("CHFPE_TMA_SLOTS", bp.P1 >= 20 ? 4 : 5);      // (20^3: 32 KB chunks, four fit beside the exchange planes)
+  bp.tma_slots = env_int("CHFPE_TMA_SLOTS", 5);                        // (20^3: 32 KB chunks, five fit beside the exchange planes: 216 KB)
   bp.tma_ring = env_int("CHFPE_TMA_RING", 1);
   bp.tma = (M == 3 && d->scheme == CHFPE_CENTRAL4 && vnq[2] <= 64 && env_int("CHFPE_TMA", 1))   // (q_3 lines of <= 64 bricks: TmaCfg::MAXQ3)
                ? tma_has_fixed(M, bp.P1, bp.P2, bp.P3, bp.tma_npart, bp.tma_nseg, bp.tma_slots, bp.tma_ring) : 0;

@@ -142,7 +142,10 @@ struct TmaCfg {
   static constexpr unsigned CHUNK = PP * PLANE * (unsigned)sizeof(double);
   static constexpr bool SHFL3 = tma_shfl3(P2, P3);
   static constexpr int G2_ROW = P3, G2_PLANE = (P2 == 1) ? 0 : (P2 + 4) * P3;       // G_2[plane][i2+2][i3]
-  static constexpr int G3_ROW = P3 + 4, G3_PLANE = SHFL3 ? 0 : P2 * (P3 + 4);       // G_3[plane][i2][i3+2]
+  // p_3 stencil: neighbour lanes (a thread owns a pair of p_3-adjacent cells).  SHFL3: the rows of P3/2 pairs tile a warp.
+  // Otherwise a row may cross a warp boundary: lane 0 / 31 of every warp leave their G_3 pairs in a small edge buffer and
+  // the thread on the other side adds the missing terms after the exchange barrier (the stencil is linear).
+  static constexpr int EB = SHFL3 ? 0 : NW * 2 * NC * 2;                            // doubles: G_3 pair [warp][side][plane]
   static constexpr int XG = (NSEG > 1) ? (NSEG - 1) * 4 * PLANE : 0;                // G_1 planes next to a segment edge
   static_assert(NPART <= 2, "a part has at most one edge inside the brick (the halo planes share one ring slot)");
   // Chunk kinds of one step (= one brick of the line), consumed in this order; kind e always uses ring slot e % SLOTS,
@@ -157,7 +160,7 @@ struct TmaCfg {
   static_assert(3 * 2 * PLANE <= PP * PLANE, "halo pieces must fit a slot");
   static_assert(NK % SLOTS == 0, "the slot of a kind must not depend on the step");
   static constexpr int MAXQ3 = 64;                                 // longest q_3 line (dU/dq_s table of the line)
-  static constexpr size_t SMEM = (size_t)SLOTS * CHUNK + sizeof(double) * (PP * G2_PLANE + PP * G3_PLANE + XG) +
+  static constexpr size_t SMEM = (size_t)SLOTS * CHUNK + sizeof(double) * (PP * G2_PLANE + EB + XG) +
                                  16 * SLOTS + 16 + 8 * NK + 8 * 3 * MAXQ3 + 16;
   static constexpr int MINB = (2 * (SMEM + 1024) <= 227 * 1024 && 2 * NT <= 1024) ? 2 : 1;
 };
@@ -185,8 +188,8 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char* ring = smem_raw;
   double* g2 = reinterpret_cast<double*>(smem_raw + (size_t)SLOTS * C::CHUNK);
-  double* g3 = g2 + PP * C::G2_PLANE;
-  double* xg = g3 + PP * C::G3_PLANE;
+  double* eb = g2 + PP * C::G2_PLANE;
+  double* xg = eb + C::EB;
   unsigned long long* full = reinterpret_cast<unsigned long long*>(xg + C::XG);       // data of a slot has landed
   unsigned long long* empty = full + SLOTS;                                           // all warps have released a slot
   unsigned long long* xbar = empty + SLOTS;                                           // exchange planes: [0] written, [1] read
@@ -292,10 +295,6 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
   for (int i = t; i < (SKIP1 ? 0 : PP * 4 * P3); i += C::NT) {
     const int pl = i / (4 * P3), rr = i - pl * (4 * P3), row = rr / P3, col = rr - row * P3;
     g2[pl * C::G2_PLANE + (row < 2 ? row : P2 + row) * C::G2_ROW + col] = 0.0;
-  }
-  for (int i = t; i < (C::SHFL3 ? 0 : PP * P2 * 4); i += C::NT) {
-    const int rw = i >> 2, c4 = i & 3;
-    g3[rw * C::G3_ROW + (c4 < 2 ? c4 : P3 + c4)] = 0.0;
   }
   __syncthreads();
 
@@ -480,25 +479,24 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
           for (int j = 0; j < NC; j++)
             *reinterpret_cast<double2*>(g2 + (jbase + j) * C::G2_PLANE + (i2 + 2) * C::G2_ROW + i3) = g[j];
         }
-      } else if (C::SHFL3) {                                        // D_{p_3} G_3 from the neighbour lanes of the row
-        constexpr int W = P3 / 2;
+      } else {                                                      // D_{p_3} G_3 from the neighbour lanes of the row
+        constexpr int W = P3 / 2, SW = C::SHFL3 ? W : 32;
         const int c = tid % W;
+        const bool nol = c == 0 || (!C::SHFL3 && lane == 0), nor = c == W - 1 || (!C::SHFL3 && lane == 31);
 #pragma unroll
         for (int j = 0; j < NC; j++) {
           const double2 own = g[j];
-          double ly = __shfl_up_sync(0xffffffffu, own.y, 1, W), rx = __shfl_down_sync(0xffffffffu, own.x, 1, W);
-          double lx = __shfl_up_sync(0xffffffffu, own.x, 1, W), ry = __shfl_down_sync(0xffffffffu, own.y, 1, W);
-          if (c == 0) { ly = 0.0; lx = 0.0; }
-          if (c == W - 1) { rx = 0.0; ry = 0.0; }
+          double ly = __shfl_up_sync(0xffffffffu, own.y, 1, SW), rx = __shfl_down_sync(0xffffffffu, own.x, 1, SW);
+          double lx = __shfl_up_sync(0xffffffffu, own.x, 1, SW), ry = __shfl_down_sync(0xffffffffu, own.y, 1, SW);
+          if (nol) { ly = 0.0; lx = 0.0; }
+          if (nor) { rx = 0.0; ry = 0.0; }
           const double e3x = fma(8.0, own.y - ly, -(rx - lx));
           const double e3y = fma(8.0, rx - own.x, -(ry - ly));
           acc[j].x = fma(w3p, e3x, acc[j].x);
           acc[j].y = fma(w3p, e3y, acc[j].y);
+          if (!C::SHFL3 && active && (lane == 0 || lane == 31))     // for the neighbour in the next / previous warp
+            *reinterpret_cast<double2*>(eb + ((warp * 2 + (lane == 31)) * NC + j) * 2) = own;
         }
-      } else if (active) {
-#pragma unroll
-        for (int j = 0; j < NC; j++)
-          *reinterpret_cast<double2*>(g3 + (jbase + j) * C::G3_PLANE + i2 * C::G3_ROW + i3 + 2) = g[j];
       }
     }
     __syncwarp();
@@ -540,7 +538,6 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
     }
     {
       const double* c2 = g2 + jbase * C::G2_PLANE + (i2 + 2) * C::G2_ROW + i3;
-      const double* c3p = g3 + jbase * C::G3_PLANE + i2 * C::G3_ROW + i3 + 2;
 #pragma unroll
       for (int j = 0; j < NC; j++) {
         if (!SKIP1) {
@@ -550,13 +547,25 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
           acc[j].x = fma(w2p, fma(8.0, u1.x - d1.x, -(u2.x - d2.x)), acc[j].x);
           acc[j].y = fma(w2p, fma(8.0, u1.y - d1.y, -(u2.y - d2.y)), acc[j].y);
         }
-        if (!C::SHFL3) {
-          const double* a3 = c3p + j * C::G3_PLANE;
-          const double2 lft = *reinterpret_cast<const double2*>(a3 - 2), rgt = *reinterpret_cast<const double2*>(a3 + 2);
-          const double2 own = *reinterpret_cast<const double2*>(a3);
-          // pair (i3, i3+1): neighbours i3-2..i3+3 = lft.x lft.y [own.x own.y] rgt.x rgt.y
-          acc[j].x = fma(w3p, fma(8.0, own.y - lft.y, -(rgt.x - lft.x)), acc[j].x);
-          acc[j].y = fma(w3p, fma(8.0, rgt.x - own.x, -(rgt.y - lft.y)), acc[j].y);
+      }
+      if (!C::SHFL3 && active) {                                    // the row continues in the previous / next warp
+        constexpr int W = P3 / 2;
+        const int c = tid % W;
+        if (lane == 0 && c != 0) {                                  // pair (i3-2, i3-1): -8 ly + lx on x, + ly on y
+#pragma unroll
+          for (int j = 0; j < NC; j++) {
+            const double2 l = *reinterpret_cast<const double2*>(eb + (((warp - 1) * 2 + 1) * NC + j) * 2);
+            acc[j].x = fma(w3p, fma(-8.0, l.y, l.x), acc[j].x);
+            acc[j].y = fma(w3p, l.y, acc[j].y);
+          }
+        }
+        if (lane == 31 && c != W - 1) {                             // pair (i3+2, i3+3): - rx on x, 8 rx - ry on y
+#pragma unroll
+          for (int j = 0; j < NC; j++) {
+            const double2 r = *reinterpret_cast<const double2*>(eb + (((warp + 1) * 2 + 0) * NC + j) * 2);
+            acc[j].x = fma(w3p, -r.x, acc[j].x);
+            acc[j].y = fma(w3p, fma(8.0, r.x, -r.y), acc[j].y);
+          }
         }
       }
     }
@@ -587,7 +596,7 @@ k_stage_tma(DevOp op, BrickPlan bp, const double* __restrict__ in, const double*
 #define TMA_SPECIALISATIONS(X) \
   X(16, 16, 16, 2, 2, 5, true) X(16, 16, 16, 2, 2, 4, true) X(16, 16, 16, 2, 2, 4, false) X(16, 16, 16, 1, 4, 5, true) X(16, 16, 16, 1, 4, 4, true) \
   X(8, 8, 8, 1, 2, 5, true) X(8, 8, 8, 1, 2, 4, true) X(8, 8, 8, 1, 2, 4, false) X(12, 12, 12, 2, 3, 5, true) X(12, 12, 12, 2, 3, 4, true) \
-  X(20, 20, 20, 2, 2, 4, true) X(20, 20, 20, 2, 2, 4, false)
+  X(20, 20, 20, 2, 2, 5, true) X(20, 20, 20, 2, 2, 4, true) X(20, 20, 20, 2, 2, 4, false)
 
 int tma_has_fixed(int M, int P1, int P2, int P3, int npart, int nseg, int slots, int ring) {
   if (M != 3) return 0;
