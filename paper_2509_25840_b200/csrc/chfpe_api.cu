@@ -262,6 +262,7 @@ extern "C" int chfpe_create(const chfpe_desc* desc, void* ws, size_t bytes, void
   memset(&op, 0, sizeof(op));
   op.M = M; op.nax = 2 * M; op.K = pl.K; op.scheme = desc->scheme; op.gauge = desc->gauge; op.beta = desc->beta;
   op.closure = desc->closure; op.depth = desc->depth;
+  op.expect_pbrick = env_int("CHFPE_EXPECT_PBRICK", 1);
   for (int s = 0; s < M; s++) {
     op.n[s] = desc->nq[s]; op.n[M + s] = desc->np[s];
     op.x0[s] = desc->qmin[s]; op.x0[M + s] = desc->pmin[s];

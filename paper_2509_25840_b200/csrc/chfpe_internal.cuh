@@ -15,6 +15,7 @@
 struct DevOp {
   int M, nax, K, scheme, gauge;
   int closure, depth;                 // CHFPE_CLOSURE_*; N (elements with sum n = N are the top level)
+  int expect_pbrick;                  // expectation values by k_expect_pbrick (CHFPE_EXPECT_PBRICK=0: generic reduction)
   int n[CHFPE_MAXAX];                 // points per internal axis
   long long st[CHFPE_MAXAX];          // internal strides (doubles)
   long long cells, nqc, pb;           // cells per element, q-points, p-brick size

@@ -372,6 +372,64 @@ __global__ void __launch_bounds__(256) k_reduce_partial(DevOp op, DevObs ob, int
   if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = r;
 }
 
+// <O> on the p-brick layout (RED_EXPECT only; p-bricks of up to EXPECT_MAXPB cells).  The observable of Eq. (13)-(14) is
+// O(q, p) = A(q) + sum_s lin_p[s] p_s and the gauge weight factorises as eU(q) * prod_s ep_s(p_s), so a CTA tabulates the
+// momentum factors of one brick once in shared memory -- wp[c] = prod_s ep_s, lp[c] = sum_s lin_p[s] p_s -- and then
+// streams its contiguous run of bricks: per cell one coalesced load, two shared loads and two FMAs instead of a full
+// index decode (six divisions) and four table loads.  Summation order: fixed by (nqc, gridDim.x, 256) alone.
+constexpr int EXPECT_MAXPB = 8192;
+template <int M>
+__global__ void __launch_bounds__(256) k_expect_pbrick(DevOp op, DevObs ob, const double* __restrict__ x, long long elem_off,
+                                                       size_t slot_stride, double* __restrict__ partial) {
+  extern __shared__ double ex_tab[];                  // wp[pb], lp[pb]
+  const int pb = (int)op.pb;
+  double* wp = ex_tab;
+  double* lp = ex_tab + pb;
+  for (int c = threadIdx.x; c < pb; c += 256) {
+    unsigned r = (unsigned)c;
+    double w = 1.0, l = 0.0;
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) {
+      const unsigned q = r / (unsigned)op.n[M + s];
+      const int i = (int)(r - q * (unsigned)op.n[M + s]);
+      r = q;
+      l = fma(ob.lin_p[s], op.x0[M + s] + i * op.h[M + s], l);
+      if (op.gauge == CHFPE_GAUGE_SQRT_EQ) w *= __ldg(op.ep[s] + i);
+    }
+    wp[c] = w; lp[c] = l;
+  }
+  __syncthreads();
+  const double* X = x + (size_t)blockIdx.y * slot_stride + elem_off;
+  const long long per = (op.nqc + gridDim.x - 1) / gridDim.x;
+  const long long lo = (long long)blockIdx.x * per;
+  long long hi = lo + per; if (hi > op.nqc) hi = op.nqc;
+  double acc = 0.0;
+  for (long long qi = lo; qi < hi; qi++) {
+    unsigned r = (unsigned)qi;
+    double q[M];
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) {
+      const unsigned d = r / (unsigned)op.n[s];
+      q[s] = op.x0[s] + (int)(r - d * (unsigned)op.n[s]) * op.h[s];
+      r = d;
+    }
+    double A = ob.c0;
+#pragma unroll
+    for (int s = 0; s < M; s++) {
+      A = fma(ob.lin_q[s], q[s], A);
+#pragma unroll
+      for (int t = 0; t < M; t++) A = fma(0.5 * ob.quad[s][t] * q[s], q[t], A);
+    }
+    const double e = (op.gauge == CHFPE_GAUGE_SQRT_EQ) ? __ldg(op.eU + qi) : 1.0;
+    const double* B = X + qi * pb;
+    double a = 0.0;
+    for (int c = threadIdx.x; c < pb; c += 256) a = fma((A + lp[c]) * wp[c], B[c], a);
+    acc = fma(e, a, acc);
+  }
+  const double r = block_sum_256(acc);
+  if (threadIdx.x == 0) partial[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = r;
+}
+
 __global__ void __launch_bounds__(256) k_reduce_final(const double* __restrict__ partial, int nblocks, double scale,
                                                       double* __restrict__ results, long long res_stride) {
   const double* P = partial + (size_t)blockIdx.x * nblocks;
@@ -539,6 +597,25 @@ int launch_reduce(const DevOp& op, const DevObs& o, int mode, const double* x, i
                   long long res_stride, cudaStream_t s) {
   dim3 grid(red_blocks, nb);
   const long long off = (long long)k * op.cells;
+  if (mode == RED_EXPECT && ncells == op.cells && op.pb <= EXPECT_MAXPB && op.pb >= 256 && op.expect_pbrick) {
+    const size_t sm = 2 * sizeof(double) * (size_t)op.pb;
+    cudaError_t e = cudaSuccess;
+    if (sm > 48 * 1024) {
+      switch (op.M) {
+        case 1: e = cudaFuncSetAttribute(k_expect_pbrick<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); break;
+        case 2: e = cudaFuncSetAttribute(k_expect_pbrick<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); break;
+        default: e = cudaFuncSetAttribute(k_expect_pbrick<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm); break;
+      }
+    }
+    if (e == cudaSuccess) {
+#define CALL(MM) k_expect_pbrick<MM><<<grid, 256, sm, s>>>(op, o, x, off, slot_stride, partial)
+      DISPATCH_M(op.M, CALL);
+#undef CALL
+      k_reduce_final<<<nb, 256, 0, s>>>(partial, red_blocks, scale, results, res_stride);
+      return 2;
+    }
+    cudaGetLastError();
+  }
 #define CALL(MM) k_reduce_partial<MM><<<grid, 256, 0, s>>>(op, o, mode, x, off, ncells, slot_stride, partial)
   DISPATCH_M(op.M, CALL);
 #undef CALL

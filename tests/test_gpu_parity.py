@@ -212,6 +212,31 @@ FAMILY_ENVS = [
 ]
 
 
+@pytest.mark.parametrize("name", ["m2_48_brick_w", "m3_cube12", "m3_cube20_c2"])
+def test_expectation_kernels_agree(name, monkeypatch):
+    """k_expect_pbrick (momentum factors of the observable and of the gauge weight tabulated per brick in shared memory; the
+    default for p-bricks of 256 ... 8192 cells) against the generic reduction (CHFPE_EXPECT_PBRICK=0) and the oracle, on
+    element 0 and on the last element, both gauges, two batch slots, general observable incl. the momentum part."""
+    cfg = dict(SMALL)[name]
+    M = cfg["n_modes"]
+    gen = dict(c0=-0.2, lin_q=[0.7, -0.4, 0.2][:M], quad=[[0.5, 0.2, -0.1][:M], [0.1, -0.3, 0.25][:M], [0.05, 0.15, 0.4][:M]][:M],
+               lin_p=[0.3, -0.2, 0.1][:M])
+    og, oo = make_obs(gpu_mod(), gen), make_obs(oracle, gen)
+    g, o = both(cfg, batch=2)
+    X = ci.seeded_state(cfg, [sum(n) for n in o.elements()], seed=6)
+    g.import_state(X); g.import_state(-3.0 * X, replica=1); o.import_state(X)
+    ref0, refK = o.expect(oo), o.expect(oo, element=o.K - 1)
+    monkeypatch.setenv("CHFPE_EXPECT_PBRICK", "0")
+    g0 = gpu_mod().CHFPE(cfg, batch=2)
+    g0.import_state(X); g0.import_state(-3.0 * X, replica=1)
+    for h in (g, g0):
+        e = h.expect(og)
+        assert abs(e[0] - ref0) <= 1e-12 * max(1.0, abs(ref0)) and abs(e[1] + 3.0 * ref0) <= 3e-12 * max(1.0, abs(ref0))
+        assert abs(h.expect_element(og, o.K - 1) - refK) <= 1e-12 * max(1.0, abs(ref0))
+    assert abs(g.expect(og)[0] - g0.expect(og)[0]) <= 1e-13 * max(1.0, abs(ref0))
+    g.close(); g0.close()
+
+
 @pytest.mark.parametrize("env,family", FAMILY_ENVS, ids=["-".join("%s%s" % (k[6:], v) for k, v in e.items()) or "default"
                                                          for e, _ in FAMILY_ENVS])
 def test_stage_kernel_families(monkeypatch, env, family):
