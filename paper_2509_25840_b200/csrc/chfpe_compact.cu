@@ -231,12 +231,15 @@ __global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double
 // with the pointwise gauge terms and the damping: one read of X_k, X_up, X_dn and one read-modify-write of `out` per
 // stage instead of one such pass per momentum axis.  The K elements of a q-point run in consecutive CTAs, so the bricks
 // of hierarchy neighbours are served by L2.  CPT cells per thread: pb <= CPT * blockDim.x.
-template <int M, int PBRICK_CPT>
+// NP > 0: cubic bricks of NP points per momentum axis with NP^M = CPT * 512 cells known at compile time (every index
+// decode, stride and loop bound becomes a constant); NP = 0: run-time brick shape.
+__host__ __device__ constexpr int pbrick_ipow(int b, int e) { return e <= 0 ? 1 : b * pbrick_ipow(b, e - 1); }
+template <int M, int PBRICK_CPT, int NP>
 __global__ void __launch_bounds__(512, (PBRICK_CPT == 8) ? 2 : 1) k_compact_pbrick(DevOp op, CompactTables ct, const double* __restrict__ in,
                                                          double* out, double c, size_t slot_stride) {
   extern __shared__ double ptile_s[];
-  const int NT = blockDim.x, t = threadIdx.x;
-  const int pb = (int)op.pb, nl = op.n[2 * M - 1];
+  const int NT = NP ? 512 : blockDim.x, t = threadIdx.x;
+  const int pb = NP ? pbrick_ipow(NP, M) : (int)op.pb, nl = NP ? NP : op.n[2 * M - 1];
   double* tile = ptile_s;                                           // G_s
   double* rt = ptile_s + (pb + pb / nl);                            // B G_s / h, then d = A^{-1} B G_s
   const long long ql = blockIdx.x / op.K;
@@ -259,13 +262,13 @@ __global__ void __launch_bounds__(512, (PBRICK_CPT == 8) ? 2 : 1) k_compact_pbri
     pcs[j] = cell + cell / nl;
     int r = cell, pk = 0;
 #pragma unroll
-    for (int s = M - 1; s >= 0; s--) { const int n = op.n[M + s]; const int q = r / n; pk |= (r - q * n) << (10 * s); r = q; }
+    for (int s = M - 1; s >= 0; s--) { const int n = NP ? NP : op.n[M + s]; const int q = r / n; pk |= (r - q * n) << (10 * s); r = q; }
     pidx[j] = pk;
   }
   const double al = 1.0 / 3.0, ca = 7.0 / 9.0, cb = 1.0 / 36.0;
 #pragma unroll
   for (int s = 0; s < M; s++) {
-    const int ap = M + s, n = op.n[ap], stb = (int)op.st[ap];       // stride of p_s inside the brick
+    const int ap = M + s, n = NP ? NP : op.n[ap], stb = NP ? pbrick_ipow(NP, M - 1 - s) : (int)op.st[ap];   // stride of p_s inside the brick
     const double q = op.x0[s] + iq[s] * op.h[s];
     const double Vp = fma(op.VSL[s], q, op.VLL[s]);
     const double ck = __ldg(op.dU[s] + ql);
@@ -310,13 +313,13 @@ __global__ void __launch_bounds__(512, (PBRICK_CPT == 8) ? 2 : 1) k_compact_pbri
         double* row = rt + base + base / nl;
         double prev = row[0] * __ldg(ibet);
         row[0] = prev;
-#pragma unroll 4
+#pragma unroll(NP ? NP : 4)
         for (int i = 1; i < n; i++) {                               // forward elimination: r'_i = (r_i - r'_{i-1}/3) / bet_i
           const double ib = __ldg(ibet + i);
           prev = fma(-al * ib, prev, row[i * pitch] * ib);
           row[i * pitch] = prev;
         }
-#pragma unroll 4
+#pragma unroll(NP ? NP : 4)
         for (int i = n - 2; i >= 0; i--) {                          // back substitution
           prev = fma(-__ldg(cfac + i + 1), prev, row[i * pitch]);
           row[i * pitch] = prev;
@@ -416,17 +419,21 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
     if (nt < 64) nt = 64;
     static bool optin = false;
     if (!optin) {
-      cudaFuncSetAttribute(k_compact_pbrick<2, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-      cudaFuncSetAttribute(k_compact_pbrick<2, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-      cudaFuncSetAttribute(k_compact_pbrick<3, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-      cudaFuncSetAttribute(k_compact_pbrick<3, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<2, 8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<2, 16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<3, 8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<3, 16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<3, 8, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
       optin = true;
     }
     const dim3 grid((unsigned)(op.nqc * op.K), 1, nb);                // element fastest: hierarchy neighbours meet in L2
-    if (op.M == 2 && cpt == 8) k_compact_pbrick<2, 8><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
-    else if (op.M == 2) k_compact_pbrick<2, 16><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
-    else if (cpt == 8) k_compact_pbrick<3, 8><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
-    else k_compact_pbrick<3, 16><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    static const bool cube_on = []() { const char* e = getenv("CHFPE_COMPACT_CUBE"); return !(e && e[0] == '0'); }();
+    const bool cube16 = cube_on && op.M == 3 && op.n[3] == 16 && op.n[4] == 16 && op.n[5] == 16 && nt == 512;
+    if (op.M == 2 && cpt == 8) k_compact_pbrick<2, 8, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else if (op.M == 2) k_compact_pbrick<2, 16, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else if (cube16) k_compact_pbrick<3, 8, 16><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else if (cpt == 8) k_compact_pbrick<3, 8, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else k_compact_pbrick<3, 16, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
     launches++;
   }
   return launches;

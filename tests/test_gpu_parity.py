@@ -596,6 +596,8 @@ COMPACT = [
     # 24 and 32 points on the contiguous axis: the transposing kernel needs > 48 KB of dynamic shared memory
     ("m1_t32", ci.config("cfg2", nq=[32], np=[32], depth=3, scheme="compact6")),
     ("m2_t24", ci.config("cfg3s", nq=[8, 8], np=[8, 24], depth=2, scheme="compact6")),
+    # 16^3 bricks (config 4's): the compile-time-shaped brick pass k_compact_pbrick<3, 8, 16>
+    ("m3_cube16", ci.config("cfg4", nq=[5, 6, 5], depth=2, scheme="compact6", mass=[1.0, 0.8, 1.2])),
 ]
 
 
