@@ -234,11 +234,14 @@ __global__ void __launch_bounds__(128) k_compact_pline_s1(DevOp op, const double
 // NP > 0: cubic bricks of NP points per momentum axis with NP^M = CPT * 512 cells known at compile time (every index
 // decode, stride and loop bound becomes a constant); NP = 0: run-time brick shape.
 __host__ __device__ constexpr int pbrick_ipow(int b, int e) { return e <= 0 ? 1 : b * pbrick_ipow(b, e - 1); }
+__host__ __device__ constexpr int pbrick_nt(int m, int cpt, int np) {   // threads per CTA of a compile-time shape (0: run time, <= 512)
+  return np ? ((pbrick_ipow(np, m) + cpt - 1) / cpt + 31) / 32 * 32 : 512;
+}
 template <int M, int PBRICK_CPT, int NP>
-__global__ void __launch_bounds__(512, (PBRICK_CPT == 8) ? 2 : 1) k_compact_pbrick(DevOp op, CompactTables ct, const double* __restrict__ in,
+__global__ void __launch_bounds__(pbrick_nt(M, PBRICK_CPT, NP), (PBRICK_CPT == 8) ? 2 : 1) k_compact_pbrick(DevOp op, CompactTables ct, const double* __restrict__ in,
                                                          double* out, double c, size_t slot_stride) {
   extern __shared__ double ptile_s[];
-  const int NT = NP ? 512 : blockDim.x, t = threadIdx.x;
+  const int NT = NP ? pbrick_nt(M, PBRICK_CPT, NP) : blockDim.x, t = threadIdx.x;
   const int pb = NP ? pbrick_ipow(NP, M) : (int)op.pb, nl = NP ? NP : op.n[2 * M - 1];
   double* tile = ptile_s;                                           // G_s
   double* rt = ptile_s + (pb + pb / nl);                            // B G_s / h, then d = A^{-1} B G_s
@@ -368,7 +371,10 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
   // (measured per stage, brick pass vs line passes: config 4 16.8 vs 18.3 ms, config 3 3.56 vs 4.58 ms; 20^3 bricks with
   // 16 cells per thread lose, 83.3 vs 74.9 ms, so they stay on the line passes unless CHFPE_COMPACT_PBRICK=2)
   static const bool pbrick_big = []() { const char* e = getenv("CHFPE_COMPACT_PBRICK"); return e && e[0] == '2'; }();
-  bool pbrick = pbrick_on && op.M >= 2 && op.pb <= (pbrick_big ? 16 : 8) * 512 && tile_bytes <= 200 * 1024 && op.nqc * op.K <= 0x7fffffffLL;
+  static const bool cube_on = []() { const char* e = getenv("CHFPE_COMPACT_CUBE"); return !(e && e[0] == '0'); }();
+  // (with the compile-time 20^3 shape the brick pass wins there as well: 55.4 vs 69.3 ms per stage at config 5)
+  const bool is20 = cube_on && op.M == 3 && op.n[3] == 20 && op.n[4] == 20 && op.n[5] == 20;
+  bool pbrick = pbrick_on && op.M >= 2 && op.pb <= ((pbrick_big || is20) ? 16 : 8) * 512 && tile_bytes <= 200 * 1024 && op.nqc * op.K <= 0x7fffffffLL;
   for (int s2 = 0; s2 < op.M; s2++) if (op.n[op.M + s2] > 1023) pbrick = false;
   for (int pa = 0; pa < (pbrick ? 1 : 2); pa++)
     for (int sI = 0; sI < op.M; sI++) {
@@ -424,12 +430,17 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
       cudaFuncSetAttribute(k_compact_pbrick<3, 8, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
       cudaFuncSetAttribute(k_compact_pbrick<3, 16, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
       cudaFuncSetAttribute(k_compact_pbrick<3, 8, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<3, 16, 20>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      cudaFuncSetAttribute(k_compact_pbrick<2, 8, 48>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
       optin = true;
     }
     const dim3 grid((unsigned)(op.nqc * op.K), 1, nb);                // element fastest: hierarchy neighbours meet in L2
-    static const bool cube_on = []() { const char* e = getenv("CHFPE_COMPACT_CUBE"); return !(e && e[0] == '0'); }();
     const bool cube16 = cube_on && op.M == 3 && op.n[3] == 16 && op.n[4] == 16 && op.n[5] == 16 && nt == 512;
-    if (op.M == 2 && cpt == 8) k_compact_pbrick<2, 8, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    const bool cube20 = cube_on && op.M == 3 && op.n[3] == 20 && op.n[4] == 20 && op.n[5] == 20 && nt == 512 && cpt == 16;
+    const bool sq48 = cube_on && op.M == 2 && op.n[2] == 48 && op.n[3] == 48 && nt == 288 && cpt == 8;
+    if (sq48) k_compact_pbrick<2, 8, 48><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else if (cube20) k_compact_pbrick<3, 16, 20><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    else if (op.M == 2 && cpt == 8) k_compact_pbrick<2, 8, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
     else if (op.M == 2) k_compact_pbrick<2, 16, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
     else if (cube16) k_compact_pbrick<3, 8, 16><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
     else if (cpt == 8) k_compact_pbrick<3, 8, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);

@@ -598,6 +598,9 @@ COMPACT = [
     ("m2_t24", ci.config("cfg3s", nq=[8, 8], np=[8, 24], depth=2, scheme="compact6")),
     # 16^3 bricks (config 4's): the compile-time-shaped brick pass k_compact_pbrick<3, 8, 16>
     ("m3_cube16", ci.config("cfg4", nq=[5, 6, 5], depth=2, scheme="compact6", mass=[1.0, 0.8, 1.2])),
+    # 48^2 (config 3) and 20^3 (config 5) bricks: k_compact_pbrick<2, 8, 48> (288 threads) and <3, 16, 20> (16 cells per thread)
+    ("m2_sq48_w", ci.config("cfg3", nq=[6, 5], depth=2, scheme="compact6", gauge="w", mass=[1.0, 1.3])),
+    ("m3_cube20", ci.config("cfg5", nq=[5, 5, 5], depth=1, scheme="compact6")),
 ]
 
 
