@@ -224,6 +224,29 @@ def test_response_2d_batched_over_t1(batch):
     assert np.array_equal(Rg[1], Rg[2])              # repeated t1 sample
 
 
+@pytest.mark.parametrize("scheme", ["central4", "compact6"])
+def test_protocols_on_the_march_kernel(scheme):
+    """The 1D and batched 2D response drivers on a three-mode n_1 x 32 x 32 mesh, i.e. with k_hermite_stage_tma under them
+    (explicit stencils: <CMP=false>; COMPACT6: <CMP=true> + the q_1 line pass): equilibrium state, kick, 40 RK4 steps with
+    batch slots at different trajectory positions, expectation values, against the oracle's plain loops."""
+    cfg = ci.config("cfg4h", nq=[6, 32, 32], np=[2, 2, 2], depth=1, scheme=scheme)
+    g, o = both(cfg, batch=3)
+    assert g.stage_kernel() == ("tma" if scheme == "central4" else "compact_tma")
+    g.equilibrate(); o.equilibrate()
+    mu, al = ci.observable("mu", 3), ci.observable("alpha", 3)
+    R1g = g.response_1d(gobs(mu), gobs(mu), 9, 5, 4e-3)
+    R1o = o.response_1d(mu, mu, 9, 5, 4e-3)
+    assert np.max(np.abs(R1o)) > 1e-3
+    assert np.max(np.abs(R1g - R1o)) <= 1e-8 * np.max(np.abs(R1o))
+    g.equilibrate(); o.equilibrate()
+    t1, t2 = [0, 4, 9], [0, 3, 8]
+    Rg = g.response_2d(gobs(mu), gobs(al), gobs(al), t1, t2, 4e-3)
+    Ro = o.response_2d(mu, al, al, t1, t2, 4e-3)
+    assert np.max(np.abs(Ro)) > 1e-5
+    assert np.max(np.abs(Rg - Ro)) <= 1e-8 * np.max(np.abs(Ro))
+    g.close()
+
+
 @pytest.mark.parametrize("batch,n2", [(3, 2), (5, 3), (4, 1), (2, 1)])
 def test_response_3d_batched(batch, n2):
     """Eq. (17): groups of (batch-1)/2 t1 samples (batch-1 for a single waiting time), ragged last group, repeated and
