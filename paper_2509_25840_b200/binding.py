@@ -488,6 +488,12 @@ class Hermite:
                  "chfpe_hermite_export_state")
         return X
 
+    def export_state_device(self, replica=0):
+        t = self._torch.empty(self.shape, dtype=self._torch.float64, device=self.device)
+        self._ck(lib().chfpe_hermite_export_state(self._h, replica, C.c_void_p(t.data_ptr()), 1),
+                 "chfpe_hermite_export_state")
+        return t
+
     def import_state(self, X, replica=0):
         if hasattr(X, "data_ptr"):
             assert X.is_cuda and X.is_contiguous() and X.numel() == self.values

@@ -413,6 +413,34 @@ def test_march_kernel_on_other_mesh_lengths(name, kw, monkeypatch):
     p.close(); g.close()
 
 
+@pytest.mark.parametrize("scheme", ["central4", "compact6"])
+def test_march_kernel_is_bitwise_reproducible_at_full_size(scheme):
+    """The march kernel synchronises its warps with mbarriers only (ring slots, exchange planes, the COMPACT6 line solves):
+    a missing wait would show up as a race, i.e. as run-to-run differences, most likely with all 10240 CTAs of the bench
+    workload in flight.  The kernel has no atomics and a fixed summation order, so two runs from the same state must agree
+    BITWISE: right-hand side twice, then two RK4 steps from the same state twice (the last stage updates y in place)."""
+    cfg = ci.config("cfg4h", scheme=scheme)
+    if torch.cuda.mem_get_info()[0] < 20e9:
+        pytest.skip("needs 20 GB of device memory")
+    g = P().Hermite(cfg)
+    assert g.stage_kernel() == ("tma" if scheme == "central4" else "compact_tma")
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    X = torch.rand(g.shape, dtype=torch.float64, device="cuda", generator=gen) - 0.5
+    g.import_state(X)
+    F1 = g.export_rhs_device().clone()
+    F2 = g.export_rhs_device()
+    assert torch.equal(F1, F2)
+    assert bool(torch.isfinite(F1).all()) and float(F1.abs().max()) > 0.0
+    del F1, F2
+    g.step(2, cfg["dt"])
+    Y1 = g.export_state_device()
+    g.import_state(X)
+    g.step(2, cfg["dt"])
+    Y2 = g.export_state_device()
+    assert torch.equal(Y1, Y2)
+    g.close()
+
+
 def test_full_size_rhs_on_an_embedded_block():
     """The bench workload (cfg4h: 32^3 q mesh, 8^3 Hermite functions, 20 elements = 3.36e8 values, launch configuration
     of bench.py --representation hermite).  The state is zero outside a 9 x 10 x 11 block of the q mesh; zero ghosts

@@ -212,6 +212,35 @@ FAMILY_ENVS = [
 ]
 
 
+@pytest.mark.parametrize("name", ["cfg4", "cfg5"])
+def test_stage_kernel_is_bitwise_reproducible_at_full_size(name):
+    """k_stage_tma synchronises its warps with mbarriers only (ring slots, exchange planes, the edge buffer of the p_3 stencil
+    at 20^3): a missing wait would be a race, i.e. run-to-run differences, most likely with every CTA of the bench workload
+    in flight.  No atomics, fixed summation order: the right-hand side of the same state must come out BITWISE equal twice,
+    and so must two RK4 steps (the last stage updates y in place)."""
+    cfg = ci.config(name)
+    P = gpu_mod()
+    arr = 8.0 * np.prod(cfg["nq"]) * np.prod(cfg["np"]) * 20           # one state array; the workspace holds three, the test three more
+    if torch.cuda.mem_get_info()[0] < 6.5 * arr + 2e9:
+        pytest.skip("needs %.0f GB of device memory" % ((6.5 * arr + 2e9) / 1e9))
+    g = P.CHFPE(cfg)
+    assert g.stage_kernel() == "tma"
+    g.equilibrate(residual=False)
+    g.kick(make_obs(P, ci.observable("mu", 3)))
+    g.step(1, cfg["dt"])                       # a state that is non-trivial on every element
+    X = g.export_state_device().clone()
+    F1 = g.export_rhs_device().clone()
+    F2 = g.export_rhs_device()
+    assert torch.equal(F1, F2) and bool(torch.isfinite(F1).all()) and float(F1.abs().max()) > 0.0
+    del F1, F2
+    g.step(2, cfg["dt"])
+    Y1 = g.export_state_device().clone()
+    g.import_state(X)
+    g.step(2, cfg["dt"])
+    assert torch.equal(Y1, g.export_state_device())
+    g.close()
+
+
 @pytest.mark.parametrize("name", ["m2_48_brick_w", "m3_cube12", "m3_cube20_c2"])
 def test_expectation_kernels_agree(name, monkeypatch):
     """k_expect_pbrick (momentum factors of the observable and of the gauge weight tabulated per brick in shared memory; the
