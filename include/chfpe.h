@@ -285,6 +285,8 @@ const char* chfpe_hermite_last_error(const chfpe_hermite_handle* h);   /* h may 
        CHFPE_KICK_BRICK=0     generic kick kernel + copy back instead of the in-place brick kick
        CHFPE_COMPACT_CUBE=0   run-time-shaped brick pass also for 16^3 / 48^2 bricks and line passes for 20^3 bricks
                               (default there: brick pass with a compile-time shape)
+       CHFPE_COMPACT_QPLANE=0 COMPACT6, three modes: one line pass per q axis instead of the fused (q_2, q_3) plane pass (16- and
+                              20-point axes)
        CHFPE_EXPECT_PBRICK=0  generic reduction (index decode per cell) instead of the factorised expectation kernel
        CHFPE_COMPACT_PBRICK=0|1|2   COMPACT6 p-derivatives: one line pass per momentum axis | one brick pass for bricks of
                               up to 4096 cells (default) | brick pass for bricks of up to 8192 cells as well

@@ -630,6 +630,9 @@ COMPACT = [
     # 48^2 (config 3) and 20^3 (config 5) bricks: k_compact_pbrick<2, 8, 48> (288 threads) and <3, 16, 20> (16 cells per thread)
     ("m2_sq48_w", ci.config("cfg3", nq=[6, 5], depth=2, scheme="compact6", gauge="w", mass=[1.0, 1.3])),
     ("m3_cube20", ci.config("cfg5", nq=[5, 5, 5], depth=1, scheme="compact6")),
+    # 16 x 16 and 20 x 20 (q_2, q_3) planes: the fused plane pass k_compact_qplane (q_2 and q_3 in one launch)
+    ("m3_qplane16_w", ci.config("cfg4s8", nq=[5, 16, 16], np=[5, 8, 8], depth=2, scheme="compact6", gauge="w", mass=[1.0, 0.8, 1.2])),
+    ("m3_qplane20", ci.config("cfg4s8", nq=[6, 20, 20], np=[5, 8, 6], depth=1, scheme="compact6")),
 ]
 
 
