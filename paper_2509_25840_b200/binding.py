@@ -355,7 +355,8 @@ class CHFPE:
     def stage_kernel_name(self):
         """Name of the CUDA kernel family behind stage_kernel() (for benchmark records)."""
         return {"generic": "k_stage_generic", "brick": "k_stage_brick3",
-                "compact": "k_compact_line passes", "tma": "k_stage_tma"}[self.stage_kernel()]
+                "compact": "COMPACT6 passes: k_compact_line / k_compact_qplane (q axes) + k_compact_pbrick (p axes)",
+                "tma": "k_stage_tma"}[self.stage_kernel()]
 
     def launch_count(self):
         n = C.c_int64()
