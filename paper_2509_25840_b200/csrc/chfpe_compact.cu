@@ -177,8 +177,13 @@ __global__ void __launch_bounds__(NQ * PC, (NQ * NQ * PC * 16 <= 72 * 1024) ? 3 
   const int iq1 = kq % op.n[0], k = kq / op.n[0];
   const size_t eoff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells + (size_t)iq1 * PTS * pb + (size_t)chunk * PC;
   const double* Xg = in + eoff;
-#pragma unroll 4
-  for (int i = t; i < TILE; i += NT) X[i] = Xg[(size_t)(i / PC) * pb + (i % PC)];
+  {                                                                  // NQ loads per thread, all in flight before the first use
+    double v[NQ];
+#pragma unroll
+    for (int j = 0; j < NQ; j++) { const int i = t + j * NT; v[j] = __ldg(Xg + (size_t)(i / PC) * pb + (i % PC)); }
+#pragma unroll
+    for (int j = 0; j < NQ; j++) X[t + j * NT] = v[j];
+  }
   __syncthreads();
   const int line = t / PC, pc = t - line * PC;
   double coef2, coef3;
@@ -220,11 +225,20 @@ __global__ void __launch_bounds__(NQ * PC, (NQ * NQ * PC * 16 <= 72 * 1024) ? 3 
   __syncthreads();
   const double* Yg = y + eoff;
   double* Og = out + eoff;
-#pragma unroll 4
-  for (int i = t; i < TILE; i += NT) {
-    const size_t g = (size_t)(i / PC) * pb + (i % PC);
-    const double v = c * A[i];
-    Og[g] = first ? fma(a, Yg[g], v) : Og[g] + v;
+  {
+    double v[NQ];
+#pragma unroll
+    for (int j = 0; j < NQ; j++) {
+      const int i = t + j * NT;
+      const size_t g = (size_t)(i / PC) * pb + (i % PC);
+      v[j] = first ? Yg[g] : Og[g];
+    }
+#pragma unroll
+    for (int j = 0; j < NQ; j++) {
+      const int i = t + j * NT;
+      const size_t g = (size_t)(i / PC) * pb + (i % PC);
+      Og[g] = first ? fma(a, v[j], c * A[i]) : v[j] + c * A[i];
+    }
   }
 }
 
