@@ -242,6 +242,50 @@ __global__ void __launch_bounds__(NQ * PC, (NQ * NQ * PC * 16 <= 72 * 1024) ? 3 
   }
 }
 
+// One q-line of compile-time length NQ per thread (q axes only): all NQ loads of the line are issued before the first use,
+// the recurrence runs in registers, then all NQ loads of the output (or of y) are issued before the first store -- the
+// memory-level parallelism of a thread is NQ instead of the one or two loads the generic kernel has in flight.
+template <int M, int NQ>
+__global__ void __launch_bounds__(128) k_compact_qline(DevOp op, const double* __restrict__ in, const double* y, double* out,
+                                                       double a, double c, int s, int first, size_t slot_stride,
+                                                       const double* __restrict__ ib, const double* __restrict__ cf) {
+  const long long st = op.st[s];
+  const long long line = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (line >= op.cells / NQ) return;
+  const int k = blockIdx.y;
+  const size_t eoff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells;
+  const long long outer = line / st, inner = line - outer * st;
+  const long long base = outer * st * NQ + inner;
+  int idx[2 * M];
+  cdecode<2 * M>(op, (unsigned)base, idx);
+  const double coef = -(op.x0[M + s] + idx[M + s] * op.h[M + s]) * op.inv_mass[s];
+  const double* Xk = in + eoff + base;
+  double f[NQ + 2];
+#pragma unroll
+  for (int i = 0; i < NQ; i++) f[i] = __ldg(Xk + (long long)i * st);
+  f[NQ] = 0.0; f[NQ + 1] = 0.0;
+  const double al = 1.0 / 3.0, ca = 7.0 / 9.0, cb = 1.0 / 36.0, inv_h = 1.0 / op.h[s];
+  double d[NQ];
+  double prev = 0.0;
+#pragma unroll
+  for (int i = 0; i < NQ; i++) {
+    const double fm1 = (i >= 1) ? f[i - 1] : 0.0, fm2 = (i >= 2) ? f[i - 2] : 0.0;
+    const double r = (ca * (f[i + 1] - fm1) + cb * (f[i + 2] - fm2)) * inv_h;
+    prev = (i == 0) ? r * __ldg(ib) : (r - al * prev) * __ldg(ib + i);
+    d[i] = prev;
+  }
+#pragma unroll
+  for (int i = NQ - 2; i >= 0; i--) d[i] = d[i] - __ldg(cf + i + 1) * d[i + 1];
+  const double cc = c * coef;
+  const double* Y = y + eoff + base;
+  double* O = out + eoff + base;
+  double o[NQ];
+#pragma unroll
+  for (int i = 0; i < NQ; i++) o[i] = first ? Y[(long long)i * st] : O[(long long)i * st];
+#pragma unroll
+  for (int i = 0; i < NQ; i++) O[(long long)i * st] = first ? fma(a, o[i], cc * d[i]) : o[i] + cc * d[i];
+}
+
 // p_M pass (the contiguous axis): one thread per line would read 8 bytes per 128-byte line and request.  A warp
 // therefore takes 32 consecutive lines (32 n contiguous doubles), loads them coalesced, forms G_M on the way and
 // transposes through a padded shared tile [32][n+1]; every lane then runs the Thomas recurrence on its row in place,
@@ -488,6 +532,20 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
       }
       const int axis = pa ? op.M + sI : sI;
       const int n = op.n[axis];
+      static const bool qline_on = []() { const char* e = getenv("CHFPE_COMPACT_QLINE"); return !(e && e[0] == '0'); }();
+      if (pa == 0 && qline_on && (n == 16 || n == 20) && op.M >= 2) {   // q lines of the BASELINE lengths: loads ahead of the recurrence
+        const dim3 grid((unsigned)((op.cells / n + 127) / 128), op.K, nb);
+#define CALLQ(MM)                                                                                                     \
+  do {                                                                                                                \
+    if (n == 16) k_compact_qline<MM, 16><<<grid, 128, 0, s>>>(op, in, y, out, a, c, sI, first, slot_stride, ct.ibet[axis], ct.cfac[axis]); \
+    else k_compact_qline<MM, 20><<<grid, 128, 0, s>>>(op, in, y, out, a, c, sI, first, slot_stride, ct.ibet[axis], ct.cfac[axis]);       \
+  } while (0)
+        CDISPATCH(op.M, CALLQ);
+#undef CALLQ
+        launches++;
+        first = 0;
+        continue;
+      }
       const unsigned lb = (unsigned)((op.cells / n + 127) / 128);
       const bool local = n <= CLINE_MAX;
 #define LINE(MM, PA, NFV, GRID, K0, B0)                                                                               \

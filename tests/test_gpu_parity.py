@@ -633,6 +633,9 @@ COMPACT = [
     # 16 x 16 and 20 x 20 (q_2, q_3) planes: the fused plane pass k_compact_qplane (q_2 and q_3 in one launch)
     ("m3_qplane16_w", ci.config("cfg4s8", nq=[5, 16, 16], np=[5, 8, 8], depth=2, scheme="compact6", gauge="w", mass=[1.0, 0.8, 1.2])),
     ("m3_qplane20", ci.config("cfg4s8", nq=[6, 20, 20], np=[5, 8, 6], depth=1, scheme="compact6")),
+    # 16- and 20-point q lines outside the plane pass: k_compact_qline (loads ahead of the recurrence), two and three modes
+    ("m3_qline16", ci.config("cfg4s8", nq=[16, 5, 6], np=[5, 6, 7], depth=2, scheme="compact6", mass=[1.0, 0.8, 1.2])),
+    ("m2_qline20_16_w", ci.config("cfg3s", nq=[20, 16], np=[9, 8], depth=2, scheme="compact6", gauge="w")),
 ]
 
 
