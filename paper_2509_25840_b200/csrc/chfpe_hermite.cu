@@ -559,12 +559,18 @@ __global__ void __launch_bounds__(128) k_hermite_compact_line_fixed(const HOp op
     Pm2 = Pm1; Pm1 = P0; P0 = P1; P1 = P2;
   }
   const double f = -c * op.a2[s];
-  double x = fwd[N - 1];
-  po[(size_t)(N - 1) * st] += f * x;
+  // back substitution in place, then the read-modify-write of the output in blocks of 8 points whose loads are all issued
+  // before the first store (the compiler cannot move a load of po[] above a store to po[]: the stride is a run-time value)
 #pragma unroll
-  for (int i = N - 2; i >= 0; i--) {
-    x = fwd[i] - __ldg(cfac + i + 1) * x;
-    po[(size_t)i * st] += f * x;
+  for (int i = N - 2; i >= 0; i--) fwd[i] = fwd[i] - __ldg(cfac + i + 1) * fwd[i + 1];
+  constexpr int B = (N % 8 == 0) ? 8 : 1;
+#pragma unroll
+  for (int i0 = 0; i0 < N; i0 += B) {
+    double o[B];
+#pragma unroll
+    for (int j = 0; j < B; j++) o[j] = po[(size_t)(i0 + j) * st];
+#pragma unroll
+    for (int j = 0; j < B; j++) po[(size_t)(i0 + j) * st] = fma(f, fwd[i0 + j], o[j]);
   }
 }
 
