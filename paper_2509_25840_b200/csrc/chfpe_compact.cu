@@ -475,6 +475,113 @@ __global__ void __launch_bounds__(pbrick_nt(M, PBRICK_CPT, NP), (PBRICK_CPT == 8
   }
 }
 
+// The brick pass for cubic three-mode bricks of NP^3 cells (NP = 16: config 4, NP = 20: config 5), thread-per-column form:
+// thread (i_2, i_3) owns the NP cells of its p_1 column in registers.  Per mode s it forms G_s on its column; the p_1 lines
+// ARE the columns, so their right-hand sides and Thomas recurrences run in registers with no shared memory and no barrier;
+// for p_2 and p_3 the columns go through one shared tile [i_1][i_2][i_3 + pad], thread (i_1, i_3) resp. (i_1, i_2) takes
+// one line into registers, solves it and puts it back, and the owners add their cells.  Same arithmetic as
+// k_compact_pbrick; about a quarter of its instructions (no index decode, no ghost predicates on shared loads, every
+// thread busy in the recurrences of modes 2 and 3).
+template <int NP>
+__global__ void __launch_bounds__((NP * NP + 31) / 32 * 32, (NP == 16) ? 3 : 1) k_compact_pcolumn(
+    DevOp op, CompactTables ct, const double* __restrict__ in, double* out, double c, size_t slot_stride) {
+  extern __shared__ double pcol_s[];
+  constexpr int M = 3, LD = NP + 1, PL = NP * NP, PB = NP * PL;
+  const int t = threadIdx.x;
+  const bool active = t < PL;
+  const int ta = active ? t : 0;
+  const int ia = ta / NP, ib = ta - ia * NP;                        // (i_2, i_3) as owner; (i_1, i_3) / (i_1, i_2) as line solver
+  const long long ql = blockIdx.x / op.K;
+  const int k = (int)(blockIdx.x - ql * op.K);
+  const size_t eoff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells + (size_t)ql * PB;
+  const double* Xk = in + eoff + ta;                                // cell (i_1, i_2, i_3) = i_1 * PL + t
+  int iq[M];
+  {
+    long long r = ql;
+#pragma unroll
+    for (int s = M - 1; s >= 0; s--) { iq[s] = (int)(r % op.n[s]); r /= op.n[s]; }
+  }
+  const double gam = __ldg(op.Gamma + k);
+  double acc[NP];
+#pragma unroll
+  for (int i = 0; i < NP; i++) acc[i] = -gam * Xk[i * PL];
+  const double al = 1.0 / 3.0, ca = 7.0 / 9.0, cb = 1.0 / 36.0;
+  auto solve = [&](double (&f)[NP], const int ap) {                 // f <- A^{-1} B f / h along one line
+    const double* __restrict__ ibet = ct.ibet[ap];
+    const double* __restrict__ cfac = ct.cfac[ap];
+    const double inv_h = 1.0 / op.h[ap];
+    double fm2 = 0.0, fm1 = 0.0, prev = 0.0;
+#pragma unroll
+    for (int i = 0; i < NP; i++) {
+      const double fp1 = (i + 1 < NP) ? f[i + 1] : 0.0, fp2 = (i + 2 < NP) ? f[i + 2] : 0.0;
+      const double r = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
+      const double ibi = __ldg(ibet + i);
+      fm2 = fm1; fm1 = f[i];
+      prev = (i == 0) ? r * ibi : fma(-al * ibi, prev, r * ibi);
+      f[i] = prev;
+    }
+#pragma unroll
+    for (int i = NP - 2; i >= 0; i--) f[i] = fma(-__ldg(cfac + i + 1), f[i + 1], f[i]);
+  };
+#pragma unroll
+  for (int s = 0; s < M; s++) {
+    const int ap = M + s;
+    const double q = op.x0[s] + iq[s] * op.h[s];
+    const double Vp = fma(op.VSL[s], q, op.VLL[s]);
+    const double ck = __ldg(op.dU[s] + ql);
+    const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+    const double cu = (ku >= 0) ? Vp : 0.0;
+    const double cd = (kd >= 0) ? __ldg(op.nvec + 3 * k + s) * op.cdn[s] * Vp : 0.0;
+    const double* Xu = Xk + ((long long)(ku >= 0 ? ku : k) - k) * op.cells;
+    const double* Xd = Xk + ((long long)(kd >= 0 ? kd : k) - k) * op.cells;
+    const double pu = op.kup[s] * cu, pd = op.kdn[s] * cd;
+    double g[NP];
+#pragma unroll
+    for (int i = 0; i < NP; i++) {                                  // G_s and the gauge terms p_s V'_s (kup X_up + n c kdn X_dn)
+      double v = ck * Xk[i * PL], pw = 0.0;
+      if (ku >= 0) { const double xu = Xu[i * PL]; v = fma(cu, xu, v); pw = pu * xu; }
+      if (kd >= 0) { const double xd = Xd[i * PL]; v = fma(cd, xd, v); pw = fma(pd, xd, pw); }
+      const int ip = (s == 0) ? i : (s == 1 ? ia : ib);
+      acc[i] = fma(op.x0[ap] + ip * op.h[ap], pw, acc[i]);
+      g[i] = v;
+    }
+    if (s == 0) {                                                   // p_1 lines: the thread's own column
+      solve(g, ap);
+#pragma unroll
+      for (int i = 0; i < NP; i++) acc[i] += g[i];
+    } else {
+      if (s == 2) __syncthreads();                                  // the owners have read the p_2 results
+      if (active) {
+#pragma unroll
+        for (int i = 0; i < NP; i++) pcol_s[(i * NP + ia) * LD + ib] = g[i];
+      }
+      __syncthreads();
+      // line of thread (ia, ib): s = 1: (i_1 = ia, i_3 = ib) along i_2; s = 2: (i_1 = ia, i_2 = ib) along i_3
+      double* L = (s == 1) ? pcol_s + ia * NP * LD + ib : pcol_s + (ia * NP + ib) * LD;
+      constexpr int one = 1;
+      const int st = (s == 1) ? LD : one;
+#pragma unroll
+      for (int i = 0; i < NP; i++) g[i] = L[i * st];
+      solve(g, ap);
+      if (active) {
+#pragma unroll
+        for (int i = 0; i < NP; i++) L[i * st] = g[i];
+      }
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < NP; i++) acc[i] += pcol_s[(i * NP + ia) * LD + ib];
+    }
+  }
+  if (active) {
+    double* O = out + eoff + ta;
+    double o[NP];
+#pragma unroll
+    for (int i = 0; i < NP; i++) o[i] = O[i * PL];
+#pragma unroll
+    for (int i = 0; i < NP; i++) O[i * PL] = fma(c, acc[i], o[i]);
+  }
+}
+
 }  // namespace
 
 #define CDISPATCH(M, CALL) do { if ((M) == 1) { CALL(1); } else if ((M) == 2) { CALL(2); } else { CALL(3); } } while (0)
@@ -604,7 +711,15 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
     const bool cube16 = cube_on && op.M == 3 && op.n[3] == 16 && op.n[4] == 16 && op.n[5] == 16 && nt == 512;
     const bool cube20 = cube_on && op.M == 3 && op.n[3] == 20 && op.n[4] == 20 && op.n[5] == 20 && nt == 512 && cpt == 16;
     const bool sq48 = cube_on && op.M == 2 && op.n[2] == 48 && op.n[3] == 48 && nt == 288 && cpt == 8;
-    if (sq48) k_compact_pbrick<2, 8, 48><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
+    static const bool pcol_on = []() { const char* e = getenv("CHFPE_COMPACT_PCOLUMN"); return !(e && e[0] == '0'); }();
+    static bool pcol_optin = false;
+    if (!pcol_optin) {
+      cudaFuncSetAttribute(k_compact_pcolumn<20>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * 20 * 20 * 21));
+      pcol_optin = true;
+    }
+    if (pcol_on && cube16) k_compact_pcolumn<16><<<grid, 256, sizeof(double) * 16 * 16 * 17, s>>>(op, ct, in, out, c, slot_stride);
+    else if (pcol_on && cube20) k_compact_pcolumn<20><<<grid, 416, sizeof(double) * 20 * 20 * 21, s>>>(op, ct, in, out, c, slot_stride);
+    else if (sq48) k_compact_pbrick<2, 8, 48><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
     else if (cube20) k_compact_pbrick<3, 16, 20><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
     else if (op.M == 2 && cpt == 8) k_compact_pbrick<2, 8, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
     else if (op.M == 2) k_compact_pbrick<2, 16, 0><<<grid, nt, tile_bytes, s>>>(op, ct, in, out, c, slot_stride);
