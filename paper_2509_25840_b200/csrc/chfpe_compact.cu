@@ -483,7 +483,7 @@ __global__ void __launch_bounds__(pbrick_nt(M, PBRICK_CPT, NP), (PBRICK_CPT == 8
 // k_compact_pbrick; about a quarter of its instructions (no index decode, no ghost predicates on shared loads, every
 // thread busy in the recurrences of modes 2 and 3).
 template <int NP>
-__global__ void __launch_bounds__((NP * NP + 31) / 32 * 32, (NP == 16) ? 3 : 1) k_compact_pcolumn(
+__global__ void __launch_bounds__((NP * NP + 31) / 32 * 32, (NP == 16) ? 2 : 1) k_compact_pcolumn(
     DevOp op, CompactTables ct, const double* __restrict__ in, double* out, double c, size_t slot_stride) {
   extern __shared__ double pcol_s[];
   constexpr int M = 3, LD = NP + 1, PL = NP * NP, PB = NP * PL;
