@@ -92,3 +92,19 @@ def test_hermite_workspace_bytes_and_validation():
     h = C.c_void_p()
     rc = P.lib().chfpe_hermite_create(C.byref(d), None, 0, None, C.byref(h))
     assert rc == -2 and not h.value          # CHFPE_ERR_WORKSPACE
+
+
+def test_every_environment_knob_is_documented_in_the_header():
+    """include/chfpe.h ("Tunables") lists every CHFPE_* environment variable the library reads (kernel variants and launch
+    plans that compute the same results): a knob added to csrc/ without a line there fails this test."""
+    import glob
+    import re
+    root = os.path.join(os.path.dirname(__file__), "..")
+    names = set()
+    for f in glob.glob(os.path.join(root, "paper_2509_25840_b200", "csrc", "*")):
+        names |= set(re.findall(r'(?:getenv|env_int)\("(CHFPE_[A-Z0-9_]+)"', open(f).read()))
+    assert len(names) >= 20
+    header = open(os.path.join(root, "include", "chfpe.h")).read()
+    missing = sorted(n for n in names if n not in header)
+    assert not missing, missing
+
