@@ -288,7 +288,8 @@ const char* chfpe_hermite_last_error(const chfpe_hermite_handle* h);   /* h may 
        CHFPE_COMPACT_QPLANE=0 COMPACT6, three modes: one line pass per q axis instead of the fused (q_2, q_3) plane pass (16- and
                               20-point axes)
        CHFPE_COMPACT_PCOLUMN=0 COMPACT6, 16^3 / 20^3 bricks: k_compact_pbrick instead of the thread-per-column brick pass
-       CHFPE_COMPACT_QLINE=0  COMPACT6: generic line kernel also for 16- and 20-point q lines (default there: k_compact_qline)
+       CHFPE_COMPACT_QLINE=0  COMPACT6: generic line kernel also for 16-, 20- and (two modes) 48-point q lines (default there:
+                              k_compact_qline / k_compact_qline_long)
        CHFPE_EXPECT_PBRICK=0  generic reduction (index decode per cell) instead of the factorised expectation kernel
        CHFPE_COMPACT_PBRICK=0|1|2   COMPACT6 p-derivatives: one line pass per momentum axis | one brick pass for bricks of
                               up to 4096 cells (default) | brick pass for bricks of up to 8192 cells as well

@@ -286,6 +286,64 @@ __global__ void __launch_bounds__(128) k_compact_qline(DevOp op, const double* _
   for (int i = 0; i < NQ; i++) O[(long long)i * st] = first ? fma(a, o[i], cc * d[i]) : o[i] + cc * d[i];
 }
 
+// The same for long lines (NQ a multiple of 8, e.g. the 48-point axes of config 3): the operand streams through a window
+// of three blocks of 8 points -- the block two ahead is requested before the current one is used -- while the NQ forward
+// values stay in registers; the output is read-modify-written in blocks of 8 with the loads ahead of the stores.
+template <int M, int NQ>
+__global__ void __launch_bounds__(128) k_compact_qline_long(DevOp op, const double* __restrict__ in, const double* y, double* out,
+                                                            double a, double c, int s, int first, size_t slot_stride,
+                                                            const double* __restrict__ ib, const double* __restrict__ cf) {
+  static_assert(NQ % 8 == 0 && NQ >= 24, "blocks of 8 points");
+  constexpr int B = 8, NB = NQ / B;
+  const long long st = op.st[s];
+  const long long line = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (line >= op.cells / NQ) return;
+  const int k = blockIdx.y;
+  const size_t eoff = (size_t)blockIdx.z * slot_stride + (size_t)k * op.cells;
+  const long long outer = line / st, inner = line - outer * st;
+  const long long base = outer * st * NQ + inner;
+  int idx[2 * M];
+  cdecode<2 * M>(op, (unsigned)base, idx);
+  const double coef = -(op.x0[M + s] + idx[M + s] * op.h[M + s]) * op.inv_mass[s];
+  const double* Xk = in + eoff + base;
+  const double al = 1.0 / 3.0, ca = 7.0 / 9.0, cb = 1.0 / 36.0, inv_h = 1.0 / op.h[s];
+  double d[NQ];
+  double cur[B], nxt[B], nn[B];
+#pragma unroll
+  for (int j = 0; j < B; j++) { cur[j] = __ldg(Xk + (long long)j * st); nxt[j] = __ldg(Xk + (long long)(B + j) * st); }
+  double fm2 = 0.0, fm1 = 0.0, prev = 0.0;
+#pragma unroll
+  for (int b = 0; b < NB; b++) {
+#pragma unroll
+    for (int j = 0; j < B; j++) nn[j] = (b + 2 < NB) ? __ldg(Xk + (long long)((b + 2) * B + j) * st) : 0.0;
+#pragma unroll
+    for (int j = 0; j < B; j++) {
+      const int i = b * B + j;
+      const double fp1 = (j + 1 < B) ? cur[j + 1] : nxt[0];          // (nxt is zero past the end of the line)
+      const double fp2 = (j + 2 < B) ? cur[j + 2] : nxt[j + 2 - B];
+      const double r = (ca * (fp1 - fm1) + cb * (fp2 - fm2)) * inv_h;
+      prev = (i == 0) ? r * __ldg(ib) : (r - al * prev) * __ldg(ib + i);
+      d[i] = prev;
+      fm2 = fm1; fm1 = cur[j];
+    }
+#pragma unroll
+    for (int j = 0; j < B; j++) { cur[j] = nxt[j]; nxt[j] = nn[j]; }
+  }
+#pragma unroll
+  for (int i = NQ - 2; i >= 0; i--) d[i] = d[i] - __ldg(cf + i + 1) * d[i + 1];
+  const double cc = c * coef;
+  const double* Y = y + eoff + base;
+  double* O = out + eoff + base;
+#pragma unroll
+  for (int b = 0; b < NB; b++) {
+    double o[B];
+#pragma unroll
+    for (int j = 0; j < B; j++) o[j] = first ? Y[(long long)(b * B + j) * st] : O[(long long)(b * B + j) * st];
+#pragma unroll
+    for (int j = 0; j < B; j++) O[(long long)(b * B + j) * st] = first ? fma(a, o[j], cc * d[b * B + j]) : o[j] + cc * d[b * B + j];
+  }
+}
+
 // p_M pass (the contiguous axis): one thread per line would read 8 bytes per 128-byte line and request.  A warp
 // therefore takes 32 consecutive lines (32 n contiguous doubles), loads them coalesced, forms G_M on the way and
 // transposes through a padded shared tile [32][n+1]; every lane then runs the Thomas recurrence on its row in place,
@@ -640,6 +698,13 @@ int launch_stage_compact(const DevOp& op, const CompactTables& ct, const double*
       const int axis = pa ? op.M + sI : sI;
       const int n = op.n[axis];
       static const bool qline_on = []() { const char* e = getenv("CHFPE_COMPACT_QLINE"); return !(e && e[0] == '0'); }();
+      if (pa == 0 && qline_on && n == 48 && op.M == 2) {                // config 3's lines: blocked window
+        const dim3 grid((unsigned)((op.cells / n + 127) / 128), op.K, nb);
+        k_compact_qline_long<2, 48><<<grid, 128, 0, s>>>(op, in, y, out, a, c, sI, first, slot_stride, ct.ibet[axis], ct.cfac[axis]);
+        launches++;
+        first = 0;
+        continue;
+      }
       if (pa == 0 && qline_on && (n == 16 || n == 20) && op.M >= 2) {   // q lines of the BASELINE lengths: loads ahead of the recurrence
         const dim3 grid((unsigned)((op.cells / n + 127) / 128), op.K, nb);
 #define CALLQ(MM)                                                                                                     \

@@ -636,6 +636,8 @@ COMPACT = [
     # 16- and 20-point q lines outside the plane pass: k_compact_qline (loads ahead of the recurrence), two and three modes
     ("m3_qline16", ci.config("cfg4s8", nq=[16, 5, 6], np=[5, 6, 7], depth=2, scheme="compact6", mass=[1.0, 0.8, 1.2])),
     ("m2_qline20_16_w", ci.config("cfg3s", nq=[20, 16], np=[9, 8], depth=2, scheme="compact6", gauge="w")),
+    # 48-point q lines of two modes (config 3): k_compact_qline_long (window of three blocks of 8 points), both axes
+    ("m2_qline48", ci.config("cfg3s", nq=[48, 48], np=[5, 6], depth=1, scheme="compact6", mass=[1.0, 1.3])),
 ]
 
 
