@@ -559,6 +559,19 @@ __global__ void __launch_bounds__((NP * NP + 31) / 32 * 32, (NP == 16) ? 2 : 1) 
 #pragma unroll
     for (int s = M - 1; s >= 0; s--) { iq[s] = (int)(r % op.n[s]); r /= op.n[s]; }
   }
+  if (t == 0) {
+    // the bricks this CTA will read later -- hierarchy neighbours of the three modes, the output -- are contiguous runs of
+    // PB doubles: ask L2 for them now, so that the three mode phases and the final read-modify-write do not each pay a
+    // DRAM latency with only two CTAs per SM to hide it
+    const double* base = in + eoff;
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(out + eoff), "r"((unsigned)(PB * sizeof(double))) : "memory");
+#pragma unroll
+    for (int s = 0; s < M; s++) {
+      const int ku = __ldg(op.up + 3 * k + s), kd = __ldg(op.dn + 3 * k + s);
+      if (ku >= 0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(base + ((long long)ku - k) * op.cells), "r"((unsigned)(PB * sizeof(double))) : "memory");
+      if (kd >= 0) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(base + ((long long)kd - k) * op.cells), "r"((unsigned)(PB * sizeof(double))) : "memory");
+    }
+  }
   const double gam = __ldg(op.Gamma + k);
   double acc[NP];
 #pragma unroll
