@@ -181,6 +181,11 @@ __global__ void __launch_bounds__(NQ * PC, (NQ * NQ * PC * 16 <= 72 * 1024) ? 3 
     double v[NQ];
 #pragma unroll
     for (int j = 0; j < NQ; j++) { const int i = t + j * NT; v[j] = __ldg(Xg + (size_t)(i / PC) * pb + (i % PC)); }
+    if ((t & 15) == 0) {                                             // the lines of the final read-modify-write: ask L2 now
+      const double* Pg = (first ? y : out) + eoff;
+#pragma unroll
+      for (int j = 0; j < NQ; j++) { const int i = t + j * NT; asm volatile("prefetch.global.L2 [%0];" ::"l"(Pg + (size_t)(i / PC) * pb + (i % PC))); }
+    }
 #pragma unroll
     for (int j = 0; j < NQ; j++) X[t + j * NT] = v[j];
   }
